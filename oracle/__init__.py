@@ -1,0 +1,167 @@
+"""ctypes front-end of the C oracle (oracle/tpcf_oracle.c).  TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import
+this package; it imports nothing from paper_1204_6630_b200.  The arithmetic is all in the C file (one
+thread per call); this module marshals arrays and, when threads > 1, splits the outer i-rows over
+Python threads that each call the same single-threaded C loop on a private histogram and sums the
+integer results (order-independent).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from concurrent.futures import ThreadPoolExecutor
+from dataclasses import dataclass
+from typing import Optional
+
+import numpy as np
+
+from .build import build as _build
+
+_lib = None
+
+
+def lib() -> ctypes.CDLL:
+    global _lib
+    if _lib is None:
+        L = ctypes.CDLL(_build())
+        vp, sz, i32, i64p = ctypes.c_void_p, ctypes.c_size_t, ctypes.c_int, ctypes.c_void_p
+        L.orc_radec_to_xyz.argtypes = [vp, sz, vp]
+        L.orc_radec_to_xyz.restype = None
+        L.orc_count_auto.argtypes = [vp, sz, sz, sz, vp, i32, vp, vp, vp]
+        L.orc_count_auto.restype = i32
+        L.orc_count_cross.argtypes = [vp, sz, sz, sz, vp, sz, vp, i32, vp, vp, vp]
+        L.orc_count_cross.restype = i32
+        L.orc_count_rows.argtypes = [vp, i64p, sz, sz, vp, sz, i32, vp, i32, vp, vp, vp]
+        L.orc_count_rows.restype = i32
+        L.orc_estimate.argtypes = [vp, vp, vp, i32, ctypes.c_uint64, ctypes.c_uint64, vp]
+        L.orc_estimate.restype = None
+        _lib = L
+    return _lib
+
+
+def host_threads() -> int:
+    try:
+        return max(1, len(os.sched_getaffinity(0)))
+    except AttributeError:  # pragma: no cover
+        return max(1, os.cpu_count() or 1)
+
+
+def _ptr(a: Optional[np.ndarray]):
+    return None if a is None else a.ctypes.data_as(ctypes.c_void_p)
+
+
+def radec_to_xyz(radec) -> np.ndarray:
+    """O1+O2: rows of (RA, Dec) degrees, float32 widened exactly to float64 -> (n, 3) unit vectors."""
+    rd = np.ascontiguousarray(np.asarray(radec, dtype=np.float64).reshape(-1, 2))
+    out = np.empty((rd.shape[0], 3), dtype=np.float64)
+    lib().orc_radec_to_xyz(_ptr(rd), rd.shape[0], _ptr(out))
+    return out
+
+
+@dataclass
+class Counts:
+    """One histogram: hist[k] for the nbins theta bins plus the out-of-range counters."""
+    hist: np.ndarray          # uint64[nbins]
+    under: int
+    over: int
+    near: Optional[np.ndarray] = None   # uint64[nbins+1], O6 near-edge counters (validation runs)
+    mismatch: Optional[int] = None      # O8 self-check counter (validation runs)
+
+    @property
+    def total(self) -> int:
+        return int(self.hist.sum(dtype=np.uint64)) + self.under + self.over
+
+    def tol(self) -> np.ndarray:
+        """Per-bin tolerance tol_k = near[k] + near[k+1] (BASELINE.json / SURVEY.md O6)."""
+        assert self.near is not None
+        return (self.near[:-1] + self.near[1:]).astype(np.int64)
+
+
+def _run(kind: str, spans, call, nbins: int, validate: bool, threads: int) -> Counts:
+    def one(span):
+        h = np.zeros(nbins + 2, dtype=np.uint64)
+        nr = np.zeros(nbins + 1, dtype=np.uint64) if validate else None
+        mm = np.zeros(1, dtype=np.uint64) if validate else None
+        rc = call(span[0], span[1], h, nr, mm)
+        if rc != 0:
+            raise ValueError(f"oracle {kind}: bad arguments (rc={rc})")
+        return h, nr, mm
+
+    if threads <= 1 or len(spans) == 1:
+        parts = [one(s) for s in spans]
+    else:
+        with ThreadPoolExecutor(max_workers=threads) as ex:
+            parts = list(ex.map(one, spans))
+    h = np.sum([p[0] for p in parts], axis=0, dtype=np.uint64)
+    near = np.sum([p[1] for p in parts], axis=0, dtype=np.uint64) if validate else None
+    mm = int(np.sum([p[2] for p in parts], dtype=np.uint64)) if validate else None
+    return Counts(h[1:-1].copy(), int(h[0]), int(h[-1]), near, mm)
+
+
+def _even_spans(n: int, parts: int):
+    cuts = np.linspace(0, n, max(1, min(parts, n)) + 1).astype(np.int64)
+    return [(int(a), int(b)) for a, b in zip(cuts[:-1], cuts[1:]) if b > a] or [(0, 0)]
+
+
+def _triangle_spans(n: int, parts: int):
+    """Split rows 0..n so each span holds about the same number of i<j pairs."""
+    parts = max(1, min(parts, n))
+    total = n * (n - 1) / 2.0
+    cuts = [0]
+    for p in range(1, parts):
+        # rows [0, c) hold c*n - c(c+1)/2 pairs; solve for the target
+        t = total * p / parts
+        c = int(n - 0.5 - np.sqrt(max((n - 0.5) ** 2 - 2.0 * t, 0.0)))
+        cuts.append(min(max(c, cuts[-1]), n))
+    cuts.append(n)
+    return [(a, b) for a, b in zip(cuts[:-1], cuts[1:]) if b > a] or [(0, 0)]
+
+
+def count_auto(xyz: np.ndarray, edges, validate: bool = False, threads: int = 1) -> Counts:
+    """DD or RR: all unordered pairs i<j of one catalog (reading A3)."""
+    xyz = np.ascontiguousarray(xyz, dtype=np.float64)
+    e = np.ascontiguousarray(edges, dtype=np.float64)
+    nb, n = e.shape[0] - 1, xyz.shape[0]
+    L = lib()
+    call = lambda a, b, h, nr, mm: L.orc_count_auto(_ptr(xyz), n, a, b, _ptr(e), nb, _ptr(h), _ptr(nr), _ptr(mm))
+    return _run("auto", _triangle_spans(n, threads * 4 if threads > 1 else 1), call, nb, validate, threads)
+
+
+def count_cross(a: np.ndarray, b: np.ndarray, edges, validate: bool = False, threads: int = 1) -> Counts:
+    """DR: all N_a * N_b ordered pairs."""
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    b = np.ascontiguousarray(b, dtype=np.float64)
+    e = np.ascontiguousarray(edges, dtype=np.float64)
+    nb = e.shape[0] - 1
+    L = lib()
+    call = lambda i0, i1, h, nr, mm: L.orc_count_cross(_ptr(a), a.shape[0], i0, i1, _ptr(b), b.shape[0], _ptr(e), nb,
+                                                       _ptr(h), _ptr(nr), _ptr(mm))
+    return _run("cross", _even_spans(a.shape[0], threads), call, nb, validate, threads)
+
+
+def count_rows(a: np.ndarray, rows, b: np.ndarray, exclude_self: bool, edges, validate: bool = False,
+               threads: int = 1) -> Counts:
+    """Row-subset mode: sum_{i in rows} sum_j, skipping j == i when exclude_self."""
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    b = np.ascontiguousarray(b, dtype=np.float64)
+    r = np.ascontiguousarray(rows, dtype=np.int64)
+    if r.size and (r.min() < 0 or r.max() >= a.shape[0]):
+        raise ValueError("row index out of range")
+    e = np.ascontiguousarray(edges, dtype=np.float64)
+    nb = e.shape[0] - 1
+    L = lib()
+    call = lambda r0, r1, h, nr, mm: L.orc_count_rows(_ptr(a), _ptr(r), r0, r1, _ptr(b), b.shape[0],
+                                                      1 if exclude_self else 0, _ptr(e), nb, _ptr(h), _ptr(nr),
+                                                      _ptr(mm))
+    return _run("rows", _even_spans(r.shape[0], threads), call, nb, validate, threads)
+
+
+def estimate(dd, dr, rr, n_d: int, n_r: int) -> np.ndarray:
+    """O7: pair-normalised Landy-Szalay w_k (Eq. 1 as read in A1)."""
+    dd = np.ascontiguousarray(dd, dtype=np.uint64)
+    dr = np.ascontiguousarray(dr, dtype=np.uint64)
+    rr = np.ascontiguousarray(rr, dtype=np.uint64)
+    w = np.empty(dd.shape[0], dtype=np.float64)
+    lib().orc_estimate(_ptr(dd), _ptr(dr), _ptr(rr), dd.shape[0], int(n_d), int(n_r), _ptr(w))
+    return w

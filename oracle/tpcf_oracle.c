@@ -1,0 +1,167 @@
+/*
+ * tpcf_oracle.c -- TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+ *
+ * Plain, slow, double-precision brute-force oracle for the angular pair counts DD, DR, RR and the
+ * Landy-Szalay estimator of arXiv:1204.6630 (reference text: PAPER.md).  It is the *definition*
+ * of the result written out: for every pair, dot product -> arc-cosine -> theta -> bin, exactly the
+ * two operations the paper names for its kernels (Section 3, first bullet), filling
+ * the three histograms of PAPER.md:25/38 (Eq. 1 and Section 3, second bullet).
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+ * load this file.  It shares no code, header, table or constant with paper_1204_6630_b200/.
+ *
+ * Readings of the paper where it is silent (restated in DESIGN.md):
+ *   A3  DD/RR count unordered pairs i<j; DR counts all N_D*N_R ordered pairs.
+ *   A5  bin k = [e_k, e_{k+1}) in theta, last bin closed at e_n (numpy.histogram convention).
+ *   A7  the dot product is clamped to [-1, 1] before acos.
+ *   A8  RA/Dec in degrees; x = cos(dec)cos(ra), y = cos(dec)sin(ra), z = sin(dec).
+ *   A1  estimator in pair-normalised form (BASELINE.json north_star), see orc_estimate.
+ *
+ * Pins (tests/test_oracle_pins.py, run with -m "not gpu"): hand catalogs P1, totals P2,
+ * numpy.histogram of arccos of a Gram matrix P3, great-circle ring closed form P4, integer
+ * identities P5, uniform-sphere closed form P6, null test P7, Eq. 1 hand case P8, acos-vs-asin P9.
+ * Unpinned: absolute w(theta) values on the MICE catalogs / Fig. 1 (data not available).
+ *
+ * Build: gcc -O2 -ffp-contract=off -fPIC -shared tpcf_oracle.c -o libtpcf_oracle.so -lm
+ */
+#include <math.h>
+#include <stddef.h>
+#include <stdint.h>
+
+#ifndef M_PI
+#define M_PI 3.14159265358979323846
+#endif
+
+/* O2 (A8): RA, Dec in degrees -> unit vector.  radec is n rows x 2, xyz is n rows x 3. */
+void orc_radec_to_xyz(const double *radec, size_t n, double *xyz)
+{
+    for (size_t i = 0; i < n; ++i) {
+        double alpha = radec[2 * i] * M_PI / 180.0;
+        double delta = radec[2 * i + 1] * M_PI / 180.0;
+        xyz[3 * i + 0] = cos(delta) * cos(alpha);
+        xyz[3 * i + 1] = cos(delta) * sin(alpha);
+        xyz[3 * i + 2] = sin(delta);
+    }
+}
+
+/* O5 (A5): slot 0 = under (theta < e_0), slots 1..n = bins, slot n+1 = over (theta > e_n). */
+static int bin_slot(double theta, const double *e, int n)
+{
+    if (theta < e[0]) return 0;
+    if (theta > e[n]) return n + 1;
+    int lo = 0, hi = n; /* invariant: e[lo] <= theta, and (hi == n or theta < e[hi]) */
+    while (hi - lo > 1) {
+        int mid = (lo + hi) / 2;
+        if (e[mid] <= theta) lo = mid; else hi = mid;
+    }
+    return lo + 1; /* largest k with e_k <= theta, capped at n-1 */
+}
+
+/* One pair: O4 (dot, clamp A7, acos), O5 (bin), optional O6 (near-edge counters), optional O8. */
+static inline void one_pair(const double *a, const double *b, const double *e, const double *cose, int n,
+                            uint64_t *hist, uint64_t *near, uint64_t *mismatch)
+{
+    double s = a[0] * b[0] + a[1] * b[1] + a[2] * b[2];
+    if (s > 1.0) s = 1.0;
+    if (s < -1.0) s = -1.0;
+    double theta = acos(s) * 180.0 / M_PI;
+    int slot = bin_slot(theta, e, n);
+    ++hist[slot];
+    if (near) {
+        /* O6: ++near[k] for every edge k with |s - cos(e_k)| <= 1e-6 (BASELINE.json tolerance).
+         * cos(e_k) decreases with k, so the edges that qualify are one contiguous run: find its
+         * start by bisection and walk it (same set as testing every k). */
+        int lo = 0, hi = n + 1; /* first k with cose[k] <= s + 1e-6 */
+        while (lo < hi) {
+            int mid = (lo + hi) / 2;
+            if (cose[mid] <= s + 1e-6) hi = mid; else lo = mid + 1;
+        }
+        for (int k = (lo > 0 ? lo - 1 : 0); k <= n && cose[k] >= s - 2e-6; ++k) /* generous window */
+            if (fabs(s - cose[k]) <= 1e-6) ++near[k];                          /* the defining test */
+    }
+    if (mismatch) {
+        /* O8 / P9: theta' = 2 asin(|a-b|/2), well conditioned at small theta; must bin identically. */
+        double dx = a[0] - b[0], dy = a[1] - b[1], dz = a[2] - b[2];
+        double h = 0.5 * sqrt(dx * dx + dy * dy + dz * dz);
+        if (h > 1.0) h = 1.0;
+        double theta2 = 2.0 * asin(h) * 180.0 / M_PI;
+        if (bin_slot(theta2, e, n) != slot) ++*mismatch;
+    }
+}
+
+#define MAX_EDGES 4100
+
+static int prep(const double *e, int n, double *cose)
+{
+    if (n < 1 || n + 1 > MAX_EDGES) return -1;
+    for (int k = 0; k <= n; ++k) cose[k] = cos(e[k] * M_PI / 180.0);
+    return 0;
+}
+
+/*
+ * Auto-pairs (DD, RR): all i<j with i in [i_begin, i_end) (A3).  hist has n+2 slots and is
+ * ACCUMULATED into (caller zeroes it); near has n+1 slots or is NULL; mismatch is one counter or NULL.
+ */
+int orc_count_auto(const double *xyz, size_t npts, size_t i_begin, size_t i_end, const double *edges, int nbins,
+                   uint64_t *hist, uint64_t *near, uint64_t *mismatch)
+{
+    double cose[MAX_EDGES];
+    if (prep(edges, nbins, cose)) return -1;
+    for (size_t i = i_begin; i < i_end && i < npts; ++i)
+        for (size_t j = i + 1; j < npts; ++j)
+            one_pair(xyz + 3 * i, xyz + 3 * j, edges, cose, nbins, hist, near, mismatch);
+    return 0;
+}
+
+/* Cross-pairs (DR): all (i, j), i in [i_begin, i_end) of a, every j of b. */
+int orc_count_cross(const double *a, size_t na, size_t i_begin, size_t i_end, const double *b, size_t nb,
+                    const double *edges, int nbins, uint64_t *hist, uint64_t *near, uint64_t *mismatch)
+{
+    double cose[MAX_EDGES];
+    if (prep(edges, nbins, cose)) return -1;
+    for (size_t i = i_begin; i < i_end && i < na; ++i)
+        for (size_t j = 0; j < nb; ++j)
+            one_pair(a + 3 * i, b + 3 * j, edges, cose, nbins, hist, near, mismatch);
+    return 0;
+}
+
+/*
+ * Row-subset mode: sum over i in rows[r_begin..r_end) of all j in b; with
+ * exclude_self != 0 (a and b are the same catalog) the pair j == rows[r] is skipped, so the total is
+ * nrows*(N-1) and both sides of the diagonal are counted.
+ */
+int orc_count_rows(const double *a, const int64_t *rows, size_t r_begin, size_t r_end, const double *b, size_t nb,
+                   int exclude_self, const double *edges, int nbins, uint64_t *hist, uint64_t *near,
+                   uint64_t *mismatch)
+{
+    double cose[MAX_EDGES];
+    if (prep(edges, nbins, cose)) return -1;
+    for (size_t r = r_begin; r < r_end; ++r) {
+        size_t i = (size_t)rows[r];
+        for (size_t j = 0; j < nb; ++j) {
+            if (exclude_self && j == i) continue;
+            one_pair(a + 3 * i, b + 3 * j, edges, cose, nbins, hist, near, mismatch);
+        }
+    }
+    return 0;
+}
+
+/*
+ * O7: Landy-Szalay in pair-count-normalised form (Eq. 1, whose extraction lost the
+ * square on N_random/N_real -- reading A1; form fixed by BASELINE.json north_star):
+ *   w_k = (DD_k/nDD - 2 DR_k/nDR + RR_k/nRR) / (RR_k/nRR),
+ *   nDD = N_D(N_D-1)/2, nDR = N_D N_R, nRR = N_R(N_R-1)/2;  RR_k = 0 -> NaN (A14).
+ * dd, dr, rr point at the nbins in-range counts (no under/over slots).
+ */
+void orc_estimate(const uint64_t *dd, const uint64_t *dr, const uint64_t *rr, int nbins, uint64_t n_d, uint64_t n_r,
+                  double *w)
+{
+    double ndd = 0.5 * (double)n_d * ((double)n_d - 1.0);
+    double ndr = (double)n_d * (double)n_r;
+    double nrr = 0.5 * (double)n_r * ((double)n_r - 1.0);
+    for (int k = 0; k < nbins; ++k) {
+        if (rr[k] == 0) { w[k] = NAN; continue; }
+        double fdd = (double)dd[k] / ndd, fdr = (double)dr[k] / ndr, frr = (double)rr[k] / nrr;
+        w[k] = (fdd - 2.0 * fdr + frr) / frr;
+    }
+}

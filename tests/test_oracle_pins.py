@@ -1,0 +1,282 @@
+"""Pins for the fp64 oracle against things that are NOT the oracle.
+
+Every pin is chosen so that a plausible slip in oracle/tpcf_oracle.c (dropped term, wrong sign or
+index, transposed operand, wrong edge convention, wrong normalisation in Eq. 1) fails at least one.
+None of these tests touches the CUDA library.
+"""
+import json
+import math
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+import synth
+
+GOLD = json.load(open(os.path.join(os.path.dirname(__file__), "golden", "hand_catalogs.json")))
+
+
+def xyz_of(radec):
+    return oracle.radec_to_xyz(np.asarray(radec, dtype=np.float64))
+
+
+def unit_bins(lo, hi):
+    """Unit-width bins centred on the integers lo..hi: edges lo-0.5, ..., hi+0.5."""
+    return np.arange(lo - 0.5, hi + 1.0, 1.0)
+
+
+# ------------------------------------------------------------------ P1 hand catalogs
+@pytest.mark.parametrize("name", ["equator", "meridian", "wrap", "poles"])
+def test_p1_hand_separations(name):
+    g = GOLD[name]
+    e = unit_bins(0, 180)                      # bins centred on 0..180 deg
+    e[0] = 0.0
+    e[-1] = 180.0
+    c = oracle.count_auto(xyz_of(g["radec"]), e)
+    want = np.zeros(181, dtype=np.uint64)
+    for s in g["separations"]:
+        want[int(round(s))] += 1
+    assert c.under == 0 and c.over == 0
+    np.testing.assert_array_equal(c.hist, want)
+    n = len(g["radec"])
+    assert c.total == n * (n - 1) // 2
+
+
+def test_p1_octahedron_closed_last_bin_and_clamp():
+    g = GOLD["octahedron"]
+    c = oracle.count_auto(xyz_of(g["radec"]), np.array(g["edges"], dtype=np.float64))
+    np.testing.assert_array_equal(c.hist, np.array(g["hist"], dtype=np.uint64))
+    assert (c.under, c.over) == (0, 0)         # 180 deg lands IN the closed last bin, not in 'over'
+
+
+def test_p1_interior_edge_is_lower_inclusive():
+    """A5: bin k = [e_k, e_{k+1}), last bin closed.  The +x, +y, +z axes are pairwise exactly 90 deg apart
+    in fp64 (dot products 6e-17 or 0, acos -> pi/2 exactly, pi/2*180/pi = 90.0), so with an interior edge
+    AT 90 the 3 pairs belong to the upper bin, and with 90 as the LAST edge they are in range."""
+    v = xyz_of([[0, 0], [90, 0], [0, 90]])
+    c = oracle.count_auto(v, np.array([0.0, 90.0, 135.0, 180.0]))
+    np.testing.assert_array_equal(c.hist, np.array([0, 3, 0], dtype=np.uint64))
+    c = oracle.count_auto(v, np.array([10.0, 90.0]))
+    assert (c.under, int(c.hist[0]), c.over) == (0, 3, 0)
+    c = oracle.count_auto(v, np.array([90.0, 100.0]))
+    assert (c.under, int(c.hist[0]), c.over) == (0, 3, 0)
+
+
+def test_p1_general_pair_two_formulas():
+    g = GOLD["general_pair"]
+    (ra1, d1), (ra2, d2) = np.radians(g["radec"])
+    law_of_cos = math.sin(d1) * math.sin(d2) + math.cos(d1) * math.cos(d2) * math.cos(ra1 - ra2)
+    hav = math.sin((d2 - d1) / 2) ** 2 + math.cos(d1) * math.cos(d2) * math.sin((ra2 - ra1) / 2) ** 2
+    assert abs(law_of_cos - g["cos_theta"]) < 1e-14
+    assert abs(math.degrees(2 * math.asin(math.sqrt(hav))) - g["theta"]) < 1e-11
+    v = xyz_of(g["radec"])
+    assert abs(float(v[0] @ v[1]) - g["cos_theta"]) < 1e-14
+    th = g["theta"]
+    c = oracle.count_auto(v, np.array([th - 1e-9, th + 1e-9]))
+    assert c.hist[0] == 1
+    c = oracle.count_auto(v, np.array([th + 1e-9, th + 1.0]))
+    assert (c.under, int(c.hist[0]), c.over) == (1, 0, 0)
+
+
+@pytest.mark.parametrize("name", ["small_ra", "small_dec"])
+def test_p1_small_angle_conditioning(name):
+    g = GOLD[name]
+    th = g["theta"]
+    c = oracle.count_auto(xyz_of(g["radec"]), np.array([th * (1 - 1e-6), th * (1 + 1e-6)]), validate=True)
+    assert c.hist[0] == 1 and c.mismatch == 0
+
+
+def test_p1_cross_counts_on_hand_points():
+    a = xyz_of(GOLD["equator"]["radec"][:2])        # RA 0, 1 on the equator
+    b = xyz_of([[3, 0], [7, 0], [15, 0]])
+    e = unit_bins(0, 20)
+    e[0] = 0.0
+    c = oracle.count_cross(a, b, e)
+    want = np.zeros(21, dtype=np.uint64)
+    for s in (3, 7, 15, 2, 6, 14):
+        want[s] += 1
+    np.testing.assert_array_equal(c.hist, want)
+    assert c.total == 6
+
+
+def test_p1_unit_vectors_convention():
+    v = xyz_of([[0, 0], [90, 0], [0, 90], [180, 0], [45, 0], [0, -90]])
+    want = np.array([[1, 0, 0], [0, 1, 0], [0, 0, 1], [-1, 0, 0], [math.sqrt(0.5), math.sqrt(0.5), 0], [0, 0, -1]])
+    np.testing.assert_allclose(v, want, atol=1.3e-16)
+    np.testing.assert_allclose(np.linalg.norm(xyz_of(synth.uniform_sphere(1000, synth.SplitMix(5))), axis=1), 1.0,
+                               atol=3e-16)
+
+
+def test_p1_float32_rows_widen_exactly():
+    rd32 = np.array([[10.1, 20.2], [33.3, -44.4]], dtype=np.float32)
+    np.testing.assert_array_equal(oracle.radec_to_xyz(rd32), oracle.radec_to_xyz(rd32.astype(np.float64)))
+
+
+# ------------------------------------------------------------------ P2 totals identity
+def test_p2_totals_auto_cross_rows():
+    D, R, e, _ = synth.make_config(1, n_d=700, n_r=500)
+    d, r = oracle.radec_to_xyz(D), oracle.radec_to_xyz(R)
+    full = np.array([0.0, 1.0, 50.0, 180.0])
+    assert oracle.count_auto(d, full).total == 700 * 699 // 2
+    assert oracle.count_auto(d, full).under == 0 and oracle.count_auto(d, full).over == 0
+    assert oracle.count_cross(d, r, e).total == 700 * 500
+    rows = synth.subset_rows(700, 50)
+    assert oracle.count_rows(d, rows, d, True, e).total == 50 * 699
+    assert oracle.count_rows(d, rows, r, False, e).total == 50 * 500
+
+
+# ------------------------------------------------------------------ P3 library routine on tiny inputs
+@pytest.mark.parametrize("idx,n", [(1, 900), (5, 700)])
+def test_p3_numpy_histogram_of_arccos_gram(idx, n):
+    D, R, e, _ = synth.make_config(idx, n_d=n, n_r=n // 2)
+    d, r = oracle.radec_to_xyz(D), oracle.radec_to_xyz(R)
+    th = np.degrees(np.arccos(np.clip(d @ d.T, -1.0, 1.0)))[np.triu_indices(n, 1)]
+    ref, _ = np.histogram(th, bins=e)
+    c = oracle.count_auto(d, e)
+    # the Gram matrix comes from BLAS (different summation order): allow the few ulp-tie pairs
+    assert np.abs(c.hist.astype(np.int64) - ref).sum() <= 2
+    assert c.under == int((th < e[0]).sum()) and c.over == int((th > e[-1]).sum())
+    thx = np.degrees(np.arccos(np.clip(d @ r.T, -1.0, 1.0))).ravel()
+    refx, _ = np.histogram(thx, bins=e)
+    assert np.abs(oracle.count_cross(d, r, e).hist.astype(np.int64) - refx).sum() <= 2
+
+
+def test_p3_explicit_python_loop_tiny():
+    """Brute force in pure Python with math.acos on 40 points, exact equality."""
+    D, _, e, _ = synth.make_config(1, n_d=40, n_r=8)
+    d = oracle.radec_to_xyz(D)
+    want = np.zeros(len(e) + 1, dtype=np.uint64)
+    for i in range(40):
+        for j in range(i + 1, 40):
+            s = d[i, 0] * d[j, 0] + d[i, 1] * d[j, 1] + d[i, 2] * d[j, 2]
+            th = math.acos(max(-1.0, min(1.0, s))) * 180.0 / math.pi
+            if th < e[0]:
+                want[0] += 1
+            elif th > e[-1]:
+                want[-1] += 1
+            else:
+                want[min(int(np.searchsorted(e, th, side="right")) - 1, len(e) - 2) + 1] += 1
+    c = oracle.count_auto(d, e)
+    np.testing.assert_array_equal(np.concatenate([[c.under], c.hist, [c.over]]).astype(np.uint64), want)
+
+
+# ------------------------------------------------------------------ P4 ring closed form
+@pytest.mark.parametrize("n", [360, 1000])
+def test_p4_ring_auto(n):
+    delta = 360.0 / n
+    v = xyz_of(synth.great_circle_ring(n))
+    e = (np.arange(0, n // 2 + 1) + 0.5) * delta      # bin m-1 = ((m-.5)d, (m+.5)d) holds separation m*d
+    e[-1] = 180.0
+    c = oracle.count_auto(v, e, validate=True)
+    want = np.full(n // 2, n, dtype=np.uint64)
+    want[-1] = n // 2                                  # antipodal pairs
+    np.testing.assert_array_equal(c.hist, want)
+    assert c.under == 0 and c.over == 0 and c.total == n * (n - 1) // 2 and c.mismatch == 0
+
+
+def test_p4_ring_cross_shifted():
+    n = 360
+    a = xyz_of(synth.great_circle_ring(n))
+    b = xyz_of(synth.great_circle_ring(n, phase_deg=0.5))
+    c = oracle.count_cross(a, b, np.arange(0.0, 181.0, 1.0))   # separations (m+1/2) deg, 2n each
+    np.testing.assert_array_equal(c.hist, np.full(180, 2 * n, dtype=np.uint64))
+    assert c.total == n * n
+
+
+# ------------------------------------------------------------------ P5 exact integer identities
+def test_p5_identities():
+    D, R, e, _ = synth.make_config(2, n_d=900, n_r=600)
+    d, r = oracle.radec_to_xyz(D), oracle.radec_to_xyz(R)
+    a, b = d[:400], d[400:]
+    H = lambda c: np.concatenate([[c.under], c.hist.astype(np.int64), [c.over]])
+    dd = H(oracle.count_auto(d, e))
+    # permutation invariance
+    perm = np.argsort(synth.SplitMix(9).u64(900))
+    np.testing.assert_array_equal(H(oracle.count_auto(d[perm], e)), dd)
+    # additivity DD(A u B) = DD(A) + DD(B) + DR(A, B)
+    np.testing.assert_array_equal(H(oracle.count_auto(a, e)) + H(oracle.count_auto(b, e)) + H(oracle.count_cross(a, b, e)), dd)
+    # DR(D, R1 u R2) = DR(D, R1) + DR(D, R2); DR(a,b) = DR(b,a)
+    dr = H(oracle.count_cross(d, r, e))
+    np.testing.assert_array_equal(H(oracle.count_cross(d, r[:250], e)) + H(oracle.count_cross(d, r[250:], e)), dr)
+    np.testing.assert_array_equal(H(oracle.count_cross(r, d, e)), dr)
+    # DR(D, D) = 2 DD + N self pairs at theta = 0 (under, because e_0 = 0.01 > 0)
+    self_dr = H(oracle.count_cross(d, d, e))
+    want = 2 * dd
+    want[0] += 900
+    np.testing.assert_array_equal(self_dr, want)
+    # subset mode over a partition of the rows sums to 2 DD
+    rows = np.arange(900)
+    parts = [rows[:300], rows[300:301], rows[301:]]
+    np.testing.assert_array_equal(sum(H(oracle.count_rows(d, p, d, True, e)) for p in parts), 2 * dd)
+    # threads do not change integers
+    np.testing.assert_array_equal(H(oracle.count_auto(d, e, threads=3)), dd)
+    np.testing.assert_array_equal(H(oracle.count_cross(d, r, e, threads=3)), dr)
+    # nested edges: merging adjacent bins = counting with the coarser edges
+    coarse = oracle.count_auto(d, e[::2])
+    np.testing.assert_array_equal(coarse.hist.astype(np.int64), dd[1:-1].reshape(-1, 2).sum(1))
+
+
+# ------------------------------------------------------------------ P6 uniform full sphere
+def test_p6_uniform_sphere_closed_form():
+    n = 6000
+    v = xyz_of(synth.uniform_sphere(n, synth.SplitMix(11)))
+    e = synth.edges(25, 0.5, 180.0, "log")
+    c = oracle.count_auto(v, e, threads=oracle.host_threads())
+    npairs = n * (n - 1) / 2
+    exp = npairs * (np.cos(np.radians(e[:-1])) - np.cos(np.radians(e[1:]))) / 2.0
+    assert np.all(np.abs(c.hist - exp) <= 5.0 * np.sqrt(exp) + 1.0)
+    assert abs(c.under - npairs * (1 - math.cos(math.radians(0.5))) / 2) <= 5 * math.sqrt(c.under + 1) + 1
+    assert c.over == 0
+    # same closed form for a linear binning and for the cross count
+    w = xyz_of(synth.uniform_sphere(3000, synth.SplitMix(12)))
+    el = synth.edges(18, 0.0, 180.0, "linear")
+    cx = oracle.count_cross(v, w, el, threads=oracle.host_threads())
+    expx = n * 3000 * (np.cos(np.radians(el[:-1])) - np.cos(np.radians(el[1:]))) / 2.0
+    assert np.all(np.abs(cx.hist - expx) <= 5.0 * np.sqrt(expx) + 1.0)
+
+
+# ------------------------------------------------------------------ P7 null test, P8 Eq. 1 algebra
+def test_p7_null_test_w_consistent_with_zero():
+    patch = (0.0, 20.0, -10.0, 10.0)
+    d = xyz_of(synth.uniform_patch(5000, patch, synth.SplitMix(21)))
+    r = xyz_of(synth.uniform_patch(7000, patch, synth.SplitMix(22)))
+    e = synth.edges(10, 0.3, 10.0, "log")
+    t = oracle.host_threads()
+    dd, dr, rr = oracle.count_auto(d, e, threads=t), oracle.count_cross(d, r, e, threads=t), oracle.count_auto(r, e, threads=t)
+    w = oracle.estimate(dd.hist, dr.hist, rr.hist, 5000, 7000)
+    assert np.all(np.abs(w) <= 5.0 / np.sqrt(np.minimum(dd.hist, rr.hist)))
+
+
+def test_p8_eq1_hand_case_and_same_catalog():
+    g = GOLD["landy_szalay_hand"]
+    w = oracle.estimate(g["dd"], g["dr"], g["rr"], g["n_d"], g["n_r"])
+    assert abs(w[0] - g["w"][0]) < 1e-15
+    assert math.isnan(oracle.estimate([1], [1], [0], 5, 5)[0])
+    # D = R (same N rows): DD_k = RR_k, DR_k = 2 DD_k in bins that exclude theta = 0  =>  w_k = 2/N exactly
+    D, _, e, _ = synth.make_config(1, n_d=500, n_r=8)
+    d = oracle.radec_to_xyz(D)
+    dd, dr = oracle.count_auto(d, e), oracle.count_cross(d, d, e)
+    w = oracle.estimate(dd.hist, dr.hist, dd.hist, 500, 500)
+    ok = dd.hist > 0
+    np.testing.assert_allclose(w[ok], 2.0 / 500, rtol=0, atol=1e-12)
+
+
+# ------------------------------------------------------------------ P9 two independent angle formulas, O6
+@pytest.mark.parametrize("idx", [1, 2, 5])
+def test_p9_acos_vs_asin_chord(idx):
+    D, R, e, _ = synth.make_config(idx, n_d=1200, n_r=800)
+    d, r = oracle.radec_to_xyz(D), oracle.radec_to_xyz(R)
+    assert oracle.count_auto(d, e, validate=True).mismatch == 0
+    assert oracle.count_cross(d, r, e, validate=True).mismatch == 0
+
+
+def test_o6_near_edge_counters_match_numpy():
+    D, R, e, _ = synth.make_config(1, n_d=600, n_r=400)
+    d, r = oracle.radec_to_xyz(D), oracle.radec_to_xyz(R)
+    s = np.clip(d @ r.T, -1, 1).ravel()
+    ce = np.cos(np.radians(e))
+    want = np.array([(np.abs(s - c) <= 1e-6).sum() for c in ce])
+    got = oracle.count_cross(d, r, e, validate=True).near
+    assert np.abs(got.astype(np.int64) - want).sum() <= 2      # BLAS-vs-loop rounding at the 1e-6 boundary
+    assert got.sum() > 0                                       # the small log bins do sit within 1e-6 in cos
