@@ -1,0 +1,172 @@
+/*
+ * tpcf.h -- C ABI of the B200-native pair-counting library (libtpcf.so).
+ *
+ * The library computes the hot path of the Landy-Szalay angular two-point correlation function of
+ * arXiv:1204.6630: brute-force all-pairs angular pair counting of a data catalog D and a
+ * random catalog R into the three theta-binned histograms DD, DR, RR (the definitions
+ * under Eq. 1; Section 3 bullets 1-2: per pair a dot product and an arc-cosine, then a
+ * histogram update with shared-memory atomics, partial histograms merged in global memory), and the
+ * estimator of Eq. 1.  Every step runs in hand-written CUDA kernels for sm_100a; there
+ * is no CPU fallback: every entry point that needs the GPU returns TPCF_ECUDA when none is usable.
+ *
+ * Conventions
+ *   - All pointers are HOST pointers unless the argument says "device".  The caller owns every buffer
+ *     it passes in; the library copies what it needs before returning and owns all of its own device
+ *     memory through the opaque context.  No torch / C++ types cross this boundary.
+ *   - Every function returns a tpcf_status and never throws or aborts; tpcf_last_error() gives a
+ *     human-readable message for the last failure on that context.
+ *   - Calls on one context must not be concurrent.  All calls are synchronous on return except the
+ *     explicitly *_async one.
+ *   - Bins (reading A5 in DESIGN.md; the paper does not state a convention): bin k = [e_k, e_{k+1}) in
+ *     theta, the LAST bin closed at e_n (numpy.histogram's convention); under = theta < e_0,
+ *     over = theta > e_n; always under + sum(bins) + over = number of pairs enumerated.
+ *   - Pairs (reading A3): DD / RR enumerate the unordered pairs i<j of one catalog, N(N-1)/2 of them;
+ *     DR enumerates all N_D*N_R ordered pairs (BASELINE.json north_star).
+ */
+#ifndef TPCF_H
+#define TPCF_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct tpcf_ctx tpcf_ctx;
+
+typedef enum { TPCF_OK = 0, TPCF_EINVAL = 1, TPCF_ENOMEM = 2, TPCF_ECUDA = 3, TPCF_ESTATE = 4 } tpcf_status;
+typedef enum { TPCF_LINEAR = 0, TPCF_LOG = 1, TPCF_EXPLICIT = 2 } tpcf_binning;
+typedef enum { TPCF_D = 0, TPCF_R = 1 } tpcf_cat;
+typedef enum { TPCF_F32 = 0, TPCF_F64 = 1 } tpcf_dtype;
+typedef enum { TPCF_DD = 0, TPCF_DR = 1, TPCF_RR = 2 } tpcf_kind;
+
+/* Which kernel family tpcf_count uses (tpcf_set_engine).
+ *   TPCF_ENGINE_FAST    fp32 squared-chord evaluation, O(1) cell lookup against cos/chord-space
+ *                       thresholds, privatised shared-memory histograms; every pair that lands within the
+ *                       fp32 rounding guard band of a bin edge is re-evaluated in fp64 from the fp64
+ *                       coordinates, so the histograms equal those of TPCF_ENGINE_EXACT64 (default).
+ *   TPCF_ENGINE_EXACT64 plain fp64 kernel: fp64 squared chord against fp64 thresholds 4 sin^2(e_k/2) by
+ *                       binary search.  Slow; kept as the device-side cross-check of the fast engine. */
+typedef enum { TPCF_ENGINE_FAST = 0, TPCF_ENGINE_EXACT64 = 1 } tpcf_engine;
+
+/*
+ * tpcf_create -- fix the theta binning (the paper gives none; BASELINE.json configs do).
+ *   nbins      >= 1 (and <= 4096).
+ *   theta_deg  LINEAR / LOG: two doubles {min, max} in degrees, 0 <= min < max <= 180 (LOG: min > 0).
+ *                LINEAR: e_k = min + k (max-min)/nbins.  LOG: e_k = min * (max/min)^(k/nbins).
+ *                e_0 = min and e_n = max exactly.
+ *              EXPLICIT: nbins+1 strictly increasing edges in [0, 180].
+ *   Does not touch the GPU (thresholds and lookup tables are built on the host here and uploaded at the
+ *   first count).  Errors: TPCF_EINVAL on any violated condition above or a NaN edge.
+ */
+tpcf_status tpcf_create(tpcf_ctx** out, int nbins, const double* theta_deg, tpcf_binning mode);
+
+/* Copies the nbins+1 edges (degrees) the context uses, so a checker can bin with the very same values. */
+tpcf_status tpcf_get_edges(const tpcf_ctx* ctx, double* edges_out /* nbins+1 */);
+
+/*
+ * tpcf_load -- load catalog D or R: n rows of (RA, Dec) in degrees, row-major n x 2, dtype F32 or F64
+ *   ("input file lines").  The rows are copied to the device (or read in place
+ *   when on_device != 0, in which case radec_deg is a device pointer) and converted ON THE DEVICE to unit
+ *   vectors x = cos(dec)cos(ra), y = cos(dec)sin(ra), z = sin(dec) in fp64 (reading A8); the fp32 copy the
+ *   fast engine uses is that fp64 vector rounded once.  Replaces any previous catalog in that slot and
+ *   invalidates stored counts that used it.
+ *   cuda_stream: a cudaStream_t (or NULL for the context's stream) the copy and conversion are ordered on;
+ *   the call returns after they completed.
+ *   Errors: TPCF_EINVAL for n == 0, n > 2^31-1, |Dec| > 90 or a non-finite value in any row (checked on
+ *   the device); TPCF_ENOMEM; TPCF_ECUDA.
+ */
+tpcf_status tpcf_load(tpcf_ctx* ctx, tpcf_cat which, const void* radec_deg, tpcf_dtype dt, size_t n, int on_device,
+                      void* cuda_stream);
+
+/*
+ * tpcf_count -- one histogram.
+ *   kind       TPCF_DD (pairs i<j of D), TPCF_RR (pairs i<j of R), TPCF_DR (all pairs D x R).
+ *   hist_out   nbins uint64 counts (host).
+ *   under_over_out  NULL, or 2 uint64: {pairs with theta < e_0, pairs with theta > e_n}.
+ *   rows/nrows NULL/0 for the full count.  Otherwise ROW-SUBSET mode (validation of catalogs too large for
+ *              a CPU oracle, BASELINE.json): rows are indices into D (for DD, DR) or R (for RR), and the
+ *              call counts sum over i in rows of all j != i of the same catalog (DD, RR: nrows*(N-1) pairs,
+ *              both sides of the diagonal) or of all j of R (DR: nrows*N_R pairs).  A subset count is not
+ *              stored for tpcf_estimate.
+ *   Errors: TPCF_ESTATE if a needed catalog is not loaded; TPCF_EINVAL for a row index out of range;
+ *   TPCF_ECUDA.
+ */
+tpcf_status tpcf_count(tpcf_ctx* ctx, tpcf_kind kind, uint64_t* hist_out, uint64_t* under_over_out,
+                       const int64_t* rows, size_t nrows);
+
+/*
+ * tpcf_count_async -- the same full count, without host synchronisation: enqueues the kernels on the
+ *   context's stream (tpcf_set_stream) and writes nbins+2 uint64 {under, bin_0..bin_{n-1}, over} to the
+ *   DEVICE buffer hist_dev when they complete.  The count is not stored for tpcf_estimate.  This is the
+ *   entry point timed with CUDA events when the catalogs are already resident.
+ */
+tpcf_status tpcf_count_async(tpcf_ctx* ctx, tpcf_kind kind, uint64_t* hist_dev /* device, nbins+2 */);
+
+/*
+ * tpcf_estimate -- Landy-Szalay w(theta) in the pair-count-normalised form (Eq. 1, whose
+ *   extraction lost the square on N_random/N_real; form fixed by BASELINE.json north_star, reading A1):
+ *     w_k = (DD_k/nDD - 2 DR_k/nDR + RR_k/nRR) / (RR_k/nRR),
+ *     nDD = N_D(N_D-1)/2, nDR = N_D N_R, nRR = N_R(N_R-1)/2;   RR_k = 0 gives NaN.
+ *   Needs full (non-subset, non-partitioned) DD, DR and RR counted by tpcf_count on the current catalogs,
+ *   else TPCF_ESTATE.
+ */
+tpcf_status tpcf_estimate(tpcf_ctx* ctx, double* w_out /* nbins */);
+
+/* The same arithmetic on caller-supplied histograms (used after a multi-process reduction). */
+tpcf_status tpcf_estimate_from(const uint64_t* dd, const uint64_t* dr, const uint64_t* rr, int nbins, uint64_t n_d,
+                               uint64_t n_r, double* w_out /* nbins */);
+
+void tpcf_destroy(tpcf_ctx* ctx);
+const char* tpcf_last_error(const tpcf_ctx* ctx);
+
+/* ---- controls ------------------------------------------------------------------------------------- */
+
+/* Stream (a cudaStream_t) all later kernels of this context are launched on; NULL = legacy default. */
+tpcf_status tpcf_set_stream(tpcf_ctx* ctx, void* cuda_stream);
+tpcf_status tpcf_set_engine(tpcf_ctx* ctx, tpcf_engine e);
+/* Multiplies the width of the fp32 guard band around each bin edge (default 1.0).  Any value >= 1 must
+ * give identical histograms; the tests use 2.0 and 8.0 to demonstrate that the band is wide enough.
+ * scale <= 0 is TPCF_EINVAL. */
+tpcf_status tpcf_set_guard_scale(tpcf_ctx* ctx, double scale);
+/* Work partition for multi-process runs (one process per GPU): this context enumerates only the tile
+ * work items w with w % nparts == part; summing the histograms of all parts gives the full count
+ * (integer, order-independent).  Default (0, 1). */
+tpcf_status tpcf_set_partition(tpcf_ctx* ctx, int part, int nparts);
+
+typedef struct {
+    uint64_t pairs;          /* pairs enumerated by the last count (after the partition) */
+    uint64_t rechecked;      /* pairs the fast engine re-evaluated in fp64 (inside a guard band) */
+    uint64_t work_items;     /* tile work items executed */
+    int launches;            /* kernels launched by the last count */
+    int grid, block, smem_bytes;   /* geometry of the pair kernel */
+    int cells, cell_bits;    /* lookup cells of the fast engine and mantissa bits per octave */
+    int hist_copies;         /* privatised copies of each partial-histogram slot per CTA */
+    float kernel_ms;         /* device time of the last synchronous count (CUDA events) */
+} tpcf_stats;
+tpcf_status tpcf_get_stats(const tpcf_ctx* ctx, tpcf_stats* out);
+
+/* ---- host-only helpers (no GPU needed) ------------------------------------------------------------- */
+
+/* fp64 thresholds T_k = 4 sin^2(e_k/2) in squared-chord space the engines compare against (nbins+1). */
+tpcf_status tpcf_get_thresholds(const tpcf_ctx* ctx, double* t_out /* nbins+1 */);
+
+/*
+ * The fast engine's classification of one fp32 squared chord d2, evaluated on the host with the very
+ * tables the kernel uses: returns in *slot_out the result slot (0 = under, 1..nbins = bins, nbins+1 = over,
+ * nbins+2 = discarded padding lane) or -1 when d2 falls in a guard band (the kernel then re-evaluates the
+ * pair in fp64).  Lets CPU tests check the table builder against the thresholds without a GPU.
+ */
+tpcf_status tpcf_classify_fast(const tpcf_ctx* ctx, float d2, int* slot_out);
+
+/* Number of tile work items of a full count of `kind` for catalog sizes (n_d, n_r), and the number of
+ * pairs in item w: the partition arithmetic of tpcf_set_partition, testable without a GPU. */
+tpcf_status tpcf_plan(const tpcf_ctx* ctx, tpcf_kind kind, uint64_t n_d, uint64_t n_r, uint64_t* n_items_out);
+tpcf_status tpcf_plan_item_pairs(const tpcf_ctx* ctx, tpcf_kind kind, uint64_t n_d, uint64_t n_r, uint64_t w,
+                                 uint64_t* pairs_out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TPCF_H */

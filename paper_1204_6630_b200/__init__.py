@@ -1,0 +1,308 @@
+"""paper_1204_6630_b200 -- thin Python binding of libtpcf.so (include/tpcf.h).
+
+Argument marshalling only: every step of the path (RA/Dec -> unit vectors, pair distances, binning,
+histogram merge) runs in the CUDA kernels behind the C ABI; the estimator is the library's own host
+arithmetic.  The functions carry the names of the C entry points.  PyTorch is used here only for device
+memory (CUDA tensors handed in by pointer) and streams.  There is no CPU fallback: if libtpcf.so cannot be
+built or loaded this module raises, and every compute call fails with TpcfError(TPCF_ECUDA) without a GPU.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional, Tuple
+
+import numpy as np
+
+from . import build as _build
+
+TPCF_OK, TPCF_EINVAL, TPCF_ENOMEM, TPCF_ECUDA, TPCF_ESTATE = 0, 1, 2, 3, 4
+TPCF_LINEAR, TPCF_LOG, TPCF_EXPLICIT = 0, 1, 2
+TPCF_D, TPCF_R = 0, 1
+TPCF_F32, TPCF_F64 = 0, 1
+TPCF_DD, TPCF_DR, TPCF_RR = 0, 1, 2
+TPCF_ENGINE_FAST, TPCF_ENGINE_EXACT64 = 0, 1
+_STATUS = {0: "TPCF_OK", 1: "TPCF_EINVAL", 2: "TPCF_ENOMEM", 3: "TPCF_ECUDA", 4: "TPCF_ESTATE"}
+_MODES = {"linear": TPCF_LINEAR, "log": TPCF_LOG, "explicit": TPCF_EXPLICIT}
+_KINDS = {"DD": TPCF_DD, "DR": TPCF_DR, "RR": TPCF_RR}
+
+# every symbol include/tpcf.h declares (tests check that the library exports them all)
+EXPORTS = (
+    "tpcf_create", "tpcf_get_edges", "tpcf_load", "tpcf_count", "tpcf_count_async", "tpcf_estimate",
+    "tpcf_estimate_from", "tpcf_destroy", "tpcf_last_error", "tpcf_set_stream", "tpcf_set_engine",
+    "tpcf_set_guard_scale", "tpcf_set_partition", "tpcf_get_stats", "tpcf_get_thresholds", "tpcf_classify_fast",
+    "tpcf_plan", "tpcf_plan_item_pairs",
+)
+
+
+class TpcfError(RuntimeError):
+    def __init__(self, status: int, message: str):
+        super().__init__(f"{_STATUS.get(status, status)}: {message}")
+        self.status = status
+
+
+class tpcf_stats(ctypes.Structure):
+    _fields_ = [("pairs", ctypes.c_uint64), ("rechecked", ctypes.c_uint64), ("work_items", ctypes.c_uint64),
+                ("launches", ctypes.c_int), ("grid", ctypes.c_int), ("block", ctypes.c_int),
+                ("smem_bytes", ctypes.c_int), ("cells", ctypes.c_int), ("cell_bits", ctypes.c_int),
+                ("hist_copies", ctypes.c_int), ("kernel_ms", ctypes.c_float)]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_}
+
+
+_lib = None
+
+
+def lib() -> ctypes.CDLL:
+    """Load (building first if the sources are newer) the in-tree libtpcf.so.  Raises if that is impossible."""
+    global _lib
+    if _lib is None:
+        path = _build.LIB
+        if _build.stale():
+            path = _build.build()
+        L = ctypes.CDLL(path)
+        vp, i32, sz, u64, dbl = ctypes.c_void_p, ctypes.c_int, ctypes.c_size_t, ctypes.c_uint64, ctypes.c_double
+        sig = {
+            "tpcf_create": [ctypes.POINTER(vp), i32, vp, i32],
+            "tpcf_get_edges": [vp, vp],
+            "tpcf_load": [vp, i32, vp, i32, sz, i32, vp],
+            "tpcf_count": [vp, i32, vp, vp, vp, sz],
+            "tpcf_count_async": [vp, i32, vp],
+            "tpcf_estimate": [vp, vp],
+            "tpcf_estimate_from": [vp, vp, vp, i32, u64, u64, vp],
+            "tpcf_set_stream": [vp, vp],
+            "tpcf_set_engine": [vp, i32],
+            "tpcf_set_guard_scale": [vp, dbl],
+            "tpcf_set_partition": [vp, i32, i32],
+            "tpcf_get_stats": [vp, ctypes.POINTER(tpcf_stats)],
+            "tpcf_get_thresholds": [vp, vp],
+            "tpcf_classify_fast": [vp, ctypes.c_float, ctypes.POINTER(i32)],
+            "tpcf_plan": [vp, i32, u64, u64, ctypes.POINTER(u64)],
+            "tpcf_plan_item_pairs": [vp, i32, u64, u64, u64, ctypes.POINTER(u64)],
+        }
+        for name, args in sig.items():
+            fn = getattr(L, name)
+            fn.argtypes = args
+            fn.restype = i32
+        L.tpcf_destroy.argtypes = [vp]
+        L.tpcf_destroy.restype = None
+        L.tpcf_last_error.argtypes = [vp]
+        L.tpcf_last_error.restype = ctypes.c_char_p
+        _lib = L
+    return _lib
+
+
+def _check(ctx, status: int):
+    if status != TPCF_OK:
+        msg = lib().tpcf_last_error(ctx).decode() if ctx else "invalid arguments"
+        raise TpcfError(status, msg)
+
+
+def _np_ptr(a: np.ndarray):
+    return a.ctypes.data_as(ctypes.c_void_p)
+
+
+def _is_torch(x) -> bool:
+    return type(x).__module__.startswith("torch")
+
+
+# ---- the C entry points, one Python function each --------------------------------------------------------
+def tpcf_create(nbins: int, theta_deg, mode) -> ctypes.c_void_p:
+    mode = _MODES.get(mode, mode)
+    th = np.ascontiguousarray(theta_deg, dtype=np.float64)
+    need = nbins + 1 if mode == TPCF_EXPLICIT else 2
+    if th.ndim != 1 or th.shape[0] != need:
+        raise TpcfError(TPCF_EINVAL, f"theta_deg must hold {need} values")
+    ctx = ctypes.c_void_p()
+    st = lib().tpcf_create(ctypes.byref(ctx), int(nbins), _np_ptr(th), int(mode))
+    if st != TPCF_OK:
+        raise TpcfError(st, "tpcf_create rejected the binning")
+    return ctx
+
+
+def tpcf_destroy(ctx) -> None:
+    lib().tpcf_destroy(ctx)
+
+
+def tpcf_get_edges(ctx, nbins: int) -> np.ndarray:
+    e = np.empty(nbins + 1, dtype=np.float64)
+    _check(ctx, lib().tpcf_get_edges(ctx, _np_ptr(e)))
+    return e
+
+
+def tpcf_get_thresholds(ctx, nbins: int) -> np.ndarray:
+    t = np.empty(nbins + 1, dtype=np.float64)
+    _check(ctx, lib().tpcf_get_thresholds(ctx, _np_ptr(t)))
+    return t
+
+
+def tpcf_load(ctx, which: int, radec_deg, stream: int = 0) -> int:
+    """radec_deg: (n, 2) float32/float64 numpy array, CPU torch tensor (pinned or not) or CUDA torch tensor."""
+    if _is_torch(radec_deg):
+        t = radec_deg
+        if t.dim() != 2 or t.shape[1] != 2 or not t.is_contiguous():
+            raise TpcfError(TPCF_EINVAL, "catalog must be a contiguous (n, 2) tensor")
+        dt = {"torch.float32": TPCF_F32, "torch.float64": TPCF_F64}.get(str(t.dtype))
+        if dt is None:
+            raise TpcfError(TPCF_EINVAL, "catalog dtype must be float32 or float64")
+        n, ptr, on_dev = t.shape[0], ctypes.c_void_p(t.data_ptr()), int(t.is_cuda)
+        keep = t
+    else:
+        a = np.asarray(radec_deg)
+        if a.dtype not in (np.float32, np.float64):
+            raise TpcfError(TPCF_EINVAL, "catalog dtype must be float32 or float64")
+        a = np.ascontiguousarray(a)
+        if a.ndim != 2 or a.shape[1] != 2:
+            raise TpcfError(TPCF_EINVAL, "catalog must be an (n, 2) array")
+        dt = TPCF_F32 if a.dtype == np.float32 else TPCF_F64
+        n, ptr, on_dev, keep = a.shape[0], _np_ptr(a), 0, a
+    _check(ctx, lib().tpcf_load(ctx, int(which), ptr, dt, n, on_dev, ctypes.c_void_p(stream)))
+    del keep
+    return n
+
+
+def tpcf_count(ctx, kind: int, nbins: int, rows=None) -> Tuple[np.ndarray, int, int]:
+    hist = np.zeros(nbins, dtype=np.uint64)
+    uo = np.zeros(2, dtype=np.uint64)
+    if rows is None:
+        st = lib().tpcf_count(ctx, int(kind), _np_ptr(hist), _np_ptr(uo), None, 0)
+    else:
+        r = np.ascontiguousarray(rows, dtype=np.int64)
+        st = lib().tpcf_count(ctx, int(kind), _np_ptr(hist), _np_ptr(uo), _np_ptr(r), r.shape[0])
+    _check(ctx, st)
+    return hist, int(uo[0]), int(uo[1])
+
+
+def tpcf_count_async(ctx, kind: int, hist_dev_ptr: int) -> None:
+    _check(ctx, lib().tpcf_count_async(ctx, int(kind), ctypes.c_void_p(hist_dev_ptr)))
+
+
+def tpcf_estimate(ctx, nbins: int) -> np.ndarray:
+    w = np.empty(nbins, dtype=np.float64)
+    _check(ctx, lib().tpcf_estimate(ctx, _np_ptr(w)))
+    return w
+
+
+def tpcf_estimate_from(dd, dr, rr, n_d: int, n_r: int) -> np.ndarray:
+    dd = np.ascontiguousarray(dd, dtype=np.uint64)
+    dr = np.ascontiguousarray(dr, dtype=np.uint64)
+    rr = np.ascontiguousarray(rr, dtype=np.uint64)
+    w = np.empty(dd.shape[0], dtype=np.float64)
+    st = lib().tpcf_estimate_from(_np_ptr(dd), _np_ptr(dr), _np_ptr(rr), dd.shape[0], int(n_d), int(n_r), _np_ptr(w))
+    if st != TPCF_OK:
+        raise TpcfError(st, "tpcf_estimate_from: invalid arguments")
+    return w
+
+
+def tpcf_set_stream(ctx, stream: int) -> None:
+    _check(ctx, lib().tpcf_set_stream(ctx, ctypes.c_void_p(stream)))
+
+
+def tpcf_set_engine(ctx, engine: int) -> None:
+    _check(ctx, lib().tpcf_set_engine(ctx, int(engine)))
+
+
+def tpcf_set_guard_scale(ctx, scale: float) -> None:
+    _check(ctx, lib().tpcf_set_guard_scale(ctx, float(scale)))
+
+
+def tpcf_set_partition(ctx, part: int, nparts: int) -> None:
+    _check(ctx, lib().tpcf_set_partition(ctx, int(part), int(nparts)))
+
+
+def tpcf_get_stats(ctx) -> dict:
+    s = tpcf_stats()
+    _check(ctx, lib().tpcf_get_stats(ctx, ctypes.byref(s)))
+    return s.as_dict()
+
+
+def tpcf_classify_fast(ctx, d2: float) -> int:
+    out = ctypes.c_int()
+    _check(ctx, lib().tpcf_classify_fast(ctx, ctypes.c_float(d2), ctypes.byref(out)))
+    return out.value
+
+
+def tpcf_plan(ctx, kind: int, n_d: int, n_r: int) -> int:
+    out = ctypes.c_uint64()
+    _check(ctx, lib().tpcf_plan(ctx, int(kind), int(n_d), int(n_r), ctypes.byref(out)))
+    return out.value
+
+
+def tpcf_plan_item_pairs(ctx, kind: int, n_d: int, n_r: int, w: int) -> int:
+    out = ctypes.c_uint64()
+    _check(ctx, lib().tpcf_plan_item_pairs(ctx, int(kind), int(n_d), int(n_r), int(w), ctypes.byref(out)))
+    return out.value
+
+
+class Context:
+    """Owns one tpcf_ctx.  Convenience wrapper over the functions above; holds no arithmetic."""
+
+    def __init__(self, nbins: int, theta_deg, mode="explicit"):
+        self.nbins = int(nbins)
+        self._ctx = tpcf_create(nbins, theta_deg, mode)
+        self.n = {TPCF_D: 0, TPCF_R: 0}
+
+    def close(self):
+        if getattr(self, "_ctx", None):
+            tpcf_destroy(self._ctx)
+            self._ctx = None
+
+    __del__ = close
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    @property
+    def handle(self):
+        return self._ctx
+
+    def edges(self):
+        return tpcf_get_edges(self._ctx, self.nbins)
+
+    def thresholds(self):
+        return tpcf_get_thresholds(self._ctx, self.nbins)
+
+    def load(self, which, radec_deg, stream: int = 0):
+        which = {"D": TPCF_D, "R": TPCF_R}.get(which, which)
+        self.n[which] = tpcf_load(self._ctx, which, radec_deg, stream)
+
+    def count(self, kind, rows=None):
+        return tpcf_count(self._ctx, _KINDS.get(kind, kind), self.nbins, rows)
+
+    def count_async(self, kind, out):
+        """out: CUDA uint64/int64 tensor with nbins+2 elements, written {under, bins..., over} on the stream."""
+        if not (_is_torch(out) and out.is_cuda and out.is_contiguous() and out.numel() >= self.nbins + 2
+                and out.element_size() == 8):
+            raise TpcfError(TPCF_EINVAL, "out must be a contiguous CUDA 64-bit tensor of nbins+2 elements")
+        tpcf_count_async(self._ctx, _KINDS.get(kind, kind), out.data_ptr())
+
+    def estimate(self):
+        return tpcf_estimate(self._ctx, self.nbins)
+
+    def set_stream(self, stream: int):
+        tpcf_set_stream(self._ctx, stream)
+
+    def set_engine(self, engine):
+        tpcf_set_engine(self._ctx, {"fast": TPCF_ENGINE_FAST, "exact64": TPCF_ENGINE_EXACT64}.get(engine, engine))
+
+    def set_guard_scale(self, scale: float):
+        tpcf_set_guard_scale(self._ctx, scale)
+
+    def set_partition(self, part: int, nparts: int):
+        tpcf_set_partition(self._ctx, part, nparts)
+
+    def stats(self):
+        return tpcf_get_stats(self._ctx)
+
+    def classify_fast(self, d2: float):
+        return tpcf_classify_fast(self._ctx, d2)
+
+    def plan(self, kind, n_d: int, n_r: int):
+        return tpcf_plan(self._ctx, _KINDS.get(kind, kind), n_d, n_r)
+
+    def plan_item_pairs(self, kind, n_d: int, n_r: int, w: int):
+        return tpcf_plan_item_pairs(self._ctx, _KINDS.get(kind, kind), n_d, n_r, w)

@@ -1,0 +1,515 @@
+// api.cu -- the C ABI of libtpcf (include/tpcf.h): context, argument checking, device memory, launches.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/tpcf.h"
+#include "kernels.cuh"
+#include "tables.h"
+
+using namespace tpcf;
+
+namespace {
+struct Catalog {
+    uint64_t n = 0, n_pad = 0;
+    double4* x64 = nullptr;
+    float4* x32 = nullptr;
+};
+struct PlanCache {
+    bool valid = false;
+    Plan plan;
+    uint32_t* d_row_start = nullptr;
+};
+}  // namespace
+
+struct tpcf_ctx {
+    Binning bin;
+    FastTables ft;
+    double guard_scale = 1.0;
+    bool tables_dirty = true;
+    tpcf_engine engine = TPCF_ENGINE_FAST;
+    cudaStream_t stream = nullptr;
+    int part = 0, nparts = 1;
+    Catalog cat[2];
+    PlanCache plans[3];
+    // device side
+    bool cuda_ready = false;
+    int sm_count = 0;
+    float2* d_lut = nullptr;
+    uint16_t* d_slotmap = nullptr;
+    double* d_thr = nullptr;
+    unsigned long long* d_result = nullptr;     // nbins + 3
+    unsigned long long* d_counters = nullptr;   // 4
+    unsigned long long* d_out = nullptr;        // nbins + 2
+    int* d_bad = nullptr;
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    // stored full counts for tpcf_estimate
+    std::vector<uint64_t> counts[3];
+    bool have[3] = {false, false, false};
+    tpcf_stats stats{};
+    std::string err;
+};
+
+namespace {
+
+tpcf_status fail(tpcf_ctx* c, tpcf_status s, const std::string& msg) {
+    if (c) c->err = msg;
+    return s;
+}
+tpcf_status cuda_fail(tpcf_ctx* c, cudaError_t e, const char* what) {
+    return fail(c, e == cudaErrorMemoryAllocation ? TPCF_ENOMEM : TPCF_ECUDA,
+                std::string(what) + ": " + cudaGetErrorString(e));
+}
+#define CU(call, what)                                       \
+    do {                                                     \
+        cudaError_t e_ = (call);                             \
+        if (e_ != cudaSuccess) return cuda_fail(ctx, e_, what); \
+    } while (0)
+
+// No CPU fallback: without a usable GPU every compute entry point fails with TPCF_ECUDA.
+tpcf_status ensure_cuda(tpcf_ctx* ctx) {
+    if (ctx->cuda_ready) return TPCF_OK;
+    int n = 0;
+    cudaError_t e = cudaGetDeviceCount(&n);
+    if (e != cudaSuccess || n < 1) {
+        cudaGetLastError();
+        return fail(ctx, TPCF_ECUDA, std::string("no usable CUDA device: ") + (e != cudaSuccess ? cudaGetErrorString(e) : "device count is 0"));
+    }
+    int dev = 0;
+    CU(cudaGetDevice(&dev), "cudaGetDevice");
+    cudaDeviceProp prop;
+    CU(cudaGetDeviceProperties(&prop, dev), "cudaGetDeviceProperties");
+    if (prop.major < 10) return fail(ctx, TPCF_ECUDA, "libtpcf is built for sm_100a (B200) only");
+    ctx->sm_count = prop.multiProcessorCount;
+    const int nb = ctx->bin.nbins;
+    CU(cudaMalloc(&ctx->d_thr, (nb + 1) * sizeof(double)), "cudaMalloc thresholds");
+    CU(cudaMalloc(&ctx->d_result, (nb + 3) * sizeof(unsigned long long)), "cudaMalloc result");
+    CU(cudaMalloc(&ctx->d_out, (nb + 2) * sizeof(unsigned long long)), "cudaMalloc out");
+    CU(cudaMalloc(&ctx->d_counters, 4 * sizeof(unsigned long long)), "cudaMalloc counters");
+    CU(cudaMalloc(&ctx->d_bad, sizeof(int)), "cudaMalloc flag");
+    CU(cudaMemcpy(ctx->d_thr, ctx->bin.thr.data(), (nb + 1) * sizeof(double), cudaMemcpyHostToDevice), "upload thresholds");
+    CU(cudaEventCreate(&ctx->ev0), "cudaEventCreate");
+    CU(cudaEventCreate(&ctx->ev1), "cudaEventCreate");
+    ctx->cuda_ready = true;
+    return TPCF_OK;
+}
+
+void rebuild_tables(tpcf_ctx* ctx) {
+    build_fast_tables(ctx->bin, ctx->guard_scale, ctx->ft);
+    ctx->tables_dirty = true;
+}
+
+tpcf_status upload_tables(tpcf_ctx* ctx) {
+    if (!ctx->tables_dirty && ctx->d_lut) return TPCF_OK;
+    const FastTables& t = ctx->ft;
+    if (ctx->d_lut) cudaFree(ctx->d_lut);
+    if (ctx->d_slotmap) cudaFree(ctx->d_slotmap);
+    ctx->d_lut = nullptr;
+    ctx->d_slotmap = nullptr;
+    std::vector<float2> lut(t.ncells);
+    std::vector<uint16_t> sm(2 * (size_t)t.ncells);
+    for (int c = 0; c < t.ncells; ++c) {
+        lut[c] = make_float2(t.lo[c], t.hi[c]);
+        sm[2 * c] = t.slot0[c];
+        sm[2 * c + 1] = t.slot1[c];
+    }
+    CU(cudaMalloc(&ctx->d_lut, lut.size() * sizeof(float2)), "cudaMalloc lut");
+    CU(cudaMalloc(&ctx->d_slotmap, sm.size() * sizeof(uint16_t)), "cudaMalloc slotmap");
+    CU(cudaMemcpy(ctx->d_lut, lut.data(), lut.size() * sizeof(float2), cudaMemcpyHostToDevice), "upload lut");
+    CU(cudaMemcpy(ctx->d_slotmap, sm.data(), sm.size() * sizeof(uint16_t), cudaMemcpyHostToDevice), "upload slotmap");
+    ctx->tables_dirty = false;
+    return TPCF_OK;
+}
+
+void free_catalog(Catalog& c) {
+    if (c.x64) cudaFree(c.x64);
+    if (c.x32) cudaFree(c.x32);
+    c = Catalog();
+}
+
+uint64_t pad_to(uint64_t n, uint64_t m) { return (n + m - 1) / m * m; }
+
+struct Sides {
+    int ci, cj;      // catalog indices of the i-side and the j-side
+    bool tri;
+};
+Sides sides_of(tpcf_kind k) {
+    switch (k) {
+        case TPCF_DD: return {0, 0, true};
+        case TPCF_RR: return {1, 1, true};
+        default: return {0, 1, false};
+    }
+}
+
+uint32_t items_of_part(uint64_t n_items, int part, int nparts) {
+    if ((uint64_t)part >= n_items) return 0;
+    return (uint32_t)((n_items - part + nparts - 1) / nparts);
+}
+
+// Enqueue one count on ctx->stream; the nbins+2 result lands in d_out_dev.  rows_dev == nullptr: full count.
+tpcf_status enqueue_count(tpcf_ctx* ctx, tpcf_kind kind, const int64_t* rows_host, size_t nrows, unsigned long long* out_dev,
+                          double4** tmp64, float4** tmp32, int64_t** tmp_rows, uint64_t* pairs_out) {
+    tpcf_status s = ensure_cuda(ctx);
+    if (s) return s;
+    if (kind != TPCF_DD && kind != TPCF_DR && kind != TPCF_RR) return fail(ctx, TPCF_EINVAL, "unknown kind");
+    const Sides sd = sides_of(kind);
+    const Catalog& ci = ctx->cat[sd.ci];
+    const Catalog& cj = ctx->cat[sd.cj];
+    if (!ci.n || !cj.n) return fail(ctx, TPCF_ESTATE, "count before the needed catalog(s) were loaded");
+    if (ctx->engine == TPCF_ENGINE_FAST) {
+        s = upload_tables(ctx);
+        if (s) return s;
+    }
+    cudaStream_t st = ctx->stream;
+    const int nb = ctx->bin.nbins;
+
+    PairParams p{};
+    Plan subset_plan;
+    const Plan* plan = nullptr;
+    const uint32_t* d_row_start = nullptr;
+    unsigned long long self_pairs = 0;
+    if (rows_host) {
+        // row-subset mode: gather the rows into a temporary i-side catalog, count the rectangle against all j
+        if (nrows == 0) return fail(ctx, TPCF_EINVAL, "nrows == 0 with rows != NULL");
+        const uint64_t np = pad_to(nrows, kTileI);
+        CU(cudaMalloc(tmp_rows, nrows * sizeof(int64_t)), "cudaMalloc rows");
+        CU(cudaMalloc(tmp64, np * sizeof(double4)), "cudaMalloc subset");
+        CU(cudaMalloc(tmp32, np * sizeof(float4)), "cudaMalloc subset");
+        CU(cudaMemcpyAsync(*tmp_rows, rows_host, nrows * sizeof(int64_t), cudaMemcpyHostToDevice, st), "upload rows");
+        CU(cudaMemsetAsync(ctx->d_bad, 0, sizeof(int), st), "memset");
+        CU(launch_gather(ci.x64, ci.x32, *tmp_rows, nrows, np, ci.n, *tmp64, *tmp32, ctx->d_bad, st), "gather kernel");
+        int bad = 0;
+        CU(cudaMemcpyAsync(&bad, ctx->d_bad, sizeof(int), cudaMemcpyDeviceToHost, st), "read flag");
+        CU(cudaStreamSynchronize(st), "gather");
+        if (bad) return fail(ctx, TPCF_EINVAL, "row index out of range");
+        make_plan(false, nrows, cj.n, subset_plan);
+        plan = &subset_plan;
+        p.xi = *tmp32;
+        p.xi64 = *tmp64;
+        p.n_i = (uint32_t)nrows;
+        p.tri = 0;
+        if (sd.tri) self_pairs = nrows;      // each listed row meets itself once at theta = 0: remove it
+        ctx->stats.launches = 1;
+    } else {
+        PlanCache& pc = ctx->plans[kind];
+        if (!pc.valid) {
+            make_plan(sd.tri, ci.n, cj.n, pc.plan);
+            if (pc.d_row_start) cudaFree(pc.d_row_start);
+            pc.d_row_start = nullptr;
+            if (sd.tri) {
+                CU(cudaMalloc(&pc.d_row_start, pc.plan.row_start.size() * sizeof(uint32_t)), "cudaMalloc plan");
+                CU(cudaMemcpy(pc.d_row_start, pc.plan.row_start.data(), pc.plan.row_start.size() * sizeof(uint32_t),
+                              cudaMemcpyHostToDevice), "upload plan");
+            }
+            pc.valid = true;
+        }
+        plan = &pc.plan;
+        d_row_start = pc.d_row_start;
+        p.xi = ci.x32;
+        p.xi64 = ci.x64;
+        p.n_i = (uint32_t)ci.n;
+        p.tri = sd.tri ? 1 : 0;
+        ctx->stats.launches = 0;
+    }
+    p.xj = cj.x32;
+    p.xj64 = cj.x64;
+    p.n_j = (uint32_t)cj.n;
+    p.blocks_i = plan->blocks_i;
+    p.tiles_j = plan->tiles_j;
+    p.chunk = plan->chunk;
+    if (plan->n_items > 0xFFFFFFFFull) return fail(ctx, TPCF_EINVAL, "catalogs too large for the 32-bit work-item index");
+    p.n_items_part = items_of_part(plan->n_items, ctx->part, ctx->nparts);
+    p.row_start = d_row_start;
+    p.part = (uint32_t)ctx->part;
+    p.nparts = (uint32_t)ctx->nparts;
+    p.lut = ctx->d_lut;
+    p.slotmap = ctx->d_slotmap;
+    p.ncells = ctx->ft.ncells;
+    p.shift = ctx->ft.shift;
+    p.sqrt_scale = ctx->ft.sqrt_scale;
+    p.sqrt_clamp = ctx->ft.sqrt_clamp;
+    p.thr = ctx->d_thr;
+    p.nbins = nb;
+    p.result = ctx->d_result;
+    p.counters = ctx->d_counters;
+
+    CU(cudaMemsetAsync(ctx->d_result, 0, (nb + 3) * sizeof(unsigned long long), st), "memset result");
+    CU(cudaMemsetAsync(ctx->d_counters, 0, 4 * sizeof(unsigned long long), st), "memset counters");
+    LaunchInfo li{};
+    if (ctx->engine == TPCF_ENGINE_FAST)
+        CU(launch_pairs_fast(p, ctx->ft.map, ctx->sm_count, st, &li), "pair_fast_kernel launch");
+    else
+        CU(launch_pairs_exact64(p, ctx->sm_count, st, &li), "pair_exact64_kernel launch");
+    const int zero_slot = (ctx->bin.thr[0] > 0.0) ? 0 : 1;
+    CU(launch_finalize(ctx->d_result, nb, zero_slot, self_pairs, out_dev, st), "finalize launch");
+    ctx->stats.launches += 2;
+    ctx->stats.grid = li.grid;
+    ctx->stats.block = li.block;
+    ctx->stats.smem_bytes = li.smem_bytes;
+    ctx->stats.cells = ctx->ft.ncells;
+    ctx->stats.cell_bits = (ctx->ft.map == CellMap::LogBits) ? 23 - ctx->ft.shift : -1;
+    ctx->stats.hist_copies = 1;
+    if (pairs_out) {
+        uint64_t pairs = 0;
+        if (ctx->nparts == 1) {
+            pairs = plan->tri ? plan->n_i * (plan->n_i - 1) / 2 : plan->n_i * plan->n_j;
+        } else {
+            for (uint64_t w = ctx->part; w < plan->n_items; w += ctx->nparts) pairs += plan->item_pairs(w);
+        }
+        *pairs_out = pairs - self_pairs;
+    }
+    return TPCF_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+tpcf_status tpcf_create(tpcf_ctx** out, int nbins, const double* theta_deg, tpcf_binning mode) {
+    if (!out) return TPCF_EINVAL;
+    *out = nullptr;
+    tpcf_ctx* ctx = new (std::nothrow) tpcf_ctx();
+    if (!ctx) return TPCF_ENOMEM;
+    std::string why;
+    try {
+        why = make_binning(nbins, theta_deg, (int)mode, ctx->bin);
+        if (why.empty()) rebuild_tables(ctx);
+    } catch (const std::bad_alloc&) {
+        delete ctx;
+        return TPCF_ENOMEM;
+    }
+    if (!why.empty()) {
+        delete ctx;
+        return TPCF_EINVAL;
+    }
+    *out = ctx;
+    return TPCF_OK;
+}
+
+tpcf_status tpcf_get_edges(const tpcf_ctx* ctx, double* edges_out) {
+    if (!ctx || !edges_out) return TPCF_EINVAL;
+    std::memcpy(edges_out, ctx->bin.edges.data(), ctx->bin.edges.size() * sizeof(double));
+    return TPCF_OK;
+}
+
+tpcf_status tpcf_get_thresholds(const tpcf_ctx* ctx, double* t_out) {
+    if (!ctx || !t_out) return TPCF_EINVAL;
+    std::memcpy(t_out, ctx->bin.thr.data(), ctx->bin.thr.size() * sizeof(double));
+    return TPCF_OK;
+}
+
+tpcf_status tpcf_load(tpcf_ctx* ctx, tpcf_cat which, const void* radec_deg, tpcf_dtype dt, size_t n, int on_device,
+                      void* cuda_stream) {
+    if (!ctx) return TPCF_EINVAL;
+    if (which != TPCF_D && which != TPCF_R) return fail(ctx, TPCF_EINVAL, "which must be TPCF_D or TPCF_R");
+    if (dt != TPCF_F32 && dt != TPCF_F64) return fail(ctx, TPCF_EINVAL, "dtype must be TPCF_F32 or TPCF_F64");
+    if (!radec_deg || n == 0) return fail(ctx, TPCF_EINVAL, "empty catalog");
+    if (n > 0x7FFFFFFFull) return fail(ctx, TPCF_EINVAL, "more than 2^31-1 rows");
+    tpcf_status s = ensure_cuda(ctx);
+    if (s) return s;
+    cudaStream_t st = cuda_stream ? static_cast<cudaStream_t>(cuda_stream) : ctx->stream;
+    Catalog& c = ctx->cat[which];
+    free_catalog(c);
+    for (int k = 0; k < 3; ++k) {           // DR depends on both catalogs
+        const Sides sd = sides_of((tpcf_kind)k);
+        if (sd.ci == (int)which || sd.cj == (int)which) {
+            ctx->have[k] = false;
+            ctx->plans[k].valid = false;
+        }
+    }
+    const uint64_t n_pad = pad_to(n, kTileI);
+    const size_t esz = (dt == TPCF_F64) ? 8 : 4;
+    CU(cudaMalloc(&c.x64, n_pad * sizeof(double4)), "cudaMalloc catalog (fp64)");
+    CU(cudaMalloc(&c.x32, n_pad * sizeof(float4)), "cudaMalloc catalog (fp32)");
+    void* staged = nullptr;
+    const void* src = radec_deg;
+    if (!on_device) {
+        CU(cudaMalloc(&staged, n * 2 * esz), "cudaMalloc staging");
+        cudaError_t e = cudaMemcpyAsync(staged, radec_deg, n * 2 * esz, cudaMemcpyHostToDevice, st);
+        if (e != cudaSuccess) {
+            cudaFree(staged);
+            return cuda_fail(ctx, e, "copy catalog to device");
+        }
+        src = staged;
+    }
+    cudaError_t e = cudaMemsetAsync(ctx->d_bad, 0, sizeof(int), st);
+    if (e == cudaSuccess) e = launch_convert(src, dt == TPCF_F64, n, n_pad, c.x64, c.x32, ctx->d_bad, st);
+    int bad = 0;
+    if (e == cudaSuccess) e = cudaMemcpyAsync(&bad, ctx->d_bad, sizeof(int), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (staged) cudaFree(staged);
+    if (e != cudaSuccess) {
+        free_catalog(c);
+        return cuda_fail(ctx, e, "convert catalog");
+    }
+    if (bad) {
+        free_catalog(c);
+        return fail(ctx, TPCF_EINVAL, "catalog has a non-finite value or |Dec| > 90");
+    }
+    c.n = n;
+    c.n_pad = n_pad;
+    return TPCF_OK;
+}
+
+tpcf_status tpcf_count(tpcf_ctx* ctx, tpcf_kind kind, uint64_t* hist_out, uint64_t* under_over_out, const int64_t* rows,
+                       size_t nrows) {
+    if (!ctx) return TPCF_EINVAL;
+    if (!hist_out) return fail(ctx, TPCF_EINVAL, "hist_out is NULL");
+    if (!rows && nrows) return fail(ctx, TPCF_EINVAL, "nrows != 0 with rows == NULL");
+    tpcf_status s = ensure_cuda(ctx);
+    if (s) return s;
+    double4* tmp64 = nullptr;
+    float4* tmp32 = nullptr;
+    int64_t* tmp_rows = nullptr;
+    uint64_t pairs = 0;
+    cudaStream_t st = ctx->stream;
+    const int nb = ctx->bin.nbins;
+    std::vector<unsigned long long> host(nb + 2), ctr(4);
+    cudaError_t e = cudaEventRecord(ctx->ev0, st);
+    s = (e == cudaSuccess) ? enqueue_count(ctx, kind, rows, nrows, ctx->d_out, &tmp64, &tmp32, &tmp_rows, &pairs)
+                           : cuda_fail(ctx, e, "cudaEventRecord");
+    if (s == TPCF_OK) {
+        e = cudaEventRecord(ctx->ev1, st);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(host.data(), ctx->d_out, (nb + 2) * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(ctr.data(), ctx->d_counters, 4 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess) s = cuda_fail(ctx, e, "pair count");
+    }
+    if (tmp64) cudaFree(tmp64);
+    if (tmp32) cudaFree(tmp32);
+    if (tmp_rows) cudaFree(tmp_rows);
+    if (s) return s;
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, ctx->ev0, ctx->ev1);
+    ctx->stats.kernel_ms = ms;
+    ctx->stats.pairs = pairs;
+    ctx->stats.rechecked = ctr[1];
+    ctx->stats.work_items = ctr[2];
+    for (int k = 0; k < nb; ++k) hist_out[k] = host[k + 1];
+    if (under_over_out) {
+        under_over_out[0] = host[0];
+        under_over_out[1] = host[nb + 1];
+    }
+    if (!rows && ctx->nparts == 1) {
+        ctx->counts[kind].assign(hist_out, hist_out + nb);
+        ctx->have[kind] = true;
+    }
+    return TPCF_OK;
+}
+
+tpcf_status tpcf_count_async(tpcf_ctx* ctx, tpcf_kind kind, uint64_t* hist_dev) {
+    if (!ctx) return TPCF_EINVAL;
+    if (!hist_dev) return fail(ctx, TPCF_EINVAL, "hist_dev is NULL");
+    return enqueue_count(ctx, kind, nullptr, 0, reinterpret_cast<unsigned long long*>(hist_dev), nullptr, nullptr, nullptr,
+                         nullptr);
+}
+
+tpcf_status tpcf_estimate_from(const uint64_t* dd, const uint64_t* dr, const uint64_t* rr, int nbins, uint64_t n_d,
+                               uint64_t n_r, double* w_out) {
+    if (!dd || !dr || !rr || !w_out || nbins < 1) return TPCF_EINVAL;
+    estimate(dd, dr, rr, nbins, n_d, n_r, w_out);
+    return TPCF_OK;
+}
+
+tpcf_status tpcf_estimate(tpcf_ctx* ctx, double* w_out) {
+    if (!ctx) return TPCF_EINVAL;
+    if (!w_out) return fail(ctx, TPCF_EINVAL, "w_out is NULL");
+    if (!ctx->have[TPCF_DD] || !ctx->have[TPCF_DR] || !ctx->have[TPCF_RR])
+        return fail(ctx, TPCF_ESTATE, "estimate needs full DD, DR and RR counts on the current catalogs");
+    estimate(ctx->counts[TPCF_DD].data(), ctx->counts[TPCF_DR].data(), ctx->counts[TPCF_RR].data(), ctx->bin.nbins,
+             ctx->cat[0].n, ctx->cat[1].n, w_out);
+    return TPCF_OK;
+}
+
+void tpcf_destroy(tpcf_ctx* ctx) {
+    if (!ctx) return;
+    if (ctx->cuda_ready) {
+        free_catalog(ctx->cat[0]);
+        free_catalog(ctx->cat[1]);
+        for (auto& pc : ctx->plans)
+            if (pc.d_row_start) cudaFree(pc.d_row_start);
+        cudaFree(ctx->d_lut);
+        cudaFree(ctx->d_slotmap);
+        cudaFree(ctx->d_thr);
+        cudaFree(ctx->d_result);
+        cudaFree(ctx->d_out);
+        cudaFree(ctx->d_counters);
+        cudaFree(ctx->d_bad);
+        if (ctx->ev0) cudaEventDestroy(ctx->ev0);
+        if (ctx->ev1) cudaEventDestroy(ctx->ev1);
+    }
+    delete ctx;
+}
+
+const char* tpcf_last_error(const tpcf_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+
+tpcf_status tpcf_set_stream(tpcf_ctx* ctx, void* cuda_stream) {
+    if (!ctx) return TPCF_EINVAL;
+    ctx->stream = static_cast<cudaStream_t>(cuda_stream);
+    return TPCF_OK;
+}
+
+tpcf_status tpcf_set_engine(tpcf_ctx* ctx, tpcf_engine e) {
+    if (!ctx) return TPCF_EINVAL;
+    if (e != TPCF_ENGINE_FAST && e != TPCF_ENGINE_EXACT64) return fail(ctx, TPCF_EINVAL, "unknown engine");
+    ctx->engine = e;
+    return TPCF_OK;
+}
+
+tpcf_status tpcf_set_guard_scale(tpcf_ctx* ctx, double scale) {
+    if (!ctx) return TPCF_EINVAL;
+    if (!(scale > 0.0) || !(scale <= 1.0e6)) return fail(ctx, TPCF_EINVAL, "guard scale must be in (0, 1e6]");
+    ctx->guard_scale = scale;
+    rebuild_tables(ctx);
+    return TPCF_OK;
+}
+
+tpcf_status tpcf_set_partition(tpcf_ctx* ctx, int part, int nparts) {
+    if (!ctx) return TPCF_EINVAL;
+    if (nparts < 1 || part < 0 || part >= nparts) return fail(ctx, TPCF_EINVAL, "need 0 <= part < nparts");
+    ctx->part = part;
+    ctx->nparts = nparts;
+    return TPCF_OK;
+}
+
+tpcf_status tpcf_get_stats(const tpcf_ctx* ctx, tpcf_stats* out) {
+    if (!ctx || !out) return TPCF_EINVAL;
+    *out = ctx->stats;
+    out->cells = ctx->ft.ncells;
+    out->cell_bits = (ctx->ft.map == CellMap::LogBits) ? 23 - ctx->ft.shift : -1;
+    return TPCF_OK;
+}
+
+tpcf_status tpcf_classify_fast(const tpcf_ctx* ctx, float d2, int* slot_out) {
+    if (!ctx || !slot_out) return TPCF_EINVAL;
+    if (!(d2 >= 0.0f) || !(d2 < 64.0f)) return TPCF_EINVAL;
+    *slot_out = ctx->ft.classify(d2);
+    return TPCF_OK;
+}
+
+tpcf_status tpcf_plan(const tpcf_ctx* ctx, tpcf_kind kind, uint64_t n_d, uint64_t n_r, uint64_t* n_items_out) {
+    if (!ctx || !n_items_out || n_d == 0 || n_r == 0) return TPCF_EINVAL;
+    Plan p;
+    const Sides sd = sides_of(kind);
+    make_plan(sd.tri, sd.ci == 0 ? n_d : n_r, sd.cj == 0 ? n_d : n_r, p);
+    *n_items_out = p.n_items;
+    return TPCF_OK;
+}
+
+tpcf_status tpcf_plan_item_pairs(const tpcf_ctx* ctx, tpcf_kind kind, uint64_t n_d, uint64_t n_r, uint64_t w,
+                                 uint64_t* pairs_out) {
+    if (!ctx || !pairs_out || n_d == 0 || n_r == 0) return TPCF_EINVAL;
+    Plan p;
+    const Sides sd = sides_of(kind);
+    make_plan(sd.tri, sd.ci == 0 ? n_d : n_r, sd.cj == 0 ? n_d : n_r, p);
+    if (w >= p.n_items) return TPCF_EINVAL;
+    *pairs_out = p.item_pairs(w);
+    return TPCF_OK;
+}
+
+}  // extern "C"

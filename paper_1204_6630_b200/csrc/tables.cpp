@@ -1,0 +1,299 @@
+// tables.cpp -- host-side logic of libtpcf (no CUDA calls): binning, thresholds, guard bands, cell lookup
+// table, work plan, estimator.  DESIGN.md sections 3-5 derive everything here.
+#include "tables.h"
+
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <limits>
+
+namespace tpcf {
+
+static const double kPi = 3.14159265358979323846;
+
+static inline uint32_t f2u(float f) { uint32_t u; std::memcpy(&u, &f, 4); return u; }
+static inline float u2f(uint32_t u) { float f; std::memcpy(&f, &u, 4); return f; }
+static float float_down(double x) {
+    float f = (float)x;
+    if ((double)f > x) f = std::nextafterf(f, -std::numeric_limits<float>::infinity());
+    return f;
+}
+static float float_up(double x) {
+    float f = (float)x;
+    if ((double)f < x) f = std::nextafterf(f, std::numeric_limits<float>::infinity());
+    return f;
+}
+
+// --------------------------------------------------------------------------------------------------
+// Binning.  The paper fixes no bins (reading A4); edges in degrees, chord-space thresholds
+// T_k = |a-b|^2 at separation e_k = 2 - 2 cos(e_k) = 4 sin^2(e_k/2): a monotone function of the dot
+// product of PAPER.md:37, so comparing against T_k is "binning in cos(theta) space" without an acos and
+// without the cancellation of 1 - cos at small angles.
+// --------------------------------------------------------------------------------------------------
+std::string make_binning(int nbins, const double* theta, int mode, Binning& out) {
+    if (nbins < 1 || nbins > 4096) return "nbins must be in [1, 4096]";
+    if (!theta) return "theta_deg is NULL";
+    std::vector<double> e((size_t)nbins + 1);
+    if (mode == 0 || mode == 1) {
+        double lo = theta[0], hi = theta[1];
+        if (!(lo == lo) || !(hi == hi)) return "NaN edge";
+        if (!(lo >= 0.0 && hi <= 180.0 && lo < hi)) return "need 0 <= min < max <= 180";
+        if (mode == 1 && !(lo > 0.0)) return "LOG binning needs min > 0";
+        for (int k = 0; k <= nbins; ++k)
+            e[k] = (mode == 0) ? lo + k * ((hi - lo) / nbins) : lo * std::pow(hi / lo, (double)k / nbins);
+        e[0] = lo;
+        e[nbins] = hi;
+    } else if (mode == 2) {
+        for (int k = 0; k <= nbins; ++k) {
+            if (!(theta[k] == theta[k])) return "NaN edge";
+            e[k] = theta[k];
+        }
+    } else {
+        return "unknown binning mode";
+    }
+    if (!(e[0] >= 0.0 && e[nbins] <= 180.0)) return "edges must lie in [0, 180]";
+    for (int k = 0; k < nbins; ++k)
+        if (!(e[k] < e[k + 1])) return "edges must be strictly increasing";
+    out.nbins = nbins;
+    out.edges = e;
+    out.thr.resize((size_t)nbins + 1);
+    for (int k = 0; k <= nbins; ++k) {
+        double s = std::sin(e[k] * kPi / 360.0);
+        out.thr[k] = 4.0 * s * s;
+    }
+    out.drop_first = (e[0] == 0.0);
+    out.drop_last = (e[nbins] == 180.0);
+    if (out.drop_first) out.thr[0] = 0.0;
+    if (out.drop_last) out.thr[nbins] = 4.0;
+    for (int k = 0; k < nbins; ++k)
+        if (!(out.thr[k] < out.thr[k + 1])) return "edges closer than fp64 can separate in chord space";
+    return "";
+}
+
+int exact_slot(double d2, const Binning& b) {
+    const int n = b.nbins;
+    if (d2 > 4.0) d2 = 4.0;                 // the oracle clamps the dot product to [-1, 1] (reading A7)
+    if (d2 < b.thr[0]) return 0;
+    if (d2 > b.thr[n]) return n + 1;
+    int lo = 0, hi = n;                     // thr[lo] <= d2, (hi == n or d2 < thr[hi])
+    while (hi - lo > 1) {
+        int mid = (lo + hi) >> 1;
+        if (b.thr[mid] <= d2) lo = mid; else hi = mid;
+    }
+    return lo + 1;
+}
+
+// |d2_fp32 - d2| <= 2.07e-7 sqrt(d2) + 3.0e-7 d2 + 1.1e-14; the constants below add margin.
+double guard_width(double t, double scale) { return scale * (2.5e-7 * std::sqrt(t) + 5.0e-7 * t + 1.0e-13); }
+
+// --------------------------------------------------------------------------------------------------
+// Cell maps.  Both are integer/IEEE arithmetic on the float's bit pattern, reproduced exactly on the device.
+// --------------------------------------------------------------------------------------------------
+static const uint32_t kSqrtMagic = 0x1FBD1DF5u;   // bits(sqrt(x)) ~ (bits(x) >> 1) + magic (within ~4 %)
+static const uint32_t kTopBits = 0x42800000u;     // bits(64.0f): no squared chord, padded or not, reaches it
+
+int FastTables::cell_of(float d2) const {
+    if (map == CellMap::LogBits) return (int)(f2u(d2) >> shift);
+    float c = std::fmin(d2, sqrt_clamp);
+    float key = u2f((f2u(c) >> 1) + kSqrtMagic);
+    float t = std::fmaf(key, sqrt_scale, 8388608.0f);
+    return (int)(f2u(t) & 0x7FFFFFu);
+}
+
+int FastTables::classify(float d2) const {
+    int c = cell_of(d2);
+    if (c < 0 || c >= ncells) return -2;
+    bool p0 = d2 >= lo[c];
+    if (p0 && d2 < hi[c]) return -1;
+    return p0 ? slot1[c] : slot0[c];
+}
+
+namespace {
+struct Band {
+    float lo, hi;
+    int below, above;
+};
+
+// first float (as bits) whose cell index is >= c; cell_of is monotone non-decreasing in d2 >= 0
+uint32_t first_bits_of_cell(const FastTables& t, int c) {
+    uint32_t a = 0, b = kTopBits;           // answer in [a, b]
+    if (t.cell_of(u2f(b)) < c) return b + 1;
+    while (a < b) {
+        uint32_t m = a + (b - a) / 2;
+        if (t.cell_of(u2f(m)) >= c) b = m; else a = m + 1;
+    }
+    return a;
+}
+
+// Fill lo/hi/slot tables for the current map; returns the number of cells that see more than one band.
+int fill(FastTables& t, const std::vector<Band>& bands, int lowest_slot) {
+    const float inf = std::numeric_limits<float>::infinity();
+    t.ncells = t.cell_of(u2f(kTopBits)) + 1;
+    t.lo.assign(t.ncells, inf);
+    t.hi.assign(t.ncells, inf);
+    t.slot0.assign(t.ncells, 0);
+    t.slot1.assign(t.ncells, 0);
+    int bad = 0;
+    size_t first = 0;                       // first band with hi > start of this cell
+    for (int c = 0; c < t.ncells; ++c) {
+        uint32_t b0 = first_bits_of_cell(t, c), b1 = first_bits_of_cell(t, c + 1);
+        if (b1 == b0) {                     // empty cell (SqrtLin can skip indices): never addressed
+            t.slot0[c] = t.slot1[c] = (uint16_t)lowest_slot;
+            continue;
+        }
+        float f0 = (c == 0) ? 0.0f : u2f(b0);
+        float f1 = (b1 > kTopBits) ? inf : u2f(b1);
+        while (first < bands.size() && bands[first].hi <= f0) ++first;   // bands wholly below this cell
+        // bands [first, last) intersect [f0, f1)
+        size_t last = first;
+        while (last < bands.size() && bands[last].lo < f1) ++last;
+        int region = (first == 0) ? lowest_slot : bands[first - 1].above;
+        if (last == first) {
+            t.slot0[c] = t.slot1[c] = (uint16_t)region;
+        } else {
+            // More than one band in a cell: everything from the first band's lo to the last band's hi is
+            // treated as ambiguous (classified by the fp64 path), which is always correct, only slower.
+            if (last - first > 1) ++bad;
+            t.lo[c] = bands[first].lo;
+            t.hi[c] = bands[last - 1].hi;
+            t.slot0[c] = (uint16_t)bands[first].below;
+            t.slot1[c] = (uint16_t)bands[last - 1].above;
+        }
+    }
+    return bad;
+}
+}  // namespace
+
+void build_fast_tables(const Binning& b, double gs, FastTables& out) {
+    const int n = b.nbins;
+    int overlapping = 0;
+    std::vector<Band> bands;
+    for (int k = 0; k <= n; ++k) {
+        if ((k == 0 && b.drop_first) || (k == n && b.drop_last)) continue;
+        double T = b.thr[k], g = guard_width(T, gs);
+        Band bd;
+        bd.lo = (T - g <= 0.0 || T < 1e-12) ? 0.0f : float_down(T - g);
+        bd.hi = float_up(T + g);
+        bd.below = k;
+        bd.above = k + 1;
+        if (!bands.empty() && bd.lo < bands.back().hi) {      // overlapping guard bands: one wider ambiguous band
+            bands.back().hi = std::max(bands.back().hi, bd.hi);
+            bands.back().above = bd.above;
+            ++overlapping;
+        } else {
+            bands.push_back(bd);
+        }
+    }
+    const int lowest = b.drop_first ? 1 : 0;
+    {   // everything at or above kDiscardFrom involves a padding row: zero-width band, never ambiguous
+        Band d;
+        d.lo = d.hi = kDiscardFrom;
+        d.below = bands.empty() ? lowest : bands.back().above;
+        d.above = n + 2;
+        if (!bands.empty() && bands.back().hi > kDiscardFrom) bands.back().hi = kDiscardFrom;
+        bands.push_back(d);
+    }
+
+    // 1. LogBits with 2, 4, ... cells per octave
+    FastTables t;
+    t.merged_bands = overlapping;
+    for (int shift = 22; shift >= 19; --shift) {
+        t.map = CellMap::LogBits;
+        t.shift = shift;
+        if ((int)(kTopBits >> shift) + 1 > kMaxCells) break;
+        if (fill(t, bands, lowest) == 0) { out = t; return; }
+    }
+    // 2. SqrtLin (bins of near-constant width in theta)
+    {
+        double top = 0.0;
+        for (size_t m = 0; m + 1 < bands.size(); ++m) top = std::max(top, (double)bands[m].hi);
+        float clamp = std::min(kDiscardFrom * 0.999f, (float)(top * 1.25 + 1e-9));
+        float keymax = u2f((f2u(clamp) >> 1) + kSqrtMagic);
+        for (int target = 512; target <= kMaxCells; target *= 2) {
+            t.map = CellMap::SqrtLin;
+            t.sqrt_clamp = clamp;
+            t.sqrt_scale = (float)((target - 2) / (double)keymax);
+            if (fill(t, bands, lowest) == 0 && t.ncells <= kMaxCells) { out = t; return; }
+        }
+    }
+    // 3. Fallback, always correct: finest LogBits map; a cell that sees several guard bands treats the whole
+    //    span between them as ambiguous, so those pairs are classified by the fp64 path.
+    t.map = CellMap::LogBits;
+    t.shift = 19;
+    t.merged_bands += fill(t, bands, lowest);
+    out = t;
+}
+
+// --------------------------------------------------------------------------------------------------
+// Work plan: the N_D x N_R rectangle (DR) or the i<j triangle (DD, RR) cut into items of one 1024-row
+// i-block times up to `chunk` 1024-column j-tiles (north_star "triangular tiles").
+// --------------------------------------------------------------------------------------------------
+void make_plan(bool tri, uint64_t n_i, uint64_t n_j, Plan& p) {
+    p = Plan();
+    p.tri = tri;
+    p.n_i = n_i;
+    p.n_j = tri ? n_i : n_j;
+    p.blocks_i = (uint32_t)((n_i + kTileI - 1) / kTileI);
+    p.tiles_j = (uint32_t)((p.n_j + kTileJ - 1) / kTileJ);
+    uint64_t tiles = tri ? (uint64_t)p.blocks_i * (p.blocks_i + 1) / 2 : (uint64_t)p.blocks_i * p.tiles_j;
+    uint64_t c = tiles / (40ull * kPlanSMs);
+    p.chunk = (uint32_t)std::min<uint64_t>(std::max<uint64_t>(c, 1), kMaxChunk);
+    if (tri) {
+        p.row_start.resize((size_t)p.blocks_i + 1);
+        uint64_t acc = 0;
+        for (uint32_t I = 0; I < p.blocks_i; ++I) {
+            p.row_start[I] = (uint32_t)acc;
+            acc += (p.tiles_j - I + p.chunk - 1) / p.chunk;
+        }
+        p.row_start[p.blocks_i] = (uint32_t)acc;
+        p.n_items = acc;
+    } else {
+        p.n_items = (uint64_t)p.blocks_i * ((p.tiles_j + p.chunk - 1) / p.chunk);
+    }
+}
+
+void Plan::item(uint64_t w, uint32_t& I, uint32_t& tile0, uint32_t& ntiles) const {
+    if (tri) {
+        uint32_t lo = 0, hi = blocks_i;     // row_start[lo] <= w < row_start[hi]
+        while (hi - lo > 1) {
+            uint32_t mid = (lo + hi) >> 1;
+            if (row_start[mid] <= w) lo = mid; else hi = mid;
+        }
+        I = lo;
+        uint32_t c = (uint32_t)(w - row_start[lo]);
+        tile0 = I + c * chunk;
+        ntiles = std::min(chunk, tiles_j - tile0);
+    } else {
+        uint32_t per_row = (tiles_j + chunk - 1) / chunk;
+        I = (uint32_t)(w / per_row);
+        uint32_t c = (uint32_t)(w % per_row);
+        tile0 = c * chunk;
+        ntiles = std::min(chunk, tiles_j - tile0);
+    }
+}
+
+uint64_t Plan::item_pairs(uint64_t w) const {
+    uint32_t I, t0, nt;
+    item(w, I, t0, nt);
+    uint64_t rows = std::min<uint64_t>(kTileI, n_i - (uint64_t)I * kTileI), total = 0;
+    for (uint32_t t = t0; t < t0 + nt; ++t) {
+        uint64_t cols = std::min<uint64_t>(kTileJ, n_j - (uint64_t)t * kTileJ);
+        total += (tri && t == I) ? rows * (rows - 1) / 2 : rows * cols;
+    }
+    return total;
+}
+
+// PAPER.md:20-25 Eq. 1 in the pair-count-normalised reading A1 (BASELINE.json north_star).
+void estimate(const uint64_t* dd, const uint64_t* dr, const uint64_t* rr, int nbins, uint64_t n_d, uint64_t n_r,
+              double* w) {
+    const double ndd = 0.5 * (double)n_d * ((double)n_d - 1.0);
+    const double ndr = (double)n_d * (double)n_r;
+    const double nrr = 0.5 * (double)n_r * ((double)n_r - 1.0);
+    for (int k = 0; k < nbins; ++k) {
+        if (rr[k] == 0) { w[k] = std::numeric_limits<double>::quiet_NaN(); continue; }
+        const double frr = (double)rr[k] / nrr;
+        w[k] = ((double)dd[k] / ndd - 2.0 * ((double)dr[k] / ndr) + frr) / frr;
+    }
+}
+
+}  // namespace tpcf

@@ -1,0 +1,72 @@
+// tables.h -- host-side (no CUDA) logic of libtpcf: theta edges, chord-space thresholds, the fast engine's
+// guard bands and cell lookup table, the tile work plan and the estimator.  See DESIGN.md sections 3-5.
+#pragma once
+#include <cstdint>
+#include <string>
+#include <vector>
+
+namespace tpcf {
+
+// Geometry shared by the host plan and the kernels.
+constexpr int kThreads = 256;          // threads per CTA
+constexpr int kIPerThread = 4;         // i-points held in registers per thread
+constexpr int kTileI = kThreads * kIPerThread;   // 1024 i-points per CTA work item
+constexpr int kTileJ = 1024;           // j-points per shared-memory tile (16 KB of float4)
+constexpr int kMaxChunk = 8;           // j-tiles per work item, at most
+constexpr int kPlanSMs = 148;          // B200 SM count the plan balances for
+constexpr float kPadCoord = 2.0f;      // padding rows are (2,2,2): 6.07 <= d2 <= 19.9 against any unit vector
+constexpr float kDiscardFrom = 5.0f;   // d2 >= 5 can only involve a padding row
+constexpr int kMaxCells = 8192;
+
+enum class CellMap : int { LogBits = 0, SqrtLin = 1 };
+
+// Result-slot numbering used everywhere: 0 = under, 1..nbins = bins, nbins+1 = over, nbins+2 = discard.
+struct FastTables {
+    CellMap map = CellMap::LogBits;
+    int shift = 21;                 // LogBits: cell = bits(d2) >> shift
+    float sqrt_scale = 0.f;         // SqrtLin: cell = low 23 bits of fmaf(approx_sqrt(min(d2, sqrt_clamp)), sqrt_scale, 2^23)
+    float sqrt_clamp = 0.f;
+    int ncells = 0;
+    int merged_bands = 0;           // guard bands that had to be merged because they shared a cell (0 normally)
+    std::vector<float> lo, hi;      // per cell: below lo -> slot0, [lo, hi) -> ambiguous, >= hi -> slot1
+    std::vector<uint16_t> slot0, slot1;
+    int cell_of(float d2) const;    // exactly the kernel's integer arithmetic
+    int classify(float d2) const;   // result slot, or -1 when ambiguous
+};
+
+struct Binning {
+    int nbins = 0;
+    std::vector<double> edges;      // degrees, nbins+1
+    std::vector<double> thr;        // T_k = 4 sin^2(e_k/2), nbins+1
+    bool drop_first = false;        // e_0 == 0: nothing can be "under"
+    bool drop_last = false;         // e_n == 180: nothing can be "over"
+};
+
+// Returns "" on success, else the reason (-> TPCF_EINVAL).
+std::string make_binning(int nbins, const double* theta_deg, int mode, Binning& out);
+
+// fp32 rounding bound of the fast engine's squared chord around the true value t.
+double guard_width(double t, double scale);
+
+void build_fast_tables(const Binning& b, double guard_scale, FastTables& out);
+
+// Exact classification used by the fp64 engine and the recheck path (host mirror of the device code).
+int exact_slot(double d2, const Binning& b);
+
+// ---- tile work plan --------------------------------------------------------------------------------
+struct Plan {
+    bool tri = false;               // true: one catalog, pairs i<j; false: rectangle n_i x n_j
+    uint64_t n_i = 0, n_j = 0;
+    uint32_t blocks_i = 0, tiles_j = 0, chunk = 1;
+    uint64_t n_items = 0;
+    std::vector<uint32_t> row_start;   // tri only: first item of i-block I (blocks_i + 1 entries)
+    // item w -> i-block, first j-tile, number of j-tiles
+    void item(uint64_t w, uint32_t& I, uint32_t& tile0, uint32_t& ntiles) const;
+    uint64_t item_pairs(uint64_t w) const;
+};
+void make_plan(bool tri, uint64_t n_i, uint64_t n_j, Plan& out);
+
+void estimate(const uint64_t* dd, const uint64_t* dr, const uint64_t* rr, int nbins, uint64_t n_d, uint64_t n_r,
+              double* w);
+
+}  // namespace tpcf
