@@ -1,0 +1,342 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for the DD+DR+RR pair-count hot path (BASELINE.json metric) on N GPUs of one node.
+
+A "step" is one full pass of the hot path over one synthetic catalog pair: the three histograms DD, DR, RR of
+the workload (default: BASELINE.json configs[2], the paper-scale 430k + 430k octant catalogs of Table 2 row 1,
+PAPER.md:61) with the catalogs already resident in HBM; `e2e` repeats it through the synchronous C-ABI calls
+with pinned HOST buffers (tpcf_load x2 + tpcf_count x3 + tpcf_estimate, host<->device copies inside the timed
+region).  `--impl reference` times the fp64 oracle (oracle/, test infrastructure) on the host cores instead.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl ours|reference]
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+import synth  # noqa: E402
+
+KINDS = ("DD", "DR", "RR")
+METRIC = "pair evals/sec (DD+DR+RR)"
+UNIT = "Gpairs/s"
+SM_COUNT = 148
+LANES_PER_CLK_PER_SM = 128      # 4 schedulers x 1 warp instruction x 32 lanes
+PAPER_CONTEXT = {"table2_row1_0.43e6_lines_seconds": {"cpu_2xE5520": 3.60e4, "gtx295": 3.01e2, "c1060": 2.91e2,
+                                                      "c2050": 2.19e2}, "source": "PAPER.md:61 (other hardware; context, not target)"}
+
+
+def total_pairs(nd: int, nr: int) -> int:
+    return nd * (nd - 1) // 2 + nd * nr + nr * (nr - 1) // 2
+
+
+def workload_name(idx: int, cfg, nd: int, nr: int) -> str:
+    return (f"BASELINE.json configs[{idx - 1}] {cfg.name}: N_D={nd}, N_R={nr}, {cfg.nbins} {cfg.mode} bins "
+            f"{cfg.theta_min}-{cfg.theta_max} deg, {total_pairs(nd, nr):.4g} pairs per step")
+
+
+class ClockSampler:
+    """nvidia-smi SM clock / throttle reasons every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc, self.lines = index, None, []
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"], stdout=subprocess.PIPE,
+                                         stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=lambda: self.lines.extend(self.proc.stdout), daemon=True)
+            self.th.start()
+        except OSError:
+            self.proc = None
+        return self
+
+    def __exit__(self, *exc):
+        if self.proc:
+            time.sleep(0.25)
+            self.proc.terminate()
+            self.th.join(timeout=2)
+
+    def summary(self):
+        sm, mx, reasons = [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0]))
+                mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for name, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def inst_per_pair(cfg_idx: int):
+    """Thread-level SASS instructions executed per pair by the pair kernel, from the committed ncu summary
+    (profiles/inst_per_pair.json: smsp__thread_inst_executed.sum / pairs); falls back to the static SASS count."""
+    path = os.path.join(ROOT, "profiles", "inst_per_pair.json")
+    try:
+        d = json.load(open(path))
+        e = d.get(f"cfg{cfg_idx}") or d["default"]
+        return float(e["inst_per_pair"]), e.get("source", path)
+    except Exception:
+        return 22.0, "static SASS count of the inner loop (no ncu summary found)"
+
+
+# ------------------------------------------------------------------------------------------------ oracle legs
+def oracle_sample_rate(D, R, e, rows_per_hist: int, threads: int):
+    """Time the oracle (as it stands) on a seeded row subset of each of DD, DR, RR; returns (pairs, seconds)."""
+    import oracle
+    d, r = oracle.radec_to_xyz(D), oracle.radec_to_xyz(R)
+    nd, nr = d.shape[0], r.shape[0]
+    rd, rr = synth.subset_rows(nd, rows_per_hist, 777), synth.subset_rows(nr, rows_per_hist, 778)
+    t0 = time.perf_counter()
+    a = oracle.count_rows(d, rd, d, True, e, threads=threads)
+    b = oracle.count_rows(d, rd, r, False, e, threads=threads)
+    c = oracle.count_rows(r, rr, r, True, e, threads=threads)
+    dt = time.perf_counter() - t0
+    return a.total + b.total + c.total, dt
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores, each step a bounded sample of the workload."""
+    import oracle
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    D, R, e, cfg = synth.make_config(args.config)
+    nd, nr = D.shape[0], R.shape[0]
+    threads = oracle.host_threads()
+    pairs, dt = oracle_sample_rate(D, R, e, 16, threads)          # probe to size the sample
+    rate = pairs / dt
+    budget = 150.0 / (args.steps + args.warmup)                   # whole run within a few minutes
+    rows = int(max(16, min(2000, rate * min(budget, 20.0) / (nd + nr + nr))))
+    for _ in range(args.warmup):
+        oracle_sample_rate(D, R, e, rows, threads)
+    t_tot, p_tot = 0.0, 0
+    for _ in range(args.steps):
+        p, t = oracle_sample_rate(D, R, e, rows, threads)
+        p_tot += p
+        t_tot += t
+    val = p_tot / t_tot / 1e9
+    sample = f"{rows} seeded rows of each of DD, DR, RR against all j ({p_tot // args.steps:.4g} pairs per step)"
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * t_tot / args.steps, "higher_is_better": True, "scaling": "strong",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_name(args.config, cfg, nd, nr), "sample": sample},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "full_workload_seconds_extrapolated": total_pairs(nd, nr) / (val * 1e9)}
+    print(json.dumps(line))
+    return 0
+
+
+# ------------------------------------------------------------------------------------------------ our arm
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    import paper_1204_6630_b200 as T
+    from paper_1204_6630_b200 import dist as tdist
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: libtpcf has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    D, R, e, cfg = synth.make_config(args.config)
+    nd, nr = D.shape[0], R.shape[0]
+    pairs_step = total_pairs(nd, nr)
+    nb = cfg.nbins
+
+    st = torch.cuda.Stream()
+    ctx = T.Context(nb, e, "explicit")
+    ctx.set_stream(st.cuda_stream)
+    ctx.load("D", D, stream=st.cuda_stream)
+    ctx.load("R", R, stream=st.cuda_stream)
+    tdist.apply_partition(ctx)
+    out = torch.zeros(3, nb + 2, dtype=torch.int64, device="cuda")
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")      # > 126 MB L2
+
+    def step():
+        with torch.cuda.stream(st):
+            flush.zero_()                                   # L2 flush between steps (inside the timed region)
+            for i, k in enumerate(KINDS):
+                ctx.count_async(k, out[i])
+            if world > 1:
+                tdist.allreduce_counts(out)                 # 3 x (nbins+2) int64 over NCCL: the only exchange
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    ctx.set_kernel_timing(True)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    kernel_ms = []
+    with ClockSampler(local) as clk:
+        barrier()
+        ev0.record(st)
+        for _ in range(args.steps):
+            step()
+        ev1.record(st)
+        barrier()
+    ms_total = ev0.elapsed_time(ev1)
+    kernel_ms = [float(x) for x in ctx.kernel_times_ms()]                # per pair-kernel launch, CUDA events on the launching stream
+    ctx.set_kernel_timing(False)
+    t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_total = float(t.item())
+    ms_step = ms_total / args.steps
+    value = pairs_step / (ms_step * 1e-3) / 1e9
+    stats = ctx.stats()
+
+    # check the result the timed steps produced (totals identity; full parity lives in tests/)
+    res = out.cpu().numpy()
+    want = (nd * (nd - 1) // 2, nd * nr, nr * (nr - 1) // 2)
+    for i in range(3):
+        assert int(res[i].sum()) == want[i], (KINDS[i], int(res[i].sum()), want[i])
+
+    # ---- end to end through the synchronous C ABI with pinned host buffers --------------------------------
+    Dp, Rp = torch.from_numpy(D).pin_memory(), torch.from_numpy(R).pin_memory()
+    e2e_steps = max(1, min(args.steps, 5))
+
+    def e2e_step():
+        ctx.load("D", Dp, stream=st.cuda_stream)            # H2D copy + on-device conversion
+        ctx.load("R", Rp, stream=st.cuda_stream)
+        tdist.apply_partition(ctx)
+        hs = [ctx.count(k) for k in KINDS]                  # D2H of each histogram inside
+        if world > 1:
+            arr = np.stack([np.concatenate([[u], h.astype(np.int64), [o]]) for h, u, o in hs])
+            arr = tdist.allreduce_counts(arr)
+            return T.tpcf_estimate_from(arr[0][1:-1], arr[1][1:-1], arr[2][1:-1], nd, nr)
+        return ctx.estimate()
+
+    e2e_step()
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        w = e2e_step()
+    barrier()
+    e2e_s = (time.perf_counter() - t0) / e2e_steps
+    t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    e2e_s = float(t.item())
+    h2d = D.nbytes + R.nbytes
+    d2h = 3 * ((nb + 2) * 8 + 4 * 8) + 2 * 4
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+
+    # ---- roofline of the dominant kernel (pair_fast_kernel): plain ALU issue --------------------------------
+    clocks = clk.summary()
+    k_inst, k_src = inst_per_pair(args.config)
+    peak_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        sm_max = float(json.load(open(peak_path))["sm_max_mhz"])
+        peak_src = "MEASURED_PEAKS.json sm_max_mhz"
+    except Exception:
+        sm_max, peak_src = 1965.0, "fallback 1965 MHz (B200_PROFILING.md nominal clocks.max.sm)"
+    peak = SM_COUNT * LANES_PER_CLK_PER_SM * sm_max * 1e6 / 1e12          # T lane-instructions/s
+    # per launch: pairs of that histogram (this rank's share) / its own duration; the three launches repeat DD, DR, RR
+    share = [w_ / world for w_ in want]
+    per_launch = [share[i % 3] / (ms * 1e-3) for i, ms in enumerate(kernel_ms)] or [pairs_step / world / (ms_step * 1e-3)]
+    pairs_per_s_kernel = sum(share[i % 3] for i in range(len(kernel_ms))) / (sum(kernel_ms) * 1e-3) if kernel_ms else per_launch[0]
+    achieved = pairs_per_s_kernel * k_inst / 1e12
+    roofline = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "Tinst/s (thread-level SASS instructions)",
+                "frac": achieved / peak, "traffic": None,
+                "kernel": "pair_fast_kernel", "inst_per_pair": k_inst, "inst_per_pair_source": k_src,
+                "kernel_pairs_per_s": pairs_per_s_kernel, "kernel_ms_avg": (sum(kernel_ms) / len(kernel_ms)) if kernel_ms else None,
+                "kernel_launches_timed": len(kernel_ms),
+                "kernel_share_of_step": (sum(kernel_ms) / ms_total) if kernel_ms else None,
+                "pairs_per_clk_per_sm_at_max_clock": pairs_per_s_kernel / (SM_COUNT * sm_max * 1e6),
+                "peak_source": f"{SM_COUNT} SMs x {LANES_PER_CLK_PER_SM} lanes/clk x {sm_max:.0f} MHz ({peak_src}); DESIGN.md section 7",
+                "frac_at_sampled_clock": (achieved / (SM_COUNT * LANES_PER_CLK_PER_SM * clocks["sm_mhz"] * 1e6 / 1e12)) if clocks.get("sm_mhz") else None}
+    try:
+        prof = json.load(open(os.path.join(ROOT, "profiles", "inst_per_pair.json")))
+        roofline["traffic"] = (prof.get(f"cfg{args.config}") or prof["default"]).get("dram_bytes_per_launch")
+    except Exception:
+        pass
+
+    # ---- the oracle timed beside it (rank 0, N = 1 only) --------------------------------------------------------
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        import oracle
+        threads = oracle.host_threads()
+        p0, t0_ = oracle_sample_rate(D, R, e, 16, threads)
+        rows = int(max(16, min(2000, (p0 / t0_) * 15.0 / (nd + nr + nr))))
+        p1, t1_ = oracle_sample_rate(D, R, e, rows, threads)
+        cpu = {"value": p1 / t1_ / 1e9, "unit": UNIT, "cores": threads, "kind": "oracle",
+               "sample": f"{rows} seeded rows of each of DD, DR, RR against all j = {p1:.4g} pairs in {t1_:.1f} s",
+               "full_workload_seconds_extrapolated": pairs_step / (p1 / t1_)}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f32",
+            "data": "synthetic",
+            "config": {"workload": workload_name(args.config, cfg, nd, nr),
+                       "l2": "256 MiB write between steps (inside the timed region); catalogs (<= 14 MB) are L2-resident by design",
+                       "engine": "fast (fp32 squared chord + fp64 recheck of guard-band pairs)",
+                       "parallelism": f"tile work items w % {world} == rank, one all-reduce of 3x{nb + 2} int64" if world > 1 else "1 GPU",
+                       "grid": stats["grid"], "block": stats["block"], "smem_bytes": stats["smem_bytes"], "cells": stats["cells"]},
+            "seconds_per_w_theta": ms_step * 1e-3,
+            "e2e": {"value": pairs_step / e2e_s / 1e9, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                    "seconds_per_step": e2e_s, "steps": e2e_steps,
+                    "path": "tpcf_load(D), tpcf_load(R) from pinned host rows + tpcf_count x3 + tpcf_estimate"},
+            "gpu_launches": args.steps * 6,
+            "gpu_launches_note": "per step: 3 x (pair_fast_kernel + finalize_kernel); memsets are driver memset nodes",
+            "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu, "paper_context": PAPER_CONTEXT}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.steps < 1:
+        ap.error("--steps must be >= 1")
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -135,6 +135,12 @@ tpcf_status tpcf_set_guard_scale(tpcf_ctx* ctx, double scale);
  * (integer, order-independent).  Default (0, 1). */
 tpcf_status tpcf_set_partition(tpcf_ctx* ctx, int part, int nparts);
 
+/* Per-kernel device timing: when enabled, every later count records a CUDA event pair around its pair
+ * kernel on the context's stream (up to 64 outstanding).  tpcf_get_kernel_times waits for them, writes the
+ * durations in milliseconds, oldest first, and clears the list.  Used by bench.py for the roofline line. */
+tpcf_status tpcf_set_kernel_timing(tpcf_ctx* ctx, int enabled);
+tpcf_status tpcf_get_kernel_times(tpcf_ctx* ctx, float* ms_out, int capacity, int* n_out);
+
 typedef struct {
     uint64_t pairs;          /* pairs enumerated by the last count (after the partition) */
     uint64_t rechecked;      /* pairs the fast engine re-evaluated in fp64 (inside a guard band) */

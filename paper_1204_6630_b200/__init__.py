@@ -31,7 +31,7 @@ EXPORTS = (
     "tpcf_create", "tpcf_get_edges", "tpcf_load", "tpcf_count", "tpcf_count_async", "tpcf_estimate",
     "tpcf_estimate_from", "tpcf_destroy", "tpcf_last_error", "tpcf_set_stream", "tpcf_set_engine",
     "tpcf_set_guard_scale", "tpcf_set_partition", "tpcf_get_stats", "tpcf_get_thresholds", "tpcf_classify_fast",
-    "tpcf_plan", "tpcf_plan_item_pairs",
+    "tpcf_plan", "tpcf_plan_item_pairs", "tpcf_set_kernel_timing", "tpcf_get_kernel_times",
 )
 
 
@@ -76,6 +76,8 @@ def lib() -> ctypes.CDLL:
             "tpcf_set_guard_scale": [vp, dbl],
             "tpcf_set_partition": [vp, i32, i32],
             "tpcf_get_stats": [vp, ctypes.POINTER(tpcf_stats)],
+            "tpcf_set_kernel_timing": [vp, i32],
+            "tpcf_get_kernel_times": [vp, vp, i32, ctypes.POINTER(i32)],
             "tpcf_get_thresholds": [vp, vp],
             "tpcf_classify_fast": [vp, ctypes.c_float, ctypes.POINTER(i32)],
             "tpcf_plan": [vp, i32, u64, u64, ctypes.POINTER(u64)],
@@ -217,6 +219,17 @@ def tpcf_get_stats(ctx) -> dict:
     return s.as_dict()
 
 
+def tpcf_set_kernel_timing(ctx, enabled: bool) -> None:
+    _check(ctx, lib().tpcf_set_kernel_timing(ctx, int(bool(enabled))))
+
+
+def tpcf_get_kernel_times(ctx) -> np.ndarray:
+    ms = np.zeros(64, dtype=np.float32)
+    n = ctypes.c_int()
+    _check(ctx, lib().tpcf_get_kernel_times(ctx, _np_ptr(ms), 64, ctypes.byref(n)))
+    return ms[: n.value].copy()
+
+
 def tpcf_classify_fast(ctx, d2: float) -> int:
     out = ctypes.c_int()
     _check(ctx, lib().tpcf_classify_fast(ctx, ctypes.c_float(d2), ctypes.byref(out)))
@@ -297,6 +310,12 @@ class Context:
 
     def stats(self):
         return tpcf_get_stats(self._ctx)
+
+    def set_kernel_timing(self, enabled: bool):
+        tpcf_set_kernel_timing(self._ctx, enabled)
+
+    def kernel_times_ms(self):
+        return tpcf_get_kernel_times(self._ctx)
 
     def classify_fast(self, d2: float):
         return tpcf_classify_fast(self._ctx, d2)

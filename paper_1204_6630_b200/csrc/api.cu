@@ -48,6 +48,8 @@ struct tpcf_ctx {
     unsigned long long* d_out = nullptr;        // nbins + 2
     int* d_bad = nullptr;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    bool time_kernels = false;
+    std::vector<std::pair<cudaEvent_t, cudaEvent_t>> kev_pool, kev_used;
     // stored full counts for tpcf_estimate
     std::vector<uint64_t> counts[3];
     bool have[3] = {false, false, false};
@@ -241,10 +243,25 @@ tpcf_status enqueue_count(tpcf_ctx* ctx, tpcf_kind kind, const int64_t* rows_hos
     CU(cudaMemsetAsync(ctx->d_result, 0, (nb + 3) * sizeof(unsigned long long), st), "memset result");
     CU(cudaMemsetAsync(ctx->d_counters, 0, 4 * sizeof(unsigned long long), st), "memset counters");
     LaunchInfo li{};
+    std::pair<cudaEvent_t, cudaEvent_t> kev{nullptr, nullptr};
+    if (ctx->time_kernels && ctx->kev_used.size() < 64) {
+        if (ctx->kev_pool.empty()) {
+            CU(cudaEventCreate(&kev.first), "cudaEventCreate");
+            CU(cudaEventCreate(&kev.second), "cudaEventCreate");
+        } else {
+            kev = ctx->kev_pool.back();
+            ctx->kev_pool.pop_back();
+        }
+        CU(cudaEventRecord(kev.first, st), "cudaEventRecord");
+    }
     if (ctx->engine == TPCF_ENGINE_FAST)
         CU(launch_pairs_fast(p, ctx->ft.map, ctx->sm_count, st, &li), "pair_fast_kernel launch");
     else
         CU(launch_pairs_exact64(p, ctx->sm_count, st, &li), "pair_exact64_kernel launch");
+    if (kev.first) {
+        CU(cudaEventRecord(kev.second, st), "cudaEventRecord");
+        ctx->kev_used.push_back(kev);
+    }
     const int zero_slot = (ctx->bin.thr[0] > 0.0) ? 0 : 1;
     CU(launch_finalize(ctx->d_result, nb, zero_slot, self_pairs, out_dev, st), "finalize launch");
     ctx->stats.launches += 2;
@@ -442,6 +459,11 @@ void tpcf_destroy(tpcf_ctx* ctx) {
         cudaFree(ctx->d_bad);
         if (ctx->ev0) cudaEventDestroy(ctx->ev0);
         if (ctx->ev1) cudaEventDestroy(ctx->ev1);
+        for (auto* v : {&ctx->kev_pool, &ctx->kev_used})
+            for (auto& kv : *v) {
+                cudaEventDestroy(kv.first);
+                cudaEventDestroy(kv.second);
+            }
     }
     delete ctx;
 }
@@ -474,6 +496,27 @@ tpcf_status tpcf_set_partition(tpcf_ctx* ctx, int part, int nparts) {
     if (nparts < 1 || part < 0 || part >= nparts) return fail(ctx, TPCF_EINVAL, "need 0 <= part < nparts");
     ctx->part = part;
     ctx->nparts = nparts;
+    return TPCF_OK;
+}
+
+tpcf_status tpcf_set_kernel_timing(tpcf_ctx* ctx, int enabled) {
+    if (!ctx) return TPCF_EINVAL;
+    ctx->time_kernels = enabled != 0;
+    return TPCF_OK;
+}
+
+tpcf_status tpcf_get_kernel_times(tpcf_ctx* ctx, float* ms_out, int capacity, int* n_out) {
+    if (!ctx || !n_out || (capacity > 0 && !ms_out)) return TPCF_EINVAL;
+    int n = 0;
+    for (auto& kv : ctx->kev_used) {
+        CU(cudaEventSynchronize(kv.second), "cudaEventSynchronize");
+        float ms = 0.f;
+        CU(cudaEventElapsedTime(&ms, kv.first, kv.second), "cudaEventElapsedTime");
+        if (n < capacity) ms_out[n++] = ms;
+        ctx->kev_pool.push_back(kv);
+    }
+    ctx->kev_used.clear();
+    *n_out = n;
     return TPCF_OK;
 }
 

@@ -1,0 +1,198 @@
+"""CPU-side checks of libtpcf (no GPU): the library loads and exports every symbol of include/tpcf.h, argument
+validation, edge/threshold generation, the fast engine's lookup tables against the thresholds, the tile work
+plan and its partition, the estimator, and the no-fallback rule (compute calls fail loudly without a GPU)."""
+import ctypes
+import json
+import math
+import os
+import re
+
+import numpy as np
+import pytest
+
+import oracle
+import paper_1204_6630_b200 as T
+import synth
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def has_gpu():
+    try:
+        import torch
+        return torch.cuda.is_available()
+    except Exception:
+        return False
+
+
+def test_library_exports_every_declared_symbol():
+    header = open(os.path.join(ROOT, "include", "tpcf.h")).read()
+    declared = set(re.findall(r"\b(tpcf_[a-z0-9_]+)\s*\(", header))
+    assert declared == set(T.EXPORTS), declared ^ set(T.EXPORTS)
+    L = T.lib()
+    for name in declared:
+        assert getattr(L, name) is not None
+
+
+def test_create_rejects_bad_binnings():
+    bad = [(0, [0.1, 1.0], "log"), (5000, [0.1, 1.0], "log"), (4, [0.0, 1.0], "log"), (4, [1.0, 1.0], "linear"),
+           (4, [2.0, 1.0], "linear"), (4, [-1.0, 1.0], "linear"), (4, [1.0, 181.0], "linear"),
+           (4, [float("nan"), 1.0], "linear"), (2, [0.0, 1.0, 1.0], "explicit"), (2, [0.0, 2.0, 1.0], "explicit"),
+           (2, [0.0, 1.0, 200.0], "explicit")]
+    for nbins, th, mode in bad:
+        with pytest.raises(T.TpcfError) as ei:
+            T.tpcf_create(nbins, th, mode)
+        assert ei.value.status == T.TPCF_EINVAL
+
+
+@pytest.mark.parametrize("idx", [1, 2, 3, 4, 5])
+def test_edges_match_the_input_recipe_and_thresholds_closed_form(idx):
+    cfg = synth.CONFIGS[idx]
+    with T.Context(cfg.nbins, [cfg.theta_min, cfg.theta_max], cfg.mode) as c:
+        e = c.edges()
+        ref = synth.config_edges(cfg)
+        assert e[0] == cfg.theta_min and e[-1] == cfg.theta_max
+        np.testing.assert_allclose(e, ref, rtol=1e-14, atol=0)
+        thr = c.thresholds()
+    # T_k = |a-b|^2 at separation e_k = 2 - 2 cos(e_k): checked with mpmath-free high precision via the
+    # half-angle form in numpy longdouble
+    el = np.asarray(ref, dtype=np.longdouble) * (np.pi / np.longdouble(360.0))
+    want = (4 * np.sin(el) ** 2).astype(np.float64)
+    np.testing.assert_allclose(thr, want, rtol=1e-15, atol=0)   # 3-4 fp64 roundings in 4 sin^2(e pi/360)
+    big = ref > 5.0                                  # where 2 - 2 cos is not cancellation-limited
+    np.testing.assert_allclose(thr[big], 2.0 - 2.0 * np.cos(np.radians(ref[big])), rtol=1e-13)
+
+
+def expected_slot(v, thr, nbins):
+    if v >= 5.0:
+        return nbins + 2
+    if v < thr[0]:
+        return 0
+    if v > thr[-1]:
+        return nbins + 1
+    return min(int(np.searchsorted(thr, v, side="right")) - 1, nbins - 1) + 1
+
+
+def fp32_bound(t):
+    """|d2_fp32 - d2| bound of DESIGN.md section 4 (without the safety margin of the implementation)."""
+    return 2.07e-7 * math.sqrt(t) + 3.0e-7 * t + 1.1e-14
+
+
+@pytest.mark.parametrize("idx", [1, 2, 3, 4, 5])
+@pytest.mark.parametrize("scale", [1.0, 8.0])
+def test_fast_tables_agree_with_thresholds_outside_the_guard_bands(idx, scale):
+    cfg = synth.CONFIGS[idx]
+    rng = np.random.default_rng(idx)
+    with T.Context(cfg.nbins, synth.config_edges(cfg), "explicit") as c:
+        c.set_guard_scale(scale)
+        thr = c.thresholds()
+        pos = thr[thr > 0]
+        near = (pos[:, None] * (1.0 + rng.normal(0.0, 2e-6, (len(pos), 24)))).ravel()
+        vals = np.concatenate([np.exp(rng.uniform(np.log(1e-13), np.log(4.0), 6000)), near,
+                               [0.0, 1e-30, 4.0, 4.0000005, 6.07, 19.9, 48.0]]).astype(np.float32)
+        n_amb = 0
+        for v in vals:
+            v = float(v)
+            s = c.classify_fast(v)
+            d = np.abs(thr - v)
+            k = int(np.argmin(d))
+            if s == -1:
+                n_amb += 1
+                # ambiguous only close to an edge: within the (scaled, margin-included) band
+                assert d[k] <= scale * (2.6e-7 * math.sqrt(thr[k]) + 5.2e-7 * thr[k] + 1.1e-13) + 1e-7 * thr[k]
+            else:
+                assert s == expected_slot(v, thr, cfg.nbins), (v, s)
+                # a decided value must be farther from every droppable edge than the fp32 rounding bound,
+                # otherwise the true d2 could be on the other side
+                live = np.ones(len(thr), bool)
+                live[0] = thr[0] > 0
+                live[-1] = thr[-1] < 4.0
+                if v < 4.5:
+                    assert np.all(d[live] > fp32_bound(v)), (v, k)
+        assert n_amb > 0
+        assert c.stats()["cells"] <= 8192
+
+
+def test_fast_tables_survive_pathological_edges():
+    # bins far narrower than the fp32 guard bands: everything near them must come back ambiguous (-1), never wrong
+    e = np.concatenate([[0.0], 1.0 + 1e-7 * np.arange(40), [90.0, 180.0]])
+    with T.Context(len(e) - 1, e, "explicit") as c:
+        thr = c.thresholds()
+        for v in np.linspace(thr[1] * 0.999, thr[40] * 1.001, 400).astype(np.float32):
+            s = c.classify_fast(float(v))
+            assert s == -1 or s == expected_slot(float(v), thr, len(e) - 1)
+        assert c.classify_fast(3.0) == len(e) - 1          # inside the last bin [90, 180]
+        assert c.classify_fast(4.0000005) == len(e) - 1    # e_n = 180: nothing is ever "over"
+        assert c.classify_fast(0.0) == 1                   # e_0 = 0: theta = 0 is in bin 0
+
+
+@pytest.mark.parametrize("n_d,n_r", [(1, 1), (5, 3), (1024, 1024), (1025, 2047), (4096, 4096), (100_000, 70_001)])
+def test_plan_covers_every_pair_exactly_once(n_d, n_r):
+    with T.Context(4, [0.1, 10.0], "log") as c:
+        for kind, total in (("DD", n_d * (n_d - 1) // 2), ("DR", n_d * n_r), ("RR", n_r * (n_r - 1) // 2)):
+            n = c.plan(kind, n_d, n_r)
+            pairs = [c.plan_item_pairs(kind, n_d, n_r, w) for w in range(n)]
+            assert sum(pairs) == total
+            for nparts in (2, 3):
+                assert sum(sum(pairs[p::nparts]) for p in range(nparts)) == total
+            with pytest.raises(T.TpcfError):
+                c.plan_item_pairs(kind, n_d, n_r, n)
+
+
+def test_plan_sizes_at_paper_scale():
+    with T.Context(4, [0.1, 10.0], "log") as c:
+        n = c.plan("DR", 430_000, 430_000)
+        assert 148 * 40 <= n <= 2 ** 32
+        assert c.plan("RR", 1_000_000, 2_000_000) < 2 ** 32
+
+
+def test_estimator_hand_case_and_against_oracle():
+    g = json.load(open(os.path.join(ROOT, "tests", "golden", "hand_catalogs.json")))["landy_szalay_hand"]
+    w = T.tpcf_estimate_from(g["dd"], g["dr"], g["rr"], g["n_d"], g["n_r"])
+    assert abs(w[0] - g["w"][0]) < 1e-15
+    rng = np.random.default_rng(3)
+    dd, dr, rr = (rng.integers(0, 10 ** 9, 50).astype(np.uint64) for _ in range(3))
+    rr[7] = 0
+    a = T.tpcf_estimate_from(dd, dr, rr, 430_000, 500_000)
+    b = oracle.estimate(dd, dr, rr, 430_000, 500_000)
+    assert math.isnan(a[7]) and math.isnan(b[7])
+    ok = ~np.isnan(b)
+    np.testing.assert_allclose(a[ok], b[ok], rtol=1e-15, atol=1e-15)
+
+
+def test_setters_validate():
+    with T.Context(4, [0.1, 10.0], "log") as c:
+        for bad in (0.0, -1.0, float("nan")):
+            with pytest.raises(T.TpcfError):
+                c.set_guard_scale(bad)
+        for part, nparts in ((0, 0), (2, 2), (-1, 2)):
+            with pytest.raises(T.TpcfError):
+                c.set_partition(part, nparts)
+        with pytest.raises(T.TpcfError):
+            c.set_engine(7)
+        c.set_partition(1, 2)
+        c.set_engine("exact64")
+
+
+@pytest.mark.skipif(has_gpu(), reason="checks the behaviour on a box without a GPU")
+def test_no_cpu_fallback_compute_calls_fail_loudly_without_a_gpu():
+    D, R, e, cfg = synth.make_config(1, n_d=64, n_r=64)
+    with T.Context(cfg.nbins, e, "explicit") as c:
+        with pytest.raises(T.TpcfError) as ei:
+            c.load("D", D)
+        assert ei.value.status == T.TPCF_ECUDA
+        with pytest.raises(T.TpcfError) as ei:
+            c.count("DD")
+        assert ei.value.status == T.TPCF_ECUDA
+        with pytest.raises(T.TpcfError) as ei:
+            c.estimate()
+        assert ei.value.status == T.TPCF_ESTATE
+
+
+def test_product_package_does_not_touch_the_oracle():
+    pkg = os.path.join(ROOT, "paper_1204_6630_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".cpp", ".h")):
+                src = open(os.path.join(dirpath, f)).read()
+                assert "import oracle" not in src and "from oracle" not in src and "tpcf_oracle" not in src, f
