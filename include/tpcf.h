@@ -130,6 +130,13 @@ tpcf_status tpcf_set_engine(tpcf_ctx* ctx, tpcf_engine e);
  * give identical histograms; the tests use 2.0 and 8.0 to demonstrate that the band is wide enough.
  * scale <= 0 is TPCF_EINVAL. */
 tpcf_status tpcf_set_guard_scale(tpcf_ctx* ctx, double scale);
+/* Window path of the fast engine on (default) / off.  On: catalogs are held in Hilbert-curve order with a bounding
+ * sphere per 32 rows; for every (lane = 4 consecutive i-rows, 32-row j-subtile) block the kernel bounds the chord
+ * lengths by the triangle inequality, and when at most 3 bin edges can be reached it classifies each pair with that
+ * many sign tests against the band midpoints (register counters, no shared-memory traffic per pair); otherwise, and
+ * always when off, each pair goes through the cell lookup.  Every pair is evaluated either way; the histograms are
+ * identical (tests). */
+tpcf_status tpcf_set_window(tpcf_ctx* ctx, int enabled);
 /* Work partition for multi-process runs (one process per GPU): this context enumerates only the tile
  * work items w with w % nparts == part; summing the histograms of all parts gives the full count
  * (integer, order-independent).  Default (0, 1). */
@@ -150,6 +157,9 @@ typedef struct {
     int cells, cell_bits;    /* lookup cells of the fast engine and mantissa bits per octave */
     int hist_copies;         /* privatised copies of each partial-histogram slot per CTA */
     float kernel_ms;         /* device time of the last synchronous count (CUDA events) */
+    uint64_t win_blocks[5];  /* (warp, 32-row j-subtile) blocks of the last synchronous count by path: counted by the
+                                1-, 2-, 3-edge window loops, by the per-pair cell lookup; [4] = lanes of window
+                                blocks recounted pair by pair because a pair came within a guard band */
 } tpcf_stats;
 tpcf_status tpcf_get_stats(const tpcf_ctx* ctx, tpcf_stats* out);
 
@@ -165,6 +175,15 @@ tpcf_status tpcf_get_thresholds(const tpcf_ctx* ctx, double* t_out /* nbins+1 */
  * pair in fp64).  Lets CPU tests check the table builder against the thresholds without a GPU.
  */
 tpcf_status tpcf_classify_fast(const tpcf_ctx* ctx, float d2, int* slot_out);
+
+/* The guard bands of the fast engine (ascending, disjoint; the last is the zero-width "discard" band that separates
+ * real pairs from padding lanes): *n_out = number of bands; if capacity >= that, lo/hi (fp32 squared chord) and the
+ * result slot just below each band are written (any of the three may be NULL). */
+tpcf_status tpcf_get_bands(const tpcf_ctx* ctx, int capacity, float* lo_out, float* hi_out, int* slot_below_out, int* n_out);
+/* Host mirror of the kernel's window selection: for a block whose fp32 squared chords all lie in [lo2, hi2], the first
+ * band that is not wholly below lo2 and the number of consecutive bands the block can reach (1..3, or 4 = too many,
+ * cell-lookup path).  0 <= lo2 <= hi2 < 64. */
+tpcf_status tpcf_window_host(const tpcf_ctx* ctx, float lo2, float hi2, int* first_band_out, int* n_edges_out);
 
 /* Number of tile work items of a full count of `kind` for catalog sizes (n_d, n_r), and the number of
  * pairs in item w: the partition arithmetic of tpcf_set_partition, testable without a GPU. */

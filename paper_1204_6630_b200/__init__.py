@@ -31,7 +31,8 @@ EXPORTS = (
     "tpcf_create", "tpcf_get_edges", "tpcf_load", "tpcf_count", "tpcf_count_async", "tpcf_estimate",
     "tpcf_estimate_from", "tpcf_destroy", "tpcf_last_error", "tpcf_set_stream", "tpcf_set_engine",
     "tpcf_set_guard_scale", "tpcf_set_partition", "tpcf_get_stats", "tpcf_get_thresholds", "tpcf_classify_fast",
-    "tpcf_plan", "tpcf_plan_item_pairs", "tpcf_set_kernel_timing", "tpcf_get_kernel_times",
+    "tpcf_plan", "tpcf_plan_item_pairs", "tpcf_set_kernel_timing", "tpcf_get_kernel_times", "tpcf_set_window",
+    "tpcf_get_bands", "tpcf_window_host",
 )
 
 
@@ -45,10 +46,12 @@ class tpcf_stats(ctypes.Structure):
     _fields_ = [("pairs", ctypes.c_uint64), ("rechecked", ctypes.c_uint64), ("work_items", ctypes.c_uint64),
                 ("launches", ctypes.c_int), ("grid", ctypes.c_int), ("block", ctypes.c_int),
                 ("smem_bytes", ctypes.c_int), ("cells", ctypes.c_int), ("cell_bits", ctypes.c_int),
-                ("hist_copies", ctypes.c_int), ("kernel_ms", ctypes.c_float)]
+                ("hist_copies", ctypes.c_int), ("kernel_ms", ctypes.c_float), ("win_blocks", ctypes.c_uint64 * 5)]
 
     def as_dict(self):
-        return {k: getattr(self, k) for k, _ in self._fields_}
+        d = {k: getattr(self, k) for k, _ in self._fields_}
+        d["win_blocks"] = [int(x) for x in self.win_blocks]
+        return d
 
 
 _lib = None
@@ -74,6 +77,9 @@ def lib() -> ctypes.CDLL:
             "tpcf_set_stream": [vp, vp],
             "tpcf_set_engine": [vp, i32],
             "tpcf_set_guard_scale": [vp, dbl],
+            "tpcf_set_window": [vp, i32],
+            "tpcf_get_bands": [vp, i32, vp, vp, vp, ctypes.POINTER(i32)],
+            "tpcf_window_host": [vp, ctypes.c_float, ctypes.c_float, ctypes.POINTER(i32), ctypes.POINTER(i32)],
             "tpcf_set_partition": [vp, i32, i32],
             "tpcf_get_stats": [vp, ctypes.POINTER(tpcf_stats)],
             "tpcf_set_kernel_timing": [vp, i32],
@@ -209,6 +215,26 @@ def tpcf_set_guard_scale(ctx, scale: float) -> None:
     _check(ctx, lib().tpcf_set_guard_scale(ctx, float(scale)))
 
 
+def tpcf_set_window(ctx, enabled: bool) -> None:
+    _check(ctx, lib().tpcf_set_window(ctx, int(bool(enabled))))
+
+
+def tpcf_get_bands(ctx):
+    """(lo, hi, slot_below) arrays of the fast engine's guard bands."""
+    n = ctypes.c_int()
+    _check(ctx, lib().tpcf_get_bands(ctx, 0, None, None, None, ctypes.byref(n)))
+    lo, hi = np.empty(n.value, dtype=np.float32), np.empty(n.value, dtype=np.float32)
+    sb = np.empty(n.value, dtype=np.int32)
+    _check(ctx, lib().tpcf_get_bands(ctx, n.value, _np_ptr(lo), _np_ptr(hi), _np_ptr(sb), ctypes.byref(n)))
+    return lo, hi, sb
+
+
+def tpcf_window_host(ctx, lo2: float, hi2: float) -> Tuple[int, int]:
+    k, e = ctypes.c_int(), ctypes.c_int()
+    _check(ctx, lib().tpcf_window_host(ctx, ctypes.c_float(lo2), ctypes.c_float(hi2), ctypes.byref(k), ctypes.byref(e)))
+    return k.value, e.value
+
+
 def tpcf_set_partition(ctx, part: int, nparts: int) -> None:
     _check(ctx, lib().tpcf_set_partition(ctx, int(part), int(nparts)))
 
@@ -304,6 +330,15 @@ class Context:
 
     def set_guard_scale(self, scale: float):
         tpcf_set_guard_scale(self._ctx, scale)
+
+    def set_window(self, enabled: bool):
+        tpcf_set_window(self._ctx, enabled)
+
+    def bands(self):
+        return tpcf_get_bands(self._ctx)
+
+    def window_host(self, lo2: float, hi2: float):
+        return tpcf_window_host(self._ctx, lo2, hi2)
 
     def set_partition(self, part: int, nparts: int):
         tpcf_set_partition(self._ctx, part, nparts)

@@ -15,10 +15,21 @@
 using namespace tpcf;
 
 namespace {
-struct Catalog {
+struct Catalog {                 // rows in Hilbert order (counts are order-invariant, reading A16)
     uint64_t n = 0, n_pad = 0;
     double4* x64 = nullptr;
     float4* x32 = nullptr;
+    uint32_t* inv = nullptr;     // caller row -> position in the sorted catalog (row-subset mode)
+    float4* sph = nullptr;       // bounding sphere of every kSubJ consecutive rows
+};
+// scratch of one spatial sort: (key, idx) ping-pong buffers and the digit counts
+struct SortScratch {
+    uint64_t *ka = nullptr, *kb = nullptr;
+    uint32_t *ia = nullptr, *ib = nullptr, *counts = nullptr;
+    void release() {
+        cudaFree(ka); cudaFree(kb); cudaFree(ia); cudaFree(ib); cudaFree(counts);
+        *this = SortScratch();
+    }
 };
 struct PlanCache {
     bool valid = false;
@@ -33,6 +44,7 @@ struct tpcf_ctx {
     double guard_scale = 1.0;
     bool tables_dirty = true;
     tpcf_engine engine = TPCF_ENGINE_FAST;
+    bool window = true;
     cudaStream_t stream = nullptr;
     int part = 0, nparts = 1;
     Catalog cat[2];
@@ -42,9 +54,11 @@ struct tpcf_ctx {
     int sm_count = 0;
     float2* d_lut = nullptr;
     uint16_t* d_slotmap = nullptr;
+    float2 *d_band_mh = nullptr, *d_band_lh = nullptr;
+    uint16_t *d_band_slot = nullptr, *d_cell_band = nullptr;
     double* d_thr = nullptr;
     unsigned long long* d_result = nullptr;     // nbins + 3
-    unsigned long long* d_counters = nullptr;   // 4
+    unsigned long long* d_counters = nullptr;   // kNumCounters
     unsigned long long* d_out = nullptr;        // nbins + 2
     int* d_bad = nullptr;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
@@ -92,7 +106,7 @@ tpcf_status ensure_cuda(tpcf_ctx* ctx) {
     CU(cudaMalloc(&ctx->d_thr, (nb + 1) * sizeof(double)), "cudaMalloc thresholds");
     CU(cudaMalloc(&ctx->d_result, (nb + 3) * sizeof(unsigned long long)), "cudaMalloc result");
     CU(cudaMalloc(&ctx->d_out, (nb + 2) * sizeof(unsigned long long)), "cudaMalloc out");
-    CU(cudaMalloc(&ctx->d_counters, 4 * sizeof(unsigned long long)), "cudaMalloc counters");
+    CU(cudaMalloc(&ctx->d_counters, kNumCounters * sizeof(unsigned long long)), "cudaMalloc counters");
     CU(cudaMalloc(&ctx->d_bad, sizeof(int)), "cudaMalloc flag");
     CU(cudaMemcpy(ctx->d_thr, ctx->bin.thr.data(), (nb + 1) * sizeof(double), cudaMemcpyHostToDevice), "upload thresholds");
     CU(cudaEventCreate(&ctx->ev0), "cudaEventCreate");
@@ -109,10 +123,14 @@ void rebuild_tables(tpcf_ctx* ctx) {
 tpcf_status upload_tables(tpcf_ctx* ctx) {
     if (!ctx->tables_dirty && ctx->d_lut) return TPCF_OK;
     const FastTables& t = ctx->ft;
-    if (ctx->d_lut) cudaFree(ctx->d_lut);
-    if (ctx->d_slotmap) cudaFree(ctx->d_slotmap);
-    ctx->d_lut = nullptr;
-    ctx->d_slotmap = nullptr;
+    cudaFree(ctx->d_lut);
+    cudaFree(ctx->d_slotmap);
+    cudaFree(ctx->d_band_mh);
+    cudaFree(ctx->d_band_lh);
+    cudaFree(ctx->d_band_slot);
+    cudaFree(ctx->d_cell_band);
+    ctx->d_lut = ctx->d_band_mh = ctx->d_band_lh = nullptr;
+    ctx->d_slotmap = ctx->d_band_slot = ctx->d_cell_band = nullptr;
     std::vector<float2> lut(t.ncells);
     std::vector<uint16_t> sm(2 * (size_t)t.ncells);
     for (int c = 0; c < t.ncells; ++c) {
@@ -124,14 +142,39 @@ tpcf_status upload_tables(tpcf_ctx* ctx) {
     CU(cudaMalloc(&ctx->d_slotmap, sm.size() * sizeof(uint16_t)), "cudaMalloc slotmap");
     CU(cudaMemcpy(ctx->d_lut, lut.data(), lut.size() * sizeof(float2), cudaMemcpyHostToDevice), "upload lut");
     CU(cudaMemcpy(ctx->d_slotmap, sm.data(), sm.size() * sizeof(uint16_t), cudaMemcpyHostToDevice), "upload slotmap");
+    std::vector<float2> mh(t.nbands), lh(t.nbands);
+    for (int b = 0; b < t.nbands; ++b) {
+        mh[b] = make_float2(t.band_mid[b], t.band_half[b]);
+        lh[b] = make_float2(t.band_lo[b], t.band_hi[b]);
+    }
+    CU(cudaMalloc(&ctx->d_band_mh, mh.size() * sizeof(float2)), "cudaMalloc bands");
+    CU(cudaMalloc(&ctx->d_band_lh, lh.size() * sizeof(float2)), "cudaMalloc bands");
+    CU(cudaMalloc(&ctx->d_band_slot, t.band_slot.size() * sizeof(uint16_t)), "cudaMalloc bands");
+    CU(cudaMalloc(&ctx->d_cell_band, t.cell_band.size() * sizeof(uint16_t)), "cudaMalloc bands");
+    CU(cudaMemcpy(ctx->d_band_mh, mh.data(), mh.size() * sizeof(float2), cudaMemcpyHostToDevice), "upload bands");
+    CU(cudaMemcpy(ctx->d_band_lh, lh.data(), lh.size() * sizeof(float2), cudaMemcpyHostToDevice), "upload bands");
+    CU(cudaMemcpy(ctx->d_band_slot, t.band_slot.data(), t.band_slot.size() * sizeof(uint16_t), cudaMemcpyHostToDevice), "upload bands");
+    CU(cudaMemcpy(ctx->d_cell_band, t.cell_band.data(), t.cell_band.size() * sizeof(uint16_t), cudaMemcpyHostToDevice), "upload bands");
     ctx->tables_dirty = false;
     return TPCF_OK;
 }
 
 void free_catalog(Catalog& c) {
-    if (c.x64) cudaFree(c.x64);
-    if (c.x32) cudaFree(c.x32);
+    cudaFree(c.x64);
+    cudaFree(c.x32);
+    cudaFree(c.inv);
+    cudaFree(c.sph);
     c = Catalog();
+}
+
+tpcf_status alloc_sort_scratch(tpcf_ctx* ctx, SortScratch& sc, uint64_t n) {
+    const uint64_t nblk = (n + kSortChunk - 1) / kSortChunk;
+    CU(cudaMalloc(&sc.ka, n * sizeof(uint64_t)), "cudaMalloc sort keys");
+    CU(cudaMalloc(&sc.kb, n * sizeof(uint64_t)), "cudaMalloc sort keys");
+    CU(cudaMalloc(&sc.ia, n * sizeof(uint32_t)), "cudaMalloc sort index");
+    CU(cudaMalloc(&sc.ib, n * sizeof(uint32_t)), "cudaMalloc sort index");
+    CU(cudaMalloc(&sc.counts, 256 * nblk * sizeof(uint32_t)), "cudaMalloc sort counts");
+    return TPCF_OK;
 }
 
 uint64_t pad_to(uint64_t n, uint64_t m) { return (n + m - 1) / m * m; }
@@ -178,16 +221,27 @@ tpcf_status enqueue_count(tpcf_ctx* ctx, tpcf_kind kind, const int64_t* rows_hos
     if (rows_host) {
         // row-subset mode: gather the rows into a temporary i-side catalog, count the rectangle against all j
         if (nrows == 0) return fail(ctx, TPCF_EINVAL, "nrows == 0 with rows != NULL");
+        if (nrows > 0x7FFFFFFFull) return fail(ctx, TPCF_EINVAL, "more than 2^31-1 rows");
         const uint64_t np = pad_to(nrows, kTileI);
         CU(cudaMalloc(tmp_rows, nrows * sizeof(int64_t)), "cudaMalloc rows");
         CU(cudaMalloc(tmp64, np * sizeof(double4)), "cudaMalloc subset");
         CU(cudaMalloc(tmp32, np * sizeof(float4)), "cudaMalloc subset");
-        CU(cudaMemcpyAsync(*tmp_rows, rows_host, nrows * sizeof(int64_t), cudaMemcpyHostToDevice, st), "upload rows");
-        CU(cudaMemsetAsync(ctx->d_bad, 0, sizeof(int), st), "memset");
-        CU(launch_gather(ci.x64, ci.x32, *tmp_rows, nrows, np, ci.n, *tmp64, *tmp32, ctx->d_bad, st), "gather kernel");
+        SortScratch sc;
+        tpcf_status ss = alloc_sort_scratch(ctx, sc, nrows);
+        if (ss) { sc.release(); return ss; }
+        // the listed rows, ordered by their position in the sorted catalog (the order of the i-rows does not
+        // change a sum over them; it keeps consecutive i-rows close on the sky for the window path)
+        cudaError_t e = cudaMemcpyAsync(*tmp_rows, rows_host, nrows * sizeof(int64_t), cudaMemcpyHostToDevice, st);
+        if (e == cudaSuccess) e = cudaMemsetAsync(ctx->d_bad, 0, sizeof(int), st);
+        if (e == cudaSuccess) e = launch_row_keys(*tmp_rows, nrows, ci.n, ci.inv, sc.ka, sc.ia, ctx->d_bad, st);
+        bool in_a = true;
+        if (e == cudaSuccess) e = launch_sort_pairs(sc.ka, sc.kb, sc.ia, sc.ib, sc.counts, (uint32_t)nrows, 32, st, &in_a);
+        if (e == cudaSuccess) e = launch_gather(ci.x64, ci.x32, in_a ? sc.ka : sc.kb, nrows, np, *tmp64, *tmp32, st);
         int bad = 0;
-        CU(cudaMemcpyAsync(&bad, ctx->d_bad, sizeof(int), cudaMemcpyDeviceToHost, st), "read flag");
-        CU(cudaStreamSynchronize(st), "gather");
+        if (e == cudaSuccess) e = cudaMemcpyAsync(&bad, ctx->d_bad, sizeof(int), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        sc.release();
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "gather subset rows");
         if (bad) return fail(ctx, TPCF_EINVAL, "row index out of range");
         make_plan(false, nrows, cj.n, subset_plan);
         plan = &subset_plan;
@@ -231,6 +285,12 @@ tpcf_status enqueue_count(tpcf_ctx* ctx, tpcf_kind kind, const int64_t* rows_hos
     p.nparts = (uint32_t)ctx->nparts;
     p.lut = ctx->d_lut;
     p.slotmap = ctx->d_slotmap;
+    p.sph_j = (ctx->window && ctx->ft.nbands >= 1) ? cj.sph : nullptr;
+    p.band_mh = ctx->d_band_mh;
+    p.band_lh = ctx->d_band_lh;
+    p.band_slot = ctx->d_band_slot;
+    p.cell_band = ctx->d_cell_band;
+    p.nbands = ctx->ft.nbands;
     p.ncells = ctx->ft.ncells;
     p.shift = ctx->ft.shift;
     p.sqrt_scale = ctx->ft.sqrt_scale;
@@ -241,7 +301,7 @@ tpcf_status enqueue_count(tpcf_ctx* ctx, tpcf_kind kind, const int64_t* rows_hos
     p.counters = ctx->d_counters;
 
     CU(cudaMemsetAsync(ctx->d_result, 0, (nb + 3) * sizeof(unsigned long long), st), "memset result");
-    CU(cudaMemsetAsync(ctx->d_counters, 0, 4 * sizeof(unsigned long long), st), "memset counters");
+    CU(cudaMemsetAsync(ctx->d_counters, 0, kNumCounters * sizeof(unsigned long long), st), "memset counters");
     LaunchInfo li{};
     std::pair<cudaEvent_t, cudaEvent_t> kev{nullptr, nullptr};
     if (ctx->time_kernels && ctx->kev_used.size() < 64) {
@@ -343,23 +403,38 @@ tpcf_status tpcf_load(tpcf_ctx* ctx, tpcf_cat which, const void* radec_deg, tpcf
     const size_t esz = (dt == TPCF_F64) ? 8 : 4;
     CU(cudaMalloc(&c.x64, n_pad * sizeof(double4)), "cudaMalloc catalog (fp64)");
     CU(cudaMalloc(&c.x32, n_pad * sizeof(float4)), "cudaMalloc catalog (fp32)");
+    CU(cudaMalloc(&c.inv, n * sizeof(uint32_t)), "cudaMalloc catalog (row map)");
+    CU(cudaMalloc(&c.sph, n_pad / kSubJ * sizeof(float4)), "cudaMalloc catalog (spheres)");
     void* staged = nullptr;
+    double4* rows64 = nullptr;
+    SortScratch sc;
+    auto cleanup = [&]() {
+        cudaFree(staged);
+        cudaFree(rows64);
+        sc.release();
+    };
+    cudaError_t e = cudaMalloc(&rows64, n * sizeof(double4));
+    if (e != cudaSuccess) { cleanup(); free_catalog(c); return cuda_fail(ctx, e, "cudaMalloc rows"); }
+    s = alloc_sort_scratch(ctx, sc, n);
+    if (s) { cleanup(); free_catalog(c); return s; }
     const void* src = radec_deg;
     if (!on_device) {
-        CU(cudaMalloc(&staged, n * 2 * esz), "cudaMalloc staging");
-        cudaError_t e = cudaMemcpyAsync(staged, radec_deg, n * 2 * esz, cudaMemcpyHostToDevice, st);
-        if (e != cudaSuccess) {
-            cudaFree(staged);
-            return cuda_fail(ctx, e, "copy catalog to device");
-        }
+        e = cudaMalloc(&staged, n * 2 * esz);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(staged, radec_deg, n * 2 * esz, cudaMemcpyHostToDevice, st);
+        if (e != cudaSuccess) { cleanup(); free_catalog(c); return cuda_fail(ctx, e, "copy catalog to device"); }
         src = staged;
     }
-    cudaError_t e = cudaMemsetAsync(ctx->d_bad, 0, sizeof(int), st);
-    if (e == cudaSuccess) e = launch_convert(src, dt == TPCF_F64, n, n_pad, c.x64, c.x32, ctx->d_bad, st);
+    // convert (fp64 unit vectors + Hilbert keys) -> sort -> sorted fp64/fp32 rows + row map -> subtile spheres
+    e = cudaMemsetAsync(ctx->d_bad, 0, sizeof(int), st);
+    if (e == cudaSuccess) e = launch_convert(src, dt == TPCF_F64, n, rows64, sc.ka, sc.ia, ctx->d_bad, st);
+    bool in_a = true;
+    if (e == cudaSuccess) e = launch_sort_pairs(sc.ka, sc.kb, sc.ia, sc.ib, sc.counts, (uint32_t)n, 63, st, &in_a);
+    if (e == cudaSuccess) e = launch_permute(rows64, in_a ? sc.ia : sc.ib, n, n_pad, c.x64, c.x32, c.inv, st);
+    if (e == cudaSuccess) e = launch_spheres(c.x64, n_pad, c.sph, st);
     int bad = 0;
     if (e == cudaSuccess) e = cudaMemcpyAsync(&bad, ctx->d_bad, sizeof(int), cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-    if (staged) cudaFree(staged);
+    cleanup();
     if (e != cudaSuccess) {
         free_catalog(c);
         return cuda_fail(ctx, e, "convert catalog");
@@ -386,14 +461,14 @@ tpcf_status tpcf_count(tpcf_ctx* ctx, tpcf_kind kind, uint64_t* hist_out, uint64
     uint64_t pairs = 0;
     cudaStream_t st = ctx->stream;
     const int nb = ctx->bin.nbins;
-    std::vector<unsigned long long> host(nb + 2), ctr(4);
+    std::vector<unsigned long long> host(nb + 2), ctr(kNumCounters);
     cudaError_t e = cudaEventRecord(ctx->ev0, st);
     s = (e == cudaSuccess) ? enqueue_count(ctx, kind, rows, nrows, ctx->d_out, &tmp64, &tmp32, &tmp_rows, &pairs)
                            : cuda_fail(ctx, e, "cudaEventRecord");
     if (s == TPCF_OK) {
         e = cudaEventRecord(ctx->ev1, st);
         if (e == cudaSuccess) e = cudaMemcpyAsync(host.data(), ctx->d_out, (nb + 2) * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st);
-        if (e == cudaSuccess) e = cudaMemcpyAsync(ctr.data(), ctx->d_counters, 4 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(ctr.data(), ctx->d_counters, kNumCounters * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st);
         if (e == cudaSuccess) e = cudaStreamSynchronize(st);
         if (e != cudaSuccess) s = cuda_fail(ctx, e, "pair count");
     }
@@ -407,6 +482,7 @@ tpcf_status tpcf_count(tpcf_ctx* ctx, tpcf_kind kind, uint64_t* hist_out, uint64
     ctx->stats.pairs = pairs;
     ctx->stats.rechecked = ctr[1];
     ctx->stats.work_items = ctr[2];
+    for (int k = 0; k < 5; ++k) ctx->stats.win_blocks[k] = ctr[3 + k];
     for (int k = 0; k < nb; ++k) hist_out[k] = host[k + 1];
     if (under_over_out) {
         under_over_out[0] = host[0];
@@ -452,6 +528,10 @@ void tpcf_destroy(tpcf_ctx* ctx) {
             if (pc.d_row_start) cudaFree(pc.d_row_start);
         cudaFree(ctx->d_lut);
         cudaFree(ctx->d_slotmap);
+        cudaFree(ctx->d_band_mh);
+        cudaFree(ctx->d_band_lh);
+        cudaFree(ctx->d_band_slot);
+        cudaFree(ctx->d_cell_band);
         cudaFree(ctx->d_thr);
         cudaFree(ctx->d_result);
         cudaFree(ctx->d_out);
@@ -480,6 +560,12 @@ tpcf_status tpcf_set_engine(tpcf_ctx* ctx, tpcf_engine e) {
     if (!ctx) return TPCF_EINVAL;
     if (e != TPCF_ENGINE_FAST && e != TPCF_ENGINE_EXACT64) return fail(ctx, TPCF_EINVAL, "unknown engine");
     ctx->engine = e;
+    return TPCF_OK;
+}
+
+tpcf_status tpcf_set_window(tpcf_ctx* ctx, int enabled) {
+    if (!ctx) return TPCF_EINVAL;
+    ctx->window = enabled != 0;
     return TPCF_OK;
 }
 
@@ -532,6 +618,26 @@ tpcf_status tpcf_classify_fast(const tpcf_ctx* ctx, float d2, int* slot_out) {
     if (!ctx || !slot_out) return TPCF_EINVAL;
     if (!(d2 >= 0.0f) || !(d2 < 64.0f)) return TPCF_EINVAL;
     *slot_out = ctx->ft.classify(d2);
+    return TPCF_OK;
+}
+
+tpcf_status tpcf_window_host(const tpcf_ctx* ctx, float lo2, float hi2, int* first_band_out, int* n_edges_out) {
+    if (!ctx || !first_band_out || !n_edges_out) return TPCF_EINVAL;
+    if (!(lo2 >= 0.0f) || !(hi2 >= lo2) || !(hi2 < 64.0f)) return TPCF_EINVAL;
+    ctx->ft.window(lo2, hi2, *first_band_out, *n_edges_out);
+    return TPCF_OK;
+}
+
+tpcf_status tpcf_get_bands(const tpcf_ctx* ctx, int capacity, float* lo_out, float* hi_out, int* slot_below_out, int* n_out) {
+    if (!ctx || !n_out) return TPCF_EINVAL;
+    const FastTables& t = ctx->ft;
+    *n_out = t.nbands;
+    if (capacity < t.nbands) return (lo_out || hi_out || slot_below_out) ? TPCF_EINVAL : TPCF_OK;
+    for (int b = 0; b < t.nbands; ++b) {
+        if (lo_out) lo_out[b] = t.band_lo[b];
+        if (hi_out) hi_out[b] = t.band_hi[b];
+        if (slot_below_out) slot_below_out[b] = t.band_slot[b];
+    }
     return TPCF_OK;
 }
 

@@ -24,22 +24,48 @@ struct PairParams {
     const uint16_t* slotmap;    // 2 x ncells: result slot of (cell, d2 < lo) and (cell, d2 >= hi)
     int ncells, shift;
     float sqrt_scale, sqrt_clamp;
+    // window path: bounding spheres of every kSubJ consecutive j rows and the guard bands
+    const float4* sph_j;        // n_j_pad / kSubJ x (cx, cy, cz, r); nullptr switches the window path off
+    const float2* band_mh;      // nbands x (mid, half width)
+    const float2* band_lh;      // nbands x (lo, hi)
+    const uint16_t* band_slot;  // nbands + 1 result slots: below band b; [nbands] = above the last band
+    const uint16_t* cell_band;  // ncells: first band whose hi lies above the start of the cell
+    int nbands;
     // exact thresholds
     const double* thr;          // nbins + 1
     int nbins;
     unsigned long long* result; // nbins + 3: under, bins, over, discard
-    unsigned long long* counters;   // [0] next work item, [1] pairs rechecked in fp64, [2] items done
+    // [0] next work item, [1] pairs rechecked in fp64, [2] items done,
+    // [3..6] (warp, subtile) blocks counted by the 1-, 2-, 3-edge window loops and by the cell-lookup loop,
+    // [7] lanes of window blocks recounted because a pair came within a guard band
+    unsigned long long* counters;
 };
 
 struct LaunchInfo {
     int grid, block, smem_bytes, launches;
 };
 
-cudaError_t launch_convert(const void* radec, int is_f64, uint64_t n, uint64_t n_pad, double4* x64, float4* x32,
+constexpr int kNumCounters = 8;
+constexpr int kSortChunk = 2048;        // elements per block of the radix sort
+
+// RA/Dec rows -> fp64 unit vectors (caller order) + 63-bit Hilbert keys + identity index
+cudaError_t launch_convert(const void* radec, int is_f64, uint64_t n, double4* x64_rows, uint64_t* keys, uint32_t* idx,
                            int* bad_flag, cudaStream_t st);
-cudaError_t launch_gather(const double4* src64, const float4* src32, const int64_t* rows, uint64_t nrows,
-                          uint64_t nrows_pad, uint64_t n_src, double4* dst64, float4* dst32, int* bad_flag,
-                          cudaStream_t st);
+// Stable LSD radix sort of (key, idx) pairs on the low `nbits` bits; buffers A hold the input, the sorted
+// result ends in A or B (*in_a).  counts: 256 * ceil(n / kSortChunk) words of scratch.
+cudaError_t launch_sort_pairs(uint64_t* keys_a, uint64_t* keys_b, uint32_t* idx_a, uint32_t* idx_b, uint32_t* counts,
+                              uint32_t n, int nbits, cudaStream_t st, bool* in_a);
+// sorted catalog: x64[k] = rows[order[k]], x32 = its rounding, inv[order[k]] = k; rows n..n_pad-1 = padding point
+cudaError_t launch_permute(const double4* x64_rows, const uint32_t* order, uint64_t n, uint64_t n_pad, double4* x64,
+                           float4* x32, uint32_t* inv, cudaStream_t st);
+// bounding sphere of every kSubJ consecutive rows of a padded catalog
+cudaError_t launch_spheres(const double4* x64, uint64_t n_pad, float4* sph, cudaStream_t st);
+// subset mode: caller rows -> positions in the sorted catalog (keys for the sort) with range check
+cudaError_t launch_row_keys(const int64_t* rows, uint64_t nrows, uint64_t n_src, const uint32_t* inv, uint64_t* keys,
+                            uint32_t* idx, int* bad_flag, cudaStream_t st);
+// dst[k] = src[pos[k]] for k < nrows, padding point after
+cudaError_t launch_gather(const double4* src64, const float4* src32, const uint64_t* pos, uint64_t nrows,
+                          uint64_t nrows_pad, double4* dst64, float4* dst32, cudaStream_t st);
 cudaError_t launch_pairs_fast(const PairParams& p, CellMap map, int sm_count, cudaStream_t st, LaunchInfo* info);
 cudaError_t launch_pairs_exact64(const PairParams& p, int sm_count, cudaStream_t st, LaunchInfo* info);
 // result[0 .. nbins+1] -> out (device), subtracting `self_pairs` from the slot that holds theta = 0

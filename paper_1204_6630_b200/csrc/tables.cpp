@@ -108,6 +108,18 @@ int FastTables::classify(float d2) const {
     return p0 ? slot1[c] : slot0[c];
 }
 
+void FastTables::window(float lo2, float hi2, int& first_band, int& n_edges) const {
+    int c = cell_of(lo2);
+    if (c < 0) c = 0;
+    if (c >= ncells) c = ncells - 1;
+    int k = cell_band[c];
+    while (k < nbands && band_hi[k] <= lo2) ++k;
+    int e = 1;
+    while (e <= kMaxWinEdges && k + e < nbands && band_lo[k + e] <= hi2) ++e;
+    first_band = k;
+    n_edges = e;
+}
+
 namespace {
 struct Band {
     float lo, hi;
@@ -133,17 +145,20 @@ int fill(FastTables& t, const std::vector<Band>& bands, int lowest_slot) {
     t.hi.assign(t.ncells, inf);
     t.slot0.assign(t.ncells, 0);
     t.slot1.assign(t.ncells, 0);
+    t.cell_band.assign(t.ncells, 0);
     int bad = 0;
     size_t first = 0;                       // first band with hi > start of this cell
     for (int c = 0; c < t.ncells; ++c) {
         uint32_t b0 = first_bits_of_cell(t, c), b1 = first_bits_of_cell(t, c + 1);
         if (b1 == b0) {                     // empty cell (SqrtLin can skip indices): never addressed
             t.slot0[c] = t.slot1[c] = (uint16_t)lowest_slot;
+            t.cell_band[c] = (uint16_t)first;
             continue;
         }
         float f0 = (c == 0) ? 0.0f : u2f(b0);
         float f1 = (b1 > kTopBits) ? inf : u2f(b1);
         while (first < bands.size() && bands[first].hi <= f0) ++first;   // bands wholly below this cell
+        t.cell_band[c] = (uint16_t)first;
         // bands [first, last) intersect [f0, f1)
         size_t last = first;
         while (last < bands.size() && bands[last].lo < f1) ++last;
@@ -164,10 +179,38 @@ int fill(FastTables& t, const std::vector<Band>& bands, int lowest_slot) {
 }
 }  // namespace
 
+static void export_bands(const std::vector<Band>& bands, FastTables& t) {
+    t.nbands = (int)bands.size();
+    t.band_lo.resize(t.nbands);
+    t.band_hi.resize(t.nbands);
+    t.band_mid.resize(t.nbands);
+    t.band_half.resize(t.nbands);
+    t.band_slot.resize((size_t)t.nbands + 1);
+    for (int k = 0; k < t.nbands; ++k) {
+        const float lo = bands[k].lo, hi = bands[k].hi;
+        const float mid = (float)(0.5 * ((double)lo + (double)hi));
+        // [mid - half, mid + half] covers [lo, hi] whatever the rounding of mid
+        const float half = float_up(std::max((double)hi - (double)mid, (double)mid - (double)lo));
+        t.band_lo[k] = lo;
+        t.band_hi[k] = hi;
+        t.band_mid[k] = mid;
+        t.band_half[k] = half;
+        t.band_slot[k] = (uint16_t)bands[k].below;   // == bands[k-1].above: the bands chain
+    }
+    t.band_slot[t.nbands] = (uint16_t)bands.back().above;
+}
+
+static void build_fast_tables_impl(const Binning& b, double gs, FastTables& out, std::vector<Band>& bands);
+
 void build_fast_tables(const Binning& b, double gs, FastTables& out) {
+    std::vector<Band> bands;
+    build_fast_tables_impl(b, gs, out, bands);
+    export_bands(bands, out);
+}
+
+static void build_fast_tables_impl(const Binning& b, double gs, FastTables& out, std::vector<Band>& bands) {
     const int n = b.nbins;
     int overlapping = 0;
-    std::vector<Band> bands;
     for (int k = 0; k <= n; ++k) {
         if ((k == 0 && b.drop_first) || (k == n && b.drop_last)) continue;
         double T = b.thr[k], g = guard_width(T, gs);

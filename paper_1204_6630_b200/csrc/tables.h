@@ -17,6 +17,8 @@ constexpr int kPlanSMs = 148;          // B200 SM count the plan balances for
 constexpr float kPadCoord = 2.0f;      // padding rows are (2,2,2): 6.07 <= d2 <= 19.9 against any unit vector
 constexpr float kDiscardFrom = 5.0f;   // d2 >= 5 can only involve a padding row
 constexpr int kMaxCells = 8192;
+constexpr int kSubJ = 32;              // j-points per window subtile (one bounding sphere each)
+constexpr int kMaxWinEdges = 3;        // a (lane, subtile) window that sees more guard bands goes to the cell-lookup path
 
 enum class CellMap : int { LogBits = 0, SqrtLin = 1 };
 
@@ -30,8 +32,19 @@ struct FastTables {
     int merged_bands = 0;           // guard bands that had to be merged because they shared a cell (0 normally)
     std::vector<float> lo, hi;      // per cell: below lo -> slot0, [lo, hi) -> ambiguous, >= hi -> slot1
     std::vector<uint16_t> slot0, slot1;
+    // The guard bands themselves, ascending and disjoint (the last one is the zero-width "discard" band at
+    // kDiscardFrom).  The window path of the kernel compares against these directly: a pair whose fp32 squared chord
+    // q satisfies |q - band_mid| > band_half is on the side of the edge its sign shows.
+    int nbands = 0;
+    std::vector<float> band_lo, band_hi, band_mid, band_half;
+    std::vector<uint16_t> band_slot;    // nbands + 1: result slot below band b; [nbands] = slot above the last band
+    std::vector<uint16_t> cell_band;    // per cell: first band whose hi lies above the start of the cell
     int cell_of(float d2) const;    // exactly the kernel's integer arithmetic
     int classify(float d2) const;   // result slot, or -1 when ambiguous
+    // Host mirror of the kernel's window selection: given bounds lo2 <= q <= hi2 on every squared chord of a
+    // (lane, subtile) block, the first band that can matter and how many consecutive bands can (1..kMaxWinEdges,
+    // or kMaxWinEdges + 1 = "too many": cell-lookup path).
+    void window(float lo2, float hi2, int& first_band, int& n_edges) const;
 };
 
 struct Binning {
