@@ -157,9 +157,10 @@ typedef struct {
     int cells, cell_bits;    /* lookup cells of the fast engine and mantissa bits per octave */
     int hist_copies;         /* privatised copies of each partial-histogram slot per CTA */
     float kernel_ms;         /* device time of the last synchronous count (CUDA events) */
-    uint64_t win_blocks[5];  /* (warp, 32-row j-subtile) blocks of the last synchronous count by path: counted by the
-                                1-, 2-, 3-edge window loops, by the per-pair cell lookup; [4] = lanes of window
-                                blocks recounted pair by pair because a pair came within a guard band */
+    uint64_t win_blocks[6];  /* (warp of 128 i-rows, 32-row j-subtile) blocks of the last synchronous count by path:
+                                counted by the 1-, 2-, 3-edge window loops, by the per-pair cell lookup; [4] = lanes of
+                                window blocks recounted pair by pair because a pair came within a guard band;
+                                [5] = blocks classified wholly in fp64 (bounding radii too large for the fp32 bound) */
 } tpcf_stats;
 tpcf_status tpcf_get_stats(const tpcf_ctx* ctx, tpcf_stats* out);
 

@@ -46,7 +46,7 @@ class tpcf_stats(ctypes.Structure):
     _fields_ = [("pairs", ctypes.c_uint64), ("rechecked", ctypes.c_uint64), ("work_items", ctypes.c_uint64),
                 ("launches", ctypes.c_int), ("grid", ctypes.c_int), ("block", ctypes.c_int),
                 ("smem_bytes", ctypes.c_int), ("cells", ctypes.c_int), ("cell_bits", ctypes.c_int),
-                ("hist_copies", ctypes.c_int), ("kernel_ms", ctypes.c_float), ("win_blocks", ctypes.c_uint64 * 5)]
+                ("hist_copies", ctypes.c_int), ("kernel_ms", ctypes.c_float), ("win_blocks", ctypes.c_uint64 * 6)]
 
     def as_dict(self):
         d = {k: getattr(self, k) for k, _ in self._fields_}

@@ -18,9 +18,9 @@ namespace {
 struct Catalog {                 // rows in Hilbert order (counts are order-invariant, reading A16)
     uint64_t n = 0, n_pad = 0;
     double4* x64 = nullptr;
-    float4* x32 = nullptr;
     uint32_t* inv = nullptr;     // caller row -> position in the sorted catalog (row-subset mode)
-    float4* sph = nullptr;       // bounding sphere of every kSubJ consecutive rows
+    float4 *xq = nullptr, *cq = nullptr;   // i-side role: rows as offsets from their 4-row quad centre; (centre, radius)
+    float4 *xs = nullptr, *cs = nullptr;   // j-side role: rows as (-2 offset, |offset|^2) from their 32-row subtile centre
 };
 // scratch of one spatial sort: (key, idx) ping-pong buffers and the digit counts
 struct SortScratch {
@@ -161,9 +161,11 @@ tpcf_status upload_tables(tpcf_ctx* ctx) {
 
 void free_catalog(Catalog& c) {
     cudaFree(c.x64);
-    cudaFree(c.x32);
     cudaFree(c.inv);
-    cudaFree(c.sph);
+    cudaFree(c.xq);
+    cudaFree(c.cq);
+    cudaFree(c.xs);
+    cudaFree(c.cs);
     c = Catalog();
 }
 
@@ -198,7 +200,7 @@ uint32_t items_of_part(uint64_t n_items, int part, int nparts) {
 
 // Enqueue one count on ctx->stream; the nbins+2 result lands in d_out_dev.  rows_dev == nullptr: full count.
 tpcf_status enqueue_count(tpcf_ctx* ctx, tpcf_kind kind, const int64_t* rows_host, size_t nrows, unsigned long long* out_dev,
-                          double4** tmp64, float4** tmp32, int64_t** tmp_rows, uint64_t* pairs_out) {
+                          Catalog* tmp, int64_t** tmp_rows, uint64_t* pairs_out) {
     tpcf_status s = ensure_cuda(ctx);
     if (s) return s;
     if (kind != TPCF_DD && kind != TPCF_DR && kind != TPCF_RR) return fail(ctx, TPCF_EINVAL, "unknown kind");
@@ -224,8 +226,9 @@ tpcf_status enqueue_count(tpcf_ctx* ctx, tpcf_kind kind, const int64_t* rows_hos
         if (nrows > 0x7FFFFFFFull) return fail(ctx, TPCF_EINVAL, "more than 2^31-1 rows");
         const uint64_t np = pad_to(nrows, kTileI);
         CU(cudaMalloc(tmp_rows, nrows * sizeof(int64_t)), "cudaMalloc rows");
-        CU(cudaMalloc(tmp64, np * sizeof(double4)), "cudaMalloc subset");
-        CU(cudaMalloc(tmp32, np * sizeof(float4)), "cudaMalloc subset");
+        CU(cudaMalloc(&tmp->x64, np * sizeof(double4)), "cudaMalloc subset");
+        CU(cudaMalloc(&tmp->xq, np * sizeof(float4)), "cudaMalloc subset");
+        CU(cudaMalloc(&tmp->cq, np / kIPerThread * sizeof(float4)), "cudaMalloc subset");
         SortScratch sc;
         tpcf_status ss = alloc_sort_scratch(ctx, sc, nrows);
         if (ss) { sc.release(); return ss; }
@@ -236,7 +239,8 @@ tpcf_status enqueue_count(tpcf_ctx* ctx, tpcf_kind kind, const int64_t* rows_hos
         if (e == cudaSuccess) e = launch_row_keys(*tmp_rows, nrows, ci.n, ci.inv, sc.ka, sc.ia, ctx->d_bad, st);
         bool in_a = true;
         if (e == cudaSuccess) e = launch_sort_pairs(sc.ka, sc.kb, sc.ia, sc.ib, sc.counts, (uint32_t)nrows, 32, st, &in_a);
-        if (e == cudaSuccess) e = launch_gather(ci.x64, ci.x32, in_a ? sc.ka : sc.kb, nrows, np, *tmp64, *tmp32, st);
+        if (e == cudaSuccess) e = launch_gather(ci.x64, in_a ? sc.ka : sc.kb, nrows, np, tmp->x64, st);
+        if (e == cudaSuccess) e = launch_quads(tmp->x64, np, tmp->xq, tmp->cq, st);
         int bad = 0;
         if (e == cudaSuccess) e = cudaMemcpyAsync(&bad, ctx->d_bad, sizeof(int), cudaMemcpyDeviceToHost, st);
         if (e == cudaSuccess) e = cudaStreamSynchronize(st);
@@ -245,8 +249,9 @@ tpcf_status enqueue_count(tpcf_ctx* ctx, tpcf_kind kind, const int64_t* rows_hos
         if (bad) return fail(ctx, TPCF_EINVAL, "row index out of range");
         make_plan(false, nrows, cj.n, subset_plan);
         plan = &subset_plan;
-        p.xi = *tmp32;
-        p.xi64 = *tmp64;
+        p.xq = tmp->xq;
+        p.cq = tmp->cq;
+        p.xi64 = tmp->x64;
         p.n_i = (uint32_t)nrows;
         p.tri = 0;
         if (sd.tri) self_pairs = nrows;      // each listed row meets itself once at theta = 0: remove it
@@ -266,13 +271,15 @@ tpcf_status enqueue_count(tpcf_ctx* ctx, tpcf_kind kind, const int64_t* rows_hos
         }
         plan = &pc.plan;
         d_row_start = pc.d_row_start;
-        p.xi = ci.x32;
+        p.xq = ci.xq;
+        p.cq = ci.cq;
         p.xi64 = ci.x64;
         p.n_i = (uint32_t)ci.n;
         p.tri = sd.tri ? 1 : 0;
         ctx->stats.launches = 0;
     }
-    p.xj = cj.x32;
+    p.xs = cj.xs;
+    p.cs = cj.cs;
     p.xj64 = cj.x64;
     p.n_j = (uint32_t)cj.n;
     p.blocks_i = plan->blocks_i;
@@ -285,7 +292,7 @@ tpcf_status enqueue_count(tpcf_ctx* ctx, tpcf_kind kind, const int64_t* rows_hos
     p.nparts = (uint32_t)ctx->nparts;
     p.lut = ctx->d_lut;
     p.slotmap = ctx->d_slotmap;
-    p.sph_j = (ctx->window && ctx->ft.nbands >= 1) ? cj.sph : nullptr;
+    p.window = (ctx->window && ctx->ft.nbands >= 1) ? 1 : 0;
     p.band_mh = ctx->d_band_mh;
     p.band_lh = ctx->d_band_lh;
     p.band_slot = ctx->d_band_slot;
@@ -402,9 +409,11 @@ tpcf_status tpcf_load(tpcf_ctx* ctx, tpcf_cat which, const void* radec_deg, tpcf
     const uint64_t n_pad = pad_to(n, kTileI);
     const size_t esz = (dt == TPCF_F64) ? 8 : 4;
     CU(cudaMalloc(&c.x64, n_pad * sizeof(double4)), "cudaMalloc catalog (fp64)");
-    CU(cudaMalloc(&c.x32, n_pad * sizeof(float4)), "cudaMalloc catalog (fp32)");
     CU(cudaMalloc(&c.inv, n * sizeof(uint32_t)), "cudaMalloc catalog (row map)");
-    CU(cudaMalloc(&c.sph, n_pad / kSubJ * sizeof(float4)), "cudaMalloc catalog (spheres)");
+    CU(cudaMalloc(&c.xq, n_pad * sizeof(float4)), "cudaMalloc catalog (quad offsets)");
+    CU(cudaMalloc(&c.cq, n_pad / kIPerThread * sizeof(float4)), "cudaMalloc catalog (quad centres)");
+    CU(cudaMalloc(&c.xs, n_pad * sizeof(float4)), "cudaMalloc catalog (subtile offsets)");
+    CU(cudaMalloc(&c.cs, n_pad / kSubJ * sizeof(float4)), "cudaMalloc catalog (subtile centres)");
     void* staged = nullptr;
     double4* rows64 = nullptr;
     SortScratch sc;
@@ -424,13 +433,14 @@ tpcf_status tpcf_load(tpcf_ctx* ctx, tpcf_cat which, const void* radec_deg, tpcf
         if (e != cudaSuccess) { cleanup(); free_catalog(c); return cuda_fail(ctx, e, "copy catalog to device"); }
         src = staged;
     }
-    // convert (fp64 unit vectors + Hilbert keys) -> sort -> sorted fp64/fp32 rows + row map -> subtile spheres
+    // convert (fp64 unit vectors + Hilbert keys) -> sort -> sorted fp64 rows + row map -> quad and subtile roles
     e = cudaMemsetAsync(ctx->d_bad, 0, sizeof(int), st);
     if (e == cudaSuccess) e = launch_convert(src, dt == TPCF_F64, n, rows64, sc.ka, sc.ia, ctx->d_bad, st);
     bool in_a = true;
     if (e == cudaSuccess) e = launch_sort_pairs(sc.ka, sc.kb, sc.ia, sc.ib, sc.counts, (uint32_t)n, 63, st, &in_a);
-    if (e == cudaSuccess) e = launch_permute(rows64, in_a ? sc.ia : sc.ib, n, n_pad, c.x64, c.x32, c.inv, st);
-    if (e == cudaSuccess) e = launch_spheres(c.x64, n_pad, c.sph, st);
+    if (e == cudaSuccess) e = launch_permute(rows64, in_a ? sc.ia : sc.ib, n, n_pad, c.x64, c.inv, st);
+    if (e == cudaSuccess) e = launch_quads(c.x64, n_pad, c.xq, c.cq, st);
+    if (e == cudaSuccess) e = launch_subtiles(c.x64, n_pad, c.xs, c.cs, st);
     int bad = 0;
     if (e == cudaSuccess) e = cudaMemcpyAsync(&bad, ctx->d_bad, sizeof(int), cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
@@ -455,15 +465,14 @@ tpcf_status tpcf_count(tpcf_ctx* ctx, tpcf_kind kind, uint64_t* hist_out, uint64
     if (!rows && nrows) return fail(ctx, TPCF_EINVAL, "nrows != 0 with rows == NULL");
     tpcf_status s = ensure_cuda(ctx);
     if (s) return s;
-    double4* tmp64 = nullptr;
-    float4* tmp32 = nullptr;
+    Catalog tmp;                 // row-subset mode: the listed rows as a temporary i-side catalog
     int64_t* tmp_rows = nullptr;
     uint64_t pairs = 0;
     cudaStream_t st = ctx->stream;
     const int nb = ctx->bin.nbins;
     std::vector<unsigned long long> host(nb + 2), ctr(kNumCounters);
     cudaError_t e = cudaEventRecord(ctx->ev0, st);
-    s = (e == cudaSuccess) ? enqueue_count(ctx, kind, rows, nrows, ctx->d_out, &tmp64, &tmp32, &tmp_rows, &pairs)
+    s = (e == cudaSuccess) ? enqueue_count(ctx, kind, rows, nrows, ctx->d_out, &tmp, &tmp_rows, &pairs)
                            : cuda_fail(ctx, e, "cudaEventRecord");
     if (s == TPCF_OK) {
         e = cudaEventRecord(ctx->ev1, st);
@@ -472,8 +481,7 @@ tpcf_status tpcf_count(tpcf_ctx* ctx, tpcf_kind kind, uint64_t* hist_out, uint64
         if (e == cudaSuccess) e = cudaStreamSynchronize(st);
         if (e != cudaSuccess) s = cuda_fail(ctx, e, "pair count");
     }
-    if (tmp64) cudaFree(tmp64);
-    if (tmp32) cudaFree(tmp32);
+    free_catalog(tmp);
     if (tmp_rows) cudaFree(tmp_rows);
     if (s) return s;
     float ms = 0.f;
@@ -481,8 +489,9 @@ tpcf_status tpcf_count(tpcf_ctx* ctx, tpcf_kind kind, uint64_t* hist_out, uint64
     ctx->stats.kernel_ms = ms;
     ctx->stats.pairs = pairs;
     ctx->stats.rechecked = ctr[1];
-    ctx->stats.work_items = ctr[2];
-    for (int k = 0; k < 5; ++k) ctx->stats.win_blocks[k] = ctr[3 + k];
+    // the fast engine executes every plan item as kWarpsPerCta warp items
+    ctx->stats.work_items = (ctx->engine == TPCF_ENGINE_FAST) ? ctr[2] / kWarpsPerCta : ctr[2];
+    for (int k = 0; k < 6; ++k) ctx->stats.win_blocks[k] = ctr[3 + k];
     for (int k = 0; k < nb; ++k) hist_out[k] = host[k + 1];
     if (under_over_out) {
         under_over_out[0] = host[0];
@@ -498,8 +507,7 @@ tpcf_status tpcf_count(tpcf_ctx* ctx, tpcf_kind kind, uint64_t* hist_out, uint64
 tpcf_status tpcf_count_async(tpcf_ctx* ctx, tpcf_kind kind, uint64_t* hist_dev) {
     if (!ctx) return TPCF_EINVAL;
     if (!hist_dev) return fail(ctx, TPCF_EINVAL, "hist_dev is NULL");
-    return enqueue_count(ctx, kind, nullptr, 0, reinterpret_cast<unsigned long long*>(hist_dev), nullptr, nullptr, nullptr,
-                         nullptr);
+    return enqueue_count(ctx, kind, nullptr, 0, reinterpret_cast<unsigned long long*>(hist_dev), nullptr, nullptr, nullptr);
 }
 
 tpcf_status tpcf_estimate_from(const uint64_t* dd, const uint64_t* dr, const uint64_t* rr, int nbins, uint64_t n_d,

@@ -1,6 +1,6 @@
 // kernels.cu -- sm_100a kernels of libtpcf.
 //
-//   convert_kernel      RA/Dec (deg) -> fp64 unit vector + Hilbert key                  (hot-path step a1)
+//   convert_kernel      RA/Dec (deg) -> fp64 unit vector + sort key                     (hot-path step a1)
 //   radix_* / permute / spheres   spatial sort of the catalog, fp32 copy, subtile bounding spheres (a1)
 //   pair_fast_kernel    the all-pairs count: fp32 squared chord; per (lane, 32-row j-subtile) window of
 //                       candidate bin edges from bounding spheres -> 1..3 threshold compares per pair with
@@ -19,8 +19,6 @@ namespace tpcf {
 namespace {
 
 constexpr int R = kIPerThread;
-constexpr int NBUF = 2;                               // j-tile buffers in shared memory
-constexpr uint32_t kTileBytes = kTileJ * sizeof(float4);
 constexpr uint32_t kSqrtMagic = 0x1FBD1DF5u;
 constexpr unsigned long long kFlushPairs = 3500000000ull;   // flush 32-bit partial counters before they can wrap
 
@@ -68,25 +66,441 @@ __device__ __forceinline__ int exact_slot_dev(double d2, const double* __restric
     return lo + 1;
 }
 
-struct SlowCtx {
+struct SlowCtx {                     // lives in shared memory
     const double4* xi64;
     const double4* xj64;
     const double* thr;
-    unsigned long long* result;
-    unsigned long long* rechecked;
+    unsigned* whist;                 // the CTA's partial histogram indexed by result slot (shared memory)
+    unsigned nrecheck;               // pairs classified in fp64 since the last flush
     int nbins;
 };
 
 // A pair whose fp32 squared chord fell inside the guard band of a bin edge: classify it from the fp64
-// coordinates.  Rare (1e-6 .. 1e-3 of the pairs), so it goes straight to the global histogram.
-__device__ __noinline__ void recheck_pair(const SlowCtx* s, uint32_t i, uint32_t j) {
+// coordinates.  Rare (1e-6 .. 1e-3 of the pairs).
+__device__ __noinline__ void recheck_pair(SlowCtx* s, uint32_t i, uint32_t j) {
     const double4 a = s->xi64[i], b = s->xj64[j];
     const int slot = exact_slot_dev(chord2_f64(a, b), s->thr, s->nbins);
-    atomicAdd(s->result + slot, 1ull);
-    atomicAdd(s->rechecked, 1ull);
+    atomicAdd(s->whist + slot, 1u);
+    atomicAdd(&s->nrecheck, 1u);
 }
 
 // ---- work items -----------------------------------------------------------------------------------------
+template <int MAP>
+__device__ __forceinline__ uint32_t cell_byte_offset(float d2, int shift, float scale, float clamp) {
+    if (MAP == (int)CellMap::LogBits) {
+        return (__float_as_uint(d2) >> (shift - 3)) & ~7u;
+    } else {
+        const float c = fminf(d2, clamp);
+        const float key = __uint_as_float((__float_as_uint(c) >> 1) + kSqrtMagic);
+        const float t = fmaf(key, scale, 8388608.0f);
+        return (__float_as_uint(t) << 3) & 0x3FFFFF8u;
+    }
+}
+
+// ---- coordinates ------------------------------------------------------------------------------------------------
+// Inside a (lane, subtile) block both points are taken relative to the subtile centre cs:
+//   s  = a' + (cq - cs)      the lane's i-point (a' = offset from its quad centre cq), formed per subtile in fp32
+//   b' = offset of the j-point from cs, stored as (-2 b', |b'|^2)
+// so |a - b|^2 = |s - b'|^2 = |s|^2 + |b'|^2 - 2 s.b'.  Every rounding is relative to |s| ~ chord or to the radii:
+// nothing is lost against the unit length of the vectors, which is what lets fp32 resolve the 0.01-degree bins.
+
+// ---- per-pair cell-lookup path ("lookup" path) ---------------------------------------------------------------
+// One pair: fp32 squared chord (difference form) -> cell -> (lo, hi) of the cell's guard band -> shared-memory
+// partial histogram, or the fp64 recheck when lo <= d2 < hi.
+template <int MAP>
+__device__ __forceinline__ void lookup_pair(float sx, float sy, float sz, const float4& b, const char* lut, char* hist,
+                                            SlowCtx* slow, uint32_t i, uint32_t j, bool valid, int shift,
+                                            float scale, float clamp) {
+    const float dx = fmaf(b.x, 0.5f, sx), dy = fmaf(b.y, 0.5f, sy), dz = fmaf(b.z, 0.5f, sz);     // s - b', one rounding each
+    const float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+    const uint32_t q8 = cell_byte_offset<MAP>(d2, shift, scale, clamp);
+    const float2 lh = *reinterpret_cast<const float2*>(lut + q8);
+    const bool above = d2 >= lh.x;
+    const bool amb = above && (d2 < lh.y);
+    if (amb) {
+        if (valid) recheck_pair(slow, i, j);
+    } else if (valid) {
+        atomicAdd(reinterpret_cast<unsigned*>(hist + q8) + (above ? 1 : 0), 1u);
+    }
+}
+
+// One subtile against this lane's R points, every pair by cell lookup.  MASK: only pairs j > i (diagonal chunk).
+template <int MAP, bool MASK>
+__device__ __forceinline__ void lookup_block(const float4* __restrict__ js, const float (&sx)[R], const float (&sy)[R],
+                                             const float (&sz)[R], const char* lut, char* hist, SlowCtx* slow,
+                                             uint32_t i0, uint32_t j0, int shift, float scale, float clamp) {
+#pragma unroll 2
+    for (int jj = 0; jj < kSubJ; ++jj) {
+        const float4 b = js[jj];                                  // one LDS.128, broadcast to the warp
+#pragma unroll
+        for (int r = 0; r < R; ++r)
+            lookup_pair<MAP>(sx[r], sy[r], sz[r], b, lut, hist, slow, i0 + r, j0 + jj, !MASK || (j0 + jj > i0 + r), shift, scale,
+                             clamp);
+    }
+}
+
+// Blocks whose bounding radii are too large for the fp32 error bound (sparse or tiny catalogs, blocks that contain
+// padding rows): every real pair is classified from the fp64 coordinates.
+__device__ __noinline__ void exact_block(SlowCtx* s, uint32_t i0, uint32_t n_i, uint32_t j0, uint32_t n_j, bool mask) {
+    for (int r = 0; r < R; ++r) {
+        const uint32_t i = i0 + r;
+        if (i >= n_i) continue;
+        for (int jj = 0; jj < kSubJ; ++jj) {
+            const uint32_t j = j0 + jj;
+            if (j >= n_j || (mask && j <= i)) continue;
+            recheck_pair(s, i, j);
+        }
+    }
+}
+
+// ---- window path ----------------------------------------------------------------------------------------------
+// The E-edge window loop over one subtile.  q = |s|^2 - mid_0 + |b'|^2 - 2 s.b' (4 FMA-pipe instructions); for each
+// of the bands k .. k+E-1 the sign bit of q + (mid_0 - mid_e) is accumulated (one LEA.HI) and the smallest
+// |q - ...| is tracked (FMNMX3, two values per instruction).  Returns true when some pair came within a band's half
+// width: this lane's counters are then not used and its pairs are recounted one by one.
+template <int E>
+__device__ __forceinline__ bool window_block(const float4* __restrict__ js, const float (&sx)[R], const float (&sy)[R],
+                                             const float (&sz)[R], const float (&nsm)[R] /* |s|^2 - mid_0 */,
+                                             const float (&dt)[kMaxWinEdges], float hmax, unsigned (&c)[kMaxWinEdges]) {
+#pragma unroll
+    for (int e = 0; e < kMaxWinEdges; ++e) c[e] = 0;
+    float m = 3.0e38f;
+#pragma unroll 8
+    for (int jj = 0; jj < kSubJ; ++jj) {
+        const float4 b = js[jj];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const float q = __fmaf_rn(sx[r], b.x, __fmaf_rn(sy[r], b.y, __fmaf_rn(sz[r], b.z, __fadd_rn(nsm[r], b.w))));
+#pragma unroll
+            for (int e = 0; e < E; ++e) {
+                const float qe = e ? __fadd_rn(q, dt[e]) : q;
+                c[e] += __float_as_uint(qe) >> 31;
+                m = fminf(m, fabsf(qe));
+            }
+        }
+    }
+    return m <= hmax;
+}
+
+struct WinTables {
+    const float2* band_mh;
+    const float2* band_lh;
+    const uint16_t* band_slot;
+    const uint16_t* cell_band;
+    unsigned* whist;            // partial histogram indexed by result slot
+    int nbands;
+};
+
+// One subtile (kSubJ rows at js, bounding sphere sp) against this lane's quad (offsets p*, centre cq*, radius ri).
+// Every lane chooses the cheapest loop that is valid for its block; the warp runs the most general of them.
+//   1..3  window loop with that many edges      4  cell lookup      5  fp64
+template <int MAP>
+__device__ __forceinline__ void subtile_pairs(const float4* __restrict__ js, const float4 sp, bool windows, bool mask,
+                                              const float (&px)[R], const float (&py)[R], const float (&pz)[R], float cqx,
+                                              float cqy, float cqz, float ri, const WinTables& wt, const char* lut,
+                                              char* hist, SlowCtx* slow, uint32_t i0, uint32_t n_i, uint32_t j0,
+                                              uint32_t n_j, int shift, float scale, float clamp, unsigned (&npath)[6]) {
+    const int lane = threadIdx.x & 31;
+    // bounds on every TRUE chord of the block from the triangle inequality: |cq - cs| -/+ (ri + rj), made safe
+    // against the fp32 evaluation (relative 4e-6 on the centre distance, 1e-7 absolute)
+    const float tx = __fsub_rn(cqx, sp.x), ty = __fsub_rn(cqy, sp.y), tz = __fsub_rn(cqz, sp.z);
+    const float dc2 = fmaf(tz, tz, fmaf(ty, ty, tx * tx));
+    float dc;
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(dc) : "f"(dc2));
+    const float rs = ri + sp.w;
+    const float lo = fmaf(dc, 1.0f - 4.0e-6f, -rs) - 1.0e-7f;
+    const float hi = fmaf(dc, 1.0f + 4.0e-6f, rs) + 1.0e-7f;
+    int mode = 4, k = 0;
+    if (rs > kRCap) {
+        mode = 5;
+    } else if (windows && !mask && lo >= kFarKappa * rs) {
+        const float lo2 = __fmul_rd(lo, lo), hi2 = __fmul_ru(hi, hi);
+        // first band that is not wholly below the window, then how many bands the window reaches
+        k = wt.cell_band[cell_byte_offset<MAP>(lo2, shift, scale, clamp) >> 3];
+        while (k < wt.nbands && wt.band_lh[k].y <= lo2) ++k;
+        int e = 1;
+        while (e <= kMaxWinEdges && k + e < wt.nbands && wt.band_lh[k + e].x <= hi2) ++e;
+        mode = e;
+    }
+    const int wmode = __reduce_max_sync(0xffffffffu, mode);
+
+    float sx[R], sy[R], sz[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        sx[r] = __fadd_rn(px[r], tx);
+        sy[r] = __fadd_rn(py[r], ty);
+        sz[r] = __fadd_rn(pz[r], tz);
+    }
+    if (wmode > kMaxWinEdges) {
+        if (mode == 5) {
+            exact_block(slow, i0, n_i, j0, n_j, mask);
+        } else if (mask) {
+            lookup_block<MAP, true>(js, sx, sy, sz, lut, hist, slow, i0, j0, shift, scale, clamp);
+        } else {
+            lookup_block<MAP, false>(js, sx, sy, sz, lut, hist, slow, i0, j0, shift, scale, clamp);
+        }
+        ++npath[wmode == 5 ? 5 : 3];
+        return;
+    }
+    // every lane runs the wmode-edge loop on bands k .. k+wmode-1; lowering k keeps the lane's window inside them
+    k = min(k, wt.nbands - wmode);
+    const float2 mh0 = wt.band_mh[k];
+    float hmax = mh0.y, dt[kMaxWinEdges], nsm[R];
+    dt[0] = 0.f;
+#pragma unroll
+    for (int e = 1; e < kMaxWinEdges; ++e) {
+        dt[e] = 0.f;
+        if (e < wmode) {
+            const float2 mh = wt.band_mh[k + e];
+            dt[e] = __fsub_rn(mh0.x, mh.x);
+            hmax = fmaxf(hmax, mh.y);
+        }
+    }
+#pragma unroll
+    for (int r = 0; r < R; ++r)
+        nsm[r] = __fsub_rn(__fmaf_rn(sz[r], sz[r], __fmaf_rn(sy[r], sy[r], __fmul_rn(sx[r], sx[r]))), mh0.x);
+    unsigned c[kMaxWinEdges], cnt[kMaxWinEdges + 1];
+    bool flagged;
+    if (wmode == 1) {
+        flagged = window_block<1>(js, sx, sy, sz, nsm, dt, hmax, c);
+        cnt[0] = c[0];
+        cnt[1] = kSubJ * R - c[0];
+        cnt[2] = cnt[3] = 0;
+        ++npath[0];
+    } else if (wmode == 2) {
+        flagged = window_block<2>(js, sx, sy, sz, nsm, dt, hmax, c);
+        cnt[0] = c[0];
+        cnt[1] = c[1] - c[0];
+        cnt[2] = kSubJ * R - c[1];
+        cnt[3] = 0;
+        ++npath[1];
+    } else {
+        flagged = window_block<3>(js, sx, sy, sz, nsm, dt, hmax, c);
+        cnt[0] = c[0];
+        cnt[1] = c[1] - c[0];
+        cnt[2] = c[2] - c[1];
+        cnt[3] = kSubJ * R - c[2];
+        ++npath[2];
+    }
+    if (!flagged) {
+#pragma unroll
+        for (int t = 0; t <= kMaxWinEdges; ++t)
+            if (cnt[t]) atomicAdd(wt.whist + wt.band_slot[k + t], cnt[t]);      // cnt[t] != 0 only for t <= wmode
+    }
+    // lanes that saw a pair inside a guard band: the warp recounts their kSubJ x R pairs together, lane l taking
+    // j-point l, through the cell-lookup path (which sends the ambiguous pairs to the fp64 recheck)
+    unsigned todo = __ballot_sync(0xffffffffu, flagged);
+    while (todo) {
+        const int src = __ffs(todo) - 1;
+        todo &= todo - 1;
+        const float4 b = js[lane];
+        const uint32_t isrc = i0 + (uint32_t)(src - lane) * R;
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const float ux = __shfl_sync(0xffffffffu, sx[r], src), uy = __shfl_sync(0xffffffffu, sy[r], src),
+                        uz = __shfl_sync(0xffffffffu, sz[r], src);
+            lookup_pair<MAP>(ux, uy, uz, b, lut, hist, slow, isrc + r, j0 + lane, true, shift, scale, clamp);
+        }
+        ++npath[4];
+    }
+}
+
+constexpr int NRING = 2;                                               // chunk slots per warp
+constexpr int kSubPerChunk = kChunkJ / kSubJ;
+constexpr uint32_t kChunkBytes = kChunkJ * sizeof(float4), kChunkSphBytes = kSubPerChunk * sizeof(float4);
+constexpr uint32_t kSlotBytes = kChunkBytes + kChunkSphBytes;
+static_assert(kSubJ == 32, "the recount of a flagged lane gives j-point l of the subtile to lane l");
+static_assert(kIPerThread == 4, "window_block's pair count assumes R = 4");
+static_assert(kChunkJ == kWarpI, "the diagonal chunk of a warp item is the chunk with the warp's own rows");
+static_assert(kTileJ % kChunkJ == 0 && kTileI % kWarpI == 0 && kTileI / kWarpI == kWarpsPerCta, "tiling");
+
+// shared-memory layout of pair_fast_kernel (byte offsets; every array 16-byte aligned)
+__host__ __device__ inline uint32_t up16(uint32_t x) { return (x + 15u) & ~15u; }
+struct FastSmem {
+    uint32_t ring, lut, hist, band_mh, band_lh, whist, cell_band, band_slot, bars, slow, total;
+};
+__host__ __device__ inline FastSmem fast_smem_layout(int ncells, int nbands, int nbins) {
+    FastSmem L;
+    uint32_t o = 0;
+    L.ring = o;       o += kWarpsPerCta * NRING * kSlotBytes;
+    L.lut = o;        o = up16(o + (uint32_t)ncells * 8);
+    L.hist = o;       o = up16(o + (uint32_t)ncells * 8);
+    L.band_mh = o;    o = up16(o + (uint32_t)nbands * 8);
+    L.band_lh = o;    o = up16(o + (uint32_t)nbands * 8);
+    L.whist = o;      o = up16(o + (uint32_t)(nbins + 3) * 4);
+    L.cell_band = o;  o = up16(o + (uint32_t)ncells * 2);
+    L.band_slot = o;  o = up16(o + (uint32_t)(nbands + 1) * 2);
+    L.bars = o;       o = up16(o + kWarpsPerCta * NRING * 8);
+    L.slow = o;       o = up16(o + (uint32_t)sizeof(SlowCtx));
+    L.total = o;
+    return L;
+}
+
+// i-block of work item w of the triangle plan: the warp probes 32 positions of row_start per round
+__device__ __forceinline__ uint32_t tri_row_of(const uint32_t* __restrict__ row_start, uint32_t blocks_i, uint32_t w, int lane) {
+    uint32_t lo = 0, hi = blocks_i;                      // row_start[lo] <= w < row_start[hi]
+    while (hi - lo > 1) {
+        const uint32_t step = (hi - lo + 32) / 33, pos = lo + (lane + 1) * step;
+        const bool ok = pos < hi && row_start[pos] <= w;
+        const uint32_t cnt = __popc(__ballot_sync(0xffffffffu, ok));      // probes are monotone: the first cnt hold
+        hi = min(hi, lo + (cnt + 1) * step);
+        lo = lo + cnt * step;
+    }
+    return lo;
+}
+
+// Add partial counters into the global uint64 result and clear them.  Integer adds: order-independent, hence
+// deterministic.  atomicExch lets one warp do this while the others keep counting.
+__device__ __forceinline__ void flush_slots(unsigned* hist, int nslots, const uint16_t* __restrict__ slotmap, unsigned* whist,
+                                            int nres, unsigned long long* result, unsigned* nrecheck,
+                                            unsigned long long* rechecked, int first, int stride) {
+    for (int s = first; s < nslots; s += stride) {
+        const unsigned v = hist[s] ? atomicExch(hist + s, 0u) : 0u;
+        if (v) atomicAdd(result + slotmap[s], (unsigned long long)v);
+    }
+    for (int s = first; s < nres; s += stride) {
+        const unsigned v = whist[s] ? atomicExch(whist + s, 0u) : 0u;
+        if (v) atomicAdd(result + s, (unsigned long long)v);
+    }
+    if (first == 0) {
+        const unsigned v = *nrecheck ? atomicExch(nrecheck, 0u) : 0u;
+        if (v) atomicAdd(rechecked, (unsigned long long)v);
+    }
+}
+
+// The pair kernel.  Persistent CTAs of 8 independent warps.  A warp item = 128 consecutive i-rows (one quad per lane)
+// against the j-rows of one plan item; the warp streams those j-rows through its own 2-slot shared-memory ring in
+// 128-row chunks (TMA bulk copies behind mbarriers, issued by lane 0), so no CTA-wide barrier sits in the loop.
+template <int MAP>
+__global__ void __launch_bounds__(kThreads, 3) pair_fast_kernel(const __grid_constant__ PairParams p) {
+    extern __shared__ __align__(128) unsigned char smem[];
+    const FastSmem L = fast_smem_layout(p.ncells, p.nbands, p.nbins);
+    char* lut = reinterpret_cast<char*>(smem + L.lut);
+    unsigned* hist = reinterpret_cast<unsigned*>(smem + L.hist);
+    SlowCtx* slow = reinterpret_cast<SlowCtx*>(smem + L.slow);
+    WinTables wt;
+    wt.band_mh = reinterpret_cast<const float2*>(smem + L.band_mh);
+    wt.band_lh = reinterpret_cast<const float2*>(smem + L.band_lh);
+    wt.band_slot = reinterpret_cast<const uint16_t*>(smem + L.band_slot);
+    wt.cell_band = reinterpret_cast<const uint16_t*>(smem + L.cell_band);
+    wt.whist = reinterpret_cast<unsigned*>(smem + L.whist);
+    wt.nbands = p.nbands;
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    unsigned char* ring = smem + L.ring + (size_t)warp * NRING * kSlotBytes;
+    const uint32_t bar0 = smem_u32(smem + L.bars + (size_t)warp * NRING * 8);
+    for (int c = tid; c < p.ncells; c += kThreads) {
+        reinterpret_cast<float2*>(lut)[c] = p.lut[c];
+        hist[2 * c] = 0;
+        hist[2 * c + 1] = 0;
+        reinterpret_cast<uint16_t*>(smem + L.cell_band)[c] = p.cell_band[c];
+    }
+    for (int b = tid; b < p.nbands; b += kThreads) {
+        reinterpret_cast<float2*>(smem + L.band_mh)[b] = p.band_mh[b];
+        reinterpret_cast<float2*>(smem + L.band_lh)[b] = p.band_lh[b];
+    }
+    for (int b = tid; b <= p.nbands; b += kThreads) reinterpret_cast<uint16_t*>(smem + L.band_slot)[b] = p.band_slot[b];
+    for (int b = tid; b < p.nbins + 3; b += kThreads) wt.whist[b] = 0;
+    if (lane == 0) {
+        for (int b = 0; b < NRING; ++b) mbar_init(bar0 + 8 * b, 1);
+        fence_barrier_init();
+    }
+    if (tid == 0) {
+        slow->xi64 = p.xi64;
+        slow->xj64 = p.xj64;
+        slow->thr = p.thr;
+        slow->whist = wt.whist;
+        slow->nrecheck = 0;
+        slow->nbins = p.nbins;
+    }
+    __syncthreads();
+
+    auto fetch_chunk = [&](uint32_t g, uint32_t ch) {      // lane 0: two bulk copies behind the slot's mbarrier
+        const uint32_t slot = g % NRING, bar = bar0 + 8 * slot;
+        unsigned char* dst = ring + (size_t)slot * kSlotBytes;
+        fence_proxy_async();
+        mbar_expect_tx(bar, kSlotBytes);
+        bulk_g2s(smem_u32(dst), p.xs + (size_t)ch * kChunkJ, kChunkBytes, bar);
+        bulk_g2s(smem_u32(dst + kChunkBytes), p.cs + (size_t)ch * kSubPerChunk, kChunkSphBytes, bar);
+    };
+
+    const unsigned long long n_witems = (unsigned long long)p.n_items_part * kWarpsPerCta;
+    const uint32_t per_row = (p.tiles_j + p.chunk - 1) / p.chunk;
+    uint32_t g = 0;                         // chunks this warp consumed so far: selects ring slot and mbarrier parity
+    unsigned long long pairs_since_flush = 0, witems_done = 0;
+    unsigned npath[6] = {0, 0, 0, 0, 0, 0};
+    for (;;) {
+        unsigned long long c = 0;
+        if (lane == 0) c = atomicAdd(p.counters, 1ull);
+        c = __shfl_sync(0xffffffffu, c, 0);
+        if (c >= n_witems) break;
+        const uint32_t w = (uint32_t)(c / kWarpsPerCta) * p.nparts + p.part, ws = (uint32_t)(c % kWarpsPerCta);
+        uint32_t I, tile0;
+        if (p.tri) {
+            I = tri_row_of(p.row_start, p.blocks_i, w, lane);
+            tile0 = I + (w - p.row_start[I]) * p.chunk;
+        } else {
+            I = w / per_row;
+            tile0 = (w % per_row) * p.chunk;
+        }
+        const uint32_t ntiles = min(p.chunk, p.tiles_j - tile0);
+
+        // this lane's quad: R consecutive rows as offsets from the quad centre.  A quad wholly past the end of the
+        // catalog is moved to (-2,-2,-2): 6 <= d2 <= 48 against every real or padding j-row, i.e. always discarded.
+        const uint32_t ibase = I * kTileI + ws * kWarpI, i0 = ibase + lane * R;
+        float4 q4 = p.cq[i0 / R];
+        float px[R], py[R], pz[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const float4 a = p.xq[i0 + r];
+            px[r] = a.x;
+            py[r] = a.y;
+            pz[r] = a.z;
+        }
+        if (i0 >= p.n_i) {
+            q4 = make_float4(-kPadCoord, -kPadCoord, -kPadCoord, 0.f);
+#pragma unroll
+            for (int r = 0; r < R; ++r) px[r] = py[r] = pz[r] = 0.f;
+        }
+
+        // chunks of kChunkJ rows; in the triangle those wholly below the warp's own rows hold no pair i<j, and the
+        // chunk of the warp's own rows is the diagonal one (masked)
+        const uint32_t dch = ibase / kChunkJ;
+        uint32_t ch = tile0 * (kTileJ / kChunkJ);
+        const uint32_t ch_end = (tile0 + ntiles) * (kTileJ / kChunkJ);
+        if (p.tri) ch = max(ch, dch);
+        if (lane == 0 && ch < ch_end) fetch_chunk(g, ch);
+        for (; ch < ch_end; ++ch, ++g) {
+            if (lane == 0 && ch + 1 < ch_end) fetch_chunk(g + 1, ch + 1);       // the other slot: released by the __syncwarp below
+            mbar_wait(bar0 + 8 * (g % NRING), (g / NRING) & 1);
+            const float4* jt = reinterpret_cast<const float4*>(ring + (size_t)(g % NRING) * kSlotBytes);
+            const float4* jsph = jt + kChunkJ;
+            const bool mask = p.tri && ch == dch;
+#pragma unroll 1
+            for (int sub = 0; sub < kSubPerChunk; ++sub)
+                subtile_pairs<MAP>(jt + sub * kSubJ, jsph[sub], p.window != 0, mask, px, py, pz, q4.x, q4.y, q4.z, q4.w, wt, lut,
+                                   reinterpret_cast<char*>(hist), slow, i0, p.n_i, ch * kChunkJ + sub * kSubJ, p.n_j, p.shift,
+                                   p.sqrt_scale, p.sqrt_clamp, npath);
+            __syncwarp();
+            pairs_since_flush += (unsigned long long)kWarpI * kChunkJ;
+        }
+        ++witems_done;
+        if (pairs_since_flush > kFlushPairs / kWarpsPerCta) {     // 8 warps x this bound < 2^32 per slot
+            flush_slots(hist, 2 * p.ncells, p.slotmap, wt.whist, p.nbins + 3, p.result, &slow->nrecheck, p.counters + 1, lane, 32);
+            pairs_since_flush = 0;
+        }
+    }
+    __syncthreads();
+    flush_slots(hist, 2 * p.ncells, p.slotmap, wt.whist, p.nbins + 3, p.result, &slow->nrecheck, p.counters + 1, tid, kThreads);
+    if (lane == 0) {
+        if (witems_done) atomicAdd(p.counters + 2, witems_done);
+#pragma unroll
+        for (int k = 0; k < 6; ++k)
+            if (npath[k]) atomicAdd(p.counters + 3 + k, (unsigned long long)npath[k]);
+    }
+}
+
+// ---- fp64 engine: work items per CTA -------------------------------------------------------------------------
 struct Item {
     uint32_t I, tile0, ntiles, valid;
 };
@@ -108,379 +522,6 @@ __device__ __forceinline__ Item decode_item(const PairParams& p, uint32_t w) {
     }
     it.ntiles = min(p.chunk, p.tiles_j - it.tile0);
     return it;
-}
-
-template <int MAP>
-__device__ __forceinline__ uint32_t cell_byte_offset(float d2, int shift, float scale, float clamp) {
-    if (MAP == (int)CellMap::LogBits) {
-        return (__float_as_uint(d2) >> (shift - 3)) & ~7u;
-    } else {
-        const float c = fminf(d2, clamp);
-        const float key = __uint_as_float((__float_as_uint(c) >> 1) + kSqrtMagic);
-        const float t = fmaf(key, scale, 8388608.0f);
-        return (__float_as_uint(t) << 3) & 0x3FFFFF8u;
-    }
-}
-
-// ---- per-pair cell-lookup path ("lookup" path) ---------------------------------------------------------------
-// One pair: fp32 squared chord -> cell -> (lo, hi) of the cell's guard band -> shared-memory partial histogram,
-// or the fp64 recheck when lo <= d2 < hi.
-template <int MAP>
-__device__ __forceinline__ void lookup_pair(float ax, float ay, float az, const float4& b, const char* lut, char* hist,
-                                            const SlowCtx* slow, uint32_t i, uint32_t j, bool valid, int shift,
-                                            float scale, float clamp) {
-    const float dx = ax - b.x, dy = ay - b.y, dz = az - b.z;
-    const float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-    const uint32_t q8 = cell_byte_offset<MAP>(d2, shift, scale, clamp);
-    const float2 lh = *reinterpret_cast<const float2*>(lut + q8);
-    const bool above = d2 >= lh.x;
-    const bool amb = above && (d2 < lh.y);
-    if (amb) {
-        if (valid) recheck_pair(slow, i, j);
-    } else if (valid) {
-        atomicAdd(reinterpret_cast<unsigned*>(hist + q8) + (above ? 1 : 0), 1u);
-    }
-}
-
-// nj consecutive j-points against this thread's R register-resident i-points, every pair by cell lookup.
-template <int MAP, bool DIAG>
-__device__ __forceinline__ void lookup_block(const float4* __restrict__ jt, int nj, const float (&ax)[R],
-                                             const float (&ay)[R], const float (&az)[R], const char* lut, char* hist,
-                                             const SlowCtx* slow, uint32_t i0 /* global index of this thread's r = 0 point */,
-                                             uint32_t j0 /* global index of jt[0] */, int shift, float scale, float clamp) {
-#pragma unroll 2
-    for (int jj = 0; jj < nj; ++jj) {
-        const float4 b = jt[jj];                                  // one LDS.128, broadcast to the warp
-#pragma unroll
-        for (int r = 0; r < R; ++r)
-            lookup_pair<MAP>(ax[r], ay[r], az[r], b, lut, hist, slow, i0 + r, j0 + jj, !DIAG || (j0 + jj > i0 + r), shift,
-                             scale, clamp);
-    }
-}
-
-// ---- window path ----------------------------------------------------------------------------------------------
-// For one lane (R consecutive rows of the spatially sorted i-catalog, bounding sphere (ci, ri)) and one j-subtile
-// (kSubJ consecutive rows, bounding sphere sp): every TRUE chord of the block lies in [dc - ri - rj, dc + ri + rj]
-// (triangle inequality in R^3).  Returns squared bounds made safe against the fp32 evaluation of the geometry.
-__device__ __forceinline__ void chord_bounds(float cx, float cy, float cz, float ri, const float4& sp, float& lo2,
-                                             float& hi2) {
-    const float dx = cx - sp.x, dy = cy - sp.y, dz = cz - sp.z;
-    const float dc2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-    float dc;
-    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(dc) : "f"(dc2));
-    const float rs = ri + sp.w;
-    const float lo = fmaf(dc, 1.0f - 4.0e-6f, -rs) - 4.0e-7f;
-    const float hi = fmaf(dc, 1.0f + 4.0e-6f, rs) + 4.0e-7f;
-    lo2 = lo > 0.f ? __fmul_rd(lo, lo) : 0.f;
-    hi2 = __fmul_ru(hi, hi);
-}
-
-// The E-edge window loop: counts, for the kSubJ x R pairs of the block, how many have q < mid_e for each of the
-// bands k .. k+E-1 (q = fp32 squared chord, accumulated starting from -mid_0 so that the test is a sign bit),
-// and tracks the smallest |q - mid_e| seen.  Returns true when some pair came within a band's half width: the
-// counters of this lane are then not used and the block is recounted pair by pair.
-template <int E>
-__device__ __forceinline__ bool window_block(const float4* __restrict__ jt, const float (&ax)[R], const float (&ay)[R],
-                                             const float (&az)[R], const float2* __restrict__ band_mh, int k,
-                                             unsigned (&c)[E]) {
-    const float2 mh0 = band_mh[k];
-    const float nm0 = -mh0.x;
-    float hmax = mh0.y, dt[E];
-    dt[0] = 0.f;
-#pragma unroll
-    for (int e = 1; e < E; ++e) {
-        const float2 mh = band_mh[k + e];
-        dt[e] = __fsub_rn(mh0.x, mh.x);
-        hmax = fmaxf(hmax, mh.y);
-    }
-#pragma unroll
-    for (int e = 0; e < E; ++e) c[e] = 0;
-    float m = 3.0e38f;
-#pragma unroll 8
-    for (int jj = 0; jj < kSubJ; ++jj) {
-        const float4 b = jt[jj];
-#pragma unroll
-        for (int r = 0; r < R; ++r) {
-            const float dx = __fsub_rn(ax[r], b.x), dy = __fsub_rn(ay[r], b.y), dz = __fsub_rn(az[r], b.z);
-            const float q = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmaf_rn(dx, dx, nm0)));
-#pragma unroll
-            for (int e = 0; e < E; ++e) {
-                const float qe = e ? __fadd_rn(q, dt[e]) : q;
-                c[e] += __float_as_uint(qe) >> 31;
-                m = fminf(m, fabsf(qe));
-            }
-        }
-    }
-    return m <= hmax;
-}
-
-struct WinTables {
-    const float2* band_mh;
-    const float2* band_lh;
-    const uint16_t* band_slot;
-    const uint16_t* cell_band;
-    unsigned* whist;            // partial histogram indexed by result slot
-    int nbands;
-};
-
-// One 1024-point j-tile against the CTA's 1024 register-resident i-points, subtile by subtile.
-template <int MAP, bool DIAG>
-__device__ __forceinline__ void tile_pairs(const float4* __restrict__ jt, const float4* __restrict__ jsph, bool windows,
-                                           const float (&ax)[R], const float (&ay)[R], const float (&az)[R], float cx,
-                                           float cy, float cz, float ri, const WinTables& wt, const char* lut, char* hist,
-                                           const SlowCtx* slow, uint32_t i0, uint32_t j0, int shift, float scale,
-                                           float clamp, unsigned (&npath)[5]) {
-    if (DIAG || !windows) {
-        lookup_block<MAP, DIAG>(jt, kTileJ, ax, ay, az, lut, hist, slow, i0, j0, shift, scale, clamp);
-        npath[3] += kTileJ / kSubJ;
-        return;
-    }
-    const int lane = threadIdx.x & 31;
-    for (int sub = 0; sub < kTileJ / kSubJ; ++sub) {
-        const float4* js = jt + sub * kSubJ;
-        float lo2, hi2;
-        chord_bounds(cx, cy, cz, ri, jsph[sub], lo2, hi2);
-        // first band that is not wholly below the window, then how many bands the window reaches
-        int k = wt.cell_band[cell_byte_offset<MAP>(lo2, shift, scale, clamp) >> 3];
-        while (k < wt.nbands && wt.band_lh[k].y <= lo2) ++k;
-        int e = 1;
-        while (e <= kMaxWinEdges && k + e < wt.nbands && wt.band_lh[k + e].x <= hi2) ++e;
-        const int emax = __reduce_max_sync(0xffffffffu, e);
-        if (emax > kMaxWinEdges) {
-            lookup_block<MAP, false>(js, kSubJ, ax, ay, az, lut, hist, slow, i0, j0 + sub * kSubJ, shift, scale, clamp);
-            ++npath[3];
-            continue;
-        }
-        // every lane runs the emax-edge loop on bands k .. k+emax-1; lowering k keeps the window inside them
-        k = min(k, wt.nbands - emax);
-        unsigned cnt[kMaxWinEdges + 1];
-        bool flagged;
-        if (emax == 1) {
-            unsigned c[1];
-            flagged = window_block<1>(js, ax, ay, az, wt.band_mh, k, c);
-            cnt[0] = c[0];
-            cnt[1] = kSubJ * R - c[0];
-            cnt[2] = cnt[3] = 0;
-            ++npath[0];
-        } else if (emax == 2) {
-            unsigned c[2];
-            flagged = window_block<2>(js, ax, ay, az, wt.band_mh, k, c);
-            cnt[0] = c[0];
-            cnt[1] = c[1] - c[0];
-            cnt[2] = kSubJ * R - c[1];
-            cnt[3] = 0;
-            ++npath[1];
-        } else {
-            unsigned c[3];
-            flagged = window_block<3>(js, ax, ay, az, wt.band_mh, k, c);
-            cnt[0] = c[0];
-            cnt[1] = c[1] - c[0];
-            cnt[2] = c[2] - c[1];
-            cnt[3] = kSubJ * R - c[2];
-            ++npath[2];
-        }
-        if (!flagged) {
-#pragma unroll
-            for (int t = 0; t <= kMaxWinEdges; ++t)
-                if (cnt[t]) atomicAdd(wt.whist + wt.band_slot[k + t], cnt[t]);      // cnt[t] != 0 only for t <= emax
-        }
-        // lanes that saw a pair inside a guard band: the warp recounts their kSubJ x R pairs together, lane l
-        // taking j-point l, through the cell-lookup path (which sends the ambiguous pairs to the fp64 recheck)
-        unsigned todo = __ballot_sync(0xffffffffu, flagged);
-        while (todo) {
-            const int src = __ffs(todo) - 1;
-            todo &= todo - 1;
-            const float4 b = js[lane];
-            const uint32_t isrc = i0 + (uint32_t)(src - lane) * R;
-#pragma unroll
-            for (int r = 0; r < R; ++r) {
-                const float sx = __shfl_sync(0xffffffffu, ax[r], src), sy = __shfl_sync(0xffffffffu, ay[r], src),
-                            sz = __shfl_sync(0xffffffffu, az[r], src);
-                lookup_pair<MAP>(sx, sy, sz, b, lut, hist, slow, isrc + r, j0 + sub * kSubJ + lane, true, shift, scale, clamp);
-            }
-            ++npath[4];
-        }
-    }
-}
-
-// Add the CTA's 32-bit partial counters into the global uint64 result (integer adds: order-independent,
-// hence deterministic) and clear them.
-__device__ __forceinline__ void flush_hist(unsigned* hist, int nslots, const uint16_t* __restrict__ slotmap,
-                                           unsigned* whist, int nres, unsigned long long* result) {
-    __syncthreads();
-    for (int s = threadIdx.x; s < nslots; s += kThreads) {
-        const unsigned v = hist[s];
-        if (v) {
-            atomicAdd(result + slotmap[s], (unsigned long long)v);
-            hist[s] = 0;
-        }
-    }
-    for (int s = threadIdx.x; s < nres; s += kThreads) {
-        const unsigned v = whist[s];
-        if (v) {
-            atomicAdd(result + s, (unsigned long long)v);
-            whist[s] = 0;
-        }
-    }
-    __syncthreads();
-}
-
-constexpr uint32_t kSphBytes = (kTileJ / kSubJ) * sizeof(float4);
-static_assert(kSubJ == 32, "the recount of a flagged lane gives j-point l of the subtile to lane l");
-static_assert(kIPerThread == 4, "window_block's pair count assumes R = 4");
-
-// shared-memory layout of pair_fast_kernel (byte offsets; every array 16-byte aligned)
-__host__ __device__ inline uint32_t up(uint32_t x) { return (x + 15u) & ~15u; }
-struct FastSmem {
-    uint32_t jbuf, jsph, lut, hist, band_mh, band_lh, whist, cell_band, band_slot, bars, item, slow, total;
-};
-__host__ __device__ inline FastSmem fast_smem_layout(int ncells, int nbands, int nbins) {
-    FastSmem L;
-    uint32_t o = 0;
-    L.jbuf = o;       o += NBUF * kTileBytes;
-    L.jsph = o;       o += NBUF * kSphBytes;
-    L.lut = o;        o = up(o + (uint32_t)ncells * 8);
-    L.hist = o;       o = up(o + (uint32_t)ncells * 8);
-    L.band_mh = o;    o = up(o + (uint32_t)nbands * 8);
-    L.band_lh = o;    o = up(o + (uint32_t)nbands * 8);
-    L.whist = o;      o = up(o + (uint32_t)(nbins + 3) * 4);
-    L.cell_band = o;  o = up(o + (uint32_t)ncells * 2);
-    L.band_slot = o;  o = up(o + (uint32_t)(nbands + 1) * 2);
-    L.bars = o;       o += 16 * ((NBUF * 8 + 15) / 16);
-    L.item = o;       o += 16;
-    L.slow = o;       o = up(o + (uint32_t)sizeof(SlowCtx));
-    L.total = o;
-    return L;
-}
-
-template <int MAP>
-__global__ void __launch_bounds__(kThreads, 3) pair_fast_kernel(const __grid_constant__ PairParams p) {
-    extern __shared__ __align__(128) unsigned char smem[];
-    const FastSmem L = fast_smem_layout(p.ncells, p.nbands, p.nbins);
-    float4* jbuf = reinterpret_cast<float4*>(smem + L.jbuf);
-    float4* jsph = reinterpret_cast<float4*>(smem + L.jsph);
-    char* lut = reinterpret_cast<char*>(smem + L.lut);
-    unsigned* hist = reinterpret_cast<unsigned*>(smem + L.hist);
-    unsigned long long* bars = reinterpret_cast<unsigned long long*>(smem + L.bars);
-    Item* s_item = reinterpret_cast<Item*>(smem + L.item);
-    SlowCtx* slow = reinterpret_cast<SlowCtx*>(smem + L.slow);
-    WinTables wt;
-    wt.band_mh = reinterpret_cast<const float2*>(smem + L.band_mh);
-    wt.band_lh = reinterpret_cast<const float2*>(smem + L.band_lh);
-    wt.band_slot = reinterpret_cast<const uint16_t*>(smem + L.band_slot);
-    wt.cell_band = reinterpret_cast<const uint16_t*>(smem + L.cell_band);
-    wt.whist = reinterpret_cast<unsigned*>(smem + L.whist);
-    wt.nbands = p.nbands;
-    const bool windows = p.sph_j != nullptr;
-    const uint32_t tile_tx = kTileBytes + (windows ? kSphBytes : 0u);
-
-    const int tid = threadIdx.x;
-    for (int c = tid; c < p.ncells; c += kThreads) {
-        reinterpret_cast<float2*>(lut)[c] = p.lut[c];
-        hist[2 * c] = 0;
-        hist[2 * c + 1] = 0;
-        reinterpret_cast<uint16_t*>(smem + L.cell_band)[c] = p.cell_band[c];
-    }
-    for (int b = tid; b < p.nbands; b += kThreads) {
-        reinterpret_cast<float2*>(smem + L.band_mh)[b] = p.band_mh[b];
-        reinterpret_cast<float2*>(smem + L.band_lh)[b] = p.band_lh[b];
-    }
-    for (int b = tid; b <= p.nbands; b += kThreads) reinterpret_cast<uint16_t*>(smem + L.band_slot)[b] = p.band_slot[b];
-    for (int b = tid; b < p.nbins + 3; b += kThreads) wt.whist[b] = 0;
-    if (tid == 0) {
-        for (int b = 0; b < NBUF; ++b) mbar_init(smem_u32(bars + b), 1);
-        fence_barrier_init();
-        slow->xi64 = p.xi64;
-        slow->xj64 = p.xj64;
-        slow->thr = p.thr;
-        slow->result = p.result;
-        slow->rechecked = p.counters + 1;
-        slow->nbins = p.nbins;
-    }
-    __syncthreads();
-
-    auto fetch_tile = [&](uint32_t g, uint32_t tile) {      // one elected thread: TMA bulk copies behind one mbarrier
-        const uint32_t buf = g % NBUF, bar = smem_u32(bars + buf);
-        mbar_expect_tx(bar, tile_tx);
-        bulk_g2s(smem_u32(jbuf + (size_t)buf * kTileJ), p.xj + (size_t)tile * kTileJ, kTileBytes, bar);
-        if (windows)
-            bulk_g2s(smem_u32(jsph + (size_t)buf * (kTileJ / kSubJ)), p.sph_j + (size_t)tile * (kTileJ / kSubJ), kSphBytes, bar);
-    };
-
-    uint32_t tiles_done = 0;                // tiles this CTA consumed so far: selects buffer and mbarrier parity
-    unsigned long long pairs_since_flush = 0, items_done = 0;
-    unsigned npath[5] = {0, 0, 0, 0, 0};
-    for (;;) {
-        if (tid == 0) {
-            const unsigned long long c = atomicAdd(p.counters, 1ull);
-            Item it;
-            it.valid = 0;
-            if (c < p.n_items_part) it = decode_item(p, (uint32_t)c * p.nparts + p.part);
-            *s_item = it;
-        }
-        __syncthreads();
-        const Item it = *s_item;
-        if (!it.valid) break;
-
-        // this thread's R consecutive i-points (rows past the end of the catalog become (-2,-2,-2): d2 >= 6
-        // against every real point and 48 against a (2,2,2) padding row, i.e. always in the discard range)
-        const uint32_t i0 = it.I * kTileI + tid * R;
-        float ax[R], ay[R], az[R];
-#pragma unroll
-        for (int r = 0; r < R; ++r) {
-            const uint32_t i = i0 + r;
-            float4 a = p.xi[i];
-            if (i >= p.n_i) a = make_float4(-kPadCoord, -kPadCoord, -kPadCoord, 0.f);
-            ax[r] = a.x;
-            ay[r] = a.y;
-            az[r] = a.z;
-        }
-        // bounding sphere of the lane's R points around their mean; the radius also covers the distance of the
-        // fp64 points from their fp32 roundings (<= 5.2e-8) and the rounding of this evaluation
-        const float cx = 0.25f * ((ax[0] + ax[1]) + (ax[2] + ax[3])), cy = 0.25f * ((ay[0] + ay[1]) + (ay[2] + ay[3])),
-                    cz = 0.25f * ((az[0] + az[1]) + (az[2] + az[3]));
-        float ri2 = 0.f;
-#pragma unroll
-        for (int r = 0; r < R; ++r) {
-            const float dx = ax[r] - cx, dy = ay[r] - cy, dz = az[r] - cz;
-            ri2 = fmaxf(ri2, fmaf(dz, dz, fmaf(dy, dy, dx * dx)));
-        }
-        const float ri = fmaf(sqrtf(ri2), 1.0f + 4.0e-6f, 2.0e-7f);
-
-        if (tid == 0) {
-            fence_proxy_async();
-            for (uint32_t t = 0; t < it.ntiles && t < NBUF; ++t) fetch_tile(tiles_done + t, it.tile0 + t);
-        }
-        for (uint32_t t = 0; t < it.ntiles; ++t) {
-            const uint32_t g = tiles_done + t, buf = g % NBUF;
-            mbar_wait(smem_u32(bars + buf), (g / NBUF) & 1);
-            const float4* jt = jbuf + (size_t)buf * kTileJ;
-            const float4* js = jsph + (size_t)buf * (kTileJ / kSubJ);
-            const uint32_t j0 = (it.tile0 + t) * kTileJ;
-            if (p.tri && it.tile0 + t == it.I)
-                tile_pairs<MAP, true>(jt, js, windows, ax, ay, az, cx, cy, cz, ri, wt, lut, reinterpret_cast<char*>(hist), slow,
-                                      i0, j0, p.shift, p.sqrt_scale, p.sqrt_clamp, npath);
-            else
-                tile_pairs<MAP, false>(jt, js, windows, ax, ay, az, cx, cy, cz, ri, wt, lut, reinterpret_cast<char*>(hist), slow,
-                                       i0, j0, p.shift, p.sqrt_scale, p.sqrt_clamp, npath);
-            __syncthreads();                // every warp is done reading buffer `buf`
-            if (tid == 0 && t + NBUF < it.ntiles) fetch_tile(g + NBUF, it.tile0 + t + NBUF);
-        }
-        tiles_done += it.ntiles;
-        ++items_done;
-        pairs_since_flush += (unsigned long long)it.ntiles * kTileI * kTileJ;
-        if (pairs_since_flush > kFlushPairs) {
-            flush_hist(hist, 2 * p.ncells, p.slotmap, wt.whist, p.nbins + 3, p.result);
-            pairs_since_flush = 0;
-        }
-    }
-    flush_hist(hist, 2 * p.ncells, p.slotmap, wt.whist, p.nbins + 3, p.result);
-    if (tid == 0 && items_done) atomicAdd(p.counters + 2, items_done);
-    if ((tid & 31) == 0) {
-#pragma unroll
-        for (int k = 0; k < 5; ++k)
-            if (npath[k]) atomicAdd(p.counters + 3 + k, (unsigned long long)npath[k]);
-    }
 }
 
 // ---- fp64 engine: same plan, no tables, no shared-memory tiles -----------------------------------------
@@ -536,47 +577,37 @@ __global__ void __launch_bounds__(kThreads) pair_exact64_kernel(const __grid_con
 }
 
 // ---- load / convert / spatial sort (step a1) -------------------------------------------------------------------
-// 63-bit Hilbert-curve index of a point of [-1, 1]^3 quantised to 21 bits per axis (Skilling's transpose
-// algorithm).  Only the ORDER it induces is used: consecutive rows of the sorted catalog are close on the sky,
-// which is what makes the bounding spheres of the window path small.  Counts do not depend on it.
+// Sort key of a unit vector: the face of the circumscribed cube it projects onto (3 bits) followed by the 56-bit
+// index of its projection along a 2-D Hilbert curve of that face (28 bits per axis).  Only the ORDER it induces is
+// used: the curve is continuous on each face, so consecutive rows of the sorted catalog are neighbours on the sky
+// (except at the <= 5 face changes), which is what keeps the bounding spheres of quads and subtiles small.  Counts
+// do not depend on it.
 __device__ inline unsigned long long hilbert_key(double x, double y, double z) {
-    constexpr int B = 21;
-    uint32_t X[3];
-    const double v[3] = {x, y, z};
-#pragma unroll
-    for (int k = 0; k < 3; ++k) {
-        double t = (v[k] + 1.0) * (double)(1u << (B - 1));
-        t = fmin(fmax(t, 0.0), (double)((1u << B) - 1));
-        X[k] = (uint32_t)t;
-    }
-    const uint32_t M = 1u << (B - 1);
-    for (uint32_t Q = M; Q > 1; Q >>= 1) {          // inverse undo
-        const uint32_t P = Q - 1;
-#pragma unroll
-        for (int i = 0; i < 3; ++i) {
-            if (X[i] & Q) {
-                X[0] ^= P;
-            } else {
-                const uint32_t t = (X[0] ^ X[i]) & P;
-                X[0] ^= t;
-                X[i] ^= t;
+    constexpr int B = 28;
+    const double ax = fabs(x), ay = fabs(y), az = fabs(z);
+    int face;
+    double u, v, m;
+    if (ax >= ay && ax >= az) { face = x >= 0 ? 0 : 1; u = y; v = z; m = ax; }
+    else if (ay >= az)        { face = y >= 0 ? 2 : 3; u = z; v = x; m = ay; }
+    else                      { face = z >= 0 ? 4 : 5; u = x; v = y; m = az; }
+    const double scale = (double)(1u << (B - 1));
+    uint32_t X = (uint32_t)fmin(fmax((u / m + 1.0) * scale, 0.0), (double)((1u << B) - 1));
+    uint32_t Y = (uint32_t)fmin(fmax((v / m + 1.0) * scale, 0.0), (double)((1u << B) - 1));
+    unsigned long long d = 0;
+    for (uint32_t s = 1u << (B - 1); s > 0; s >>= 1) {
+        const uint32_t rx = (X & s) ? 1u : 0u, ry = (Y & s) ? 1u : 0u;
+        d += (unsigned long long)s * s * ((3u * rx) ^ ry);
+        if (ry == 0) {                                  // rotate the quadrant
+            if (rx == 1) {
+                X = (1u << B) - 1 - X;
+                Y = (1u << B) - 1 - Y;
             }
+            const uint32_t t = X;
+            X = Y;
+            Y = t;
         }
     }
-    X[1] ^= X[0];                                    // Gray encode
-    X[2] ^= X[1];
-    uint32_t t = 0;
-    for (uint32_t Q = M; Q > 1; Q >>= 1)
-        if (X[2] & Q) t ^= Q - 1;
-    X[0] ^= t;
-    X[1] ^= t;
-    X[2] ^= t;
-    unsigned long long key = 0;
-    for (int b = B - 1; b >= 0; --b) {
-#pragma unroll
-        for (int k = 0; k < 3; ++k) key = (key << 1) | ((X[k] >> b) & 1u);
-    }
-    return key;
+    return ((unsigned long long)face << (2 * B)) | d;
 }
 
 // x = cos(dec) cos(ra), y = cos(dec) sin(ra), z = sin(dec) in fp64 (reading A8), in the caller's row order.
@@ -669,10 +700,10 @@ __global__ void radix_scatter_kernel(const unsigned long long* __restrict__ keys
     }
 }
 
-// The sorted catalog: fp64 rows in Hilbert order, the fp32 copy (that vector rounded once, reading A17), the
-// inverse permutation for row-subset mode; rows n..n_pad-1 become the padding point (2,2,2).
+// The sorted catalog: fp64 rows in Hilbert order and the inverse permutation for row-subset mode; rows n..n_pad-1
+// become the padding point (2,2,2).
 __global__ void permute_kernel(const double4* __restrict__ x64_rows, const uint32_t* __restrict__ order, uint64_t n,
-                               uint64_t n_pad, double4* __restrict__ x64, float4* __restrict__ x32, uint32_t* __restrict__ inv) {
+                               uint64_t n_pad, double4* __restrict__ x64, uint32_t* __restrict__ inv) {
     for (uint64_t k = blockIdx.x * (uint64_t)blockDim.x + threadIdx.x; k < n_pad; k += (uint64_t)gridDim.x * blockDim.x) {
         double4 v = make_double4((double)kPadCoord, (double)kPadCoord, (double)kPadCoord, 0.0);
         if (k < n) {
@@ -681,13 +712,38 @@ __global__ void permute_kernel(const double4* __restrict__ x64_rows, const uint3
             inv[src] = (uint32_t)k;
         }
         x64[k] = v;
-        x32[k] = make_float4((float)v.x, (float)v.y, (float)v.z, 0.f);
     }
 }
 
-// Bounding sphere of each kSubJ = 32 consecutive rows (one warp each): centre = fp32 rounding of the mean,
-// radius = max fp64 distance of the fp64 rows from that fp32 centre, rounded up with slack.
-__global__ void spheres_kernel(const double4* __restrict__ x64, uint64_t nsub, float4* __restrict__ sph) {
+// i-side role of a catalog: every kIPerThread = 4 consecutive rows form a quad (one lane of the pair kernel).
+// cq = (fp32 centre, radius): the centre is the fp32 rounding of the mean, the radius bounds the fp64 distance of
+// the fp64 rows from that fp32 point (rounded up, with slack).  xq = fp32 rounding of (row - centre), formed in fp64:
+// its error is 2^-24 of the OFFSET, not of the unit vector.
+__global__ void quads_kernel(const double4* __restrict__ x64, uint64_t nquads, float4* __restrict__ xq, float4* __restrict__ cq) {
+    for (uint64_t q = blockIdx.x * (uint64_t)blockDim.x + threadIdx.x; q < nquads; q += (uint64_t)gridDim.x * blockDim.x) {
+        double4 v[kIPerThread];
+        double sx = 0, sy = 0, sz = 0;
+#pragma unroll
+        for (int r = 0; r < kIPerThread; ++r) {
+            v[r] = x64[q * kIPerThread + r];
+            sx += v[r].x; sy += v[r].y; sz += v[r].z;
+        }
+        const float cx = (float)(sx / kIPerThread), cy = (float)(sy / kIPerThread), cz = (float)(sz / kIPerThread);
+        double rad = 0;
+#pragma unroll
+        for (int r = 0; r < kIPerThread; ++r) {
+            const double dx = v[r].x - (double)cx, dy = v[r].y - (double)cy, dz = v[r].z - (double)cz;
+            rad = fmax(rad, sqrt(dx * dx + dy * dy + dz * dz));
+            xq[q * kIPerThread + r] = make_float4((float)dx, (float)dy, (float)dz, 0.f);
+        }
+        cq[q] = make_float4(cx, cy, cz, __double2float_ru(rad * (1.0 + 1.0e-7) + 1.0e-12));
+    }
+}
+
+// j-side role: every kSubJ = 32 consecutive rows form a subtile (one warp here).  cs = (fp32 centre, radius) as
+// above; xs = (-2 b', |b'|^2) with b' the fp32 rounding of (row - centre) formed in fp64 and |b'|^2 the fp32
+// rounding of the fp64 square of that rounded offset (the window loops evaluate |a - b|^2 = |a|^2 + |b|^2 - 2 a.b).
+__global__ void subtiles_kernel(const double4* __restrict__ x64, uint64_t nsub, float4* __restrict__ xs, float4* __restrict__ cs) {
     const uint64_t w = (blockIdx.x * (uint64_t)blockDim.x + threadIdx.x) >> 5;
     const int lane = threadIdx.x & 31;
     if (w >= nsub) return;
@@ -704,7 +760,10 @@ __global__ void spheres_kernel(const double4* __restrict__ x64, uint64_t nsub, f
     double r = sqrt(dx * dx + dy * dy + dz * dz);
 #pragma unroll
     for (int off = 16; off; off >>= 1) r = fmax(r, __shfl_xor_sync(0xffffffffu, r, off));
-    if (lane == 0) sph[w] = make_float4(cx, cy, cz, __double2float_ru(r * (1.0 + 1.0e-7) + 1.0e-9));
+    const float bx = (float)dx, by = (float)dy, bz = (float)dz;
+    const double nb = (double)bx * bx + (double)by * by + (double)bz * bz;
+    xs[w * kSubJ + lane] = make_float4(-2.f * bx, -2.f * by, -2.f * bz, (float)nb);
+    if (lane == 0) cs[w] = make_float4(cx, cy, cz, __double2float_ru(r * (1.0 + 1.0e-7) + 1.0e-12));
 }
 
 // row-subset mode: position of each requested row in the sorted catalog (the key the subset is then sorted by,
@@ -720,19 +779,10 @@ __global__ void row_keys_kernel(const int64_t* __restrict__ rows, uint64_t nrows
     }
 }
 
-__global__ void gather_kernel(const double4* __restrict__ src64, const float4* __restrict__ src32,
-                              const unsigned long long* __restrict__ pos, uint64_t nrows, uint64_t nrows_pad,
-                              double4* __restrict__ dst64, float4* __restrict__ dst32) {
-    for (uint64_t k = blockIdx.x * (uint64_t)blockDim.x + threadIdx.x; k < nrows_pad; k += (uint64_t)gridDim.x * blockDim.x) {
-        double4 v = make_double4((double)kPadCoord, (double)kPadCoord, (double)kPadCoord, 0.0);
-        float4 f = make_float4(kPadCoord, kPadCoord, kPadCoord, 0.f);
-        if (k < nrows) {
-            v = src64[pos[k]];
-            f = src32[pos[k]];
-        }
-        dst64[k] = v;
-        dst32[k] = f;
-    }
+__global__ void gather_kernel(const double4* __restrict__ src64, const unsigned long long* __restrict__ pos, uint64_t nrows,
+                              uint64_t nrows_pad, double4* __restrict__ dst64) {
+    for (uint64_t k = blockIdx.x * (uint64_t)blockDim.x + threadIdx.x; k < nrows_pad; k += (uint64_t)gridDim.x * blockDim.x)
+        dst64[k] = (k < nrows) ? src64[pos[k]] : make_double4((double)kPadCoord, (double)kPadCoord, (double)kPadCoord, 0.0);
 }
 
 __global__ void finalize_kernel(const unsigned long long* __restrict__ result, int nbins, int zero_slot,
@@ -773,16 +823,22 @@ cudaError_t launch_sort_pairs(uint64_t* keys_a, uint64_t* keys_b, uint32_t* idx_
 }
 
 cudaError_t launch_permute(const double4* x64_rows, const uint32_t* order, uint64_t n, uint64_t n_pad, double4* x64,
-                           float4* x32, uint32_t* inv, cudaStream_t st) {
+                           uint32_t* inv, cudaStream_t st) {
     const int block = 256;
-    permute_kernel<<<grid_for(n_pad, block), block, 0, st>>>(x64_rows, order, n, n_pad, x64, x32, inv);
+    permute_kernel<<<grid_for(n_pad, block), block, 0, st>>>(x64_rows, order, n, n_pad, x64, inv);
     return cudaGetLastError();
 }
 
-cudaError_t launch_spheres(const double4* x64, uint64_t n_pad, float4* sph, cudaStream_t st) {
+cudaError_t launch_quads(const double4* x64, uint64_t n_pad, float4* xq, float4* cq, cudaStream_t st) {
+    const int block = 128;
+    quads_kernel<<<grid_for(n_pad / kIPerThread, block), block, 0, st>>>(x64, n_pad / kIPerThread, xq, cq);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_subtiles(const double4* x64, uint64_t n_pad, float4* xs, float4* cs, cudaStream_t st) {
     const uint64_t nsub = n_pad / kSubJ;
     const int block = 256;
-    spheres_kernel<<<(unsigned)((nsub * 32 + block - 1) / block), block, 0, st>>>(x64, nsub, sph);
+    subtiles_kernel<<<(unsigned)((nsub * 32 + block - 1) / block), block, 0, st>>>(x64, nsub, xs, cs);
     return cudaGetLastError();
 }
 
@@ -794,11 +850,11 @@ cudaError_t launch_row_keys(const int64_t* rows, uint64_t nrows, uint64_t n_src,
     return cudaGetLastError();
 }
 
-cudaError_t launch_gather(const double4* src64, const float4* src32, const uint64_t* pos, uint64_t nrows,
-                          uint64_t nrows_pad, double4* dst64, float4* dst32, cudaStream_t st) {
+cudaError_t launch_gather(const double4* src64, const uint64_t* pos, uint64_t nrows, uint64_t nrows_pad, double4* dst64,
+                          cudaStream_t st) {
     const int block = 256;
-    gather_kernel<<<grid_for(nrows_pad, block), block, 0, st>>>(src64, src32, reinterpret_cast<const unsigned long long*>(pos),
-                                                                nrows, nrows_pad, dst64, dst32);
+    gather_kernel<<<grid_for(nrows_pad, block), block, 0, st>>>(src64, reinterpret_cast<const unsigned long long*>(pos), nrows,
+                                                                nrows_pad, dst64);
     return cudaGetLastError();
 }
 

@@ -9,12 +9,17 @@ namespace tpcf {
 
 // One pair-count launch: i-points x j-points over the work plan.  All pointers are device pointers.
 struct PairParams {
-    const float4* xi;           // fp32 unit vectors of the i-side catalog, padded to a multiple of kTileI with (2,2,2,0)
-    const float4* xj;           // j-side, padded to a multiple of kTileJ
-    const double4* xi64;        // fp64 unit vectors (same padding); the recheck path and the fp64 engine read these
+    // i side: rows as fp32 offsets from the centre of their 4-row quad, and the quads' (centre, radius)
+    const float4* xq;
+    const float4* cq;
+    // j side: rows as (-2 offset, |offset|^2) from the centre of their 32-row subtile, and the subtiles' (centre, radius)
+    const float4* xs;
+    const float4* cs;
+    const double4* xi64;        // fp64 unit vectors (padded with (2,2,2)); the recheck path and the fp64 engine read these
     const double4* xj64;
     uint32_t n_i, n_j;          // real (unpadded) sizes
-    int tri;                    // 1: xi == xj and only pairs i<j are enumerated
+    int tri;                    // 1: i and j are the same catalog and only pairs i<j are enumerated
+    int window;                 // 1: window loops enabled (tpcf_set_window)
     uint32_t blocks_i, tiles_j, chunk;
     uint32_t n_items_part;      // items this launch executes (after the partition)
     const uint32_t* row_start;  // tri: first item of i-block I (blocks_i + 1 entries)
@@ -24,8 +29,6 @@ struct PairParams {
     const uint16_t* slotmap;    // 2 x ncells: result slot of (cell, d2 < lo) and (cell, d2 >= hi)
     int ncells, shift;
     float sqrt_scale, sqrt_clamp;
-    // window path: bounding spheres of every kSubJ consecutive j rows and the guard bands
-    const float4* sph_j;        // n_j_pad / kSubJ x (cx, cy, cz, r); nullptr switches the window path off
     const float2* band_mh;      // nbands x (mid, half width)
     const float2* band_lh;      // nbands x (lo, hi)
     const uint16_t* band_slot;  // nbands + 1 result slots: below band b; [nbands] = above the last band
@@ -35,9 +38,9 @@ struct PairParams {
     const double* thr;          // nbins + 1
     int nbins;
     unsigned long long* result; // nbins + 3: under, bins, over, discard
-    // [0] next work item, [1] pairs rechecked in fp64, [2] items done,
-    // [3..6] (warp, subtile) blocks counted by the 1-, 2-, 3-edge window loops and by the cell-lookup loop,
-    // [7] lanes of window blocks recounted because a pair came within a guard band
+    // [0] next work item (fast engine: next warp item), [1] pairs rechecked in fp64, [2] items done,
+    // [3..6] (lane-quad x subtile) warp blocks counted by the 1-, 2-, 3-edge window loops and by the cell-lookup loop,
+    // [7] lanes of window blocks recounted because a pair came within a guard band, [8] warp blocks sent to the fp64 loop
     unsigned long long* counters;
 };
 
@@ -45,7 +48,7 @@ struct LaunchInfo {
     int grid, block, smem_bytes, launches;
 };
 
-constexpr int kNumCounters = 8;
+constexpr int kNumCounters = 10;
 constexpr int kSortChunk = 2048;        // elements per block of the radix sort
 
 // RA/Dec rows -> fp64 unit vectors (caller order) + 63-bit Hilbert keys + identity index
@@ -55,17 +58,19 @@ cudaError_t launch_convert(const void* radec, int is_f64, uint64_t n, double4* x
 // result ends in A or B (*in_a).  counts: 256 * ceil(n / kSortChunk) words of scratch.
 cudaError_t launch_sort_pairs(uint64_t* keys_a, uint64_t* keys_b, uint32_t* idx_a, uint32_t* idx_b, uint32_t* counts,
                               uint32_t n, int nbits, cudaStream_t st, bool* in_a);
-// sorted catalog: x64[k] = rows[order[k]], x32 = its rounding, inv[order[k]] = k; rows n..n_pad-1 = padding point
+// sorted catalog: x64[k] = rows[order[k]], inv[order[k]] = k; rows n..n_pad-1 = padding point
 cudaError_t launch_permute(const double4* x64_rows, const uint32_t* order, uint64_t n, uint64_t n_pad, double4* x64,
-                           float4* x32, uint32_t* inv, cudaStream_t st);
-// bounding sphere of every kSubJ consecutive rows of a padded catalog
-cudaError_t launch_spheres(const double4* x64, uint64_t n_pad, float4* sph, cudaStream_t st);
+                           uint32_t* inv, cudaStream_t st);
+// i-side role: per 4-row quad its (centre, radius) and the rows as fp32 offsets from the centre
+cudaError_t launch_quads(const double4* x64, uint64_t n_pad, float4* xq, float4* cq, cudaStream_t st);
+// j-side role: per 32-row subtile its (centre, radius) and the rows as (-2 offset, |offset|^2)
+cudaError_t launch_subtiles(const double4* x64, uint64_t n_pad, float4* xs, float4* cs, cudaStream_t st);
 // subset mode: caller rows -> positions in the sorted catalog (keys for the sort) with range check
 cudaError_t launch_row_keys(const int64_t* rows, uint64_t nrows, uint64_t n_src, const uint32_t* inv, uint64_t* keys,
                             uint32_t* idx, int* bad_flag, cudaStream_t st);
 // dst[k] = src[pos[k]] for k < nrows, padding point after
-cudaError_t launch_gather(const double4* src64, const float4* src32, const uint64_t* pos, uint64_t nrows,
-                          uint64_t nrows_pad, double4* dst64, float4* dst32, cudaStream_t st);
+cudaError_t launch_gather(const double4* src64, const uint64_t* pos, uint64_t nrows, uint64_t nrows_pad, double4* dst64,
+                          cudaStream_t st);
 cudaError_t launch_pairs_fast(const PairParams& p, CellMap map, int sm_count, cudaStream_t st, LaunchInfo* info);
 cudaError_t launch_pairs_exact64(const PairParams& p, int sm_count, cudaStream_t st, LaunchInfo* info);
 // result[0 .. nbins+1] -> out (device), subtracting `self_pairs` from the slot that holds theta = 0

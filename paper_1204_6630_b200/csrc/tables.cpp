@@ -83,8 +83,13 @@ int exact_slot(double d2, const Binning& b) {
     return lo + 1;
 }
 
-// |d2_fp32 - d2| <= 2.07e-7 sqrt(d2) + 3.0e-7 d2 + 1.1e-14; the constants below add margin.
-double guard_width(double t, double scale) { return scale * (2.5e-7 * std::sqrt(t) + 5.0e-7 * t + 1.0e-13); }
+// Bound on |q_fp32 - q| of the fast engine around a threshold t.  Coordinates are held relative
+// to the centre of their 4-row quad (i side) and 32-row subtile (j side), so every error is relative to the chord d
+// or to the radii r = ri + rj <= kRCap:
+//   difference form (cell-lookup path):      2^-24 (9 d^2 + 9.6 d r)            <= 5.4e-7 t + 5.8e-8 sqrt(t)
+//   expanded form (window path, d >= 4 r):   2^-24 (22 + 42/4 + 36/16) d^2      <= 2.07e-6 t
+// The constants below add margin (x1.7 on the sqrt term, x1.2 on the linear one).
+double guard_width(double t, double scale) { return scale * (1.0e-7 * std::sqrt(t) + 2.5e-6 * t + 1.0e-13); }
 
 // --------------------------------------------------------------------------------------------------
 // Cell maps.  Both are integer/IEEE arithmetic on the float's bit pattern, reproduced exactly on the device.

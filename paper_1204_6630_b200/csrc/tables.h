@@ -18,6 +18,11 @@ constexpr float kPadCoord = 2.0f;      // padding rows are (2,2,2): 6.07 <= d2 <
 constexpr float kDiscardFrom = 5.0f;   // d2 >= 5 can only involve a padding row
 constexpr int kMaxCells = 8192;
 constexpr int kSubJ = 32;              // j-points per window subtile (one bounding sphere each)
+constexpr int kChunkJ = 128;           // j-points per bulk copy into a warp's shared-memory ring (= i-points per warp)
+constexpr int kWarpsPerCta = kThreads / 32;
+constexpr int kWarpI = 32 * kIPerThread;   // i-points per warp work item
+constexpr float kRCap = 0.1f;          // blocks whose bounding radii sum to more go to the fp64 path (guard_width assumes it)
+constexpr float kFarKappa = 4.0f;      // the expanded-form window loops need  min chord >= kFarKappa * (ri + rj)
 constexpr int kMaxWinEdges = 3;        // a (lane, subtile) window that sees more guard bands goes to the cell-lookup path
 
 enum class CellMap : int { LogBits = 0, SqrtLin = 1 };
