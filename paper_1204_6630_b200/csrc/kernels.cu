@@ -139,18 +139,31 @@ __device__ __forceinline__ void lookup_block(const float4* __restrict__ js, cons
     }
 }
 
-// Blocks whose bounding radii are too large for the fp32 error bound (sparse or tiny catalogs, blocks that contain
-// padding rows): every real pair is classified from the fp64 coordinates.
-__device__ __noinline__ void exact_block(SlowCtx* s, uint32_t i0, uint32_t n_i, uint32_t j0, uint32_t n_j, bool mask) {
-    for (int r = 0; r < R; ++r) {
-        const uint32_t i = i0 + r;
-        if (i >= n_i) continue;
-        for (int jj = 0; jj < kSubJ; ++jj) {
-            const uint32_t j = j0 + jj;
-            if (j >= n_j || (mask && j <= i)) continue;
-            recheck_pair(s, i, j);
+// Blocks whose bounding radii are too large for the fp32 error bound (sparse or tiny catalogs, quads or subtiles that
+// straddle a jump of the sort curve or contain padding rows): every real pair is classified from the fp64
+// coordinates.  The warp works together on the lanes in `todo`, one after the other: lane l takes j-row j0 + l.
+__device__ __noinline__ void exact_lanes(SlowCtx* s, unsigned todo, uint32_t ibase, uint32_t n_i, uint32_t j0, uint32_t n_j,
+                                         bool mask) {
+    const int lane = threadIdx.x & 31;
+    const uint32_t j = j0 + lane;
+    const double4 b = s->xj64[j];                   // rows up to the padded size exist
+    unsigned cnt = 0;
+    while (todo) {
+        const int src = __ffs(todo) - 1;
+        todo &= todo - 1;
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const uint32_t i = ibase + src * R + r;
+            if (i >= n_i) break;                    // uniform across the warp
+            const int slot = exact_slot_dev(chord2_f64(s->xi64[i], b), s->thr, s->nbins);
+            if (j < n_j && (!mask || j > i)) {
+                atomicAdd(s->whist + slot, 1u);
+                ++cnt;
+            }
         }
     }
+    cnt = __reduce_add_sync(0xffffffffu, cnt);
+    if (lane == 0 && cnt) atomicAdd(&s->nrecheck, cnt);
 }
 
 // ---- window path ----------------------------------------------------------------------------------------------
@@ -233,12 +246,13 @@ __device__ __forceinline__ void subtile_pairs(const float4* __restrict__ js, con
     }
     if (wmode > kMaxWinEdges) {
         if (mode == 5) {
-            exact_block(slow, i0, n_i, j0, n_j, mask);
+            // counted below, by the whole warp
         } else if (mask) {
             lookup_block<MAP, true>(js, sx, sy, sz, lut, hist, slow, i0, j0, shift, scale, clamp);
         } else {
             lookup_block<MAP, false>(js, sx, sy, sz, lut, hist, slow, i0, j0, shift, scale, clamp);
         }
+        if (wmode == 5) exact_lanes(slow, __ballot_sync(0xffffffffu, mode == 5), i0 - lane * R, n_i, j0, n_j, mask);
         ++npath[wmode == 5 ? 5 : 3];
         return;
     }
@@ -317,7 +331,7 @@ static_assert(kTileJ % kChunkJ == 0 && kTileI % kWarpI == 0 && kTileI / kWarpI =
 // shared-memory layout of pair_fast_kernel (byte offsets; every array 16-byte aligned)
 __host__ __device__ inline uint32_t up16(uint32_t x) { return (x + 15u) & ~15u; }
 struct FastSmem {
-    uint32_t ring, lut, hist, band_mh, band_lh, whist, cell_band, band_slot, bars, slow, total;
+    uint32_t ring, lut, hist, band_mh, band_lh, thr, whist, cell_band, band_slot, bars, slow, total;
 };
 __host__ __device__ inline FastSmem fast_smem_layout(int ncells, int nbands, int nbins) {
     FastSmem L;
@@ -327,6 +341,7 @@ __host__ __device__ inline FastSmem fast_smem_layout(int ncells, int nbands, int
     L.hist = o;       o = up16(o + (uint32_t)ncells * 8);
     L.band_mh = o;    o = up16(o + (uint32_t)nbands * 8);
     L.band_lh = o;    o = up16(o + (uint32_t)nbands * 8);
+    L.thr = o;        o = up16(o + (uint32_t)(nbins + 1) * 8);
     L.whist = o;      o = up16(o + (uint32_t)(nbins + 3) * 4);
     L.cell_band = o;  o = up16(o + (uint32_t)ncells * 2);
     L.band_slot = o;  o = up16(o + (uint32_t)(nbands + 1) * 2);
@@ -401,6 +416,7 @@ __global__ void __launch_bounds__(kThreads, 3) pair_fast_kernel(const __grid_con
     }
     for (int b = tid; b <= p.nbands; b += kThreads) reinterpret_cast<uint16_t*>(smem + L.band_slot)[b] = p.band_slot[b];
     for (int b = tid; b < p.nbins + 3; b += kThreads) wt.whist[b] = 0;
+    for (int b = tid; b <= p.nbins; b += kThreads) reinterpret_cast<double*>(smem + L.thr)[b] = p.thr[b];
     if (lane == 0) {
         for (int b = 0; b < NRING; ++b) mbar_init(bar0 + 8 * b, 1);
         fence_barrier_init();
@@ -408,7 +424,7 @@ __global__ void __launch_bounds__(kThreads, 3) pair_fast_kernel(const __grid_con
     if (tid == 0) {
         slow->xi64 = p.xi64;
         slow->xj64 = p.xj64;
-        slow->thr = p.thr;
+        slow->thr = reinterpret_cast<const double*>(smem + L.thr);
         slow->whist = wt.whist;
         slow->nrecheck = 0;
         slow->nbins = p.nbins;
