@@ -48,6 +48,25 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     } while (!ok);
 }
 
+// ---- packed fp32 pairs (sm_100 f32x2: one instruction, two IEEE round-to-nearest results) --------------------
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pack2(float lo, float hi) {
+    f32x2 d;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(d) : "f"(lo), "f"(hi));
+    return d;
+}
+__device__ __forceinline__ void unpack2(f32x2 v, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) {
+    f32x2 d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) {
+    f32x2 d;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+
 // ---- exact classification (fp64), shared by the recheck path and the fp64 engine -----------------------
 __device__ __forceinline__ double chord2_f64(const double4& a, const double4& b) {
     double dx = a.x - b.x, dy = a.y - b.y, dz = a.z - b.z;
@@ -145,20 +164,24 @@ __device__ __forceinline__ void lookup_block(const float4* __restrict__ js, cons
 __device__ __noinline__ void exact_lanes(SlowCtx* s, unsigned todo, uint32_t ibase, uint32_t n_i, uint32_t j0, uint32_t n_j,
                                          bool mask) {
     const int lane = threadIdx.x & 31;
-    const uint32_t j = j0 + lane;
-    const double4 b = s->xj64[j];                   // rows up to the padded size exist
     unsigned cnt = 0;
-    while (todo) {
-        const int src = __ffs(todo) - 1;
-        todo &= todo - 1;
+#pragma unroll 1
+    for (int h = 0; h < kSubJ / 32; ++h) {
+        const uint32_t j = j0 + h * 32 + lane;
+        const double4 b = s->xj64[j];               // rows up to the padded size exist
+        unsigned rest = todo;
+        while (rest) {
+            const int src = __ffs(rest) - 1;
+            rest &= rest - 1;
 #pragma unroll
-        for (int r = 0; r < R; ++r) {
-            const uint32_t i = ibase + src * R + r;
-            if (i >= n_i) break;                    // uniform across the warp
-            const int slot = exact_slot_dev(chord2_f64(s->xi64[i], b), s->thr, s->nbins);
-            if (j < n_j && (!mask || j > i)) {
-                atomicAdd(s->whist + slot, 1u);
-                ++cnt;
+            for (int r = 0; r < R; ++r) {
+                const uint32_t i = ibase + src * R + r;
+                if (i >= n_i) break;                // uniform across the warp
+                const int slot = exact_slot_dev(chord2_f64(s->xi64[i], b), s->thr, s->nbins);
+                if (j < n_j && (!mask || j > i)) {
+                    atomicAdd(s->whist + slot, 1u);
+                    ++cnt;
+                }
             }
         }
     }
@@ -175,20 +198,35 @@ template <int E>
 __device__ __forceinline__ bool window_block(const float4* __restrict__ js, const float (&sx)[R], const float (&sy)[R],
                                              const float (&sz)[R], const float (&nsm)[R] /* |s|^2 - mid_0 */,
                                              const float (&dt)[kMaxWinEdges], float hmax, unsigned (&c)[kMaxWinEdges]) {
+    // two i-rows per f32x2 register; the j-row is broadcast to both halves
+    f32x2 sx2[R / 2], sy2[R / 2], sz2[R / 2], nsm2[R / 2], dt2[kMaxWinEdges];
 #pragma unroll
-    for (int e = 0; e < kMaxWinEdges; ++e) c[e] = 0;
+    for (int r = 0; r < R / 2; ++r) {
+        sx2[r] = pack2(sx[2 * r], sx[2 * r + 1]);
+        sy2[r] = pack2(sy[2 * r], sy[2 * r + 1]);
+        sz2[r] = pack2(sz[2 * r], sz[2 * r + 1]);
+        nsm2[r] = pack2(nsm[2 * r], nsm[2 * r + 1]);
+    }
+#pragma unroll
+    for (int e = 0; e < kMaxWinEdges; ++e) {
+        c[e] = 0;
+        dt2[e] = pack2(dt[e], dt[e]);
+    }
     float m = 3.0e38f;
-#pragma unroll 8
+#pragma unroll 4
     for (int jj = 0; jj < kSubJ; ++jj) {
         const float4 b = js[jj];
+        const f32x2 bx = pack2(b.x, b.x), by = pack2(b.y, b.y), bz = pack2(b.z, b.z), bw = pack2(b.w, b.w);
 #pragma unroll
-        for (int r = 0; r < R; ++r) {
-            const float q = __fmaf_rn(sx[r], b.x, __fmaf_rn(sy[r], b.y, __fmaf_rn(sz[r], b.z, __fadd_rn(nsm[r], b.w))));
+        for (int r = 0; r < R / 2; ++r) {
+            const f32x2 q = fma2(sx2[r], bx, fma2(sy2[r], by, fma2(sz2[r], bz, add2(nsm2[r], bw))));
 #pragma unroll
             for (int e = 0; e < E; ++e) {
-                const float qe = e ? __fadd_rn(q, dt[e]) : q;
-                c[e] += __float_as_uint(qe) >> 31;
-                m = fminf(m, fabsf(qe));
+                float q0, q1;
+                unpack2(e ? add2(q, dt2[e]) : q, q0, q1);
+                c[e] += __float_as_uint(q0) >> 31;
+                c[e] += __float_as_uint(q1) >> 31;
+                m = fminf(m, fminf(fabsf(q0), fabsf(q1)));
             }
         }
     }
@@ -307,13 +345,14 @@ __device__ __forceinline__ void subtile_pairs(const float4* __restrict__ js, con
     while (todo) {
         const int src = __ffs(todo) - 1;
         todo &= todo - 1;
-        const float4 b = js[lane];
         const uint32_t isrc = i0 + (uint32_t)(src - lane) * R;
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const float ux = __shfl_sync(0xffffffffu, sx[r], src), uy = __shfl_sync(0xffffffffu, sy[r], src),
                         uz = __shfl_sync(0xffffffffu, sz[r], src);
-            lookup_pair<MAP>(ux, uy, uz, b, lut, hist, slow, isrc + r, j0 + lane, true, shift, scale, clamp);
+#pragma unroll
+            for (int h = 0; h < kSubJ / 32; ++h)
+                lookup_pair<MAP>(ux, uy, uz, js[h * 32 + lane], lut, hist, slow, isrc + r, j0 + h * 32 + lane, true, shift, scale, clamp);
         }
         ++npath[4];
     }
@@ -323,9 +362,9 @@ constexpr int NRING = 2;                                               // chunk 
 constexpr int kSubPerChunk = kChunkJ / kSubJ;
 constexpr uint32_t kChunkBytes = kChunkJ * sizeof(float4), kChunkSphBytes = kSubPerChunk * sizeof(float4);
 constexpr uint32_t kSlotBytes = kChunkBytes + kChunkSphBytes;
-static_assert(kSubJ == 32, "the recount of a flagged lane gives j-point l of the subtile to lane l");
-static_assert(kIPerThread == 4, "window_block's pair count assumes R = 4");
-static_assert(kChunkJ == kWarpI, "the diagonal chunk of a warp item is the chunk with the warp's own rows");
+static_assert(kSubJ % 32 == 0, "the recount of a flagged lane gives j-points l, l + 32, .. of the subtile to lane l");
+static_assert(kIPerThread % 2 == 0, "window_block packs two i-rows per f32x2 register");
+static_assert(kWarpI % kChunkJ == 0, "the diagonal chunks of a warp item are the chunks with the warp's own rows");
 static_assert(kTileJ % kChunkJ == 0 && kTileI % kWarpI == 0 && kTileI / kWarpI == kWarpsPerCta, "tiling");
 
 // shared-memory layout of pair_fast_kernel (byte offsets; every array 16-byte aligned)
@@ -387,7 +426,7 @@ __device__ __forceinline__ void flush_slots(unsigned* hist, int nslots, const ui
 // against the j-rows of one plan item; the warp streams those j-rows through its own 2-slot shared-memory ring in
 // 128-row chunks (TMA bulk copies behind mbarriers, issued by lane 0), so no CTA-wide barrier sits in the loop.
 template <int MAP>
-__global__ void __launch_bounds__(kThreads, 3) pair_fast_kernel(const __grid_constant__ PairParams p) {
+__global__ void __launch_bounds__(kThreads, 2) pair_fast_kernel(const __grid_constant__ PairParams p) {
     extern __shared__ __align__(128) unsigned char smem[];
     const FastSmem L = fast_smem_layout(p.ncells, p.nbands, p.nbins);
     char* lut = reinterpret_cast<char*>(smem + L.lut);
@@ -480,8 +519,8 @@ __global__ void __launch_bounds__(kThreads, 3) pair_fast_kernel(const __grid_con
         }
 
         // chunks of kChunkJ rows; in the triangle those wholly below the warp's own rows hold no pair i<j, and the
-        // chunk of the warp's own rows is the diagonal one (masked)
-        const uint32_t dch = ibase / kChunkJ;
+        // chunks of the warp's own rows are the diagonal ones (masked)
+        const uint32_t dch = ibase / kChunkJ, dch_end = (ibase + kWarpI) / kChunkJ;
         uint32_t ch = tile0 * (kTileJ / kChunkJ);
         const uint32_t ch_end = (tile0 + ntiles) * (kTileJ / kChunkJ);
         if (p.tri) ch = max(ch, dch);
@@ -491,7 +530,7 @@ __global__ void __launch_bounds__(kThreads, 3) pair_fast_kernel(const __grid_con
             mbar_wait(bar0 + 8 * (g % NRING), (g / NRING) & 1);
             const float4* jt = reinterpret_cast<const float4*>(ring + (size_t)(g % NRING) * kSlotBytes);
             const float4* jsph = jt + kChunkJ;
-            const bool mask = p.tri && ch == dch;
+            const bool mask = p.tri && ch < dch_end;        // a chunk of the warp's own rows: pairs j > i only
 #pragma unroll 1
             for (int sub = 0; sub < kSubPerChunk; ++sub)
                 subtile_pairs<MAP>(jt + sub * kSubJ, jsph[sub], p.window != 0, mask, px, py, pz, q4.x, q4.y, q4.z, q4.w, wt, lut,

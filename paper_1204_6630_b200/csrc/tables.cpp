@@ -83,13 +83,13 @@ int exact_slot(double d2, const Binning& b) {
     return lo + 1;
 }
 
-// Bound on |q_fp32 - q| of the fast engine around a threshold t.  Coordinates are held relative
-// to the centre of their 4-row quad (i side) and 32-row subtile (j side), so every error is relative to the chord d
-// or to the radii r = ri + rj <= kRCap:
-//   difference form (cell-lookup path):      2^-24 (9 d^2 + 9.6 d r)            <= 5.4e-7 t + 5.8e-8 sqrt(t)
-//   expanded form (window path, d >= 4 r):   2^-24 (22 + 42/4 + 36/16) d^2      <= 2.07e-6 t
-// The constants below add margin (x1.7 on the sqrt term, x1.2 on the linear one).
-double guard_width(double t, double scale) { return scale * (1.0e-7 * std::sqrt(t) + 2.5e-6 * t + 1.0e-13); }
+// Bound on |q_fp32 - q| of the fast engine around a threshold t, u = 2^-24.  Coordinates are
+// held relative to the centre of their kIPerThread-row group (i side) and kSubJ-row subtile (j side), so every error is
+// relative to the chord d or to the radii r = ri + rj <= kRCap:
+//   difference form (cell-lookup path):                   (9 d^2 + 10 d r) u   <= 5.4e-7 t + 6.0e-8 sqrt(t)
+//   expanded form (window path, d >= kFarKappa r = 2.5 r): 29.1 d^2 u          <= 1.74e-6 t
+// The constants below add margin (x1.67 on the sqrt term, x1.72 on the linear one).
+double guard_width(double t, double scale) { return scale * (1.0e-7 * std::sqrt(t) + 3.0e-6 * t + 1.0e-13); }
 
 // --------------------------------------------------------------------------------------------------
 // Cell maps.  Both are integer/IEEE arithmetic on the float's bit pattern, reproduced exactly on the device.
@@ -273,8 +273,8 @@ static void build_fast_tables_impl(const Binning& b, double gs, FastTables& out,
 }
 
 // --------------------------------------------------------------------------------------------------
-// Work plan: the N_D x N_R rectangle (DR) or the i<j triangle (DD, RR) cut into items of one 1024-row
-// i-block times up to `chunk` 1024-column j-tiles (north_star "triangular tiles").
+// Work plan: the N_D x N_R rectangle (DR) or the i<j triangle (DD, RR) cut into items of one kTileI-row
+// i-block times up to `chunk` kTileJ-column j-tiles (north_star "triangular tiles").
 // --------------------------------------------------------------------------------------------------
 void make_plan(bool tri, uint64_t n_i, uint64_t n_j, Plan& p) {
     p = Plan();

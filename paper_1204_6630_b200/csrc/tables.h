@@ -9,9 +9,9 @@ namespace tpcf {
 
 // Geometry shared by the host plan and the kernels.
 constexpr int kThreads = 256;          // threads per CTA
-constexpr int kIPerThread = 4;         // i-points held in registers per thread
-constexpr int kTileI = kThreads * kIPerThread;   // 1024 i-points per CTA work item
-constexpr int kTileJ = 1024;           // j-points per shared-memory tile (16 KB of float4)
+constexpr int kIPerThread = 8;         // i-points held in registers per thread (one "group": they share a bounding sphere)
+constexpr int kTileI = kThreads * kIPerThread;   // 2048 i-points per plan item
+constexpr int kTileJ = kTileI;         // j-points per plan tile (the triangle plan needs kTileJ == kTileI)
 constexpr int kMaxChunk = 8;           // j-tiles per work item, at most
 constexpr int kPlanSMs = 148;          // B200 SM count the plan balances for
 constexpr float kPadCoord = 2.0f;      // padding rows are (2,2,2): 6.07 <= d2 <= 19.9 against any unit vector
@@ -22,7 +22,7 @@ constexpr int kChunkJ = 128;           // j-points per bulk copy into a warp's s
 constexpr int kWarpsPerCta = kThreads / 32;
 constexpr int kWarpI = 32 * kIPerThread;   // i-points per warp work item
 constexpr float kRCap = 0.1f;          // blocks whose bounding radii sum to more go to the fp64 path (guard_width assumes it)
-constexpr float kFarKappa = 4.0f;      // the expanded-form window loops need  min chord >= kFarKappa * (ri + rj)
+constexpr float kFarKappa = 2.5f;      // the expanded-form window loops need  min chord >= kFarKappa * (ri + rj)
 constexpr int kMaxWinEdges = 3;        // a (lane, subtile) window that sees more guard bands goes to the cell-lookup path
 
 enum class CellMap : int { LogBits = 0, SqrtLin = 1 };
