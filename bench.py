@@ -91,16 +91,20 @@ class ClockSampler:
         return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def inst_per_pair(cfg_idx: int):
-    """Thread-level SASS instructions executed per pair by the pair kernel, from the committed ncu summary
-    (profiles/inst_per_pair.json: smsp__thread_inst_executed.sum / pairs); falls back to the static SASS count."""
+# Algorithmic work of one pair: the dot product of PAPER.md:37 in expanded form, 4 FP32
+# lane-operations on the FMA pipes (1 add + 3 fused multiply-adds), and its bin decision against one edge, 1.5
+# lane-operations on the ALU pipe (sign-bit add + half of a 3-input minimum for the guard band).
+OPS_PER_PAIR = 5.5
+
+
+def profile_summary(cfg_idx: int):
+    """Executed-instruction figures of the pair kernel from the committed ncu capture (profiles/inst_per_pair.json)."""
     path = os.path.join(ROOT, "profiles", "inst_per_pair.json")
     try:
         d = json.load(open(path))
-        e = d.get(f"cfg{cfg_idx}") or d["default"]
-        return float(e["inst_per_pair"]), e.get("source", path)
+        return d.get(f"cfg{cfg_idx}") or d["default"]
     except Exception:
-        return 22.0, "static SASS count of the inner loop (no ncu summary found)"
+        return {}
 
 
 # ------------------------------------------------------------------------------------------------ oracle legs
@@ -260,33 +264,32 @@ def run_ours(args):
 
     # ---- roofline of the dominant kernel (pair_fast_kernel): plain ALU issue --------------------------------
     clocks = clk.summary()
-    k_inst, k_src = inst_per_pair(args.config)
+    prof = profile_summary(args.config)
     peak_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     try:
         sm_max = float(json.load(open(peak_path))["sm_max_mhz"])
         peak_src = "MEASURED_PEAKS.json sm_max_mhz"
     except Exception:
         sm_max, peak_src = 1965.0, "fallback 1965 MHz (B200_PROFILING.md nominal clocks.max.sm)"
-    peak = SM_COUNT * LANES_PER_CLK_PER_SM * sm_max * 1e6 / 1e12          # T lane-instructions/s
+    peak = SM_COUNT * LANES_PER_CLK_PER_SM * sm_max * 1e6 / 1e12          # T lane-operations/s
     # per launch: pairs of that histogram (this rank's share) / its own duration; the three launches repeat DD, DR, RR
     share = [w_ / world for w_ in want]
-    per_launch = [share[i % 3] / (ms * 1e-3) for i, ms in enumerate(kernel_ms)] or [pairs_step / world / (ms_step * 1e-3)]
-    pairs_per_s_kernel = sum(share[i % 3] for i in range(len(kernel_ms))) / (sum(kernel_ms) * 1e-3) if kernel_ms else per_launch[0]
-    achieved = pairs_per_s_kernel * k_inst / 1e12
-    roofline = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "Tinst/s (thread-level SASS instructions)",
-                "frac": achieved / peak, "traffic": None,
-                "kernel": "pair_fast_kernel", "inst_per_pair": k_inst, "inst_per_pair_source": k_src,
+    pairs_per_s_kernel = (sum(share[i % 3] for i in range(len(kernel_ms))) / (sum(kernel_ms) * 1e-3)) if kernel_ms \
+        else pairs_step / world / (ms_step * 1e-3)
+    achieved = pairs_per_s_kernel * OPS_PER_PAIR / 1e12
+    roofline = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "T lane-operations/s (FP32 FMA-pipe + ALU-pipe operations)",
+                "frac": achieved / peak, "traffic": prof.get("dram_bytes_per_launch"),
+                "kernel": "pair_fast_kernel", "ops_per_pair": OPS_PER_PAIR,
+                "ops_per_pair_source": "DESIGN.md section 7: 4 FMA-pipe + 1.5 ALU-pipe lane-operations per pair (1-edge window loop)",
+                "executed_inst_per_pair": prof.get("inst_per_pair"), "issue_active_pct": prof.get("issue_active_pct"),
+                "executed_source": prof.get("source"),
                 "kernel_pairs_per_s": pairs_per_s_kernel, "kernel_ms_avg": (sum(kernel_ms) / len(kernel_ms)) if kernel_ms else None,
                 "kernel_launches_timed": len(kernel_ms),
                 "kernel_share_of_step": (sum(kernel_ms) / ms_total) if kernel_ms else None,
                 "pairs_per_clk_per_sm_at_max_clock": pairs_per_s_kernel / (SM_COUNT * sm_max * 1e6),
-                "peak_source": f"{SM_COUNT} SMs x {LANES_PER_CLK_PER_SM} lanes/clk x {sm_max:.0f} MHz ({peak_src}); DESIGN.md section 7",
+                "fma_pipe_bound_pairs_per_clk_per_sm": LANES_PER_CLK_PER_SM / 4.0,
+                "peak_source": f"{SM_COUNT} SMs x {LANES_PER_CLK_PER_SM} FP32 lanes/clk x {sm_max:.0f} MHz ({peak_src}); DESIGN.md section 7",
                 "frac_at_sampled_clock": (achieved / (SM_COUNT * LANES_PER_CLK_PER_SM * clocks["sm_mhz"] * 1e6 / 1e12)) if clocks.get("sm_mhz") else None}
-    try:
-        prof = json.load(open(os.path.join(ROOT, "profiles", "inst_per_pair.json")))
-        roofline["traffic"] = (prof.get(f"cfg{args.config}") or prof["default"]).get("dram_bytes_per_launch")
-    except Exception:
-        pass
 
     # ---- the oracle timed beside it (rank 0, N = 1 only) --------------------------------------------------------
     cpu = None
@@ -313,7 +316,7 @@ def run_ours(args):
                     "seconds_per_step": e2e_s, "steps": e2e_steps,
                     "path": "tpcf_load(D), tpcf_load(R) from pinned host rows + tpcf_count x3 + tpcf_estimate"},
             "gpu_launches": args.steps * 6,
-            "gpu_launches_note": "per step: 3 x (pair_fast_kernel + finalize_kernel); memsets are driver memset nodes",
+            "gpu_launches_note": "per step: 3 x (pair_fast_kernel + finalize_kernel); memsets are driver memset nodes; the e2e leg adds 2 x 28 load kernels per step",
             "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu, "paper_context": PAPER_CONTEXT}
     print(json.dumps(line))
     if world > 1:

@@ -19,7 +19,7 @@ struct Catalog {                 // rows in Hilbert order (counts are order-inva
     uint64_t n = 0, n_pad = 0;
     double4* x64 = nullptr;
     uint32_t* inv = nullptr;     // caller row -> position in the sorted catalog (row-subset mode)
-    float4 *xq = nullptr, *cq = nullptr;   // i-side role: rows as offsets from their 4-row quad centre; (centre, radius)
+    float4 *xq = nullptr, *cq = nullptr;   // i-side role: rows as offsets from their 8-row group ("quad") centre; (centre, radius)
     float4 *xs = nullptr, *cs = nullptr;   // j-side role: rows as (-2 offset, |offset|^2) from their 32-row subtile centre
 };
 // scratch of one spatial sort: (key, idx) ping-pong buffers and the digit counts
@@ -433,7 +433,7 @@ tpcf_status tpcf_load(tpcf_ctx* ctx, tpcf_cat which, const void* radec_deg, tpcf
         if (e != cudaSuccess) { cleanup(); free_catalog(c); return cuda_fail(ctx, e, "copy catalog to device"); }
         src = staged;
     }
-    // convert (fp64 unit vectors + Hilbert keys) -> sort -> sorted fp64 rows + row map -> quad and subtile roles
+    // convert (fp64 unit vectors + sort keys) -> sort -> sorted fp64 rows + row map -> quad and subtile roles
     e = cudaMemsetAsync(ctx->d_bad, 0, sizeof(int), st);
     if (e == cudaSuccess) e = launch_convert(src, dt == TPCF_F64, n, rows64, sc.ka, sc.ia, ctx->d_bad, st);
     bool in_a = true;

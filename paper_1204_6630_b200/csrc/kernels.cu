@@ -61,6 +61,11 @@ __device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) {
     asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
     return d;
 }
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) {
+    f32x2 d;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
 __device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) {
     f32x2 d;
     asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
@@ -195,18 +200,11 @@ __device__ __noinline__ void exact_lanes(SlowCtx* s, unsigned todo, uint32_t iba
 // |q - ...| is tracked (FMNMX3, two values per instruction).  Returns true when some pair came within a band's half
 // width: this lane's counters are then not used and its pairs are recounted one by one.
 template <int E>
-__device__ __forceinline__ bool window_block(const float4* __restrict__ js, const float (&sx)[R], const float (&sy)[R],
-                                             const float (&sz)[R], const float (&nsm)[R] /* |s|^2 - mid_0 */,
+__device__ __forceinline__ bool window_block(const float4* __restrict__ js, const f32x2 (&sx2)[R / 2], const f32x2 (&sy2)[R / 2],
+                                             const f32x2 (&sz2)[R / 2], const f32x2 (&nsm2)[R / 2] /* |s|^2 - mid_0 */,
                                              const float (&dt)[kMaxWinEdges], float hmax, unsigned (&c)[kMaxWinEdges]) {
     // two i-rows per f32x2 register; the j-row is broadcast to both halves
-    f32x2 sx2[R / 2], sy2[R / 2], sz2[R / 2], nsm2[R / 2], dt2[kMaxWinEdges];
-#pragma unroll
-    for (int r = 0; r < R / 2; ++r) {
-        sx2[r] = pack2(sx[2 * r], sx[2 * r + 1]);
-        sy2[r] = pack2(sy[2 * r], sy[2 * r + 1]);
-        sz2[r] = pack2(sz[2 * r], sz[2 * r + 1]);
-        nsm2[r] = pack2(nsm[2 * r], nsm[2 * r + 1]);
-    }
+    f32x2 dt2[kMaxWinEdges];
 #pragma unroll
     for (int e = 0; e < kMaxWinEdges; ++e) {
         c[e] = 0;
@@ -247,7 +245,7 @@ struct WinTables {
 //   1..3  window loop with that many edges      4  cell lookup      5  fp64
 template <int MAP>
 __device__ __forceinline__ void subtile_pairs(const float4* __restrict__ js, const float4 sp, bool windows, bool mask,
-                                              const float (&px)[R], const float (&py)[R], const float (&pz)[R], float cqx,
+                                              const f32x2 (&px2)[R / 2], const f32x2 (&py2)[R / 2], const f32x2 (&pz2)[R / 2], float cqx,
                                               float cqy, float cqz, float ri, const WinTables& wt, const char* lut,
                                               char* hist, SlowCtx* slow, uint32_t i0, uint32_t n_i, uint32_t j0,
                                               uint32_t n_j, int shift, float scale, float clamp, unsigned (&npath)[6]) {
@@ -275,12 +273,19 @@ __device__ __forceinline__ void subtile_pairs(const float4* __restrict__ js, con
     }
     const int wmode = __reduce_max_sync(0xffffffffu, mode);
 
-    float sx[R], sy[R], sz[R];
+    f32x2 sx2[R / 2], sy2[R / 2], sz2[R / 2];
+    float sx[R], sy[R], sz[R];                      // the same registers, one row at a time
+    {
+        const f32x2 tx2 = pack2(tx, tx), ty2 = pack2(ty, ty), tz2 = pack2(tz, tz);
 #pragma unroll
-    for (int r = 0; r < R; ++r) {
-        sx[r] = __fadd_rn(px[r], tx);
-        sy[r] = __fadd_rn(py[r], ty);
-        sz[r] = __fadd_rn(pz[r], tz);
+        for (int r = 0; r < R / 2; ++r) {
+            sx2[r] = add2(px2[r], tx2);
+            sy2[r] = add2(py2[r], ty2);
+            sz2[r] = add2(pz2[r], tz2);
+            unpack2(sx2[r], sx[2 * r], sx[2 * r + 1]);
+            unpack2(sy2[r], sy[2 * r], sy[2 * r + 1]);
+            unpack2(sz2[r], sz[2 * r], sz[2 * r + 1]);
+        }
     }
     if (wmode > kMaxWinEdges) {
         if (mode == 5) {
@@ -297,7 +302,7 @@ __device__ __forceinline__ void subtile_pairs(const float4* __restrict__ js, con
     // every lane runs the wmode-edge loop on bands k .. k+wmode-1; lowering k keeps the lane's window inside them
     k = min(k, wt.nbands - wmode);
     const float2 mh0 = wt.band_mh[k];
-    float hmax = mh0.y, dt[kMaxWinEdges], nsm[R];
+    float hmax = mh0.y, dt[kMaxWinEdges];
     dt[0] = 0.f;
 #pragma unroll
     for (int e = 1; e < kMaxWinEdges; ++e) {
@@ -308,26 +313,29 @@ __device__ __forceinline__ void subtile_pairs(const float4* __restrict__ js, con
             hmax = fmaxf(hmax, mh.y);
         }
     }
+    f32x2 nsm2[R / 2];
+    {
+        const f32x2 nmid = pack2(-mh0.x, -mh0.x);
 #pragma unroll
-    for (int r = 0; r < R; ++r)
-        nsm[r] = __fsub_rn(__fmaf_rn(sz[r], sz[r], __fmaf_rn(sy[r], sy[r], __fmul_rn(sx[r], sx[r]))), mh0.x);
+        for (int r = 0; r < R / 2; ++r) nsm2[r] = add2(fma2(sz2[r], sz2[r], fma2(sy2[r], sy2[r], mul2(sx2[r], sx2[r]))), nmid);
+    }
     unsigned c[kMaxWinEdges], cnt[kMaxWinEdges + 1];
     bool flagged;
     if (wmode == 1) {
-        flagged = window_block<1>(js, sx, sy, sz, nsm, dt, hmax, c);
+        flagged = window_block<1>(js, sx2, sy2, sz2, nsm2, dt, hmax, c);
         cnt[0] = c[0];
         cnt[1] = kSubJ * R - c[0];
         cnt[2] = cnt[3] = 0;
         ++npath[0];
     } else if (wmode == 2) {
-        flagged = window_block<2>(js, sx, sy, sz, nsm, dt, hmax, c);
+        flagged = window_block<2>(js, sx2, sy2, sz2, nsm2, dt, hmax, c);
         cnt[0] = c[0];
         cnt[1] = c[1] - c[0];
         cnt[2] = kSubJ * R - c[1];
         cnt[3] = 0;
         ++npath[1];
     } else {
-        flagged = window_block<3>(js, sx, sy, sz, nsm, dt, hmax, c);
+        flagged = window_block<3>(js, sx2, sy2, sz2, nsm2, dt, hmax, c);
         cnt[0] = c[0];
         cnt[1] = c[1] - c[0];
         cnt[2] = c[2] - c[1];
@@ -422,7 +430,7 @@ __device__ __forceinline__ void flush_slots(unsigned* hist, int nslots, const ui
     }
 }
 
-// The pair kernel.  Persistent CTAs of 8 independent warps.  A warp item = 128 consecutive i-rows (one quad per lane)
+// The pair kernel.  Persistent CTAs of 8 independent warps.  A warp item = kWarpI = 256 consecutive i-rows (one 8-row group per lane)
 // against the j-rows of one plan item; the warp streams those j-rows through its own 2-slot shared-memory ring in
 // 128-row chunks (TMA bulk copies behind mbarriers, issued by lane 0), so no CTA-wide barrier sits in the loop.
 template <int MAP>
@@ -504,19 +512,16 @@ __global__ void __launch_bounds__(kThreads, 2) pair_fast_kernel(const __grid_con
         // catalog is moved to (-2,-2,-2): 6 <= d2 <= 48 against every real or padding j-row, i.e. always discarded.
         const uint32_t ibase = I * kTileI + ws * kWarpI, i0 = ibase + lane * R;
         float4 q4 = p.cq[i0 / R];
-        float px[R], py[R], pz[R];
+        f32x2 px2[R / 2], py2[R / 2], pz2[R / 2];
 #pragma unroll
-        for (int r = 0; r < R; ++r) {
-            const float4 a = p.xq[i0 + r];
-            px[r] = a.x;
-            py[r] = a.y;
-            pz[r] = a.z;
+        for (int r = 0; r < R / 2; ++r) {
+            float4 a0 = p.xq[i0 + 2 * r], a1 = p.xq[i0 + 2 * r + 1];
+            if (i0 >= p.n_i) a0 = a1 = make_float4(0.f, 0.f, 0.f, 0.f);
+            px2[r] = pack2(a0.x, a1.x);
+            py2[r] = pack2(a0.y, a1.y);
+            pz2[r] = pack2(a0.z, a1.z);
         }
-        if (i0 >= p.n_i) {
-            q4 = make_float4(-kPadCoord, -kPadCoord, -kPadCoord, 0.f);
-#pragma unroll
-            for (int r = 0; r < R; ++r) px[r] = py[r] = pz[r] = 0.f;
-        }
+        if (i0 >= p.n_i) q4 = make_float4(-kPadCoord, -kPadCoord, -kPadCoord, 0.f);
 
         // chunks of kChunkJ rows; in the triangle those wholly below the warp's own rows hold no pair i<j, and the
         // chunks of the warp's own rows are the diagonal ones (masked)
@@ -533,7 +538,7 @@ __global__ void __launch_bounds__(kThreads, 2) pair_fast_kernel(const __grid_con
             const bool mask = p.tri && ch < dch_end;        // a chunk of the warp's own rows: pairs j > i only
 #pragma unroll 1
             for (int sub = 0; sub < kSubPerChunk; ++sub)
-                subtile_pairs<MAP>(jt + sub * kSubJ, jsph[sub], p.window != 0, mask, px, py, pz, q4.x, q4.y, q4.z, q4.w, wt, lut,
+                subtile_pairs<MAP>(jt + sub * kSubJ, jsph[sub], p.window != 0, mask, px2, py2, pz2, q4.x, q4.y, q4.z, q4.w, wt, lut,
                                    reinterpret_cast<char*>(hist), slow, i0, p.n_i, ch * kChunkJ + sub * kSubJ, p.n_j, p.shift,
                                    p.sqrt_scale, p.sqrt_clamp, npath);
             __syncwarp();
@@ -770,7 +775,8 @@ __global__ void permute_kernel(const double4* __restrict__ x64_rows, const uint3
     }
 }
 
-// i-side role of a catalog: every kIPerThread = 4 consecutive rows form a quad (one lane of the pair kernel).
+// i-side role of a catalog: every kIPerThread = 8 consecutive rows form a group ("quad" in the names below: one lane
+// of the pair kernel).
 // cq = (fp32 centre, radius): the centre is the fp32 rounding of the mean, the radius bounds the fp64 distance of
 // the fp64 rows from that fp32 point (rounded up, with slack).  xq = fp32 rounding of (row - centre), formed in fp64:
 // its error is 2^-24 of the OFFSET, not of the unit vector.

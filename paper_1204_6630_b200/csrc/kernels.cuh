@@ -9,7 +9,7 @@ namespace tpcf {
 
 // One pair-count launch: i-points x j-points over the work plan.  All pointers are device pointers.
 struct PairParams {
-    // i side: rows as fp32 offsets from the centre of their 4-row quad, and the quads' (centre, radius)
+    // i side: rows as fp32 offsets from the centre of their 8-row group ("quad"), and the groups' (centre, radius)
     const float4* xq;
     const float4* cq;
     // j side: rows as (-2 offset, |offset|^2) from the centre of their 32-row subtile, and the subtiles' (centre, radius)
@@ -61,7 +61,7 @@ cudaError_t launch_sort_pairs(uint64_t* keys_a, uint64_t* keys_b, uint32_t* idx_
 // sorted catalog: x64[k] = rows[order[k]], inv[order[k]] = k; rows n..n_pad-1 = padding point
 cudaError_t launch_permute(const double4* x64_rows, const uint32_t* order, uint64_t n, uint64_t n_pad, double4* x64,
                            uint32_t* inv, cudaStream_t st);
-// i-side role: per 4-row quad its (centre, radius) and the rows as fp32 offsets from the centre
+// i-side role: per kIPerThread-row group ("quad") its (centre, radius) and the rows as fp32 offsets from the centre
 cudaError_t launch_quads(const double4* x64, uint64_t n_pad, float4* xq, float4* cq, cudaStream_t st);
 // j-side role: per 32-row subtile its (centre, radius) and the rows as (-2 offset, |offset|^2)
 cudaError_t launch_subtiles(const double4* x64, uint64_t n_pad, float4* xs, float4* cs, cudaStream_t st);
