@@ -165,6 +165,54 @@ def test_full_size_configs_on_row_subset_and_identities(idx, nrows, oracle_threa
         assert abs(int(f["RR"][-1]) - totals(nd, nr)["RR"] / 2) <= 6.0 * math.sqrt(totals(nd, nr)["RR"] / 2)
 
 
+@pytest.mark.parametrize("idx,nd,nr", [(3, 60_000, 50_000), (5, 40_000, 30_000), (2, 30_000, 30_000)])
+def test_every_kernel_path_gives_the_same_histogram(idx, nd, nr):
+    """The window loops (1-3 candidate edges per block), the per-pair cell lookup, the fp64 blocks and the plain fp64
+    engine are four ways to the same integers: bit-identical histograms, and the path
+    statistics show that each of them was really exercised."""
+    D, R, e, cfg = synth.make_config(idx, n_d=nd, n_r=nr)
+    with T.Context(cfg.nbins, e, "explicit") as c:
+        c.load("D", D)
+        c.load("R", R)
+        win, used = {}, np.zeros(6, dtype=np.int64)
+        for k in KINDS:
+            win[k] = full(*c.count(k))
+            st = c.stats()
+            used += np.asarray(st["win_blocks"], dtype=np.int64)
+            assert int(win[k].sum()) == totals(nd, nr)[k] == st["pairs"]
+        assert used[0] + used[1] + used[2] > 0, "no block took a window loop"
+        assert used[3] > 0, "no block took the cell-lookup path (diagonal chunks always do)"
+        c.set_window(False)
+        for k in KINDS:
+            np.testing.assert_array_equal(full(*c.count(k)), win[k])
+            assert sum(c.stats()["win_blocks"][:3]) == 0
+        c.set_window(True)
+        c.set_guard_scale(8.0)                       # 8x wider guard bands: more fp64 rechecks, same integers
+        np.testing.assert_array_equal(full(*c.count("DR")), win["DR"])
+        c.set_guard_scale(1.0)
+        c.set_engine("exact64")
+        for k in KINDS:
+            np.testing.assert_array_equal(full(*c.count(k)), win[k])
+
+
+def test_sparse_catalogs_fall_back_to_fp64_blocks(oracle_threads):
+    """A few hundred points on the whole sky: every bounding radius exceeds the cap of the fp32 error bound, so all
+    blocks are classified from the fp64 coordinates -- and still match the oracle."""
+    rng = np.random.default_rng(11)
+    def sky(n):
+        return np.stack([rng.uniform(0.0, 360.0, n), np.degrees(np.arcsin(rng.uniform(-1.0, 1.0, n)))], 1)
+    D, R = sky(700), sky(900)
+    e = np.linspace(0.0, 180.0, 37)
+    with T.Context(36, e, "explicit") as c:
+        c.load("D", D)
+        c.load("R", R)
+        g = gpu_all(c)
+        assert c.stats()["win_blocks"][5] > 0
+        o = oracle_all(D, R, c.edges(), oracle_threads)
+        for k in KINDS:
+            assert_parity(g[k], o[k], totals(700, 900)[k])
+
+
 def test_config5_shuffled_rows_give_the_same_histogram():
     D, R, e, cfg = synth.make_config(5, n_d=60_000, n_r=1000)
     S, _, _, _ = synth.make_config(5, n_d=60_000, n_r=1000, shuffle_d=True)
