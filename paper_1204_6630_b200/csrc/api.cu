@@ -61,6 +61,8 @@ struct tpcf_ctx {
     unsigned long long* d_counters = nullptr;   // kNumCounters
     unsigned long long* d_out = nullptr;        // nbins + 2
     int* d_bad = nullptr;
+    void* arena = nullptr;                      // scratch of tpcf_load, grown on demand, kept until destroy
+    size_t arena_bytes = 0;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
     bool time_kernels = false;
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> kev_pool, kev_used;
@@ -178,6 +180,28 @@ tpcf_status alloc_sort_scratch(tpcf_ctx* ctx, SortScratch& sc, uint64_t n) {
     CU(cudaMalloc(&sc.counts, 256 * nblk * sizeof(uint32_t)), "cudaMalloc sort counts");
     return TPCF_OK;
 }
+
+// One device block for the scratch of a load, reused by later loads (a load ends with a stream synchronize, so no
+// work is in flight on it when the next one starts): no cudaMalloc / cudaFree on the steady-state path.
+tpcf_status arena_reserve(tpcf_ctx* ctx, size_t bytes) {
+    if (ctx->arena_bytes >= bytes) return TPCF_OK;
+    cudaFree(ctx->arena);
+    ctx->arena = nullptr;
+    ctx->arena_bytes = 0;
+    CU(cudaMalloc(&ctx->arena, bytes), "cudaMalloc load scratch");
+    ctx->arena_bytes = bytes;
+    return TPCF_OK;
+}
+struct Carver {
+    char* base;
+    size_t off = 0;
+    template <typename T>
+    T* take(size_t count) {
+        T* p = reinterpret_cast<T*>(base + off);
+        off += (count * sizeof(T) + 255) & ~size_t(255);
+        return p;
+    }
+};
 
 uint64_t pad_to(uint64_t n, uint64_t m) { return (n + m - 1) / m * m; }
 
@@ -398,7 +422,8 @@ tpcf_status tpcf_load(tpcf_ctx* ctx, tpcf_cat which, const void* radec_deg, tpcf
     if (s) return s;
     cudaStream_t st = cuda_stream ? static_cast<cudaStream_t>(cuda_stream) : ctx->stream;
     Catalog& c = ctx->cat[which];
-    free_catalog(c);
+    // the arrays of the catalog being replaced may still be read by counts enqueued on the context's stream
+    if (st != ctx->stream) CU(cudaStreamSynchronize(ctx->stream), "cudaStreamSynchronize");
     for (int k = 0; k < 3; ++k) {           // DR depends on both catalogs
         const Sides sd = sides_of((tpcf_kind)k);
         if (sd.ci == (int)which || sd.cj == (int)which) {
@@ -408,29 +433,36 @@ tpcf_status tpcf_load(tpcf_ctx* ctx, tpcf_cat which, const void* radec_deg, tpcf
     }
     const uint64_t n_pad = pad_to(n, kTileI);
     const size_t esz = (dt == TPCF_F64) ? 8 : 4;
-    CU(cudaMalloc(&c.x64, n_pad * sizeof(double4)), "cudaMalloc catalog (fp64)");
-    CU(cudaMalloc(&c.inv, n * sizeof(uint32_t)), "cudaMalloc catalog (row map)");
-    CU(cudaMalloc(&c.xq, n_pad * sizeof(float4)), "cudaMalloc catalog (quad offsets)");
-    CU(cudaMalloc(&c.cq, n_pad / kIPerThread * sizeof(float4)), "cudaMalloc catalog (quad centres)");
-    CU(cudaMalloc(&c.xs, n_pad * sizeof(float4)), "cudaMalloc catalog (subtile offsets)");
-    CU(cudaMalloc(&c.cs, n_pad / kSubJ * sizeof(float4)), "cudaMalloc catalog (subtile centres)");
-    void* staged = nullptr;
-    double4* rows64 = nullptr;
+    if (c.x64 && c.n_pad == n_pad && c.n == n) {
+        c.n = 0;                                // same shape as the catalog it replaces: keep the device arrays
+    } else {
+        free_catalog(c);
+        CU(cudaMalloc(&c.x64, n_pad * sizeof(double4)), "cudaMalloc catalog (fp64)");
+        CU(cudaMalloc(&c.inv, n * sizeof(uint32_t)), "cudaMalloc catalog (row map)");
+        CU(cudaMalloc(&c.xq, n_pad * sizeof(float4)), "cudaMalloc catalog (quad offsets)");
+        CU(cudaMalloc(&c.cq, n_pad / kIPerThread * sizeof(float4)), "cudaMalloc catalog (quad centres)");
+        CU(cudaMalloc(&c.xs, n_pad * sizeof(float4)), "cudaMalloc catalog (subtile offsets)");
+        CU(cudaMalloc(&c.cs, n_pad / kSubJ * sizeof(float4)), "cudaMalloc catalog (subtile centres)");
+    }
+    const uint64_t nblk = (n + kSortChunk - 1) / kSortChunk;
+    const size_t need = n * sizeof(double4) + 2 * n * sizeof(uint64_t) + 2 * n * sizeof(uint32_t) + 256 * nblk * sizeof(uint32_t) +
+                        (on_device ? 0 : n * 2 * esz) + 8 * 256;
+    s = arena_reserve(ctx, need);
+    if (s) { free_catalog(c); return s; }
+    Carver cv{static_cast<char*>(ctx->arena)};
+    double4* rows64 = cv.take<double4>(n);
     SortScratch sc;
-    auto cleanup = [&]() {
-        cudaFree(staged);
-        cudaFree(rows64);
-        sc.release();
-    };
-    cudaError_t e = cudaMalloc(&rows64, n * sizeof(double4));
-    if (e != cudaSuccess) { cleanup(); free_catalog(c); return cuda_fail(ctx, e, "cudaMalloc rows"); }
-    s = alloc_sort_scratch(ctx, sc, n);
-    if (s) { cleanup(); free_catalog(c); return s; }
+    sc.ka = cv.take<uint64_t>(n);
+    sc.kb = cv.take<uint64_t>(n);
+    sc.ia = cv.take<uint32_t>(n);
+    sc.ib = cv.take<uint32_t>(n);
+    sc.counts = cv.take<uint32_t>(256 * nblk);
+    cudaError_t e = cudaSuccess;
     const void* src = radec_deg;
     if (!on_device) {
-        e = cudaMalloc(&staged, n * 2 * esz);
-        if (e == cudaSuccess) e = cudaMemcpyAsync(staged, radec_deg, n * 2 * esz, cudaMemcpyHostToDevice, st);
-        if (e != cudaSuccess) { cleanup(); free_catalog(c); return cuda_fail(ctx, e, "copy catalog to device"); }
+        void* staged = cv.take<char>(n * 2 * esz);
+        e = cudaMemcpyAsync(staged, radec_deg, n * 2 * esz, cudaMemcpyHostToDevice, st);
+        if (e != cudaSuccess) { free_catalog(c); return cuda_fail(ctx, e, "copy catalog to device"); }
         src = staged;
     }
     // convert (fp64 unit vectors + sort keys) -> sort -> sorted fp64 rows + row map -> quad and subtile roles
@@ -444,7 +476,6 @@ tpcf_status tpcf_load(tpcf_ctx* ctx, tpcf_cat which, const void* radec_deg, tpcf
     int bad = 0;
     if (e == cudaSuccess) e = cudaMemcpyAsync(&bad, ctx->d_bad, sizeof(int), cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-    cleanup();
     if (e != cudaSuccess) {
         free_catalog(c);
         return cuda_fail(ctx, e, "convert catalog");
@@ -545,6 +576,7 @@ void tpcf_destroy(tpcf_ctx* ctx) {
         cudaFree(ctx->d_out);
         cudaFree(ctx->d_counters);
         cudaFree(ctx->d_bad);
+        cudaFree(ctx->arena);
         if (ctx->ev0) cudaEventDestroy(ctx->ev0);
         if (ctx->ev1) cudaEventDestroy(ctx->ev1);
         for (auto* v : {&ctx->kev_pool, &ctx->kev_used})

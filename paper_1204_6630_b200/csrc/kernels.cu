@@ -801,15 +801,21 @@ __global__ void quads_kernel(const double4* __restrict__ x64, uint64_t nquads, f
     }
 }
 
-// j-side role: every kSubJ = 32 consecutive rows form a subtile (one warp here).  cs = (fp32 centre, radius) as
+// j-side role: every kSubJ consecutive rows form a subtile (one warp here).  cs = (fp32 centre, radius) as
 // above; xs = (-2 b', |b'|^2) with b' the fp32 rounding of (row - centre) formed in fp64 and |b'|^2 the fp32
 // rounding of the fp64 square of that rounded offset (the window loops evaluate |a - b|^2 = |a|^2 + |b|^2 - 2 a.b).
 __global__ void subtiles_kernel(const double4* __restrict__ x64, uint64_t nsub, float4* __restrict__ xs, float4* __restrict__ cs) {
+    constexpr int H = kSubJ / 32;                   // rows per lane
     const uint64_t w = (blockIdx.x * (uint64_t)blockDim.x + threadIdx.x) >> 5;
     const int lane = threadIdx.x & 31;
     if (w >= nsub) return;
-    const double4 v = x64[w * kSubJ + lane];
-    double sx = v.x, sy = v.y, sz = v.z;
+    double4 v[H];
+    double sx = 0, sy = 0, sz = 0;
+#pragma unroll
+    for (int h = 0; h < H; ++h) {
+        v[h] = x64[w * kSubJ + h * 32 + lane];
+        sx += v[h].x; sy += v[h].y; sz += v[h].z;
+    }
 #pragma unroll
     for (int off = 16; off; off >>= 1) {
         sx += __shfl_xor_sync(0xffffffffu, sx, off);
@@ -817,13 +823,17 @@ __global__ void subtiles_kernel(const double4* __restrict__ x64, uint64_t nsub, 
         sz += __shfl_xor_sync(0xffffffffu, sz, off);
     }
     const float cx = (float)(sx / kSubJ), cy = (float)(sy / kSubJ), cz = (float)(sz / kSubJ);
-    const double dx = v.x - (double)cx, dy = v.y - (double)cy, dz = v.z - (double)cz;
-    double r = sqrt(dx * dx + dy * dy + dz * dz);
+    double r = 0;
+#pragma unroll
+    for (int h = 0; h < H; ++h) {
+        const double dx = v[h].x - (double)cx, dy = v[h].y - (double)cy, dz = v[h].z - (double)cz;
+        r = fmax(r, sqrt(dx * dx + dy * dy + dz * dz));
+        const float bx = (float)dx, by = (float)dy, bz = (float)dz;
+        const double nb = (double)bx * bx + (double)by * by + (double)bz * bz;
+        xs[w * kSubJ + h * 32 + lane] = make_float4(-2.f * bx, -2.f * by, -2.f * bz, (float)nb);
+    }
 #pragma unroll
     for (int off = 16; off; off >>= 1) r = fmax(r, __shfl_xor_sync(0xffffffffu, r, off));
-    const float bx = (float)dx, by = (float)dy, bz = (float)dz;
-    const double nb = (double)bx * bx + (double)by * by + (double)bz * bz;
-    xs[w * kSubJ + lane] = make_float4(-2.f * bx, -2.f * by, -2.f * bz, (float)nb);
     if (lane == 0) cs[w] = make_float4(cx, cy, cz, __double2float_ru(r * (1.0 + 1.0e-7) + 1.0e-12));
 }
 

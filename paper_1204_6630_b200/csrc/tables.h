@@ -17,7 +17,7 @@ constexpr int kPlanSMs = 148;          // B200 SM count the plan balances for
 constexpr float kPadCoord = 2.0f;      // padding rows are (2,2,2): 6.07 <= d2 <= 19.9 against any unit vector
 constexpr float kDiscardFrom = 5.0f;   // d2 >= 5 can only involve a padding row
 constexpr int kMaxCells = 8192;
-constexpr int kSubJ = 32;              // j-points per window subtile (one bounding sphere each)
+constexpr int kSubJ = 64;              // j-points per window subtile (one bounding sphere each)
 constexpr int kChunkJ = 128;           // j-points per bulk copy into a warp's shared-memory ring (= i-points per warp)
 constexpr int kWarpsPerCta = kThreads / 32;
 constexpr int kWarpI = 32 * kIPerThread;   // i-points per warp work item

@@ -114,6 +114,89 @@ def test_fast_tables_agree_with_thresholds_outside_the_guard_bands(idx, scale):
         assert c.stats()["cells"] <= 8192
 
 
+@pytest.mark.parametrize("idx", [1, 3, 5])
+def test_guard_bands_and_window_selection(idx):
+    """The guard bands the window loops compare against, and the host mirror of the kernel's window selection
+    (tpcf_window_host) against a brute-force scan of the band list."""
+    cfg = synth.CONFIGS[idx]
+    rng = np.random.default_rng(100 + idx)
+    with T.Context(cfg.nbins, synth.config_edges(cfg), "explicit") as c:
+        thr = c.thresholds()
+        lo, hi, below = c.bands()
+        n = len(lo)
+        assert np.all(lo[1:] >= hi[:-1]) and np.all(hi >= lo), "bands ascending and disjoint"
+        assert lo[-1] == hi[-1] == 5.0 and below[-1] <= cfg.nbins + 1, "last band: the zero-width discard edge"
+        live = [k for k in range(cfg.nbins + 1) if not (k == 0 and thr[0] == 0.0) and not (k == cfg.nbins and thr[-1] >= 4.0)]
+        assert n == len(live) + 1, "one band per droppable edge (none merged on the BASELINE configs) + discard"
+        for b, k in enumerate(live):
+            g = fp32_bound(thr[k])
+            assert lo[b] <= thr[k] - g and thr[k] + g <= hi[b], "band covers the edge by more than the fp32 bound"
+            assert below[b] == k, "result slot just below band b is the bin below edge k"
+        for _ in range(4000):
+            a = float(np.float32(np.exp(rng.uniform(np.log(1e-9), np.log(4.0)))))
+            w = float(np.float32(a * (1.0 + np.exp(rng.uniform(np.log(1e-4), np.log(3.0))))))
+            k, e = T.tpcf_window_host(c._ctx, a, w)
+            touch = [b for b in range(n) if hi[b] > a and lo[b] <= w]          # bands the interval [a, w] can reach
+            assert all(hi[b] <= a for b in range(k)), "no band below the first one reaches the interval"
+            if e <= 3:
+                assert set(touch) <= set(range(k, k + e)), (a, w, k, e, touch)
+            else:
+                assert len(touch) > 3 or (touch and touch[-1] - k >= 3)
+
+
+def _f32(x):
+    return np.asarray(x, dtype=np.float32)
+
+
+def _fma32(a, b, c):
+    """fp32 fused multiply-add: the product of two fp32 numbers is exact in fp64; one rounding to fp32 follows."""
+    return _f32(a.astype(np.float64) * b.astype(np.float64) + c.astype(np.float64))
+
+
+def test_fp32_error_bounds_of_design_section_4():
+    """DESIGN.md section 4 in numbers: the kernel's two fp32 evaluations of the squared chord, replayed here in numpy
+    fp32 on random (group, subtile) geometry, against the fp64 value.  Expanded form (window loops, chord >= 2.5 r):
+    |error| <= 29.1 u max(d^2, mid); difference form (cell lookup): |error| <= (9 d^2 + 10 d r) u; u = 2^-24."""
+    rng = np.random.default_rng(7)
+    u = 2.0 ** -24
+    n = 400_000
+    def unit(v):
+        return v / np.linalg.norm(v, axis=1, keepdims=True)
+    cq64 = unit(rng.normal(size=(n, 3)))
+    ri = np.exp(rng.uniform(np.log(1e-6), np.log(0.04), n))
+    rj = np.exp(rng.uniform(np.log(1e-6), np.log(0.05), n))
+    sep = (ri + rj) * np.exp(rng.uniform(np.log(3.6), np.log(400.0), n))      # centre distance: blocks from 2.6 r out
+    cs64 = unit(cq64 + unit(np.cross(cq64, rng.normal(size=(n, 3)))) * sep[:, None])
+    cq, cs = _f32(cq64), _f32(cs64)                                            # fp32 centres (exact values from here on)
+    a = cq.astype(np.float64) + unit(rng.normal(size=(n, 3))) * (ri * rng.uniform(0, 1, n))[:, None]    # fp64 rows
+    b = cs.astype(np.float64) + unit(rng.normal(size=(n, 3))) * (rj * rng.uniform(0, 1, n))[:, None]
+    r = np.linalg.norm(a - cq, axis=1) + np.linalg.norm(b - cs, axis=1)
+    d2 = ((a - b) ** 2).sum(1)
+    d = np.sqrt(d2)
+    ok = d >= 2.5 * (ri + rj)
+    ap, bp = _f32(a - cq), _f32(b - cs)                                        # stored offsets (rounded once)
+    bw = _f32((bp.astype(np.float64) ** 2).sum(1))                             # |b'|^2 formed in fp64, rounded once
+    t = _f32(cq - cs)
+    s = _f32(ap + t)
+    # expanded form around a band centre mid (any value within a factor of the chord: the bound uses max(d2, mid))
+    mid = _f32(d2 * np.exp(rng.uniform(np.log(0.3), np.log(3.0), n)))
+    n2 = _fma32(s[:, 2], s[:, 2], _fma32(s[:, 1], s[:, 1], _f32(s[:, 0] * s[:, 0])))
+    nsm = _f32(n2 - mid)
+    m2b = _f32(-2.0 * bp)
+    q = _fma32(s[:, 0], m2b[:, 0], _fma32(s[:, 1], m2b[:, 1], _fma32(s[:, 2], m2b[:, 2], _f32(nsm + bw))))
+    err = np.abs(q.astype(np.float64) - (d2 - mid.astype(np.float64)))
+    ratio = err[ok] / (u * np.maximum(d2[ok], mid[ok]))
+    assert ok.sum() > n // 2 and ratio.max() <= 29.1, ratio.max()
+    # difference form
+    df = _f32(s - bp)
+    qd = _fma32(df[:, 2], df[:, 2], _fma32(df[:, 1], df[:, 1], _f32(df[:, 0] * df[:, 0])))
+    errd = np.abs(qd.astype(np.float64) - d2)
+    assert np.all(errd <= (9.0 * d2 + 10.0 * d * r) * u)
+    # and both stay inside the guard band width the tables are built with (margin included)
+    g = 1.0e-7 * d + 3.0e-6 * np.maximum(d2, mid)
+    assert np.all(err[ok] < g[ok] / 1.5) and np.all(errd < (1.0e-7 * d + 3.0e-6 * d2) / 1.5)
+
+
 def test_fast_tables_survive_pathological_edges():
     # bins far narrower than the fp32 guard bands: everything near them must come back ambiguous (-1), never wrong
     e = np.concatenate([[0.0], 1.0 + 1e-7 * np.arange(40), [90.0, 180.0]])
