@@ -307,7 +307,7 @@ def run_ours(args):
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f32",
             "data": "synthetic",
             "config": {"workload": workload_name(args.config, cfg, nd, nr),
-                       "l2": "256 MiB write between steps (inside the timed region); catalogs (<= 14 MB) are L2-resident by design",
+                       "l2": "256 MiB write between steps (inside the timed region); catalogs (28 MB each) are L2-resident by design",
                        "engine": "fast (fp32 squared chord + fp64 recheck of guard-band pairs)",
                        "parallelism": f"tile work items w % {world} == rank, one all-reduce of 3x{nb + 2} int64" if world > 1 else "1 GPU",
                        "grid": stats["grid"], "block": stats["block"], "smem_bytes": stats["smem_bytes"], "cells": stats["cells"]},

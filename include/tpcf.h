@@ -69,9 +69,12 @@ tpcf_status tpcf_get_edges(const tpcf_ctx* ctx, double* edges_out /* nbins+1 */)
  * tpcf_load -- load catalog D or R: n rows of (RA, Dec) in degrees, row-major n x 2, dtype F32 or F64
  *   ("input file lines").  The rows are copied to the device (or read in place
  *   when on_device != 0, in which case radec_deg is a device pointer) and converted ON THE DEVICE to unit
- *   vectors x = cos(dec)cos(ra), y = cos(dec)sin(ra), z = sin(dec) in fp64 (reading A8); the fp32 copy the
- *   fast engine uses is that fp64 vector rounded once.  Replaces any previous catalog in that slot and
- *   invalidates stored counts that used it.
+ *   vectors x = cos(dec)cos(ra), y = cos(dec)sin(ra), z = sin(dec) in fp64 (reading A8), sorted along a space-
+ *   filling curve (counts do not depend on the order; `rows` of tpcf_count always index the caller's order) and
+ *   stored a second time as fp32 offsets from the centres of small groups of consecutive rows (what the fast
+ *   engine reads).  Replaces any previous catalog in that slot and invalidates stored
+ *   counts that used it; device arrays are reused when the size is unchanged, so do not call it while a
+ *   tpcf_count_async on another stream than cuda_stream / the context's stream is still reading them.
  *   cuda_stream: a cudaStream_t (or NULL for the context's stream) the copy and conversion are ordered on;
  *   the call returns after they completed.
  *   Errors: TPCF_EINVAL for n == 0, n > 2^31-1, |Dec| > 90 or a non-finite value in any row (checked on
