@@ -108,6 +108,31 @@ __device__ __noinline__ void recheck_pair(SlowCtx* s, uint32_t i, uint32_t j) {
     atomicAdd(&s->nrecheck, 1u);
 }
 
+// Pairs inside a guard band are rare (1e-5 .. 1e-3) and scattered over the lanes: instead of each lane branching off
+// to its own recheck, they are queued per warp in shared memory and rechecked 32 at a time, one per lane.
+// rq holds kRecheckQueue entries (i, j); qn (warp-uniform, < 32 between calls) is the fill level.
+constexpr int kRecheckQueue = 64;
+__device__ __forceinline__ void rq_push(uint2* rq, unsigned& qn, bool has, uint32_t i, uint32_t j, SlowCtx* slow) {
+    const int lane = threadIdx.x & 31;
+    const unsigned bal = __ballot_sync(0xffffffffu, has);
+    if (!bal) return;
+    if (has) rq[qn + __popc(bal & ((1u << lane) - 1u))] = make_uint2(i, j);
+    qn += __popc(bal);
+    __syncwarp();
+    if (qn >= 32) {
+        qn -= 32;
+        const uint2 e = rq[qn + lane];
+        __syncwarp();
+        recheck_pair(slow, e.x, e.y);
+    }
+}
+__device__ __forceinline__ void rq_drain(uint2* rq, unsigned& qn, SlowCtx* slow) {
+    const int lane = threadIdx.x & 31;
+    if (lane < (int)qn) recheck_pair(slow, rq[lane].x, rq[lane].y);
+    qn = 0;
+    __syncwarp();
+}
+
 // ---- work items -----------------------------------------------------------------------------------------
 template <int MAP>
 __device__ __forceinline__ uint32_t cell_byte_offset(float d2, int shift, float scale, float clamp) {
@@ -131,35 +156,39 @@ __device__ __forceinline__ uint32_t cell_byte_offset(float d2, int shift, float 
 // ---- per-pair cell-lookup path ("lookup" path) ---------------------------------------------------------------
 // One pair: fp32 squared chord (difference form) -> cell -> (lo, hi) of the cell's guard band -> shared-memory
 // partial histogram, or the fp64 recheck when lo <= d2 < hi.
+// Returns true when the pair is valid and fell inside a guard band (the caller then rechecks it in fp64); every other
+// valid pair is counted here.  No call and no branch in here, so the pairs of one j-row overlap in the pipes.
 template <int MAP>
-__device__ __forceinline__ void lookup_pair(float sx, float sy, float sz, const float4& b, const char* lut, char* hist,
-                                            SlowCtx* slow, uint32_t i, uint32_t j, bool valid, int shift,
-                                            float scale, float clamp) {
+__device__ __forceinline__ bool lookup_pair(float sx, float sy, float sz, const float4& b, const char* lut, char* hist,
+                                            bool valid, int shift, float scale, float clamp) {
     const float dx = fmaf(b.x, 0.5f, sx), dy = fmaf(b.y, 0.5f, sy), dz = fmaf(b.z, 0.5f, sz);     // s - b', one rounding each
     const float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
     const uint32_t q8 = cell_byte_offset<MAP>(d2, shift, scale, clamp);
     const float2 lh = *reinterpret_cast<const float2*>(lut + q8);
     const bool above = d2 >= lh.x;
     const bool amb = above && (d2 < lh.y);
-    if (amb) {
-        if (valid) recheck_pair(slow, i, j);
-    } else if (valid) {
-        atomicAdd(reinterpret_cast<unsigned*>(hist + q8) + (above ? 1 : 0), 1u);
-    }
+    if (valid && !amb) atomicAdd(reinterpret_cast<unsigned*>(hist + q8) + (above ? 1 : 0), 1u);
+    return valid && amb;
 }
 
 // One subtile against this lane's R points, every pair by cell lookup.  MASK: only pairs j > i (diagonal chunk).
+// Called by the whole warp; lanes with active == false count nothing.
 template <int MAP, bool MASK>
 __device__ __forceinline__ void lookup_block(const float4* __restrict__ js, const float (&sx)[R], const float (&sy)[R],
-                                             const float (&sz)[R], const char* lut, char* hist, SlowCtx* slow,
-                                             uint32_t i0, uint32_t j0, int shift, float scale, float clamp) {
+                                             const float (&sz)[R], bool active, const char* lut, char* hist, SlowCtx* slow,
+                                             uint2* rq, unsigned& qn, uint32_t i0, uint32_t j0, int shift, float scale,
+                                             float clamp) {
 #pragma unroll 2
     for (int jj = 0; jj < kSubJ; ++jj) {
         const float4 b = js[jj];                                  // one LDS.128, broadcast to the warp
+        unsigned amb = 0;
 #pragma unroll
         for (int r = 0; r < R; ++r)
-            lookup_pair<MAP>(sx[r], sy[r], sz[r], b, lut, hist, slow, i0 + r, j0 + jj, !MASK || (j0 + jj > i0 + r), shift, scale,
-                             clamp);
+            amb |= (lookup_pair<MAP>(sx[r], sy[r], sz[r], b, lut, hist, active && (!MASK || (j0 + jj > i0 + r)), shift, scale, clamp) ? 1u : 0u) << r;
+        if (__any_sync(0xffffffffu, amb != 0)) {                  // rare: pairs inside a guard band
+#pragma unroll 1
+            for (int r = 0; r < R; ++r) rq_push(rq, qn, (amb >> r) & 1u, i0 + r, j0 + jj, slow);
+        }
     }
 }
 
@@ -247,8 +276,9 @@ template <int MAP>
 __device__ __forceinline__ void subtile_pairs(const float4* __restrict__ js, const float4 sp, bool windows, bool mask,
                                               const f32x2 (&px2)[R / 2], const f32x2 (&py2)[R / 2], const f32x2 (&pz2)[R / 2], float cqx,
                                               float cqy, float cqz, float ri, const WinTables& wt, const char* lut,
-                                              char* hist, SlowCtx* slow, uint32_t i0, uint32_t n_i, uint32_t j0,
-                                              uint32_t n_j, int shift, float scale, float clamp, unsigned (&npath)[6]) {
+                                              char* hist, SlowCtx* slow, uint2* rq, unsigned& qn, uint32_t i0, uint32_t n_i,
+                                              uint32_t j0, uint32_t n_j, int shift, float scale, float clamp,
+                                              unsigned (&npath)[6]) {
     const int lane = threadIdx.x & 31;
     // bounds on every TRUE chord of the block from the triangle inequality: |cq - cs| -/+ (ri + rj), made safe
     // against the fp32 evaluation (relative 4e-6 on the centre distance, 1e-7 absolute)
@@ -288,13 +318,15 @@ __device__ __forceinline__ void subtile_pairs(const float4* __restrict__ js, con
         }
     }
     if (wmode > kMaxWinEdges) {
-        if (mode == 5) {
-            // counted below, by the whole warp
-        } else if (mask) {
-            lookup_block<MAP, true>(js, sx, sy, sz, lut, hist, slow, i0, j0, shift, scale, clamp);
-        } else {
-            lookup_block<MAP, false>(js, sx, sy, sz, lut, hist, slow, i0, j0, shift, scale, clamp);
+        const bool act = mode != 5;                 // lanes with mode 5 are counted below, by the whole warp, in fp64
+        if (!act) {
+#pragma unroll
+            for (int r = 0; r < R; ++r) sx[r] = sy[r] = sz[r] = 0.f;      // keeps their (unused) cells inside the table
         }
+        if (mask)
+            lookup_block<MAP, true>(js, sx, sy, sz, act, lut, hist, slow, rq, qn, i0, j0, shift, scale, clamp);
+        else
+            lookup_block<MAP, false>(js, sx, sy, sz, act, lut, hist, slow, rq, qn, i0, j0, shift, scale, clamp);
         if (wmode == 5) exact_lanes(slow, __ballot_sync(0xffffffffu, mode == 5), i0 - lane * R, n_i, j0, n_j, mask);
         ++npath[wmode == 5 ? 5 : 3];
         return;
@@ -360,7 +392,8 @@ __device__ __forceinline__ void subtile_pairs(const float4* __restrict__ js, con
                         uz = __shfl_sync(0xffffffffu, sz[r], src);
 #pragma unroll
             for (int h = 0; h < kSubJ / 32; ++h)
-                lookup_pair<MAP>(ux, uy, uz, js[h * 32 + lane], lut, hist, slow, isrc + r, j0 + h * 32 + lane, true, shift, scale, clamp);
+                rq_push(rq, qn, lookup_pair<MAP>(ux, uy, uz, js[h * 32 + lane], lut, hist, true, shift, scale, clamp), isrc + r,
+                        j0 + h * 32 + lane, slow);
         }
         ++npath[4];
     }
@@ -378,7 +411,7 @@ static_assert(kTileJ % kChunkJ == 0 && kTileI % kWarpI == 0 && kTileI / kWarpI =
 // shared-memory layout of pair_fast_kernel (byte offsets; every array 16-byte aligned)
 __host__ __device__ inline uint32_t up16(uint32_t x) { return (x + 15u) & ~15u; }
 struct FastSmem {
-    uint32_t ring, lut, hist, band_mh, band_lh, thr, whist, cell_band, band_slot, bars, slow, total;
+    uint32_t ring, lut, hist, band_mh, band_lh, thr, whist, cell_band, band_slot, bars, slow, rq, total;
 };
 __host__ __device__ inline FastSmem fast_smem_layout(int ncells, int nbands, int nbins) {
     FastSmem L;
@@ -394,6 +427,7 @@ __host__ __device__ inline FastSmem fast_smem_layout(int ncells, int nbands, int
     L.band_slot = o;  o = up16(o + (uint32_t)(nbands + 1) * 2);
     L.bars = o;       o = up16(o + kWarpsPerCta * NRING * 8);
     L.slow = o;       o = up16(o + (uint32_t)sizeof(SlowCtx));
+    L.rq = o;         o += kWarpsPerCta * kRecheckQueue * 8;
     L.total = o;
     return L;
 }
@@ -489,6 +523,8 @@ __global__ void __launch_bounds__(kThreads, 2) pair_fast_kernel(const __grid_con
 
     const unsigned long long n_witems = (unsigned long long)p.n_items_part * kWarpsPerCta;
     const uint32_t per_row = (p.tiles_j + p.chunk - 1) / p.chunk;
+    uint2* rq = reinterpret_cast<uint2*>(smem + L.rq) + (size_t)warp * kRecheckQueue;
+    unsigned qn = 0;                        // fill level of this warp's recheck queue
     uint32_t g = 0;                         // chunks this warp consumed so far: selects ring slot and mbarrier parity
     unsigned long long pairs_since_flush = 0, witems_done = 0;
     unsigned npath[6] = {0, 0, 0, 0, 0, 0};
@@ -539,7 +575,7 @@ __global__ void __launch_bounds__(kThreads, 2) pair_fast_kernel(const __grid_con
 #pragma unroll 1
             for (int sub = 0; sub < kSubPerChunk; ++sub)
                 subtile_pairs<MAP>(jt + sub * kSubJ, jsph[sub], p.window != 0, mask, px2, py2, pz2, q4.x, q4.y, q4.z, q4.w, wt, lut,
-                                   reinterpret_cast<char*>(hist), slow, i0, p.n_i, ch * kChunkJ + sub * kSubJ, p.n_j, p.shift,
+                                   reinterpret_cast<char*>(hist), slow, rq, qn, i0, p.n_i, ch * kChunkJ + sub * kSubJ, p.n_j, p.shift,
                                    p.sqrt_scale, p.sqrt_clamp, npath);
             __syncwarp();
             pairs_since_flush += (unsigned long long)kWarpI * kChunkJ;
@@ -550,6 +586,7 @@ __global__ void __launch_bounds__(kThreads, 2) pair_fast_kernel(const __grid_con
             pairs_since_flush = 0;
         }
     }
+    rq_drain(rq, qn, slow);
     __syncthreads();
     flush_slots(hist, 2 * p.ncells, p.slotmap, wt.whist, p.nbins + 3, p.result, &slow->nrecheck, p.counters + 1, tid, kThreads);
     if (lane == 0) {

@@ -90,6 +90,9 @@ int exact_slot(double d2, const Binning& b) {
 //   expanded form (window path, d >= kFarKappa r = 2.5 r): 29.1 d^2 u          <= 1.74e-6 t
 // The constants below add margin (x1.67 on the sqrt term, x1.72 on the linear one).
 double guard_width(double t, double scale) { return scale * (1.0e-7 * std::sqrt(t) + 3.0e-6 * t + 1.0e-13); }
+// The cell-lookup path only ever evaluates the difference form: its bands need not cover the expanded form's error.
+// (9 d^2 + 10 d r) u <= 5.4e-7 t + 6.0e-8 sqrt(t); margins x1.85 and x1.67.
+double guard_width_lookup(double t, double scale) { return scale * (1.0e-7 * std::sqrt(t) + 1.0e-6 * t + 1.0e-13); }
 
 // --------------------------------------------------------------------------------------------------
 // Cell maps.  Both are integer/IEEE arithmetic on the float's bit pattern, reproduced exactly on the device.
@@ -205,20 +208,15 @@ static void export_bands(const std::vector<Band>& bands, FastTables& t) {
     t.band_slot[t.nbands] = (uint16_t)bands.back().above;
 }
 
-static void build_fast_tables_impl(const Binning& b, double gs, FastTables& out, std::vector<Band>& bands);
-
-void build_fast_tables(const Binning& b, double gs, FastTables& out) {
-    std::vector<Band> bands;
-    build_fast_tables_impl(b, gs, out, bands);
-    export_bands(bands, out);
-}
-
-static void build_fast_tables_impl(const Binning& b, double gs, FastTables& out, std::vector<Band>& bands) {
+// Guard bands around the droppable edges (ascending, overlapping ones merged) + the zero-width discard band.
+// Returns the number of merges.
+static int make_bands(const Binning& b, double gs, bool lookup, std::vector<Band>& bands) {
     const int n = b.nbins;
     int overlapping = 0;
+    bands.clear();
     for (int k = 0; k <= n; ++k) {
         if ((k == 0 && b.drop_first) || (k == n && b.drop_last)) continue;
-        double T = b.thr[k], g = guard_width(T, gs);
+        double T = b.thr[k], g = lookup ? guard_width_lookup(T, gs) : guard_width(T, gs);
         Band bd;
         bd.lo = (T - g <= 0.0 || T < 1e-12) ? 0.0f : float_down(T - g);
         bd.hi = float_up(T + g);
@@ -241,6 +239,36 @@ static void build_fast_tables_impl(const Binning& b, double gs, FastTables& out,
         if (!bands.empty() && bands.back().hi > kDiscardFrom) bands.back().hi = kDiscardFrom;
         bands.push_back(d);
     }
+    return overlapping;
+}
+
+// per cell: first window band whose hi lies above the start of the cell (the kernel's window search starts there)
+static void fill_cell_band(FastTables& t, const std::vector<Band>& bands) {
+    t.cell_band.assign(t.ncells, 0);
+    size_t first = 0;
+    for (int c = 0; c < t.ncells; ++c) {
+        const uint32_t b0 = first_bits_of_cell(t, c), b1 = first_bits_of_cell(t, c + 1);
+        if (b1 != b0) {
+            const float f0 = (c == 0) ? 0.0f : u2f(b0);
+            while (first < bands.size() && bands[first].hi <= f0) ++first;
+        }
+        t.cell_band[c] = (uint16_t)first;
+    }
+}
+
+static void build_fast_tables_impl(const Binning& b, const std::vector<Band>& bands, int overlapping, FastTables& out);
+
+void build_fast_tables(const Binning& b, double gs, FastTables& out) {
+    std::vector<Band> lookup_bands, window_bands;
+    const int ov = make_bands(b, gs, true, lookup_bands);
+    make_bands(b, gs, false, window_bands);
+    build_fast_tables_impl(b, lookup_bands, ov, out);      // cell map + (lo, hi, slots) per cell: the lookup path
+    export_bands(window_bands, out);                       // the bands the window loops compare against
+    fill_cell_band(out, window_bands);
+}
+
+static void build_fast_tables_impl(const Binning& b, const std::vector<Band>& bands, int overlapping, FastTables& out) {
+    const int lowest = b.drop_first ? 1 : 0;
 
     // 1. LogBits with 2, 4, ... cells per octave
     FastTables t;

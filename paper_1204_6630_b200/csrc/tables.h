@@ -65,6 +65,8 @@ std::string make_binning(int nbins, const double* theta_deg, int mode, Binning& 
 
 // fp32 rounding bound of the fast engine's squared chord around the true value t.
 double guard_width(double t, double scale);
+// ... and of the difference form alone (the bands of the cell-lookup tables)
+double guard_width_lookup(double t, double scale);
 
 void build_fast_tables(const Binning& b, double guard_scale, FastTables& out);
 
