@@ -112,6 +112,7 @@ __device__ __noinline__ void recheck_pair(SlowCtx* s, uint32_t i, uint32_t j) {
 // to its own recheck, they are queued per warp in shared memory and rechecked 32 at a time, one per lane.
 // rq holds kRecheckQueue entries (i, j); qn (warp-uniform, < 32 between calls) is the fill level.
 constexpr int kRecheckQueue = 64;
+constexpr int kMaxSlowLanes = 16;         // lookup / fp64 lanes a window block may carry (subtile_pairs)
 __device__ __forceinline__ void rq_push(uint2* rq, unsigned& qn, bool has, uint32_t i, uint32_t j, SlowCtx* slow) {
     const int lane = threadIdx.x & 31;
     const unsigned bal = __ballot_sync(0xffffffffu, has);
@@ -301,7 +302,12 @@ __device__ __forceinline__ void subtile_pairs(const float4* __restrict__ js, con
         while (e <= kMaxWinEdges && k + e < wt.nbands && wt.band_lh[k + e].x <= hi2) ++e;
         mode = e;
     }
-    const int wmode = __reduce_max_sync(0xffffffffu, mode);
+    // A few lanes that need the cell lookup (or fp64) do not drag the whole warp into lookup_block: the warp runs the
+    // window loop of the other lanes, those lanes' counters are dropped and their pairs are recounted by the whole
+    // warp together (lookup lanes: the recount of flagged lanes below; fp64 lanes: exact_lanes).
+    const unsigned slow_lanes = __ballot_sync(0xffffffffu, mode > kMaxWinEdges);
+    const bool hybrid = slow_lanes != 0 && !mask && __popc(slow_lanes) <= kMaxSlowLanes;
+    const int wmode = __reduce_max_sync(0xffffffffu, (hybrid && mode > kMaxWinEdges) ? 1 : mode);
 
     f32x2 sx2[R / 2], sy2[R / 2], sz2[R / 2];
     float sx[R], sy[R], sz[R];                      // the same registers, one row at a time
@@ -374,11 +380,12 @@ __device__ __forceinline__ void subtile_pairs(const float4* __restrict__ js, con
         cnt[3] = kSubJ * R - c[2];
         ++npath[2];
     }
-    if (!flagged) {
+    if (!flagged && mode <= kMaxWinEdges) {
 #pragma unroll
         for (int t = 0; t <= kMaxWinEdges; ++t)
             if (cnt[t]) atomicAdd(wt.whist + wt.band_slot[k + t], cnt[t]);      // cnt[t] != 0 only for t <= wmode
     }
+    flagged = (flagged && mode <= kMaxWinEdges) || mode == 4;
     // lanes that saw a pair inside a guard band: the warp recounts their kSubJ x R pairs together, lane l taking
     // j-point l, through the cell-lookup path (which sends the ambiguous pairs to the fp64 recheck)
     unsigned todo = __ballot_sync(0xffffffffu, flagged);
@@ -396,6 +403,13 @@ __device__ __forceinline__ void subtile_pairs(const float4* __restrict__ js, con
                         j0 + h * 32 + lane, slow);
         }
         ++npath[4];
+    }
+    if (hybrid) {
+        const unsigned ex = __ballot_sync(0xffffffffu, mode == 5);
+        if (ex) {
+            exact_lanes(slow, ex, i0 - lane * R, n_i, j0, n_j, false);
+            ++npath[5];
+        }
     }
 }
 

@@ -312,7 +312,7 @@ void make_plan(bool tri, uint64_t n_i, uint64_t n_j, Plan& p) {
     p.blocks_i = (uint32_t)((n_i + kTileI - 1) / kTileI);
     p.tiles_j = (uint32_t)((p.n_j + kTileJ - 1) / kTileJ);
     uint64_t tiles = tri ? (uint64_t)p.blocks_i * (p.blocks_i + 1) / 2 : (uint64_t)p.blocks_i * p.tiles_j;
-    uint64_t c = tiles / (40ull * kPlanSMs);
+    uint64_t c = tiles / (160ull * kPlanSMs);
     p.chunk = (uint32_t)std::min<uint64_t>(std::max<uint64_t>(c, 1), kMaxChunk);
     if (tri) {
         p.row_start.resize((size_t)p.blocks_i + 1);
