@@ -312,6 +312,11 @@ tpcf_status enqueue_count(tpcf_ctx* ctx, tpcf_kind kind, const int64_t* rows_hos
     if (plan->n_items > 0xFFFFFFFFull) return fail(ctx, TPCF_EINVAL, "catalogs too large for the 32-bit work-item index");
     p.n_items_part = items_of_part(plan->n_items, ctx->part, ctx->nparts);
     p.row_start = d_row_start;
+    // small catalogs: split the j-tile of every warp item until each resident warp gets ~32 of them
+    p.jsplit = 1;
+    while (p.chunk == 1 && p.jsplit < (uint32_t)(kTileJ / kChunkJ) &&
+           (uint64_t)p.n_items_part * kWarpsPerCta * p.jsplit < 32ull * kPlanSMs * 2 * kWarpsPerCta)
+        p.jsplit *= 2;
     p.part = (uint32_t)ctx->part;
     p.nparts = (uint32_t)ctx->nparts;
     p.lut = ctx->d_lut;

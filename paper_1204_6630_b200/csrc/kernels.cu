@@ -535,7 +535,8 @@ __global__ void __launch_bounds__(kThreads, 2) pair_fast_kernel(const __grid_con
         bulk_g2s(smem_u32(dst + kChunkBytes), p.cs + (size_t)ch * kSubPerChunk, kChunkSphBytes, bar);
     };
 
-    const unsigned long long n_witems = (unsigned long long)p.n_items_part * kWarpsPerCta;
+    const uint32_t per_item = kWarpsPerCta * p.jsplit;      // warp items per plan item
+    const unsigned long long n_witems = (unsigned long long)p.n_items_part * per_item;
     const uint32_t per_row = (p.tiles_j + p.chunk - 1) / p.chunk;
     uint2* rq = reinterpret_cast<uint2*>(smem + L.rq) + (size_t)warp * kRecheckQueue;
     unsigned qn = 0;                        // fill level of this warp's recheck queue
@@ -547,7 +548,8 @@ __global__ void __launch_bounds__(kThreads, 2) pair_fast_kernel(const __grid_con
         if (lane == 0) c = atomicAdd(p.counters, 1ull);
         c = __shfl_sync(0xffffffffu, c, 0);
         if (c >= n_witems) break;
-        const uint32_t w = (uint32_t)(c / kWarpsPerCta) * p.nparts + p.part, ws = (uint32_t)(c % kWarpsPerCta);
+        const uint32_t w = (uint32_t)(c / per_item) * p.nparts + p.part, ws = (uint32_t)(c % per_item) / p.jsplit,
+                       js = (uint32_t)(c % p.jsplit);
         uint32_t I, tile0;
         if (p.tri) {
             I = tri_row_of(p.row_start, p.blocks_i, w, lane);
@@ -577,7 +579,11 @@ __global__ void __launch_bounds__(kThreads, 2) pair_fast_kernel(const __grid_con
         // chunks of the warp's own rows are the diagonal ones (masked)
         const uint32_t dch = ibase / kChunkJ, dch_end = (ibase + kWarpI) / kChunkJ;
         uint32_t ch = tile0 * (kTileJ / kChunkJ);
-        const uint32_t ch_end = (tile0 + ntiles) * (kTileJ / kChunkJ);
+        uint32_t ch_end = (tile0 + ntiles) * (kTileJ / kChunkJ);
+        if (p.jsplit > 1) {                                  // chunk == 1: part js of the single tile
+            ch += js * ((kTileJ / kChunkJ) / p.jsplit);
+            ch_end = ch + (kTileJ / kChunkJ) / p.jsplit;
+        }
         if (p.tri) ch = max(ch, dch);
         if (lane == 0 && ch < ch_end) fetch_chunk(g, ch);
         for (; ch < ch_end; ++ch, ++g) {
@@ -594,7 +600,7 @@ __global__ void __launch_bounds__(kThreads, 2) pair_fast_kernel(const __grid_con
             __syncwarp();
             pairs_since_flush += (unsigned long long)kWarpI * kChunkJ;
         }
-        ++witems_done;
+        if (js == 0) ++witems_done;
         if (pairs_since_flush > kFlushPairs / kWarpsPerCta) {     // 8 warps x this bound < 2^32 per slot
             flush_slots(hist, 2 * p.ncells, p.slotmap, wt.whist, p.nbins + 3, p.result, &slow->nrecheck, p.counters + 1, lane, 32);
             pairs_since_flush = 0;
@@ -990,7 +996,7 @@ cudaError_t launch_pairs_fast(const PairParams& p, CellMap map, int sm_count, cu
     if (e != cudaSuccess) return e;
     if (per_sm < 1) return cudaErrorLaunchOutOfResources;
     // persistent CTAs: a whole number of CTAs per SM, never more than there are work items
-    int grid = (int)std::min<uint64_t>((uint64_t)sm_count * per_sm, std::max<uint32_t>(p.n_items_part, 1));
+    int grid = (int)std::min<uint64_t>((uint64_t)sm_count * per_sm, std::max<uint64_t>((uint64_t)p.n_items_part * p.jsplit, 1));
     kern<<<grid, kThreads, smem, st>>>(p);
     if (info) *info = LaunchInfo{grid, kThreads, (int)smem, 1};
     return cudaGetLastError();

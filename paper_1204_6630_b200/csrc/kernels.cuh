@@ -24,6 +24,8 @@ struct PairParams {
     uint32_t n_items_part;      // items this launch executes (after the partition)
     const uint32_t* row_start;  // tri: first item of i-block I (blocks_i + 1 entries)
     uint32_t part, nparts;      // item w of the full plan is executed iff w % nparts == part
+    uint32_t jsplit;            // fast engine: a warp item covers 1/jsplit of its item's (single) j-tile; 1, 2, 4, 8 or 16,
+                                // > 1 only when chunk == 1 (small catalogs: more, shorter warp items for the tail)
     // fast engine tables
     const float2* lut;          // ncells x (lo, hi)
     const uint16_t* slotmap;    // 2 x ncells: result slot of (cell, d2 < lo) and (cell, d2 >= hi)
