@@ -21,7 +21,7 @@ TPCF_LINEAR, TPCF_LOG, TPCF_EXPLICIT = 0, 1, 2
 TPCF_D, TPCF_R = 0, 1
 TPCF_F32, TPCF_F64 = 0, 1
 TPCF_DD, TPCF_DR, TPCF_RR = 0, 1, 2
-TPCF_ENGINE_FAST, TPCF_ENGINE_EXACT64 = 0, 1
+TPCF_ENGINE_FAST, TPCF_ENGINE_EXACT64, TPCF_ENGINE_TENSOR = 0, 1, 2
 _STATUS = {0: "TPCF_OK", 1: "TPCF_EINVAL", 2: "TPCF_ENOMEM", 3: "TPCF_ECUDA", 4: "TPCF_ESTATE"}
 _MODES = {"linear": TPCF_LINEAR, "log": TPCF_LOG, "explicit": TPCF_EXPLICIT}
 _KINDS = {"DD": TPCF_DD, "DR": TPCF_DR, "RR": TPCF_RR}
@@ -326,7 +326,7 @@ class Context:
         tpcf_set_stream(self._ctx, stream)
 
     def set_engine(self, engine):
-        tpcf_set_engine(self._ctx, {"fast": TPCF_ENGINE_FAST, "exact64": TPCF_ENGINE_EXACT64}.get(engine, engine))
+        tpcf_set_engine(self._ctx, {"fast": TPCF_ENGINE_FAST, "exact64": TPCF_ENGINE_EXACT64, "tensor": TPCF_ENGINE_TENSOR}.get(engine, engine))
 
     def set_guard_scale(self, scale: float):
         tpcf_set_guard_scale(self._ctx, scale)

@@ -21,6 +21,7 @@ struct Catalog {                 // rows in Hilbert order (counts are order-inva
     uint32_t* inv = nullptr;     // caller row -> position in the sorted catalog (row-subset mode)
     float4 *xq = nullptr, *cq = nullptr;   // i-side role: rows as offsets from their 8-row group ("quad") centre; (centre, radius)
     float4 *xs = nullptr, *cs = nullptr;   // j-side role: rows as (-2 offset, |offset|^2) from their 32-row subtile centre
+    float* xb = nullptr;                   // j-side role, tensor engine: per subtile a kSubJ x 16 TF32 operand tile (kernels.cuh)
 };
 // scratch of one spatial sort: (key, idx) ping-pong buffers and the digit counts
 struct SortScratch {
@@ -168,6 +169,7 @@ void free_catalog(Catalog& c) {
     cudaFree(c.cq);
     cudaFree(c.xs);
     cudaFree(c.cs);
+    cudaFree(c.xb);
     c = Catalog();
 }
 
@@ -232,7 +234,7 @@ tpcf_status enqueue_count(tpcf_ctx* ctx, tpcf_kind kind, const int64_t* rows_hos
     const Catalog& ci = ctx->cat[sd.ci];
     const Catalog& cj = ctx->cat[sd.cj];
     if (!ci.n || !cj.n) return fail(ctx, TPCF_ESTATE, "count before the needed catalog(s) were loaded");
-    if (ctx->engine == TPCF_ENGINE_FAST) {
+    if (ctx->engine != TPCF_ENGINE_EXACT64) {
         s = upload_tables(ctx);
         if (s) return s;
     }
@@ -304,6 +306,7 @@ tpcf_status enqueue_count(tpcf_ctx* ctx, tpcf_kind kind, const int64_t* rows_hos
     }
     p.xs = cj.xs;
     p.cs = cj.cs;
+    p.xb = cj.xb;
     p.xj64 = cj.x64;
     p.n_j = (uint32_t)cj.n;
     p.blocks_i = plan->blocks_i;
@@ -352,6 +355,8 @@ tpcf_status enqueue_count(tpcf_ctx* ctx, tpcf_kind kind, const int64_t* rows_hos
     }
     if (ctx->engine == TPCF_ENGINE_FAST)
         CU(launch_pairs_fast(p, ctx->ft.map, ctx->sm_count, st, &li), "pair_fast_kernel launch");
+    else if (ctx->engine == TPCF_ENGINE_TENSOR)
+        CU(launch_pairs_tensor(p, ctx->ft.map, ctx->sm_count, st, &li), "pair_tensor_kernel launch");
     else
         CU(launch_pairs_exact64(p, ctx->sm_count, st, &li), "pair_exact64_kernel launch");
     if (kev.first) {
@@ -448,6 +453,7 @@ tpcf_status tpcf_load(tpcf_ctx* ctx, tpcf_cat which, const void* radec_deg, tpcf
         CU(cudaMalloc(&c.cq, n_pad / kIPerThread * sizeof(float4)), "cudaMalloc catalog (quad centres)");
         CU(cudaMalloc(&c.xs, n_pad * sizeof(float4)), "cudaMalloc catalog (subtile offsets)");
         CU(cudaMalloc(&c.cs, n_pad / kSubJ * sizeof(float4)), "cudaMalloc catalog (subtile centres)");
+        CU(cudaMalloc(&c.xb, n_pad * kTcK * sizeof(float)), "cudaMalloc catalog (subtile TF32 tiles)");
     }
     const uint64_t nblk = (n + kSortChunk - 1) / kSortChunk;
     const size_t need = n * sizeof(double4) + 2 * n * sizeof(uint64_t) + 2 * n * sizeof(uint32_t) + 256 * nblk * sizeof(uint32_t) +
@@ -477,7 +483,7 @@ tpcf_status tpcf_load(tpcf_ctx* ctx, tpcf_cat which, const void* radec_deg, tpcf
     if (e == cudaSuccess) e = launch_sort_pairs(sc.ka, sc.kb, sc.ia, sc.ib, sc.counts, (uint32_t)n, 63, st, &in_a);
     if (e == cudaSuccess) e = launch_permute(rows64, in_a ? sc.ia : sc.ib, n, n_pad, c.x64, c.inv, st);
     if (e == cudaSuccess) e = launch_quads(c.x64, n_pad, c.xq, c.cq, st);
-    if (e == cudaSuccess) e = launch_subtiles(c.x64, n_pad, c.xs, c.cs, st);
+    if (e == cudaSuccess) e = launch_subtiles(c.x64, n_pad, c.xs, c.cs, c.xb, st);
     int bad = 0;
     if (e == cudaSuccess) e = cudaMemcpyAsync(&bad, ctx->d_bad, sizeof(int), cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
@@ -603,7 +609,7 @@ tpcf_status tpcf_set_stream(tpcf_ctx* ctx, void* cuda_stream) {
 
 tpcf_status tpcf_set_engine(tpcf_ctx* ctx, tpcf_engine e) {
     if (!ctx) return TPCF_EINVAL;
-    if (e != TPCF_ENGINE_FAST && e != TPCF_ENGINE_EXACT64) return fail(ctx, TPCF_EINVAL, "unknown engine");
+    if (e != TPCF_ENGINE_FAST && e != TPCF_ENGINE_EXACT64 && e != TPCF_ENGINE_TENSOR) return fail(ctx, TPCF_EINVAL, "unknown engine");
     ctx->engine = e;
     return TPCF_OK;
 }

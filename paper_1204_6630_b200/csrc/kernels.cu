@@ -13,6 +13,8 @@
 // "later combined in a single histogram, in global memory").  How it is computed differs:
 // the angle is never formed; |a-b|^2 = 2 - 2 cos(theta) is compared with per-edge thresholds.
 #include "kernels.cuh"
+#include <cstdio>
+#include <cstdlib>
 
 namespace tpcf {
 
@@ -71,6 +73,10 @@ __device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) {
     asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
     return d;
 }
+
+// TF32 split of an fp32 value: hi = x with the low 13 mantissa bits cleared (exactly representable in TF32 whatever the
+// tensor core does with those bits), x - hi is exact in fp32
+__device__ __forceinline__ float tf32_hi(float x) { return __uint_as_float(__float_as_uint(x) & 0xFFFFE000u); }
 
 // ---- exact classification (fp64), shared by the recheck path and the fp64 engine -----------------------
 __device__ __forceinline__ double chord2_f64(const double4& a, const double4& b) {
@@ -617,6 +623,455 @@ __global__ void __launch_bounds__(kThreads, 2) pair_fast_kernel(const __grid_con
     }
 }
 
+// ---- tensor engine (TPCF_ENGINE_TENSOR) ---------------------------------------------------------------------
+// The window quantity q = |s|^2 - mid_0 + |b'|^2 - 2 s.b' of a (128 i-rows) x (64-row subtile) block is one
+// 128 x 64 x 16 tcgen05.mma (kind::tf32, two K = 8 steps) whose operands carry the fp32 values split into TF32 parts
+// (3xTF32: s_hi m_hi + s_hi m_lo + s_lo m_hi, the two norms as three parts each against columns of ones); the fp32
+// accumulators live in tensor memory, one TMEM lane = one i-row = one thread, and come back with tcgen05.ld for the
+// same bin decision as the FFMA2 loop (sign count per edge + min |q| against the band half width).  A CTA is 4 warps
+// = one 128-row MMA tile.  Windows are per (8-row quad, subtile) exactly as in pair_fast_kernel; rows whose block
+// needs the cell lookup, the diagonal mask or fp64 are counted by their warp together, lane l taking j-rows l, l + 32.
+#ifndef TPCF_TC_ARRIVE
+#define TPCF_TC_ARRIVE 0
+#endif
+constexpr int kTcThreads = 128;
+constexpr int kTcRing = 3;                                                      // chunk slots per CTA
+constexpr uint32_t kTcABytes = kTcThreads * kTcK * 4, kTcBBytes = kSubJ * kTcK * 4;
+constexpr uint32_t kTcALbo = kTcThreads * 16, kTcBLbo = kSubJ * 16, kTcSbo = 128;
+constexpr uint32_t kTcSlotBytes = kSubPerChunk * kTcBBytes + kChunkBytes + kChunkSphBytes;   // B tiles, xs rows, spheres
+constexpr uint32_t kTcCols = 2 * kSubJ;                                         // two accumulator buffers
+constexpr uint32_t kTcIdesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(kSubJ >> 3) << 17) | ((uint32_t)(kTcThreads >> 4) << 24);
+static_assert(kChunkJ == kTcThreads, "the diagonal chunk of a tensor-engine CTA is the chunk of its own 128 rows");
+static_assert(kSubJ == 64, "tcgen05.ld below reads 2 x 32 columns");
+
+__device__ __forceinline__ uint64_t umma_desc(uint32_t saddr, uint32_t lbo, uint32_t sbo) {
+    return (uint64_t)((saddr & 0x3FFFFu) >> 4) | ((uint64_t)(lbo >> 4) << 16) | ((uint64_t)(sbo >> 4) << 32) | (1ull << 46);
+}
+#define TPCF_TMEM_LD32(r, o, addr)                                                                                            \
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x32.b32 "                                                                    \
+                 "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28," \
+                 "%29,%30,%31}, [%32];"                                                                                       \
+                 : "=r"(r[o + 0]), "=r"(r[o + 1]), "=r"(r[o + 2]), "=r"(r[o + 3]), "=r"(r[o + 4]), "=r"(r[o + 5]), "=r"(r[o + 6]),   \
+                   "=r"(r[o + 7]), "=r"(r[o + 8]), "=r"(r[o + 9]), "=r"(r[o + 10]), "=r"(r[o + 11]), "=r"(r[o + 12]),            \
+                   "=r"(r[o + 13]), "=r"(r[o + 14]), "=r"(r[o + 15]), "=r"(r[o + 16]), "=r"(r[o + 17]), "=r"(r[o + 18]),         \
+                   "=r"(r[o + 19]), "=r"(r[o + 20]), "=r"(r[o + 21]), "=r"(r[o + 22]), "=r"(r[o + 23]), "=r"(r[o + 24]),         \
+                   "=r"(r[o + 25]), "=r"(r[o + 26]), "=r"(r[o + 27]), "=r"(r[o + 28]), "=r"(r[o + 29]), "=r"(r[o + 30]),         \
+                   "=r"(r[o + 31])                                                                                            \
+                 : "r"(addr))
+
+// window of one (quad, subtile) block: mode 1..3 = edges of the window loop, 4 = cell lookup, 5 = fp64; k = first band
+template <int MAP>
+__device__ __forceinline__ void window_of(const float4 cq, const float4 sp, bool windows, const WinTables& wt, int shift, float scale,
+                                          float clamp, int& mode, int& k) {
+    const float tx = __fsub_rn(cq.x, sp.x), ty = __fsub_rn(cq.y, sp.y), tz = __fsub_rn(cq.z, sp.z);
+    const float dc2 = fmaf(tz, tz, fmaf(ty, ty, tx * tx));
+    float dc;
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(dc) : "f"(dc2));
+    const float rs = cq.w + sp.w;
+    const float lo = fmaf(dc, 1.0f - 4.0e-6f, -rs) - 1.0e-7f;
+    const float hi = fmaf(dc, 1.0f + 4.0e-6f, rs) + 1.0e-7f;
+    mode = 4;
+    k = 0;
+    if (rs > kRCap) {
+        mode = 5;
+    } else if (windows && lo >= kFarKappa * rs) {
+        const float lo2 = __fmul_rd(lo, lo), hi2 = __fmul_ru(hi, hi);
+        k = wt.cell_band[cell_byte_offset<MAP>(lo2, shift, scale, clamp) >> 3];
+        while (k < wt.nbands && wt.band_lh[k].y <= lo2) ++k;
+        int e = 1;
+        while (e <= kMaxWinEdges && k + e < wt.nbands && wt.band_lh[k + e].x <= hi2) ++e;
+        mode = e;
+    }
+}
+
+struct TcSmem {
+    uint32_t ring, abuf, lut, hist, band_mh, band_lh, thr, whist, cell_band, band_slot, bars, slow, rq, misc, total;
+};
+__host__ __device__ inline TcSmem tc_smem_layout(int ncells, int nbands, int nbins) {
+    TcSmem L;
+    uint32_t o = 0;
+    L.ring = o;       o += kTcRing * ((kTcSlotBytes + 127u) & ~127u);
+    L.abuf = o;       o += 2 * kTcABytes;
+    L.lut = o;        o = up16(o + (uint32_t)ncells * 8);
+    L.hist = o;       o = up16(o + (uint32_t)ncells * 8);
+    L.band_mh = o;    o = up16(o + (uint32_t)nbands * 8);
+    L.band_lh = o;    o = up16(o + (uint32_t)nbands * 8);
+    L.thr = o;        o = up16(o + (uint32_t)(nbins + 1) * 8);
+    L.whist = o;      o = up16(o + (uint32_t)(nbins + 3) * 4);
+    L.cell_band = o;  o = up16(o + (uint32_t)ncells * 2);
+    L.band_slot = o;  o = up16(o + (uint32_t)(nbands + 1) * 2);
+    L.bars = o;       o = up16(o + (kTcRing + 4) * 8);
+    L.slow = o;       o = up16(o + (uint32_t)sizeof(SlowCtx));
+    L.rq = o;         o += (kTcThreads / 32) * kRecheckQueue * 8;
+    L.misc = o;       o += 16;
+    L.total = o;
+    return L;
+}
+
+// rows of `todo` (one bit per lane = i-row) against the 64 j-rows at xs: every pair through the cell lookup, the warp
+// working together on one row at a time (lane l takes j-rows l and l + 32)
+template <int MAP>
+__device__ __forceinline__ void tc_lookup_rows(unsigned todo, float sx, float sy, float sz, const float4* __restrict__ xs, const char* lut,
+                                               char* hist, SlowCtx* slow, uint2* rq, unsigned& qn, uint32_t iwarp, uint32_t j0, bool mask,
+                                               int shift, float scale, float clamp) {
+    const int lane = threadIdx.x & 31;
+    while (todo) {
+        const int src = __ffs(todo) - 1;
+        todo &= todo - 1;
+        const uint32_t i = iwarp + src;
+        const float ux = __shfl_sync(0xffffffffu, sx, src), uy = __shfl_sync(0xffffffffu, sy, src), uz = __shfl_sync(0xffffffffu, sz, src);
+#pragma unroll
+        for (int h = 0; h < kSubJ / 32; ++h) {
+            const uint32_t j = j0 + h * 32 + lane;
+            rq_push(rq, qn, lookup_pair<MAP>(ux, uy, uz, xs[h * 32 + lane], lut, hist, !mask || j > i, shift, scale, clamp), i, j, slow);
+        }
+    }
+}
+
+// rows of `todo` against 64 j-rows in fp64 (radii too large for the fp32 bound, padding rows)
+__device__ __noinline__ void tc_exact_rows(SlowCtx* s, unsigned todo, uint32_t iwarp, uint32_t n_i, uint32_t j0, uint32_t n_j, bool mask) {
+    const int lane = threadIdx.x & 31;
+    unsigned cnt = 0;
+    while (todo) {
+        const int src = __ffs(todo) - 1;
+        todo &= todo - 1;
+        const uint32_t i = iwarp + src;
+        if (i >= n_i) continue;
+        const double4 a = s->xi64[i];
+#pragma unroll 1
+        for (int h = 0; h < kSubJ / 32; ++h) {
+            const uint32_t j = j0 + h * 32 + lane;
+            if (j < n_j && (!mask || j > i)) {
+                atomicAdd(s->whist + exact_slot_dev(chord2_f64(a, s->xj64[j]), s->thr, s->nbins), 1u);
+                ++cnt;
+            }
+        }
+    }
+    cnt = __reduce_add_sync(0xffffffffu, cnt);
+    if (lane == 0 && cnt) atomicAdd(&s->nrecheck, cnt);
+}
+
+// what a thread keeps of a subtile between forming its operand row and binning its accumulators one step later
+struct TcPending {
+    float sx, sy, sz;           // the row relative to the subtile centre (for the lookup recount)
+    float dt1, dt2, hmax;       // mid_0 - mid_e of the further edges, largest band half width
+    int mode, k, we;            // this row's mode, first band, edges the warp runs
+    uint32_t j0;                // first j-row of the subtile
+    const float4* xs;           // its rows in the ring slot
+    bool mask, valid;
+};
+
+// Bin the 64 accumulators of this thread's row (subtile pd) and count or recount the row.
+template <int MAP>
+__device__ __forceinline__ void tc_bin(const TcPending& pd, uint32_t taddr, const WinTables& wt, const char* lut, char* hist,
+                                       SlowCtx* slow, uint2* rq, unsigned& qn, uint32_t iwarp, uint32_t n_i, uint32_t n_j, int shift,
+                                       float scale, float clamp, unsigned (&npath)[6]) {
+    const bool win = pd.mode <= kMaxWinEdges;
+    bool flagged = false;
+    if (pd.we <= kMaxWinEdges) {                    // warp-uniform
+        uint32_t v[kSubJ];
+        TPCF_TMEM_LD32(v, 0, taddr);
+        TPCF_TMEM_LD32(v, 32, taddr + 32);
+        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+        unsigned c0 = 0, c1 = 0, c2 = 0;
+        float m = 3.0e38f;
+        if (pd.we == 1) {
+            unsigned ca = 0, cb = 0, cc = 0, cd = 0;        // independent chains
+            float ma = 3.0e38f, mb = 3.0e38f;
+#pragma unroll
+            for (int j = 0; j < kSubJ; j += 4) {
+                ca += v[j] >> 31;
+                cb += v[j + 1] >> 31;
+                cc += v[j + 2] >> 31;
+                cd += v[j + 3] >> 31;
+                ma = fminf(ma, fminf(fabsf(__uint_as_float(v[j])), fabsf(__uint_as_float(v[j + 1]))));
+                mb = fminf(mb, fminf(fabsf(__uint_as_float(v[j + 2])), fabsf(__uint_as_float(v[j + 3]))));
+            }
+            c0 = (ca + cb) + (cc + cd);
+            m = fminf(ma, mb);
+        } else if (pd.we == 2) {
+#pragma unroll
+            for (int j = 0; j < kSubJ; ++j) {
+                const float q = __uint_as_float(v[j]), q1 = __fadd_rn(q, pd.dt1);
+                c0 += __float_as_uint(q) >> 31;
+                c1 += __float_as_uint(q1) >> 31;
+                m = fminf(m, fminf(fabsf(q), fabsf(q1)));
+            }
+        } else {
+#pragma unroll
+            for (int j = 0; j < kSubJ; ++j) {
+                const float q = __uint_as_float(v[j]), q1 = __fadd_rn(q, pd.dt1), q2 = __fadd_rn(q, pd.dt2);
+                c0 += __float_as_uint(q) >> 31;
+                c1 += __float_as_uint(q1) >> 31;
+                c2 += __float_as_uint(q2) >> 31;
+                m = fminf(fminf(m, fabsf(q)), fminf(fabsf(q1), fabsf(q2)));
+            }
+        }
+        flagged = m <= pd.hmax;
+        if (win && !flagged) {
+            // c_e = pairs below edge e (e < we); the rest of the 64 lies above the last edge
+            const unsigned n0 = c0, n1 = (pd.we >= 2 ? c1 : (unsigned)kSubJ) - c0, n2 = pd.we >= 2 ? (pd.we >= 3 ? c2 : (unsigned)kSubJ) - c1 : 0u,
+                           n3 = pd.we >= 3 ? (unsigned)kSubJ - c2 : 0u;
+            if (n0) atomicAdd(wt.whist + wt.band_slot[pd.k], n0);
+            if (n1) atomicAdd(wt.whist + wt.band_slot[pd.k + 1], n1);
+            if (n2) atomicAdd(wt.whist + wt.band_slot[pd.k + 2], n2);
+            if (n3) atomicAdd(wt.whist + wt.band_slot[pd.k + 3], n3);
+        }
+        ++npath[pd.we - 1];
+    } else {
+        ++npath[3];
+    }
+    const unsigned lk = __ballot_sync(0xffffffffu, (win && flagged) || pd.mode == 4);
+    const unsigned ex = __ballot_sync(0xffffffffu, pd.mode == 5);
+    if (lk) {
+        tc_lookup_rows<MAP>(lk, pd.sx, pd.sy, pd.sz, pd.xs, lut, hist, slow, rq, qn, iwarp, pd.j0, pd.mask, shift, scale, clamp);
+        npath[4] += __popc(lk);
+    }
+    if (ex) {
+        tc_exact_rows(slow, ex, iwarp, n_i, pd.j0, n_j, pd.mask);
+        ++npath[5];
+    }
+}
+
+template <int MAP>
+__global__ void __launch_bounds__(kTcThreads, 4) pair_tensor_kernel(const __grid_constant__ PairParams p) {
+    extern __shared__ __align__(128) unsigned char smem[];
+    const TcSmem L = tc_smem_layout(p.ncells, p.nbands, p.nbins);
+    char* lut = reinterpret_cast<char*>(smem + L.lut);
+    unsigned* hist = reinterpret_cast<unsigned*>(smem + L.hist);
+    SlowCtx* slow = reinterpret_cast<SlowCtx*>(smem + L.slow);
+    WinTables wt;
+    wt.band_mh = reinterpret_cast<const float2*>(smem + L.band_mh);
+    wt.band_lh = reinterpret_cast<const float2*>(smem + L.band_lh);
+    wt.band_slot = reinterpret_cast<const uint16_t*>(smem + L.band_slot);
+    wt.cell_band = reinterpret_cast<const uint16_t*>(smem + L.cell_band);
+    wt.whist = reinterpret_cast<unsigned*>(smem + L.whist);
+    wt.nbands = p.nbands;
+    volatile uint32_t* misc = reinterpret_cast<volatile uint32_t*>(smem + L.misc);      // [0] TMEM base, [2..3] next work item
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    constexpr uint32_t kSlotStride = (kTcSlotBytes + 127u) & ~127u;
+    unsigned char* ring = smem + L.ring;
+    const uint32_t ring_bar = smem_u32(smem + L.bars), full_bar = ring_bar + 8 * kTcRing, arr_bar = full_bar + 16;
+    for (int c = tid; c < p.ncells; c += kTcThreads) {
+        reinterpret_cast<float2*>(lut)[c] = p.lut[c];
+        hist[2 * c] = 0;
+        hist[2 * c + 1] = 0;
+        reinterpret_cast<uint16_t*>(smem + L.cell_band)[c] = p.cell_band[c];
+    }
+    for (int b = tid; b < p.nbands; b += kTcThreads) {
+        reinterpret_cast<float2*>(smem + L.band_mh)[b] = p.band_mh[b];
+        reinterpret_cast<float2*>(smem + L.band_lh)[b] = p.band_lh[b];
+    }
+    for (int b = tid; b <= p.nbands; b += kTcThreads) reinterpret_cast<uint16_t*>(smem + L.band_slot)[b] = p.band_slot[b];
+    for (int b = tid; b < p.nbins + 3; b += kTcThreads) wt.whist[b] = 0;
+    for (int b = tid; b <= p.nbins; b += kTcThreads) reinterpret_cast<double*>(smem + L.thr)[b] = p.thr[b];
+    // operand row of this thread in the two A buffers: K chunk 3 = (1, 1, 1, 0) never changes
+    unsigned char* arow = smem + L.abuf + (tid / 8) * kTcSbo + (tid % 8) * 16;
+    *reinterpret_cast<float4*>(arow + 3 * kTcALbo) = make_float4(1.f, 1.f, 1.f, 0.f);
+    *reinterpret_cast<float4*>(arow + kTcABytes + 3 * kTcALbo) = make_float4(1.f, 1.f, 1.f, 0.f);
+    if (tid == 0) {
+        for (int b = 0; b < kTcRing + 2; ++b) mbar_init(ring_bar + 8 * b, 1);
+        mbar_init(arr_bar, kTcThreads);
+        mbar_init(arr_bar + 8, kTcThreads);
+        fence_barrier_init();
+        slow->xi64 = p.xi64;
+        slow->xj64 = p.xj64;
+        slow->thr = reinterpret_cast<const double*>(smem + L.thr);
+        slow->whist = wt.whist;
+        slow->nrecheck = 0;
+        slow->nbins = p.nbins;
+    }
+    if (warp == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(smem + L.misc)), "r"(kTcCols));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    }
+    fence_proxy_async();
+    asm volatile("tcgen05.fence::before_thread_sync;");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;");
+    const uint32_t tmem = misc[0];
+    const uint32_t tlane = tmem + ((uint32_t)warp * 32u << 16);
+
+    auto fetch_chunk = [&](uint32_t n, uint32_t ch) {      // thread 0: chunk ch into the slot of running chunk number n
+        const uint32_t slot = n % kTcRing, bar = ring_bar + 8 * slot;
+        const uint32_t dst = smem_u32(ring + (size_t)slot * kSlotStride);
+        fence_proxy_async();
+        mbar_expect_tx(bar, kTcSlotBytes);
+        bulk_g2s(dst, p.xb + (size_t)ch * kChunkJ * kTcK, kSubPerChunk * kTcBBytes, bar);
+        bulk_g2s(dst + kSubPerChunk * kTcBBytes, p.xs + (size_t)ch * kChunkJ, kChunkBytes, bar);
+        bulk_g2s(dst + kSubPerChunk * kTcBBytes + kChunkBytes, p.cs + (size_t)ch * kSubPerChunk, kChunkSphBytes, bar);
+    };
+
+    constexpr uint32_t kCtasPerItem = kTileI / kTcThreads;
+    const uint32_t per_item = kCtasPerItem * p.jsplit;
+    const unsigned long long n_citems = (unsigned long long)p.n_items_part * per_item;
+    const uint32_t per_row = (p.tiles_j + p.chunk - 1) / p.chunk;
+    uint2* rq = reinterpret_cast<uint2*>(smem + L.rq) + (size_t)warp * kRecheckQueue;
+    unsigned qn = 0;
+    uint32_t gch = 0, gs = 0, na = 0;       // chunks fetched / subtiles issued / arrive phases so far: ring slot, buffers, mbarrier parities
+    unsigned long long pairs_since_flush = 0, items_done = 0;
+    unsigned npath[6] = {0, 0, 0, 0, 0, 0};
+    for (;;) {
+        if (tid == 0) {
+            const unsigned long long c = atomicAdd(p.counters, 1ull);
+            misc[2] = (uint32_t)c;
+            misc[3] = (uint32_t)(c >> 32);
+        }
+        __syncthreads();
+        const unsigned long long c = ((unsigned long long)misc[3] << 32) | misc[2];
+        if (c >= n_citems) break;
+        const uint32_t w = (uint32_t)(c / per_item) * p.nparts + p.part, ws = (uint32_t)(c % per_item) / p.jsplit, js = (uint32_t)(c % p.jsplit);
+        uint32_t I, tile0;
+        if (p.tri) {
+            I = tri_row_of(p.row_start, p.blocks_i, w, lane);
+            tile0 = I + (w - p.row_start[I]) * p.chunk;
+        } else {
+            I = w / per_row;
+            tile0 = (w % per_row) * p.chunk;
+        }
+        const uint32_t ntiles = min(p.chunk, p.tiles_j - tile0);
+        // this thread's row as an offset from the centre of its 8-row quad; a quad wholly past the end of the catalog
+        // is moved to (-2,-2,-2) as in pair_fast_kernel
+        const uint32_t ibase = I * kTileI + ws * kTcThreads, i = ibase + tid, iq = i & ~(uint32_t)(R - 1);
+        float4 a = p.xq[i], cq = p.cq[i / R];
+        if (iq >= p.n_i) {
+            a = make_float4(0.f, 0.f, 0.f, 0.f);
+            cq = make_float4(-kPadCoord, -kPadCoord, -kPadCoord, 0.f);
+        }
+        const uint32_t dch = ibase / kChunkJ;
+        uint32_t ch = tile0 * (kTileJ / kChunkJ), ch_end = (tile0 + ntiles) * (kTileJ / kChunkJ);
+        if (p.jsplit > 1) {
+            ch += js * ((kTileJ / kChunkJ) / p.jsplit);
+            ch_end = ch + (kTileJ / kChunkJ) / p.jsplit;
+        }
+        if (p.tri) ch = max(ch, dch);
+        const uint32_t nchunks = ch < ch_end ? ch_end - ch : 0u, nsub = nchunks * kSubPerChunk;
+        if (tid == 0)
+            for (uint32_t n = 0; n < min(nchunks, (uint32_t)kTcRing); ++n) fetch_chunk(gch + n, ch + n);
+
+        TcPending pd;
+        pd.valid = false;
+        int bmode = 4, bk = 0;              // window of (this thread's quad, subtile (lane & 7) of the current batch of 8)
+        for (uint32_t s = 0; s <= nsub; ++s) {
+            TcPending cur;
+            cur.valid = false;
+            if (s < nsub) {
+                const uint32_t lc = s / kSubPerChunk, sub = s % kSubPerChunk, n = gch + lc, sabs = (ch + lc) * kSubPerChunk + sub;
+                unsigned char* slot = ring + (size_t)(n % kTcRing) * kSlotStride;
+                if (sub == 0) mbar_wait(ring_bar + 8 * (n % kTcRing), (n / kTcRing) & 1);
+                const bool mask = p.tri && (ch + lc) == dch;
+                if (s == 0 || (sabs & 7u) == 0) {           // windows of 8 subtiles at a time, one per lane of the quad
+                    const uint32_t su = (sabs & ~7u) + (lane & 7);
+                    window_of<MAP>(cq, p.cs[su], p.window != 0, wt, p.shift, p.sqrt_scale, p.sqrt_clamp, bmode, bk);
+                }
+                const int owner = (lane & ~7) | (int)(sabs & 7u);
+                int mode = __shfl_sync(0xffffffffu, bmode, owner), k = __shfl_sync(0xffffffffu, bk, owner);
+                if (mask && mode <= kMaxWinEdges) mode = 4;
+                const int wmax = __reduce_max_sync(0xffffffffu, mode <= kMaxWinEdges ? mode : 0);
+                const int we = wmax ? wmax : kMaxWinEdges + 1;
+                if (mode > kMaxWinEdges) k = 0;
+                else k = min(k, p.nbands - we);
+                const float4 sp = reinterpret_cast<const float4*>(slot + kSubPerChunk * kTcBBytes + kChunkBytes)[sub];
+                const float tx = __fsub_rn(cq.x, sp.x), ty = __fsub_rn(cq.y, sp.y), tz = __fsub_rn(cq.z, sp.z);
+                const float sx = __fadd_rn(a.x, tx), sy = __fadd_rn(a.y, ty), sz = __fadd_rn(a.z, tz);
+                const float2 mh0 = wt.band_mh[k];
+                float hmax = mh0.y, dt1 = 0.f, dt2 = 0.f;
+                if (we <= kMaxWinEdges && we >= 2) {
+                    const float2 mh = wt.band_mh[k + 1];
+                    dt1 = __fsub_rn(mh0.x, mh.x);
+                    hmax = fmaxf(hmax, mh.y);
+                }
+                if (we == 3) {
+                    const float2 mh = wt.band_mh[k + 2];
+                    dt2 = __fsub_rn(mh0.x, mh.x);
+                    hmax = fmaxf(hmax, mh.y);
+                }
+                const float nsm = __fadd_rn(fmaf(sz, sz, fmaf(sy, sy, sx * sx)), -mh0.x);
+                const float xh = tf32_hi(sx), yh = tf32_hi(sy), zh = tf32_hi(sz);
+                const float xl = tf32_hi(sx - xh), yl = tf32_hi(sy - yh), zl = tf32_hi(sz - zh);
+                const float nh = tf32_hi(nsm), nm = tf32_hi(nsm - nh), nl = tf32_hi((nsm - nh) - nm);
+                unsigned char* ar = arow + (gs & 1) * kTcABytes;
+                *reinterpret_cast<float4*>(ar) = make_float4(xh, yh, zh, xh);
+                *reinterpret_cast<float4*>(ar + kTcALbo) = make_float4(yh, zh, xl, yl);
+                *reinterpret_cast<float4*>(ar + 2 * kTcALbo) = make_float4(zl, nh, nm, nl);
+                fence_proxy_async();
+                cur.sx = sx; cur.sy = sy; cur.sz = sz;
+                cur.dt1 = dt1; cur.dt2 = dt2; cur.hmax = hmax;
+                cur.mode = mode; cur.k = k; cur.we = we;
+                cur.j0 = sabs * kSubJ;
+                cur.xs = reinterpret_cast<const float4*>(slot + kSubPerChunk * kTcBBytes) + sub * kSubJ;
+                cur.mask = mask;
+                cur.valid = true;
+            }
+            // "operand rows written, previous accumulators read": all threads arrive, only the issuing thread waits
+            asm volatile("tcgen05.fence::before_thread_sync;");
+            // (two barriers in turn: a thread can be one step ahead of the slowest, never two -- its next bin needs the MMA
+            // that the issuing thread only starts after this wait)
+#if TPCF_TC_ARRIVE
+            asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(arr_bar + 8 * (na & 1)) : "memory");
+#else
+            __syncthreads();
+#endif
+            if (tid == 0) {
+#if TPCF_TC_ARRIVE
+                mbar_wait(arr_bar + 8 * (na & 1), (na >> 1) & 1);
+#endif
+                asm volatile("tcgen05.fence::after_thread_sync;");
+                if (s < nsub) {
+                    const uint32_t lc = s / kSubPerChunk, sub = s % kSubPerChunk, n = gch + lc;
+                    const uint32_t sa = smem_u32(smem + L.abuf) + (gs & 1) * kTcABytes;
+                    const uint32_t sb = smem_u32(ring + (size_t)(n % kTcRing) * kSlotStride) + sub * kTcBBytes;
+                    const uint32_t d = tmem + (gs & 1) * kSubJ;
+#pragma unroll
+                    for (int ks = 0; ks < kTcK / 8; ++ks) {
+                        const uint64_t da = umma_desc(sa + ks * 2 * kTcALbo, kTcALbo, kTcSbo), db = umma_desc(sb + ks * 2 * kTcBLbo, kTcBLbo, kTcSbo);
+                        asm volatile("{\n .reg .pred p;\n setp.ne.b32 p, %4, 0;\n tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n}" ::"r"(d),
+                                     "l"(da), "l"(db), "r"(kTcIdesc), "r"(ks)
+                                     : "memory");
+                    }
+                    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(full_bar + 8 * (gs & 1)) : "memory");
+                }
+                // every thread is past the bin of subtile s - 2: the chunk of subtiles s - 3, s - 2 is free for a new one
+                if (s >= 3 && (s & 1)) {
+                    const uint32_t lc = (s - 3) / 2;
+                    if (lc + kTcRing < nchunks) fetch_chunk(gch + lc + kTcRing, ch + lc + kTcRing);
+                }
+            }
+            if (pd.valid) {
+                const uint32_t ps = gs - 1;
+                mbar_wait(full_bar + 8 * (ps & 1), (ps >> 1) & 1);
+                asm volatile("tcgen05.fence::after_thread_sync;");
+                tc_bin<MAP>(pd, tlane + (ps & 1) * kSubJ, wt, lut, reinterpret_cast<char*>(hist), slow, rq, qn, ibase + warp * 32, p.n_i, p.n_j,
+                            p.shift, p.sqrt_scale, p.sqrt_clamp, npath);
+            }
+            pd = cur;
+            if (s < nsub) ++gs;
+            ++na;
+        }
+        gch += nchunks;
+        pairs_since_flush += (unsigned long long)nchunks * kChunkJ * kTcThreads;
+        if (tid == 0 && ws == 0 && js == 0) ++items_done;
+        __syncthreads();
+        if (pairs_since_flush > kFlushPairs) {
+            flush_slots(hist, 2 * p.ncells, p.slotmap, wt.whist, p.nbins + 3, p.result, &slow->nrecheck, p.counters + 1, tid, kTcThreads);
+            pairs_since_flush = 0;
+            __syncthreads();
+        }
+    }
+    rq_drain(rq, qn, slow);
+    asm volatile("tcgen05.fence::before_thread_sync;");
+    __syncthreads();
+    flush_slots(hist, 2 * p.ncells, p.slotmap, wt.whist, p.nbins + 3, p.result, &slow->nrecheck, p.counters + 1, tid, kTcThreads);
+    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(kTcCols));
+    if (tid == 0 && items_done) atomicAdd(p.counters + 2, items_done);
+    if (lane == 0) {
+#pragma unroll
+        for (int k = 0; k < 6; ++k)
+            if (npath[k]) atomicAdd(p.counters + 3 + k, (unsigned long long)npath[k]);
+    }
+}
+
 // ---- fp64 engine: work items per CTA -------------------------------------------------------------------------
 struct Item {
     uint32_t I, tile0, ntiles, valid;
@@ -861,7 +1316,8 @@ __global__ void quads_kernel(const double4* __restrict__ x64, uint64_t nquads, f
 // j-side role: every kSubJ consecutive rows form a subtile (one warp here).  cs = (fp32 centre, radius) as
 // above; xs = (-2 b', |b'|^2) with b' the fp32 rounding of (row - centre) formed in fp64 and |b'|^2 the fp32
 // rounding of the fp64 square of that rounded offset (the window loops evaluate |a - b|^2 = |a|^2 + |b|^2 - 2 a.b).
-__global__ void subtiles_kernel(const double4* __restrict__ x64, uint64_t nsub, float4* __restrict__ xs, float4* __restrict__ cs) {
+__global__ void subtiles_kernel(const double4* __restrict__ x64, uint64_t nsub, float4* __restrict__ xs, float4* __restrict__ cs,
+                                float* __restrict__ xb) {
     constexpr int H = kSubJ / 32;                   // rows per lane
     const uint64_t w = (blockIdx.x * (uint64_t)blockDim.x + threadIdx.x) >> 5;
     const int lane = threadIdx.x & 31;
@@ -888,6 +1344,22 @@ __global__ void subtiles_kernel(const double4* __restrict__ x64, uint64_t nsub, 
         const float bx = (float)dx, by = (float)dy, bz = (float)dz;
         const double nb = (double)bx * bx + (double)by * by + (double)bz * bz;
         xs[w * kSubJ + h * 32 + lane] = make_float4(-2.f * bx, -2.f * by, -2.f * bz, (float)nb);
+        {   // the same row as a K = 16 TF32 operand row of the tensor engine (layout: kernels.cuh)
+            const int j = h * 32 + lane;
+            float* t = xb + (size_t)w * kSubJ * kTcK + (j / 8) * 32 + (j % 8) * 4;
+            const float m[3] = {-2.f * bx, -2.f * by, -2.f * bz};
+            float mh[3], ml[3];
+#pragma unroll
+            for (int d = 0; d < 3; ++d) {
+                mh[d] = tf32_hi(m[d]);
+                ml[d] = tf32_hi(m[d] - mh[d]);
+            }
+            const float wv = (float)nb, wh = tf32_hi(wv), wm = tf32_hi(wv - wh), wl = tf32_hi((wv - wh) - wm);
+            *reinterpret_cast<float4*>(t + 0 * kSubJ * 4) = make_float4(mh[0], mh[1], mh[2], ml[0]);
+            *reinterpret_cast<float4*>(t + 1 * kSubJ * 4) = make_float4(ml[1], ml[2], mh[0], mh[1]);
+            *reinterpret_cast<float4*>(t + 2 * kSubJ * 4) = make_float4(mh[2], 1.f, 1.f, 1.f);
+            *reinterpret_cast<float4*>(t + 3 * kSubJ * 4) = make_float4(wh, wm, wl, 0.f);
+        }
     }
 #pragma unroll
     for (int off = 16; off; off >>= 1) r = fmax(r, __shfl_xor_sync(0xffffffffu, r, off));
@@ -963,10 +1435,10 @@ cudaError_t launch_quads(const double4* x64, uint64_t n_pad, float4* xq, float4*
     return cudaGetLastError();
 }
 
-cudaError_t launch_subtiles(const double4* x64, uint64_t n_pad, float4* xs, float4* cs, cudaStream_t st) {
+cudaError_t launch_subtiles(const double4* x64, uint64_t n_pad, float4* xs, float4* cs, float* xb, cudaStream_t st) {
     const uint64_t nsub = n_pad / kSubJ;
     const int block = 256;
-    subtiles_kernel<<<(unsigned)((nsub * 32 + block - 1) / block), block, 0, st>>>(x64, nsub, xs, cs);
+    subtiles_kernel<<<(unsigned)((nsub * 32 + block - 1) / block), block, 0, st>>>(x64, nsub, xs, cs, xb);
     return cudaGetLastError();
 }
 
@@ -999,6 +1471,34 @@ cudaError_t launch_pairs_fast(const PairParams& p, CellMap map, int sm_count, cu
     int grid = (int)std::min<uint64_t>((uint64_t)sm_count * per_sm, std::max<uint64_t>((uint64_t)p.n_items_part * p.jsplit, 1));
     kern<<<grid, kThreads, smem, st>>>(p);
     if (info) *info = LaunchInfo{grid, kThreads, (int)smem, 1};
+    return cudaGetLastError();
+}
+
+cudaError_t launch_pairs_tensor(const PairParams& p, CellMap map, int sm_count, cudaStream_t st, LaunchInfo* info) {
+    const size_t smem = tc_smem_layout(p.ncells, p.nbands, p.nbins).total;
+    auto kern = (map == CellMap::LogBits) ? pair_tensor_kernel<(int)CellMap::LogBits> : pair_tensor_kernel<(int)CellMap::SqrtLin>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    if (e != cudaSuccess) return e;
+    // cudaOccupancyMaxActiveBlocksPerMultiprocessor answers 1 for a kernel that allocates tensor memory, whatever it
+    // allocates; the SM does co-schedule CTAs whose allocations fit (measured: 1, 2, 4 CTAs/SM -> 80, 44, 27 ms).  So
+    // the resident CTAs per SM are worked out here from shared memory, registers and the 512 TMEM columns.
+    cudaFuncAttributes fa;
+    e = cudaFuncGetAttributes(&fa, kern);
+    if (e != cudaSuccess) return e;
+    int dev = 0, smem_sm = 0, regs_sm = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev);
+    cudaDeviceGetAttribute(&regs_sm, cudaDevAttrMaxRegistersPerMultiprocessor, dev);
+    const int regs_cta = ((fa.numRegs + 7) / 8 * 8) * kTcThreads;
+    int per_sm = std::min<int>(smem_sm / (int)(smem + fa.sharedSizeBytes + 1024), regs_sm / std::max(regs_cta, 1));
+    per_sm = std::min(per_sm, (int)(512 / kTcCols));
+    if (per_sm < 1) return cudaErrorLaunchOutOfResources;
+    const uint64_t citems = (uint64_t)p.n_items_part * (kTileI / kTcThreads) * p.jsplit;
+    int grid = (int)std::min<uint64_t>((uint64_t)sm_count * per_sm, std::max<uint64_t>(citems, 1));
+    kern<<<grid, kTcThreads, smem, st>>>(p);
+    if (info) *info = LaunchInfo{grid, kTcThreads, (int)smem, 1};
     return cudaGetLastError();
 }
 
