@@ -21,7 +21,8 @@ struct Catalog {                 // rows in Hilbert order (counts are order-inva
     uint32_t* inv = nullptr;     // caller row -> position in the sorted catalog (row-subset mode)
     float4 *xq = nullptr, *cq = nullptr;   // i-side role: rows as offsets from their 8-row group ("quad") centre; (centre, radius)
     float4 *xs = nullptr, *cs = nullptr;   // j-side role: rows as (-2 offset, |offset|^2) from their 32-row subtile centre
-    float* xb = nullptr;                   // j-side role, tensor engine: per subtile a kSubJ x 16 TF32 operand tile (kernels.cuh)
+    float4 *xt = nullptr, *ct = nullptr;   // j-side role of the tensor engine: the same for 128-row tiles
+    float* xb = nullptr;                   // ... and per tile a 128 x 16 TF32 operand block (kernels.cuh)
 };
 // scratch of one spatial sort: (key, idx) ping-pong buffers and the digit counts
 struct SortScratch {
@@ -170,6 +171,8 @@ void free_catalog(Catalog& c) {
     cudaFree(c.xs);
     cudaFree(c.cs);
     cudaFree(c.xb);
+    cudaFree(c.xt);
+    cudaFree(c.ct);
     c = Catalog();
 }
 
@@ -307,6 +310,8 @@ tpcf_status enqueue_count(tpcf_ctx* ctx, tpcf_kind kind, const int64_t* rows_hos
     p.xs = cj.xs;
     p.cs = cj.cs;
     p.xb = cj.xb;
+    p.xt = cj.xt;
+    p.ct = cj.ct;
     p.xj64 = cj.x64;
     p.n_j = (uint32_t)cj.n;
     p.blocks_i = plan->blocks_i;
@@ -453,7 +458,9 @@ tpcf_status tpcf_load(tpcf_ctx* ctx, tpcf_cat which, const void* radec_deg, tpcf
         CU(cudaMalloc(&c.cq, n_pad / kIPerThread * sizeof(float4)), "cudaMalloc catalog (quad centres)");
         CU(cudaMalloc(&c.xs, n_pad * sizeof(float4)), "cudaMalloc catalog (subtile offsets)");
         CU(cudaMalloc(&c.cs, n_pad / kSubJ * sizeof(float4)), "cudaMalloc catalog (subtile centres)");
-        CU(cudaMalloc(&c.xb, n_pad * kTcK * sizeof(float)), "cudaMalloc catalog (subtile TF32 tiles)");
+        CU(cudaMalloc(&c.xb, n_pad * kTcK * sizeof(float)), "cudaMalloc catalog (TF32 tiles)");
+        CU(cudaMalloc(&c.xt, n_pad * sizeof(float4)), "cudaMalloc catalog (tile offsets)");
+        CU(cudaMalloc(&c.ct, n_pad / kTcSubJ * sizeof(float4)), "cudaMalloc catalog (tile centres)");
     }
     const uint64_t nblk = (n + kSortChunk - 1) / kSortChunk;
     const size_t need = n * sizeof(double4) + 2 * n * sizeof(uint64_t) + 2 * n * sizeof(uint32_t) + 256 * nblk * sizeof(uint32_t) +
@@ -483,7 +490,7 @@ tpcf_status tpcf_load(tpcf_ctx* ctx, tpcf_cat which, const void* radec_deg, tpcf
     if (e == cudaSuccess) e = launch_sort_pairs(sc.ka, sc.kb, sc.ia, sc.ib, sc.counts, (uint32_t)n, 63, st, &in_a);
     if (e == cudaSuccess) e = launch_permute(rows64, in_a ? sc.ia : sc.ib, n, n_pad, c.x64, c.inv, st);
     if (e == cudaSuccess) e = launch_quads(c.x64, n_pad, c.xq, c.cq, st);
-    if (e == cudaSuccess) e = launch_subtiles(c.x64, n_pad, c.xs, c.cs, c.xb, st);
+    if (e == cudaSuccess) e = launch_subtiles(c.x64, n_pad, c.xs, c.cs, c.xt, c.ct, c.xb, st);
     int bad = 0;
     if (e == cudaSuccess) e = cudaMemcpyAsync(&bad, ctx->d_bad, sizeof(int), cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);

@@ -624,25 +624,23 @@ __global__ void __launch_bounds__(kThreads, 2) pair_fast_kernel(const __grid_con
 }
 
 // ---- tensor engine (TPCF_ENGINE_TENSOR) ---------------------------------------------------------------------
-// The window quantity q = |s|^2 - mid_0 + |b'|^2 - 2 s.b' of a (128 i-rows) x (64-row subtile) block is one
-// 128 x 64 x 16 tcgen05.mma (kind::tf32, two K = 8 steps) whose operands carry the fp32 values split into TF32 parts
+// The window quantity q = |s|^2 - mid_0 + |b'|^2 - 2 s.b' of a (128 i-rows) x (128 j-rows) block is one
+// 128 x 128 x 16 tcgen05.mma (kind::tf32, two K = 8 steps) whose operands carry the fp32 values split into TF32 parts
 // (3xTF32: s_hi m_hi + s_hi m_lo + s_lo m_hi, the two norms as three parts each against columns of ones); the fp32
 // accumulators live in tensor memory, one TMEM lane = one i-row = one thread, and come back with tcgen05.ld for the
 // same bin decision as the FFMA2 loop (sign count per edge + min |q| against the band half width).  A CTA is 4 warps
-// = one 128-row MMA tile.  Windows are per (8-row quad, subtile) exactly as in pair_fast_kernel; rows whose block
-// needs the cell lookup, the diagonal mask or fp64 are counted by their warp together, lane l taking j-rows l, l + 32.
-#ifndef TPCF_TC_ARRIVE
-#define TPCF_TC_ARRIVE 0
-#endif
+// = one 128-row MMA tile; the j side comes in tiles of kTcSubJ = 128 rows (own spheres and offsets: PairParams xt, ct, xb).
+// Windows are per (8-row quad, j-tile) as in pair_fast_kernel; rows whose block needs the cell lookup, the diagonal mask or
+// fp64 are counted by their warp together, lane l taking j-rows l, l + 32, ..
 constexpr int kTcThreads = 128;
 constexpr int kTcRing = 3;                                                      // chunk slots per CTA
-constexpr uint32_t kTcABytes = kTcThreads * kTcK * 4, kTcBBytes = kSubJ * kTcK * 4;
-constexpr uint32_t kTcALbo = kTcThreads * 16, kTcBLbo = kSubJ * 16, kTcSbo = 128;
-constexpr uint32_t kTcSlotBytes = kSubPerChunk * kTcBBytes + kChunkBytes + kChunkSphBytes;   // B tiles, xs rows, spheres
-constexpr uint32_t kTcCols = 2 * kSubJ;                                         // two accumulator buffers
-constexpr uint32_t kTcIdesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(kSubJ >> 3) << 17) | ((uint32_t)(kTcThreads >> 4) << 24);
-static_assert(kChunkJ == kTcThreads, "the diagonal chunk of a tensor-engine CTA is the chunk of its own 128 rows");
-static_assert(kSubJ == 64, "tcgen05.ld below reads 2 x 32 columns");
+constexpr uint32_t kTcABytes = kTcThreads * kTcK * 4, kTcBBytes = kTcSubJ * kTcK * 4, kTcRowBytes = kTcSubJ * sizeof(float4);
+constexpr uint32_t kTcALbo = kTcThreads * 16, kTcBLbo = kTcSubJ * 16, kTcSbo = 128;
+constexpr uint32_t kTcSlotBytes = kTcBBytes + kTcRowBytes + sizeof(float4);     // operand tile, fp32 rows, sphere
+constexpr uint32_t kTcCols = kTcSubJ;                                           // one 128 x 128 fp32 accumulator tile
+constexpr uint32_t kTcIdesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(kTcSubJ >> 3) << 17) | ((uint32_t)(kTcThreads >> 4) << 24);
+static_assert(kTcSubJ == kTcThreads && kTcSubJ == kChunkJ, "the diagonal tile of a tensor-engine CTA is the tile of its own 128 rows");
+static_assert(kTcSubJ % 64 == 0, "the accumulators are read back 64 columns at a time");
 
 __device__ __forceinline__ uint64_t umma_desc(uint32_t saddr, uint32_t lbo, uint32_t sbo) {
     return (uint64_t)((saddr & 0x3FFFFu) >> 4) | ((uint64_t)(lbo >> 4) << 16) | ((uint64_t)(sbo >> 4) << 32) | (1ull << 46);
@@ -691,7 +689,7 @@ __host__ __device__ inline TcSmem tc_smem_layout(int ncells, int nbands, int nbi
     TcSmem L;
     uint32_t o = 0;
     L.ring = o;       o += kTcRing * ((kTcSlotBytes + 127u) & ~127u);
-    L.abuf = o;       o += 2 * kTcABytes;
+    L.abuf = o;       o += kTcABytes;
     L.lut = o;        o = up16(o + (uint32_t)ncells * 8);
     L.hist = o;       o = up16(o + (uint32_t)ncells * 8);
     L.band_mh = o;    o = up16(o + (uint32_t)nbands * 8);
@@ -700,7 +698,7 @@ __host__ __device__ inline TcSmem tc_smem_layout(int ncells, int nbands, int nbi
     L.whist = o;      o = up16(o + (uint32_t)(nbins + 3) * 4);
     L.cell_band = o;  o = up16(o + (uint32_t)ncells * 2);
     L.band_slot = o;  o = up16(o + (uint32_t)(nbands + 1) * 2);
-    L.bars = o;       o = up16(o + (kTcRing + 4) * 8);
+    L.bars = o;       o = up16(o + (kTcRing + 1) * 8);
     L.slow = o;       o = up16(o + (uint32_t)sizeof(SlowCtx));
     L.rq = o;         o += (kTcThreads / 32) * kRecheckQueue * 8;
     L.misc = o;       o += 16;
@@ -708,8 +706,8 @@ __host__ __device__ inline TcSmem tc_smem_layout(int ncells, int nbands, int nbi
     return L;
 }
 
-// rows of `todo` (one bit per lane = i-row) against the 64 j-rows at xs: every pair through the cell lookup, the warp
-// working together on one row at a time (lane l takes j-rows l and l + 32)
+// rows of `todo` (one bit per lane = i-row) against the kTcSubJ j-rows at xs: every pair through the cell lookup, the warp
+// working together on one row at a time (lane l takes j-rows l, l + 32, ..)
 template <int MAP>
 __device__ __forceinline__ void tc_lookup_rows(unsigned todo, float sx, float sy, float sz, const float4* __restrict__ xs, const char* lut,
                                                char* hist, SlowCtx* slow, uint2* rq, unsigned& qn, uint32_t iwarp, uint32_t j0, bool mask,
@@ -721,14 +719,14 @@ __device__ __forceinline__ void tc_lookup_rows(unsigned todo, float sx, float sy
         const uint32_t i = iwarp + src;
         const float ux = __shfl_sync(0xffffffffu, sx, src), uy = __shfl_sync(0xffffffffu, sy, src), uz = __shfl_sync(0xffffffffu, sz, src);
 #pragma unroll
-        for (int h = 0; h < kSubJ / 32; ++h) {
+        for (int h = 0; h < kTcSubJ / 32; ++h) {
             const uint32_t j = j0 + h * 32 + lane;
             rq_push(rq, qn, lookup_pair<MAP>(ux, uy, uz, xs[h * 32 + lane], lut, hist, !mask || j > i, shift, scale, clamp), i, j, slow);
         }
     }
 }
 
-// rows of `todo` against 64 j-rows in fp64 (radii too large for the fp32 bound, padding rows)
+// rows of `todo` against the kTcSubJ j-rows from j0 on in fp64 (radii too large for the fp32 bound, padding rows)
 __device__ __noinline__ void tc_exact_rows(SlowCtx* s, unsigned todo, uint32_t iwarp, uint32_t n_i, uint32_t j0, uint32_t n_j, bool mask) {
     const int lane = threadIdx.x & 31;
     unsigned cnt = 0;
@@ -739,7 +737,7 @@ __device__ __noinline__ void tc_exact_rows(SlowCtx* s, unsigned todo, uint32_t i
         if (i >= n_i) continue;
         const double4 a = s->xi64[i];
 #pragma unroll 1
-        for (int h = 0; h < kSubJ / 32; ++h) {
+        for (int h = 0; h < kTcSubJ / 32; ++h) {
             const uint32_t j = j0 + h * 32 + lane;
             if (j < n_j && (!mask || j > i)) {
                 atomicAdd(s->whist + exact_slot_dev(chord2_f64(a, s->xj64[j]), s->thr, s->nbins), 1u);
@@ -751,84 +749,88 @@ __device__ __noinline__ void tc_exact_rows(SlowCtx* s, unsigned todo, uint32_t i
     if (lane == 0 && cnt) atomicAdd(&s->nrecheck, cnt);
 }
 
-// what a thread keeps of a subtile between forming its operand row and binning its accumulators one step later
-struct TcPending {
-    float sx, sy, sz;           // the row relative to the subtile centre (for the lookup recount)
+
+// per-thread window parameters of one (row, j-tile) block
+struct TcRow {
+    float sx, sy, sz;           // the row relative to the tile centre (for the lookup recount)
     float dt1, dt2, hmax;       // mid_0 - mid_e of the further edges, largest band half width
     int mode, k, we;            // this row's mode, first band, edges the warp runs
-    uint32_t j0;                // first j-row of the subtile
-    const float4* xs;           // its rows in the ring slot
-    bool mask, valid;
 };
 
-// Bin the 64 accumulators of this thread's row (subtile pd) and count or recount the row.
+// Bin the kTcSubJ accumulators of this thread's row and count or recount the row.
 template <int MAP>
-__device__ __forceinline__ void tc_bin(const TcPending& pd, uint32_t taddr, const WinTables& wt, const char* lut, char* hist,
-                                       SlowCtx* slow, uint2* rq, unsigned& qn, uint32_t iwarp, uint32_t n_i, uint32_t n_j, int shift,
-                                       float scale, float clamp, unsigned (&npath)[6]) {
+__device__ __forceinline__ void tc_bin(const TcRow& pd, uint32_t taddr, const float4* __restrict__ xs, uint32_t j0, bool mask,
+                                       const WinTables& wt, const char* lut, char* hist, SlowCtx* slow, uint2* rq, unsigned& qn,
+                                       uint32_t iwarp, uint32_t n_i, uint32_t n_j, int shift, float scale, float clamp,
+                                       unsigned (&npath)[6]) {
     const bool win = pd.mode <= kMaxWinEdges;
     bool flagged = false;
     if (pd.we <= kMaxWinEdges) {                    // warp-uniform
-        uint32_t v[kSubJ];
-        TPCF_TMEM_LD32(v, 0, taddr);
-        TPCF_TMEM_LD32(v, 32, taddr + 32);
-        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
         unsigned c0 = 0, c1 = 0, c2 = 0;
         float m = 3.0e38f;
-        if (pd.we == 1) {
-            unsigned ca = 0, cb = 0, cc = 0, cd = 0;        // independent chains
-            float ma = 3.0e38f, mb = 3.0e38f;
+#pragma unroll 1
+        for (int half = 0; half < kTcSubJ / 64; ++half) {
+            uint32_t v[64];
+            TPCF_TMEM_LD32(v, 0, taddr + half * 64);
+            TPCF_TMEM_LD32(v, 32, taddr + half * 64 + 32);
+            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+            if (pd.we == 1) {
+                unsigned ca = 0, cb = 0;                // independent chains
+                float ma = 3.0e38f, mb = 3.0e38f;
 #pragma unroll
-            for (int j = 0; j < kSubJ; j += 4) {
-                ca += v[j] >> 31;
-                cb += v[j + 1] >> 31;
-                cc += v[j + 2] >> 31;
-                cd += v[j + 3] >> 31;
-                ma = fminf(ma, fminf(fabsf(__uint_as_float(v[j])), fabsf(__uint_as_float(v[j + 1]))));
-                mb = fminf(mb, fminf(fabsf(__uint_as_float(v[j + 2])), fabsf(__uint_as_float(v[j + 3]))));
-            }
-            c0 = (ca + cb) + (cc + cd);
-            m = fminf(ma, mb);
-        } else if (pd.we == 2) {
+                for (int j = 0; j < 64; j += 4) {
+                    ca += v[j] >> 31;
+                    cb += v[j + 1] >> 31;
+                    ca += v[j + 2] >> 31;
+                    cb += v[j + 3] >> 31;
+                    ma = fminf(ma, fminf(fabsf(__uint_as_float(v[j])), fabsf(__uint_as_float(v[j + 1]))));
+                    mb = fminf(mb, fminf(fabsf(__uint_as_float(v[j + 2])), fabsf(__uint_as_float(v[j + 3]))));
+                }
+                c0 += ca + cb;
+                m = fminf(m, fminf(ma, mb));
+            } else if (pd.we == 2) {
 #pragma unroll
-            for (int j = 0; j < kSubJ; ++j) {
-                const float q = __uint_as_float(v[j]), q1 = __fadd_rn(q, pd.dt1);
-                c0 += __float_as_uint(q) >> 31;
-                c1 += __float_as_uint(q1) >> 31;
-                m = fminf(m, fminf(fabsf(q), fabsf(q1)));
-            }
-        } else {
+                for (int j = 0; j < 64; ++j) {
+                    const float q = __uint_as_float(v[j]), q1 = __fadd_rn(q, pd.dt1);
+                    c0 += __float_as_uint(q) >> 31;
+                    c1 += __float_as_uint(q1) >> 31;
+                    m = fminf(m, fminf(fabsf(q), fabsf(q1)));
+                }
+            } else {
 #pragma unroll
-            for (int j = 0; j < kSubJ; ++j) {
-                const float q = __uint_as_float(v[j]), q1 = __fadd_rn(q, pd.dt1), q2 = __fadd_rn(q, pd.dt2);
-                c0 += __float_as_uint(q) >> 31;
-                c1 += __float_as_uint(q1) >> 31;
-                c2 += __float_as_uint(q2) >> 31;
-                m = fminf(fminf(m, fabsf(q)), fminf(fabsf(q1), fabsf(q2)));
+                for (int j = 0; j < 64; ++j) {
+                    const float q = __uint_as_float(v[j]), q1 = __fadd_rn(q, pd.dt1), q2 = __fadd_rn(q, pd.dt2);
+                    c0 += __float_as_uint(q) >> 31;
+                    c1 += __float_as_uint(q1) >> 31;
+                    c2 += __float_as_uint(q2) >> 31;
+                    m = fminf(fminf(m, fabsf(q)), fminf(fabsf(q1), fabsf(q2)));
+                }
             }
         }
         flagged = m <= pd.hmax;
         if (win && !flagged) {
-            // c_e = pairs below edge e (e < we); the rest of the 64 lies above the last edge
-            const unsigned n0 = c0, n1 = (pd.we >= 2 ? c1 : (unsigned)kSubJ) - c0, n2 = pd.we >= 2 ? (pd.we >= 3 ? c2 : (unsigned)kSubJ) - c1 : 0u,
-                           n3 = pd.we >= 3 ? (unsigned)kSubJ - c2 : 0u;
+            // c_e = pairs below edge e (e < we); the rest of the kTcSubJ lies above the last edge
+            const unsigned T = kTcSubJ;
+            const unsigned n0 = c0, n1 = (pd.we >= 2 ? c1 : T) - c0, n2 = pd.we >= 2 ? (pd.we >= 3 ? c2 : T) - c1 : 0u, n3 = pd.we >= 3 ? T - c2 : 0u;
             if (n0) atomicAdd(wt.whist + wt.band_slot[pd.k], n0);
             if (n1) atomicAdd(wt.whist + wt.band_slot[pd.k + 1], n1);
             if (n2) atomicAdd(wt.whist + wt.band_slot[pd.k + 2], n2);
             if (n3) atomicAdd(wt.whist + wt.band_slot[pd.k + 3], n3);
         }
-        ++npath[pd.we - 1];
+        npath[0] += pd.we == 1;
+        npath[1] += pd.we == 2;
+        npath[2] += pd.we == 3;
     } else {
         ++npath[3];
     }
     const unsigned lk = __ballot_sync(0xffffffffu, (win && flagged) || pd.mode == 4);
     const unsigned ex = __ballot_sync(0xffffffffu, pd.mode == 5);
     if (lk) {
-        tc_lookup_rows<MAP>(lk, pd.sx, pd.sy, pd.sz, pd.xs, lut, hist, slow, rq, qn, iwarp, pd.j0, pd.mask, shift, scale, clamp);
+        tc_lookup_rows<MAP>(lk, pd.sx, pd.sy, pd.sz, xs, lut, hist, slow, rq, qn, iwarp, j0, mask, shift, scale, clamp);
         npath[4] += __popc(lk);
     }
     if (ex) {
-        tc_exact_rows(slow, ex, iwarp, n_i, pd.j0, n_j, pd.mask);
+        tc_exact_rows(slow, ex, iwarp, n_i, j0, n_j, mask);
         ++npath[5];
     }
 }
@@ -852,7 +854,7 @@ __global__ void __launch_bounds__(kTcThreads, 4) pair_tensor_kernel(const __grid
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     constexpr uint32_t kSlotStride = (kTcSlotBytes + 127u) & ~127u;
     unsigned char* ring = smem + L.ring;
-    const uint32_t ring_bar = smem_u32(smem + L.bars), full_bar = ring_bar + 8 * kTcRing, arr_bar = full_bar + 16;
+    const uint32_t ring_bar = smem_u32(smem + L.bars), full_bar = ring_bar + 8 * kTcRing;      // kTcRing slot barriers, "accumulators ready"
     for (int c = tid; c < p.ncells; c += kTcThreads) {
         reinterpret_cast<float2*>(lut)[c] = p.lut[c];
         hist[2 * c] = 0;
@@ -866,14 +868,11 @@ __global__ void __launch_bounds__(kTcThreads, 4) pair_tensor_kernel(const __grid
     for (int b = tid; b <= p.nbands; b += kTcThreads) reinterpret_cast<uint16_t*>(smem + L.band_slot)[b] = p.band_slot[b];
     for (int b = tid; b < p.nbins + 3; b += kTcThreads) wt.whist[b] = 0;
     for (int b = tid; b <= p.nbins; b += kTcThreads) reinterpret_cast<double*>(smem + L.thr)[b] = p.thr[b];
-    // operand row of this thread in the two A buffers: K chunk 3 = (1, 1, 1, 0) never changes
+    // operand row of this thread in the A tile: K chunk 3 = (1, 1, 1, 0) never changes
     unsigned char* arow = smem + L.abuf + (tid / 8) * kTcSbo + (tid % 8) * 16;
     *reinterpret_cast<float4*>(arow + 3 * kTcALbo) = make_float4(1.f, 1.f, 1.f, 0.f);
-    *reinterpret_cast<float4*>(arow + kTcABytes + 3 * kTcALbo) = make_float4(1.f, 1.f, 1.f, 0.f);
     if (tid == 0) {
-        for (int b = 0; b < kTcRing + 2; ++b) mbar_init(ring_bar + 8 * b, 1);
-        mbar_init(arr_bar, kTcThreads);
-        mbar_init(arr_bar + 8, kTcThreads);
+        for (int b = 0; b < kTcRing + 1; ++b) mbar_init(ring_bar + 8 * b, 1);
         fence_barrier_init();
         slow->xi64 = p.xi64;
         slow->xj64 = p.xj64;
@@ -893,14 +892,14 @@ __global__ void __launch_bounds__(kTcThreads, 4) pair_tensor_kernel(const __grid
     const uint32_t tmem = misc[0];
     const uint32_t tlane = tmem + ((uint32_t)warp * 32u << 16);
 
-    auto fetch_chunk = [&](uint32_t n, uint32_t ch) {      // thread 0: chunk ch into the slot of running chunk number n
+    auto fetch_tile = [&](uint32_t n, uint32_t t) {       // thread 0: j-tile t into the slot of running tile number n
         const uint32_t slot = n % kTcRing, bar = ring_bar + 8 * slot;
         const uint32_t dst = smem_u32(ring + (size_t)slot * kSlotStride);
         fence_proxy_async();
         mbar_expect_tx(bar, kTcSlotBytes);
-        bulk_g2s(dst, p.xb + (size_t)ch * kChunkJ * kTcK, kSubPerChunk * kTcBBytes, bar);
-        bulk_g2s(dst + kSubPerChunk * kTcBBytes, p.xs + (size_t)ch * kChunkJ, kChunkBytes, bar);
-        bulk_g2s(dst + kSubPerChunk * kTcBBytes + kChunkBytes, p.cs + (size_t)ch * kSubPerChunk, kChunkSphBytes, bar);
+        bulk_g2s(dst, p.xb + (size_t)t * kTcSubJ * kTcK, kTcBBytes, bar);
+        bulk_g2s(dst + kTcBBytes, p.xt + (size_t)t * kTcSubJ, kTcRowBytes, bar);
+        bulk_g2s(dst + kTcBBytes + kTcRowBytes, p.ct + t, sizeof(float4), bar);
     };
 
     constexpr uint32_t kCtasPerItem = kTileI / kTcThreads;
@@ -909,7 +908,7 @@ __global__ void __launch_bounds__(kTcThreads, 4) pair_tensor_kernel(const __grid
     const uint32_t per_row = (p.tiles_j + p.chunk - 1) / p.chunk;
     uint2* rq = reinterpret_cast<uint2*>(smem + L.rq) + (size_t)warp * kRecheckQueue;
     unsigned qn = 0;
-    uint32_t gch = 0, gs = 0, na = 0;       // chunks fetched / subtiles issued / arrive phases so far: ring slot, buffers, mbarrier parities
+    uint32_t gch = 0, gs = 0;               // j-tiles fetched / multiplied so far: ring slot and mbarrier parities
     unsigned long long pairs_since_flush = 0, items_done = 0;
     unsigned npath[6] = {0, 0, 0, 0, 0, 0};
     for (;;) {
@@ -946,109 +945,80 @@ __global__ void __launch_bounds__(kTcThreads, 4) pair_tensor_kernel(const __grid
             ch_end = ch + (kTileJ / kChunkJ) / p.jsplit;
         }
         if (p.tri) ch = max(ch, dch);
-        const uint32_t nchunks = ch < ch_end ? ch_end - ch : 0u, nsub = nchunks * kSubPerChunk;
+        const uint32_t ntile = ch < ch_end ? ch_end - ch : 0u;      // j-tiles of this item (a tile = a 128-row chunk)
         if (tid == 0)
-            for (uint32_t n = 0; n < min(nchunks, (uint32_t)kTcRing); ++n) fetch_chunk(gch + n, ch + n);
+            for (uint32_t n = 0; n < min(ntile, (uint32_t)kTcRing); ++n) fetch_tile(gch + n, ch + n);
 
-        TcPending pd;
-        pd.valid = false;
-        int bmode = 4, bk = 0;              // window of (this thread's quad, subtile (lane & 7) of the current batch of 8)
-        for (uint32_t s = 0; s <= nsub; ++s) {
-            TcPending cur;
-            cur.valid = false;
-            if (s < nsub) {
-                const uint32_t lc = s / kSubPerChunk, sub = s % kSubPerChunk, n = gch + lc, sabs = (ch + lc) * kSubPerChunk + sub;
-                unsigned char* slot = ring + (size_t)(n % kTcRing) * kSlotStride;
-                if (sub == 0) mbar_wait(ring_bar + 8 * (n % kTcRing), (n / kTcRing) & 1);
-                const bool mask = p.tri && (ch + lc) == dch;
-                if (s == 0 || (sabs & 7u) == 0) {           // windows of 8 subtiles at a time, one per lane of the quad
-                    const uint32_t su = (sabs & ~7u) + (lane & 7);
-                    window_of<MAP>(cq, p.cs[su], p.window != 0, wt, p.shift, p.sqrt_scale, p.sqrt_clamp, bmode, bk);
-                }
-                const int owner = (lane & ~7) | (int)(sabs & 7u);
-                int mode = __shfl_sync(0xffffffffu, bmode, owner), k = __shfl_sync(0xffffffffu, bk, owner);
-                if (mask && mode <= kMaxWinEdges) mode = 4;
-                const int wmax = __reduce_max_sync(0xffffffffu, mode <= kMaxWinEdges ? mode : 0);
-                const int we = wmax ? wmax : kMaxWinEdges + 1;
-                if (mode > kMaxWinEdges) k = 0;
-                else k = min(k, p.nbands - we);
-                const float4 sp = reinterpret_cast<const float4*>(slot + kSubPerChunk * kTcBBytes + kChunkBytes)[sub];
-                const float tx = __fsub_rn(cq.x, sp.x), ty = __fsub_rn(cq.y, sp.y), tz = __fsub_rn(cq.z, sp.z);
-                const float sx = __fadd_rn(a.x, tx), sy = __fadd_rn(a.y, ty), sz = __fadd_rn(a.z, tz);
-                const float2 mh0 = wt.band_mh[k];
-                float hmax = mh0.y, dt1 = 0.f, dt2 = 0.f;
-                if (we <= kMaxWinEdges && we >= 2) {
-                    const float2 mh = wt.band_mh[k + 1];
-                    dt1 = __fsub_rn(mh0.x, mh.x);
-                    hmax = fmaxf(hmax, mh.y);
-                }
-                if (we == 3) {
-                    const float2 mh = wt.band_mh[k + 2];
-                    dt2 = __fsub_rn(mh0.x, mh.x);
-                    hmax = fmaxf(hmax, mh.y);
-                }
-                const float nsm = __fadd_rn(fmaf(sz, sz, fmaf(sy, sy, sx * sx)), -mh0.x);
-                const float xh = tf32_hi(sx), yh = tf32_hi(sy), zh = tf32_hi(sz);
-                const float xl = tf32_hi(sx - xh), yl = tf32_hi(sy - yh), zl = tf32_hi(sz - zh);
+        int bmode = 4, bk = 0;              // window of (this thread's quad, tile (lane & 7) of the current batch of 8)
+        for (uint32_t t = 0; t < ntile; ++t) {
+            const uint32_t n = gch + t, tabs = ch + t;
+            unsigned char* slot = ring + (size_t)(n % kTcRing) * kSlotStride;
+            mbar_wait(ring_bar + 8 * (n % kTcRing), (n / kTcRing) & 1);
+            const bool mask = p.tri && tabs == dch;
+            if (t == 0 || (tabs & 7u) == 0) {               // windows of 8 tiles at a time, one per lane of the quad
+                const uint32_t su = (tabs & ~7u) + (lane & 7);
+                window_of<MAP>(cq, p.ct[su], p.window != 0, wt, p.shift, p.sqrt_scale, p.sqrt_clamp, bmode, bk);
+            }
+            const int owner = (lane & ~7) | (int)(tabs & 7u);
+            TcRow rw;
+            rw.mode = __shfl_sync(0xffffffffu, bmode, owner);
+            rw.k = __shfl_sync(0xffffffffu, bk, owner);
+            if (mask && rw.mode <= kMaxWinEdges) rw.mode = 4;
+            const int wmax = __reduce_max_sync(0xffffffffu, rw.mode <= kMaxWinEdges ? rw.mode : 0);
+            rw.we = wmax ? wmax : kMaxWinEdges + 1;
+            rw.k = rw.mode > kMaxWinEdges ? 0 : min(rw.k, p.nbands - rw.we);
+            const float4 sp = *reinterpret_cast<const float4*>(slot + kTcBBytes + kTcRowBytes);
+            const float tx = __fsub_rn(cq.x, sp.x), ty = __fsub_rn(cq.y, sp.y), tz = __fsub_rn(cq.z, sp.z);
+            rw.sx = __fadd_rn(a.x, tx);
+            rw.sy = __fadd_rn(a.y, ty);
+            rw.sz = __fadd_rn(a.z, tz);
+            const float2 mh0 = wt.band_mh[rw.k];
+            rw.hmax = mh0.y;
+            rw.dt1 = rw.dt2 = 0.f;
+            if (rw.we == 2 || rw.we == 3) {
+                const float2 mh = wt.band_mh[rw.k + 1];
+                rw.dt1 = __fsub_rn(mh0.x, mh.x);
+                rw.hmax = fmaxf(rw.hmax, mh.y);
+            }
+            if (rw.we == 3) {
+                const float2 mh = wt.band_mh[rw.k + 2];
+                rw.dt2 = __fsub_rn(mh0.x, mh.x);
+                rw.hmax = fmaxf(rw.hmax, mh.y);
+            }
+            {
+                const float nsm = __fadd_rn(fmaf(rw.sz, rw.sz, fmaf(rw.sy, rw.sy, rw.sx * rw.sx)), -mh0.x);
+                const float xh = tf32_hi(rw.sx), yh = tf32_hi(rw.sy), zh = tf32_hi(rw.sz);
+                const float xl = tf32_hi(rw.sx - xh), yl = tf32_hi(rw.sy - yh), zl = tf32_hi(rw.sz - zh);
                 const float nh = tf32_hi(nsm), nm = tf32_hi(nsm - nh), nl = tf32_hi((nsm - nh) - nm);
-                unsigned char* ar = arow + (gs & 1) * kTcABytes;
-                *reinterpret_cast<float4*>(ar) = make_float4(xh, yh, zh, xh);
-                *reinterpret_cast<float4*>(ar + kTcALbo) = make_float4(yh, zh, xl, yl);
-                *reinterpret_cast<float4*>(ar + 2 * kTcALbo) = make_float4(zl, nh, nm, nl);
-                fence_proxy_async();
-                cur.sx = sx; cur.sy = sy; cur.sz = sz;
-                cur.dt1 = dt1; cur.dt2 = dt2; cur.hmax = hmax;
-                cur.mode = mode; cur.k = k; cur.we = we;
-                cur.j0 = sabs * kSubJ;
-                cur.xs = reinterpret_cast<const float4*>(slot + kSubPerChunk * kTcBBytes) + sub * kSubJ;
-                cur.mask = mask;
-                cur.valid = true;
+                *reinterpret_cast<float4*>(arow) = make_float4(xh, yh, zh, xh);
+                *reinterpret_cast<float4*>(arow + kTcALbo) = make_float4(yh, zh, xl, yl);
+                *reinterpret_cast<float4*>(arow + 2 * kTcALbo) = make_float4(zl, nh, nm, nl);
             }
-            // "operand rows written, previous accumulators read": all threads arrive, only the issuing thread waits
+            fence_proxy_async();
+            // operand rows written and the accumulators of the previous tile read by every thread
             asm volatile("tcgen05.fence::before_thread_sync;");
-            // (two barriers in turn: a thread can be one step ahead of the slowest, never two -- its next bin needs the MMA
-            // that the issuing thread only starts after this wait)
-#if TPCF_TC_ARRIVE
-            asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(arr_bar + 8 * (na & 1)) : "memory");
-#else
             __syncthreads();
-#endif
+            asm volatile("tcgen05.fence::after_thread_sync;");
             if (tid == 0) {
-#if TPCF_TC_ARRIVE
-                mbar_wait(arr_bar + 8 * (na & 1), (na >> 1) & 1);
-#endif
-                asm volatile("tcgen05.fence::after_thread_sync;");
-                if (s < nsub) {
-                    const uint32_t lc = s / kSubPerChunk, sub = s % kSubPerChunk, n = gch + lc;
-                    const uint32_t sa = smem_u32(smem + L.abuf) + (gs & 1) * kTcABytes;
-                    const uint32_t sb = smem_u32(ring + (size_t)(n % kTcRing) * kSlotStride) + sub * kTcBBytes;
-                    const uint32_t d = tmem + (gs & 1) * kSubJ;
+                const uint32_t sa = smem_u32(smem + L.abuf), sb = smem_u32(slot);
 #pragma unroll
-                    for (int ks = 0; ks < kTcK / 8; ++ks) {
-                        const uint64_t da = umma_desc(sa + ks * 2 * kTcALbo, kTcALbo, kTcSbo), db = umma_desc(sb + ks * 2 * kTcBLbo, kTcBLbo, kTcSbo);
-                        asm volatile("{\n .reg .pred p;\n setp.ne.b32 p, %4, 0;\n tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n}" ::"r"(d),
-                                     "l"(da), "l"(db), "r"(kTcIdesc), "r"(ks)
-                                     : "memory");
-                    }
-                    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(full_bar + 8 * (gs & 1)) : "memory");
+                for (int ks = 0; ks < kTcK / 8; ++ks) {
+                    const uint64_t da = umma_desc(sa + ks * 2 * kTcALbo, kTcALbo, kTcSbo), db = umma_desc(sb + ks * 2 * kTcBLbo, kTcBLbo, kTcSbo);
+                    asm volatile("{\n .reg .pred p;\n setp.ne.b32 p, %4, 0;\n tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n}" ::"r"(tmem),
+                                 "l"(da), "l"(db), "r"(kTcIdesc), "r"(ks)
+                                 : "memory");
                 }
-                // every thread is past the bin of subtile s - 2: the chunk of subtiles s - 3, s - 2 is free for a new one
-                if (s >= 3 && (s & 1)) {
-                    const uint32_t lc = (s - 3) / 2;
-                    if (lc + kTcRing < nchunks) fetch_chunk(gch + lc + kTcRing, ch + lc + kTcRing);
-                }
+                asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(full_bar) : "memory");
+                // every thread is past the bin of tile t - 1: its slot takes tile t + 2
+                if (t >= 1 && t + kTcRing - 1 < ntile) fetch_tile(n + kTcRing - 1, tabs + kTcRing - 1);
             }
-            if (pd.valid) {
-                const uint32_t ps = gs - 1;
-                mbar_wait(full_bar + 8 * (ps & 1), (ps >> 1) & 1);
-                asm volatile("tcgen05.fence::after_thread_sync;");
-                tc_bin<MAP>(pd, tlane + (ps & 1) * kSubJ, wt, lut, reinterpret_cast<char*>(hist), slow, rq, qn, ibase + warp * 32, p.n_i, p.n_j,
-                            p.shift, p.sqrt_scale, p.sqrt_clamp, npath);
-            }
-            pd = cur;
-            if (s < nsub) ++gs;
-            ++na;
+            mbar_wait(full_bar, gs & 1);
+            asm volatile("tcgen05.fence::after_thread_sync;");
+            tc_bin<MAP>(rw, tlane, reinterpret_cast<const float4*>(slot + kTcBBytes), tabs * kTcSubJ, mask, wt, lut, reinterpret_cast<char*>(hist),
+                        slow, rq, qn, ibase + warp * 32, p.n_i, p.n_j, p.shift, p.sqrt_scale, p.sqrt_clamp, npath);
+            ++gs;
         }
+        const uint32_t nchunks = ntile;
         gch += nchunks;
         pairs_since_flush += (unsigned long long)nchunks * kChunkJ * kTcThreads;
         if (tid == 0 && ws == 0 && js == 0) ++items_done;
@@ -1316,9 +1286,10 @@ __global__ void quads_kernel(const double4* __restrict__ x64, uint64_t nquads, f
 // j-side role: every kSubJ consecutive rows form a subtile (one warp here).  cs = (fp32 centre, radius) as
 // above; xs = (-2 b', |b'|^2) with b' the fp32 rounding of (row - centre) formed in fp64 and |b'|^2 the fp32
 // rounding of the fp64 square of that rounded offset (the window loops evaluate |a - b|^2 = |a|^2 + |b|^2 - 2 a.b).
+template <int SUBJ>
 __global__ void subtiles_kernel(const double4* __restrict__ x64, uint64_t nsub, float4* __restrict__ xs, float4* __restrict__ cs,
                                 float* __restrict__ xb) {
-    constexpr int H = kSubJ / 32;                   // rows per lane
+    constexpr int H = SUBJ / 32;                   // rows per lane
     const uint64_t w = (blockIdx.x * (uint64_t)blockDim.x + threadIdx.x) >> 5;
     const int lane = threadIdx.x & 31;
     if (w >= nsub) return;
@@ -1326,7 +1297,7 @@ __global__ void subtiles_kernel(const double4* __restrict__ x64, uint64_t nsub, 
     double sx = 0, sy = 0, sz = 0;
 #pragma unroll
     for (int h = 0; h < H; ++h) {
-        v[h] = x64[w * kSubJ + h * 32 + lane];
+        v[h] = x64[w * SUBJ + h * 32 + lane];
         sx += v[h].x; sy += v[h].y; sz += v[h].z;
     }
 #pragma unroll
@@ -1335,7 +1306,7 @@ __global__ void subtiles_kernel(const double4* __restrict__ x64, uint64_t nsub, 
         sy += __shfl_xor_sync(0xffffffffu, sy, off);
         sz += __shfl_xor_sync(0xffffffffu, sz, off);
     }
-    const float cx = (float)(sx / kSubJ), cy = (float)(sy / kSubJ), cz = (float)(sz / kSubJ);
+    const float cx = (float)(sx / SUBJ), cy = (float)(sy / SUBJ), cz = (float)(sz / SUBJ);
     double r = 0;
 #pragma unroll
     for (int h = 0; h < H; ++h) {
@@ -1343,10 +1314,10 @@ __global__ void subtiles_kernel(const double4* __restrict__ x64, uint64_t nsub, 
         r = fmax(r, sqrt(dx * dx + dy * dy + dz * dz));
         const float bx = (float)dx, by = (float)dy, bz = (float)dz;
         const double nb = (double)bx * bx + (double)by * by + (double)bz * bz;
-        xs[w * kSubJ + h * 32 + lane] = make_float4(-2.f * bx, -2.f * by, -2.f * bz, (float)nb);
-        {   // the same row as a K = 16 TF32 operand row of the tensor engine (layout: kernels.cuh)
+        xs[w * SUBJ + h * 32 + lane] = make_float4(-2.f * bx, -2.f * by, -2.f * bz, (float)nb);
+        if (xb) {   // the same row as a K = 16 TF32 operand row of the tensor engine (layout: kernels.cuh)
             const int j = h * 32 + lane;
-            float* t = xb + (size_t)w * kSubJ * kTcK + (j / 8) * 32 + (j % 8) * 4;
+            float* t = xb + (size_t)w * SUBJ * kTcK + (j / 8) * 32 + (j % 8) * 4;
             const float m[3] = {-2.f * bx, -2.f * by, -2.f * bz};
             float mh[3], ml[3];
 #pragma unroll
@@ -1355,10 +1326,10 @@ __global__ void subtiles_kernel(const double4* __restrict__ x64, uint64_t nsub, 
                 ml[d] = tf32_hi(m[d] - mh[d]);
             }
             const float wv = (float)nb, wh = tf32_hi(wv), wm = tf32_hi(wv - wh), wl = tf32_hi((wv - wh) - wm);
-            *reinterpret_cast<float4*>(t + 0 * kSubJ * 4) = make_float4(mh[0], mh[1], mh[2], ml[0]);
-            *reinterpret_cast<float4*>(t + 1 * kSubJ * 4) = make_float4(ml[1], ml[2], mh[0], mh[1]);
-            *reinterpret_cast<float4*>(t + 2 * kSubJ * 4) = make_float4(mh[2], 1.f, 1.f, 1.f);
-            *reinterpret_cast<float4*>(t + 3 * kSubJ * 4) = make_float4(wh, wm, wl, 0.f);
+            *reinterpret_cast<float4*>(t + 0 * SUBJ * 4) = make_float4(mh[0], mh[1], mh[2], ml[0]);
+            *reinterpret_cast<float4*>(t + 1 * SUBJ * 4) = make_float4(ml[1], ml[2], mh[0], mh[1]);
+            *reinterpret_cast<float4*>(t + 2 * SUBJ * 4) = make_float4(mh[2], 1.f, 1.f, 1.f);
+            *reinterpret_cast<float4*>(t + 3 * SUBJ * 4) = make_float4(wh, wm, wl, 0.f);
         }
     }
 #pragma unroll
@@ -1435,10 +1406,12 @@ cudaError_t launch_quads(const double4* x64, uint64_t n_pad, float4* xq, float4*
     return cudaGetLastError();
 }
 
-cudaError_t launch_subtiles(const double4* x64, uint64_t n_pad, float4* xs, float4* cs, float* xb, cudaStream_t st) {
-    const uint64_t nsub = n_pad / kSubJ;
+cudaError_t launch_subtiles(const double4* x64, uint64_t n_pad, float4* xs, float4* cs, float4* xt, float4* ct, float* xb,
+                            cudaStream_t st) {
     const int block = 256;
-    subtiles_kernel<<<(unsigned)((nsub * 32 + block - 1) / block), block, 0, st>>>(x64, nsub, xs, cs, xb);
+    const uint64_t nsub = n_pad / kSubJ, ntile = n_pad / kTcSubJ;
+    subtiles_kernel<kSubJ><<<(unsigned)((nsub * 32 + block - 1) / block), block, 0, st>>>(x64, nsub, xs, cs, nullptr);
+    subtiles_kernel<kTcSubJ><<<(unsigned)((ntile * 32 + block - 1) / block), block, 0, st>>>(x64, ntile, xt, ct, xb);
     return cudaGetLastError();
 }
 

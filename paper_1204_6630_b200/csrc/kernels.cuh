@@ -15,9 +15,12 @@ struct PairParams {
     // j side: rows as (-2 offset, |offset|^2) from the centre of their 32-row subtile, and the subtiles' (centre, radius)
     const float4* xs;
     const float4* cs;
-    // j side, tensor engine: per subtile a kSubJ x kTcK tile of TF32 values in the K-major no-swizzle core-matrix layout
-    // (8 rows x 16 bytes contiguous; 8-row groups 128 B apart, the four 16-byte K chunks kSubJ * 16 B apart).  Row j:
-    // m_hi(3) m_lo(3) m_hi(3) 1 1 1 w_hi w_mid w_lo 0 with m = -2 offset, w = |offset|^2 split into TF32 parts
+    // j side, tensor engine: the same roles for kTcSubJ = 128-row tiles (rows xt, spheres ct), and per tile a
+    // kTcSubJ x kTcK block of TF32 values in the K-major no-swizzle core-matrix layout (8 rows x 16 bytes contiguous;
+    // 8-row groups 128 B apart, the four 16-byte K chunks kTcSubJ * 16 B apart).  Row j: m_hi(3) m_lo(3) m_hi(3) 1 1 1
+    // w_hi w_mid w_lo 0 with m = -2 offset, w = |offset|^2 split into TF32 parts
+    const float4* xt;
+    const float4* ct;
     const float* xb;
     const double4* xi64;        // fp64 unit vectors (padded with (2,2,2)); the recheck path and the fp64 engine read these
     const double4* xj64;
@@ -55,6 +58,7 @@ struct LaunchInfo {
 };
 
 constexpr int kNumCounters = 10;
+constexpr int kTcSubJ = 128;           // j-rows per tile of the tensor engine (one bounding sphere, one MMA)
 constexpr int kTcK = 16;               // K of the tensor engine's operand tiles (two tcgen05.mma kind::tf32 steps of 8)
 constexpr int kSortChunk = 2048;        // elements per block of the radix sort
 
@@ -71,7 +75,8 @@ cudaError_t launch_permute(const double4* x64_rows, const uint32_t* order, uint6
 // i-side role: per kIPerThread-row group ("quad") its (centre, radius) and the rows as fp32 offsets from the centre
 cudaError_t launch_quads(const double4* x64, uint64_t n_pad, float4* xq, float4* cq, cudaStream_t st);
 // j-side role: per 32-row subtile its (centre, radius) and the rows as (-2 offset, |offset|^2)
-cudaError_t launch_subtiles(const double4* x64, uint64_t n_pad, float4* xs, float4* cs, float* xb, cudaStream_t st);
+cudaError_t launch_subtiles(const double4* x64, uint64_t n_pad, float4* xs, float4* cs, float4* xt, float4* ct, float* xb,
+                            cudaStream_t st);
 // subset mode: caller rows -> positions in the sorted catalog (keys for the sort) with range check
 cudaError_t launch_row_keys(const int64_t* rows, uint64_t nrows, uint64_t n_src, const uint32_t* inv, uint64_t* keys,
                             uint32_t* idx, int* bad_flag, cudaStream_t st);
