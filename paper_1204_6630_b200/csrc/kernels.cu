@@ -1467,7 +1467,9 @@ cudaError_t launch_pairs_tensor(const PairParams& p, CellMap map, int sm_count, 
     const int regs_cta = ((fa.numRegs + 7) / 8 * 8) * kTcThreads;
     int per_sm = std::min<int>(smem_sm / (int)(smem + fa.sharedSizeBytes + 1024), regs_sm / std::max(regs_cta, 1));
     per_sm = std::min(per_sm, (int)(512 / kTcCols));
-    if (per_sm < 1) return cudaErrorLaunchOutOfResources;
+    // fine binnings (thousands of lookup cells: config 5) leave room for fewer than 3 such CTAs per SM, i.e. too few
+    // warps to hide the step-by-step MMA pipeline: those run the FFMA2 kernel
+    if (per_sm < 3) return launch_pairs_fast(p, map, sm_count, st, info);
     const uint64_t citems = (uint64_t)p.n_items_part * (kTileI / kTcThreads) * p.jsplit;
     int grid = (int)std::min<uint64_t>((uint64_t)sm_count * per_sm, std::max<uint64_t>(citems, 1));
     kern<<<grid, kTcThreads, smem, st>>>(p);

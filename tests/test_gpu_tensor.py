@@ -1,0 +1,131 @@
+"""GPU parity of the tensor engine (TPCF_ENGINE_TENSOR: the window quantity by 3xTF32 tcgen05.mma into tensor memory,
+DESIGN.md section 6): against the fp64 oracle element by element where the oracle finishes in seconds, and -- at the
+sizes bench.py times -- against the fast and the fp64 engines, whose histograms it must reproduce bit for bit (the
+tensor core only changes how q is formed for pairs outside the guard bands; every pair inside one is rechecked in fp64).
+"""
+import numpy as np
+import pytest
+
+import oracle
+import paper_1204_6630_b200 as T
+import synth
+from test_gpu_parity import KINDS, assert_parity, assert_w, full, gpu_all, oracle_all, totals
+
+pytestmark = pytest.mark.gpu
+
+
+def tensor_ctx(nbins, e):
+    c = T.Context(nbins, e, "explicit")
+    c.set_engine("tensor")
+    return c
+
+
+@pytest.mark.parametrize("idx,nd,nr", [(1, None, None), (2, 20_000, 17_777), (3, 9_000, 11_111), (4, 6_000, 12_345),
+                                       (5, 20_000, 20_000)])
+def test_tensor_engine_matches_oracle(idx, nd, nr, oracle_threads):
+    D, R, e, cfg = synth.make_config(idx, n_d=nd, n_r=nr)
+    nd, nr = D.shape[0], R.shape[0]
+    o = oracle_all(D, R, e, oracle_threads)
+    with tensor_ctx(cfg.nbins, e) as c:
+        c.load("D", D)
+        c.load("R", R)
+        g = gpu_all(c)
+        wg = c.estimate()
+        used = np.asarray(c.stats()["win_blocks"])
+        c.set_engine("exact64")
+        gx = gpu_all(c)
+    for k in KINDS:
+        assert_parity(g[k], o[k], totals(nd, nr)[k])
+        np.testing.assert_array_equal(g[k], gx[k])            # tensor engine == fp64 engine, bit for bit
+    assert_w(wg, oracle.estimate(o["DD"].hist, o["DR"].hist, o["RR"].hist, nd, nr))
+    if idx != 5:                                              # config 5's 8192 lookup cells run the FFMA2 kernel instead
+        assert used[:3].sum() > 0, "no block went through the tensor-core window path"
+
+
+@pytest.mark.parametrize("idx", [2, 3, 4])
+def test_tensor_engine_full_size_equals_fast_engine(idx):
+    """Configs 2-4 at BASELINE.json's sizes, in the launch configuration bench.py times: every histogram of the tensor
+    engine equals the fast engine's (which the other tests tie to the oracle on row subsets and to the fp64 engine)."""
+    D, R, e, cfg = synth.make_config(idx)
+    nd, nr = D.shape[0], R.shape[0]
+    res = {}
+    for eng in ("fast", "tensor"):
+        with T.Context(cfg.nbins, e, "explicit") as c:
+            c.set_engine(eng)
+            c.load("D", D)
+            c.load("R", R)
+            res[eng] = gpu_all(c)
+            if eng == "tensor":
+                assert c.stats()["block"] == 128              # the tensor kernel really ran (4-warp CTAs)
+    for k in KINDS:
+        assert int(res["tensor"][k].sum()) == totals(nd, nr)[k]
+        np.testing.assert_array_equal(res["tensor"][k], res["fast"][k])
+
+
+@pytest.mark.parametrize("idx,nrows", [(3, 2000), (4, 2000)])
+def test_tensor_engine_row_subset_against_oracle(idx, nrows, oracle_threads):
+    D, R, e, cfg = synth.make_config(idx)
+    nd, nr = D.shape[0], R.shape[0]
+    rows_d, rows_r = synth.subset_rows(nd, nrows, 12345), synth.subset_rows(nr, nrows, 12346)
+    d, r = oracle.radec_to_xyz(D), oracle.radec_to_xyz(R)
+    with tensor_ctx(cfg.nbins, e) as c:
+        c.load("D", D)
+        c.load("R", R)
+        g = gpu_all(c, {"DD": rows_d, "DR": rows_d, "RR": rows_r})
+    o = {"DD": oracle.count_rows(d, rows_d, d, True, e, validate=True, threads=oracle_threads),
+         "DR": oracle.count_rows(d, rows_d, r, False, e, validate=True, threads=oracle_threads),
+         "RR": oracle.count_rows(r, rows_r, r, True, e, validate=True, threads=oracle_threads)}
+    exp = {"DD": nrows * (nd - 1), "DR": nrows * nr, "RR": nrows * (nr - 1)}
+    for k in KINDS:
+        assert_parity(g[k], o[k], exp[k])
+
+
+@pytest.mark.parametrize("nd,nr", [(1, 1), (2, 3), (127, 129), (1023, 1025), (2049, 1), (3000, 5000)])
+def test_tensor_engine_ragged_sizes(nd, nr):
+    D, R, _, _ = synth.make_config(1, n_d=nd, n_r=nr)
+    e = np.array([0.0, 0.05, 0.5, 2.0, 180.0])
+    o = oracle_all(D, R, e, 1)
+    with tensor_ctx(4, e) as c:
+        c.load("D", D)
+        c.load("R", R)
+        g = gpu_all(c)
+    for k in KINDS:
+        assert_parity(g[k], o[k], totals(nd, nr)[k])
+
+
+def test_tensor_engine_sparse_and_duplicate_rows(oracle_threads):
+    rng = np.random.default_rng(11)
+    def sky(n):
+        return np.stack([rng.uniform(0.0, 360.0, n), np.degrees(np.arcsin(rng.uniform(-1.0, 1.0, n)))], 1)
+    D, R = sky(700), sky(900)
+    e = np.linspace(0.0, 180.0, 37)
+    with tensor_ctx(36, e) as c:
+        c.load("D", D)
+        c.load("R", R)
+        g = gpu_all(c)
+        o = oracle_all(D, R, c.edges(), oracle_threads)
+        for k in KINDS:
+            assert_parity(g[k], o[k], totals(700, 900)[k])
+    P = np.array([[10.0, 20.0], [10.0, 20.0], [10.0, 20.0], [50.0, -30.0]])
+    with tensor_ctx(2, [0.0, 1.0, 180.0]) as c:
+        c.load("D", P)
+        c.load("R", P)
+        assert tuple(full(*c.count("DD"))) == (0, 3, 3, 0)
+        assert tuple(full(*c.count("DR"))) == (0, 10, 6, 0)
+
+
+def test_tensor_engine_guard_scale_and_partition_leave_the_counts_unchanged():
+    D, R, e, cfg = synth.make_config(3, n_d=60_000, n_r=50_000)
+    with tensor_ctx(cfg.nbins, e) as c:
+        c.load("D", D)
+        c.load("R", R)
+        base = gpu_all(c)
+        c.set_guard_scale(8.0)                       # 8x wider guard bands: more fp64 rechecks, same integers
+        np.testing.assert_array_equal(full(*c.count("DR")), base["DR"])
+        c.set_guard_scale(1.0)
+        parts = np.zeros_like(base["DD"])
+        for part in range(3):                        # work-item partition of the multi-GPU path
+            c.set_partition(part, 3)
+            parts += full(*c.count("DD"))
+        c.set_partition(0, 1)
+        np.testing.assert_array_equal(parts, base["DD"])
