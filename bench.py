@@ -97,11 +97,13 @@ class ClockSampler:
 OPS_PER_PAIR = 5.5
 
 
-def profile_summary(cfg_idx: int):
+def profile_summary(cfg_idx: int, engine: str = "fast"):
     """Executed-instruction figures of the pair kernel from the committed ncu capture (profiles/inst_per_pair.json)."""
     path = os.path.join(ROOT, "profiles", "inst_per_pair.json")
     try:
         d = json.load(open(path))
+        if engine == "tensor":
+            return d.get(f"cfg{cfg_idx}_tensor") or d.get("default_tensor") or {}
         return d.get(f"cfg{cfg_idx}") or d["default"]
     except Exception:
         return {}
@@ -179,6 +181,7 @@ def run_ours(args):
     st = torch.cuda.Stream()
     ctx = T.Context(nb, e, "explicit")
     ctx.set_stream(st.cuda_stream)
+    ctx.set_engine(args.engine)
     ctx.load("D", D, stream=st.cuda_stream)
     ctx.load("R", R, stream=st.cuda_stream)
     tdist.apply_partition(ctx)
@@ -228,6 +231,30 @@ def run_ours(args):
     for i in range(3):
         assert int(res[i].sum()) == want[i], (KINDS[i], int(res[i].sum()), want[i])
 
+    # the other engine on the same resident catalogs, a few steps, for the record (its histograms must be the same integers)
+    other = None
+    if world == 1 and args.engine == "tensor":
+        ctx.set_engine("fast")
+        out2 = torch.zeros_like(out)
+        def step2():
+            with torch.cuda.stream(st):
+                flush.zero_()
+                for i, k in enumerate(KINDS):
+                    ctx.count_async(k, out2[i])
+        step2()
+        barrier()
+        ev2, ev3 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev2.record(st)
+        for _ in range(3):
+            step2()
+        ev3.record(st)
+        barrier()
+        ms2 = ev2.elapsed_time(ev3) / 3
+        assert torch.equal(out2, out), "fast and tensor engines disagree"
+        other = {"engine": "fast (FFMA2 window loops)", "value": pairs_step / (ms2 * 1e-3) / 1e9, "unit": UNIT, "ms_per_step": ms2, "steps": 3,
+                 "histograms_identical_to_the_timed_engine": True}
+        ctx.set_engine(args.engine)
+
     # ---- end to end through the synchronous C ABI with pinned host buffers --------------------------------
     Dp, Rp = torch.from_numpy(D).pin_memory(), torch.from_numpy(R).pin_memory()
     e2e_steps = max(1, min(args.steps, 5))
@@ -264,7 +291,8 @@ def run_ours(args):
 
     # ---- roofline of the dominant kernel (pair_fast_kernel): plain ALU issue --------------------------------
     clocks = clk.summary()
-    prof = profile_summary(args.config)
+    prof = profile_summary(args.config, args.engine if stats["block"] == 128 else "fast")
+    tensor_ran = stats["block"] == 128          # fine binnings (config 5) run the FFMA2 kernel under either engine
     peak_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     try:
         sm_max = float(json.load(open(peak_path))["sm_max_mhz"])
@@ -279,8 +307,10 @@ def run_ours(args):
     achieved = pairs_per_s_kernel * OPS_PER_PAIR / 1e12
     roofline = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "T lane-operations/s (FP32 FMA-pipe + ALU-pipe operations)",
                 "frac": achieved / peak, "traffic": prof.get("dram_bytes_per_launch"),
-                "kernel": "pair_fast_kernel", "ops_per_pair": OPS_PER_PAIR,
-                "ops_per_pair_source": "DESIGN.md section 7: 4 FMA-pipe + 1.5 ALU-pipe lane-operations per pair (1-edge window loop)",
+                "kernel": "pair_tensor_kernel" if tensor_ran else "pair_fast_kernel", "ops_per_pair": OPS_PER_PAIR,
+                "ops_per_pair_source": "DESIGN.md section 7: 4 FMA-pipe + 1.5 ALU-pipe lane-operations per pair (1-edge window loop)" +
+                                       ("; in the tensor engine the 4 dot-product operations run as a 3xTF32 tcgen05.mma, the 1.5 bin-decision "
+                                        "operations on the ALU pipe (bound 42.7 pairs/clk/SM)" if tensor_ran else ""),
                 "executed_inst_per_pair": prof.get("inst_per_pair"), "issue_active_pct": prof.get("issue_active_pct"),
                 "executed_source": prof.get("source"),
                 "kernel_pairs_per_s": pairs_per_s_kernel, "kernel_ms_avg": (sum(kernel_ms) / len(kernel_ms)) if kernel_ms else None,
@@ -308,7 +338,9 @@ def run_ours(args):
             "data": "synthetic",
             "config": {"workload": workload_name(args.config, cfg, nd, nr),
                        "l2": "256 MiB write between steps (inside the timed region); catalogs (28 MB each) are L2-resident by design",
-                       "engine": "fast (fp32 squared chord + fp64 recheck of guard-band pairs)",
+                       "engine": ("tensor (window quantity by 3xTF32 tcgen05.mma into TMEM + tcgen05.ld read-back; guard bands, cell lookup and "
+                                  "fp64 recheck as in the fast engine)" if tensor_ran else
+                                  "fast (fp32 squared chord by FFMA2 + fp64 recheck of guard-band pairs)"),
                        "parallelism": f"tile work items w % {world} == rank, one all-reduce of 3x{nb + 2} int64" if world > 1 else "1 GPU",
                        "grid": stats["grid"], "block": stats["block"], "smem_bytes": stats["smem_bytes"], "cells": stats["cells"]},
             "seconds_per_w_theta": ms_step * 1e-3,
@@ -316,7 +348,8 @@ def run_ours(args):
                     "seconds_per_step": e2e_s, "steps": e2e_steps,
                     "path": "tpcf_load(D), tpcf_load(R) from pinned host rows + tpcf_count x3 + tpcf_estimate"},
             "gpu_launches": args.steps * 6,
-            "gpu_launches_note": "per step: 3 x (pair_fast_kernel + finalize_kernel); memsets are driver memset nodes; the e2e leg adds 2 x 28 load kernels per step",
+            "gpu_launches_note": f"per step: 3 x ({'pair_tensor_kernel' if tensor_ran else 'pair_fast_kernel'} + finalize_kernel); memsets are driver memset nodes; the e2e leg adds 2 x 29 load kernels per step",
+            "other_engine": other,
             "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu, "paper_context": PAPER_CONTEXT}
     print(json.dumps(line))
     if world > 1:
@@ -332,6 +365,8 @@ def main():
     ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--engine", default="tensor", choices=["tensor", "fast"],
+                    help="pair kernel family (include/tpcf.h tpcf_engine); both give the same histograms")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.steps < 1:
