@@ -6,7 +6,9 @@
 //                       candidate bin edges from bounding spheres -> 1..3 threshold compares per pair with
 //                       register counters, else O(1) cell lookup + shared-memory partial histogram;
 //                       guard band -> fp64 recheck; uint64 merge                        (steps a3-a7)
-//   pair_exact64_kernel plain fp64 count, the device-side cross-check of the fast kernel
+//   pair_tensor_kernel  the same count with the window quantity formed by a 3xTF32 tcgen05.mma into tensor memory
+//                       (one i-row per thread, tcgen05.ld read-back), everything else shared with pair_fast_kernel
+//   pair_exact64_kernel plain fp64 count, the device-side cross-check of the other two
 //
 // What is computed per pair is PAPER.md:37 ("dot product and arc-cosine ... to extract the angle between
 // two objects") followed by PAPER.md:38 (histogram fill with shared-memory atomics, partial histograms
