@@ -32,7 +32,7 @@ EXPORTS = (
     "tpcf_estimate_from", "tpcf_destroy", "tpcf_last_error", "tpcf_set_stream", "tpcf_set_engine",
     "tpcf_set_guard_scale", "tpcf_set_partition", "tpcf_get_stats", "tpcf_get_thresholds", "tpcf_classify_fast",
     "tpcf_plan", "tpcf_plan_item_pairs", "tpcf_set_kernel_timing", "tpcf_get_kernel_times", "tpcf_set_window",
-    "tpcf_get_bands", "tpcf_window_host",
+    "tpcf_get_bands", "tpcf_window_host", "tpcf_tensor_probe",
 )
 
 
@@ -80,6 +80,7 @@ def lib() -> ctypes.CDLL:
             "tpcf_set_window": [vp, i32],
             "tpcf_get_bands": [vp, i32, vp, vp, vp, ctypes.POINTER(i32)],
             "tpcf_window_host": [vp, ctypes.c_float, ctypes.c_float, ctypes.POINTER(i32), ctypes.POINTER(i32)],
+            "tpcf_tensor_probe": [vp, vp, vp, ctypes.c_size_t, vp],
             "tpcf_set_partition": [vp, i32, i32],
             "tpcf_get_stats": [vp, ctypes.POINTER(tpcf_stats)],
             "tpcf_set_kernel_timing": [vp, i32],
@@ -254,6 +255,18 @@ def tpcf_get_kernel_times(ctx) -> np.ndarray:
     n = ctypes.c_int()
     _check(ctx, lib().tpcf_get_kernel_times(ctx, _np_ptr(ms), 64, ctypes.byref(n)))
     return ms[: n.value].copy()
+
+
+def tpcf_tensor_probe(ctx, s_rows: np.ndarray, b_rows: np.ndarray) -> np.ndarray:
+    """q tiles of the tensor engine's MMA: s_rows, b_rows (ntiles, 128, 4) float32 -> (ntiles, 128, 128) float32."""
+    s_rows = np.ascontiguousarray(s_rows, dtype=np.float32)
+    b_rows = np.ascontiguousarray(b_rows, dtype=np.float32)
+    if s_rows.ndim != 3 or s_rows.shape[1:] != (128, 4) or b_rows.shape != s_rows.shape:
+        raise ValueError("s_rows and b_rows must both be (ntiles, 128, 4)")
+    q = np.empty((s_rows.shape[0], 128, 128), dtype=np.float32)
+    _check(ctx, lib().tpcf_tensor_probe(ctx, s_rows.ctypes.data_as(ctypes.c_void_p), b_rows.ctypes.data_as(ctypes.c_void_p),
+                                        s_rows.shape[0], q.ctypes.data_as(ctypes.c_void_p)))
+    return q
 
 
 def tpcf_classify_fast(ctx, d2: float) -> int:

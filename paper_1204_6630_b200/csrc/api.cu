@@ -679,6 +679,29 @@ tpcf_status tpcf_classify_fast(const tpcf_ctx* ctx, float d2, int* slot_out) {
     return TPCF_OK;
 }
 
+tpcf_status tpcf_tensor_probe(tpcf_ctx* ctx, const float* s_rows, const float* b_rows, size_t ntiles, float* q_out) {
+    if (!ctx) return TPCF_EINVAL;
+    if (!s_rows || !b_rows || !q_out || ntiles == 0 || ntiles > 65535) return fail(ctx, TPCF_EINVAL, "tpcf_tensor_probe: bad argument");
+    tpcf_status s = ensure_cuda(ctx);
+    if (s) return s;
+    const size_t rows = ntiles * 128;
+    float4 *ds = nullptr, *db = nullptr;
+    float* dq = nullptr;
+    cudaError_t e = cudaMalloc(&ds, rows * sizeof(float4));
+    if (e == cudaSuccess) e = cudaMalloc(&db, rows * sizeof(float4));
+    if (e == cudaSuccess) e = cudaMalloc(&dq, rows * 128 * sizeof(float));
+    if (e == cudaSuccess) e = cudaMemcpyAsync(ds, s_rows, rows * sizeof(float4), cudaMemcpyHostToDevice, ctx->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(db, b_rows, rows * sizeof(float4), cudaMemcpyHostToDevice, ctx->stream);
+    if (e == cudaSuccess) e = launch_tensor_probe(ds, db, dq, (uint32_t)ntiles, ctx->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(q_out, dq, rows * 128 * sizeof(float), cudaMemcpyDeviceToHost, ctx->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    cudaFree(ds);
+    cudaFree(db);
+    cudaFree(dq);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "tpcf_tensor_probe");
+    return TPCF_OK;
+}
+
 tpcf_status tpcf_window_host(const tpcf_ctx* ctx, float lo2, float hi2, int* first_band_out, int* n_edges_out) {
     if (!ctx || !first_band_out || !n_edges_out) return TPCF_EINVAL;
     if (!(lo2 >= 0.0f) || !(hi2 >= lo2) || !(hi2 < 64.0f)) return TPCF_EINVAL;

@@ -1044,6 +1044,76 @@ __global__ void __launch_bounds__(kTcThreads, 4) pair_tensor_kernel(const __grid
     }
 }
 
+// One (128 i-rows) x (128 j-rows) tile through exactly the operand preparation, MMA and read-back of pair_tensor_kernel,
+// returning the accumulators instead of binning them: the measurement behind the tensor engine's error bound
+// (tpcf_tensor_probe, tests/test_gpu_tensor.py).  srows = (s, |s|^2 - mid_0) per i-row, brows = (-2 b', |b'|^2) per j-row.
+__global__ void __launch_bounds__(kTcThreads) tensor_probe_kernel(const float4* __restrict__ srows, const float4* __restrict__ brows,
+                                                                  float* __restrict__ q) {
+    __shared__ __align__(128) unsigned char sA[kTcABytes];
+    __shared__ __align__(128) unsigned char sB[kTcBBytes];
+    __shared__ __align__(8) unsigned long long bar;
+    __shared__ uint32_t tbase;
+    const int tid = threadIdx.x, warp = tid >> 5;
+    const float4 sr = srows[(size_t)blockIdx.x * kTcThreads + tid], br = brows[(size_t)blockIdx.x * kTcSubJ + tid];
+    unsigned char* ar = sA + (tid / 8) * kTcSbo + (tid % 8) * 16;
+    unsigned char* bp = sB + (tid / 8) * kTcSbo + (tid % 8) * 16;
+    {
+        const float xh = tf32_hi(sr.x), yh = tf32_hi(sr.y), zh = tf32_hi(sr.z);
+        const float xl = tf32_hi(sr.x - xh), yl = tf32_hi(sr.y - yh), zl = tf32_hi(sr.z - zh);
+        const float nh = tf32_hi(sr.w), nm = tf32_hi(sr.w - nh), nl = tf32_hi((sr.w - nh) - nm);
+        *reinterpret_cast<float4*>(ar) = make_float4(xh, yh, zh, xh);
+        *reinterpret_cast<float4*>(ar + kTcALbo) = make_float4(yh, zh, xl, yl);
+        *reinterpret_cast<float4*>(ar + 2 * kTcALbo) = make_float4(zl, nh, nm, nl);
+        *reinterpret_cast<float4*>(ar + 3 * kTcALbo) = make_float4(1.f, 1.f, 1.f, 0.f);
+        const float mh0 = tf32_hi(br.x), mh1 = tf32_hi(br.y), mh2 = tf32_hi(br.z);
+        const float ml0 = tf32_hi(br.x - mh0), ml1 = tf32_hi(br.y - mh1), ml2 = tf32_hi(br.z - mh2);
+        const float wh = tf32_hi(br.w), wm = tf32_hi(br.w - wh), wl = tf32_hi((br.w - wh) - wm);
+        *reinterpret_cast<float4*>(bp) = make_float4(mh0, mh1, mh2, ml0);
+        *reinterpret_cast<float4*>(bp + kTcBLbo) = make_float4(ml1, ml2, mh0, mh1);
+        *reinterpret_cast<float4*>(bp + 2 * kTcBLbo) = make_float4(mh2, 1.f, 1.f, 1.f);
+        *reinterpret_cast<float4*>(bp + 3 * kTcBLbo) = make_float4(wh, wm, wl, 0.f);
+    }
+    if (warp == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tbase)), "r"(kTcCols));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    }
+    if (tid == 0) {
+        mbar_init(smem_u32(&bar), 1);
+        fence_barrier_init();
+    }
+    fence_proxy_async();
+    asm volatile("tcgen05.fence::before_thread_sync;");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;");
+    const uint32_t tmem = tbase;
+    if (tid == 0) {
+#pragma unroll
+        for (int ks = 0; ks < kTcK / 8; ++ks) {
+            const uint64_t da = umma_desc(smem_u32(sA) + ks * 2 * kTcALbo, kTcALbo, kTcSbo), db = umma_desc(smem_u32(sB) + ks * 2 * kTcBLbo, kTcBLbo, kTcSbo);
+            asm volatile("{\n .reg .pred p;\n setp.ne.b32 p, %4, 0;\n tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n}" ::"r"(tmem), "l"(da),
+                         "l"(db), "r"(kTcIdesc), "r"(ks)
+                         : "memory");
+        }
+        asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(&bar)) : "memory");
+    }
+    mbar_wait(smem_u32(&bar), 0);
+    asm volatile("tcgen05.fence::after_thread_sync;");
+    float* out = q + ((size_t)blockIdx.x * kTcThreads + tid) * kTcSubJ;
+#pragma unroll 1
+    for (int half = 0; half < kTcSubJ / 64; ++half) {
+        uint32_t v[64];
+        const uint32_t ta = tmem + ((uint32_t)warp * 32u << 16) + half * 64;
+        TPCF_TMEM_LD32(v, 0, ta);
+        TPCF_TMEM_LD32(v, 32, ta + 32);
+        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+        for (int j = 0; j < 64; ++j) out[half * 64 + j] = __uint_as_float(v[j]);
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;");
+    __syncthreads();
+    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(kTcCols));
+}
+
 // ---- fp64 engine: work items per CTA -------------------------------------------------------------------------
 struct Item {
     uint32_t I, tile0, ntiles, valid;
@@ -1476,6 +1546,11 @@ cudaError_t launch_pairs_tensor(const PairParams& p, CellMap map, int sm_count, 
     int grid = (int)std::min<uint64_t>((uint64_t)sm_count * per_sm, std::max<uint64_t>(citems, 1));
     kern<<<grid, kTcThreads, smem, st>>>(p);
     if (info) *info = LaunchInfo{grid, kTcThreads, (int)smem, 1};
+    return cudaGetLastError();
+}
+
+cudaError_t launch_tensor_probe(const float4* srows, const float4* brows, float* q, uint32_t ntiles, cudaStream_t st) {
+    tensor_probe_kernel<<<ntiles, kTcThreads, 0, st>>>(srows, brows, q);
     return cudaGetLastError();
 }
 

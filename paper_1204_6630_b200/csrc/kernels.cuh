@@ -85,6 +85,8 @@ cudaError_t launch_gather(const double4* src64, const uint64_t* pos, uint64_t nr
                           cudaStream_t st);
 cudaError_t launch_pairs_fast(const PairParams& p, CellMap map, int sm_count, cudaStream_t st, LaunchInfo* info);
 cudaError_t launch_pairs_tensor(const PairParams& p, CellMap map, int sm_count, cudaStream_t st, LaunchInfo* info);
+// ntiles x (128 x 128) accumulator tiles of the tensor engine's MMA for given operand rows (device pointers)
+cudaError_t launch_tensor_probe(const float4* srows, const float4* brows, float* q, uint32_t ntiles, cudaStream_t st);
 cudaError_t launch_pairs_exact64(const PairParams& p, int sm_count, cudaStream_t st, LaunchInfo* info);
 // result[0 .. nbins+1] -> out (device), subtracting `self_pairs` from the slot that holds theta = 0
 cudaError_t launch_finalize(const unsigned long long* result, int nbins, int zero_slot, unsigned long long self_pairs,

@@ -129,3 +129,45 @@ def test_tensor_engine_guard_scale_and_partition_leave_the_counts_unchanged():
             parts += full(*c.count("DD"))
         c.set_partition(0, 1)
         np.testing.assert_array_equal(parts, base["DD"])
+
+
+def tensor_core_error_sample(ntiles=384, seed=20240607):
+    """Random blocks in the geometry of the window path (centre distance D, radii down to D >= 3.5 (r_i + r_j), the limit
+    of kFarKappa = 2.5) through tpcf_tensor_probe -- the kernel's own operand split, instruction and read-back -- against the
+    fp64 value of the same fp32 inputs.  Returns per tile: max |q_tc - q_fp64|, the band half width, t = D^2."""
+    rng = np.random.default_rng(seed)
+    s_rows = np.empty((ntiles, 128, 4), dtype=np.float32)
+    b_rows = np.empty((ntiles, 128, 4), dtype=np.float32)
+    tscale = np.empty(ntiles)
+    for t in range(ntiles):
+        D = 0.02 * 50.0 ** rng.uniform()                       # centre distance 0.02 .. 1
+        rs = D / rng.uniform(3.5, 40.0)                        # r_i + r_j
+        ri, rj = rs / 3.0, rs * 2.0 / 3.0
+        c = rng.normal(size=3)
+        c *= D / np.linalg.norm(c)
+        s = (c + ri * rng.uniform(-1, 1, size=(128, 3)) / np.sqrt(3.0)).astype(np.float32)
+        b = (rj * rng.uniform(-1, 1, size=(128, 3)) / np.sqrt(3.0)).astype(np.float32)
+        mid = np.float32(D * D * (1.0 + rng.uniform(-1, 1) * 2.0 * rs / D))      # an edge inside the window
+        sx, sy, sz = s[:, 0], s[:, 1], s[:, 2]
+        norm = (sz * sz + (sy * sy + sx * sx).astype(np.float32)).astype(np.float32)     # fp32, like the kernel (up to fma)
+        s_rows[t, :, :3] = s
+        s_rows[t, :, 3] = norm - mid
+        b_rows[t, :, :3] = np.float32(-2.0) * b
+        b_rows[t, :, 3] = (b.astype(np.float64) ** 2).sum(axis=1).astype(np.float32)
+        tscale[t] = D * D
+    with T.Context(4, [0.0, 1.0, 2.0, 3.0, 180.0], "explicit") as c:
+        q = T.tpcf_tensor_probe(c.handle, s_rows, b_rows).astype(np.float64)
+    S, B = s_rows.astype(np.float64), b_rows.astype(np.float64)
+    exact = S[:, :, None, 3] + B[:, None, :, 3] + np.einsum("tik,tjk->tij", S[:, :, :3], B[:, :, :3])
+    assert np.all(np.isfinite(q))
+    # a dot product at all: relative to the size of q the error is ~1e-6
+    assert np.all(np.abs(q - exact).max(axis=(1, 2)) < 2.0e-6 * np.abs(exact).max(axis=(1, 2)) + 1e-12)
+    return np.abs(q - exact).max(axis=(1, 2)), 3.0e-6 * tscale + 1.0e-7 * np.sqrt(tscale), tscale
+
+
+def test_tensor_core_accumulation_error_stays_well_inside_the_guard_band():
+    """The one step of the tensor engine that is not IEEE arithmetic is the accumulation inside tcgen05.mma.  Measure it
+    (6.3e6 values): the counters are only trusted for |q| beyond the band half width 3.0e-6 t + 1e-7 sqrt(t)
+    (tables.cpp guard_width); the error has to stay below a third of that."""
+    err, band, _ = tensor_core_error_sample()
+    assert np.all(err < band / 3.0), float((err / band).max())
