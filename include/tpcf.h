@@ -48,10 +48,12 @@ typedef enum { TPCF_DD = 0, TPCF_DR = 1, TPCF_RR = 2 } tpcf_kind;
  *                       coordinates, so the histograms equal those of TPCF_ENGINE_EXACT64 (default).
  *   TPCF_ENGINE_EXACT64 plain fp64 kernel: fp64 squared chord against fp64 thresholds 4 sin^2(e_k/2) by
  *                       binary search.  Slow; kept as the device-side cross-check of the fast engine.
- *   TPCF_ENGINE_TENSOR  experimental: the window quantity q of TPCF_ENGINE_FAST's far blocks is formed by a 3xTF32
- *                       tcgen05.mma (fp32 accumulators in tensor memory, one i-row per thread) instead of the FFMA2
- *                       chain; everything else (windows, guard bands, cell lookup, fp64 recheck) is the same.  The
- *                       tensor core's accumulation error is measured, not proven.
+ *   TPCF_ENGINE_TENSOR  the window quantity q of TPCF_ENGINE_FAST's far blocks is formed by a 3xTF32 tcgen05.mma
+ *                       (fp32 accumulators in tensor memory, one i-row per thread) instead of the FFMA2 chain;
+ *                       everything else (windows, guard bands, cell lookup, fp64 recheck) is the same, and so are the
+ *                       histograms.  Faster on all but fine binnings (which run the FFMA2 kernel under this engine
+ *                       too).  Not the default because the tensor core's accumulation error is measured (a factor 12
+ *                       inside the guard band, tpcf_tensor_probe), not proven.
  */
 typedef enum { TPCF_ENGINE_FAST = 0, TPCF_ENGINE_EXACT64 = 1, TPCF_ENGINE_TENSOR = 2 } tpcf_engine;
 
