@@ -171,3 +171,45 @@ def test_tensor_core_accumulation_error_stays_well_inside_the_guard_band():
     (tables.cpp guard_width); the error has to stay below a third of that."""
     err, band, _ = tensor_core_error_sample()
     assert np.all(err < band / 3.0), float((err / band).max())
+
+
+@pytest.mark.parametrize("case", ["window_off", "guard_half", "guard_16", "one_bin", "one_narrow_bin", "far_bins",
+                                  "linear_64_whole_range", "linear_300_fine", "tiny"])
+def test_tensor_engine_equals_fp64_engine_on_unusual_binnings_and_settings(case):
+    """Bit-identical to the plain fp64 kernel whatever the binning and the tuning knobs (window loops off: every row takes
+    the cell lookup; narrower and wider guard bands; one bin; bins far from 0; linear bins; fewer rows than one tile)."""
+    D, R, e, cfg = synth.make_config(3, n_d=30_000, n_r=20_000)
+    nb, mode, kw = cfg.nbins, "explicit", {}
+    if case == "window_off":
+        kw["window"] = False
+    elif case == "guard_half":
+        kw["gs"] = 0.5
+    elif case == "guard_16":
+        kw["gs"] = 16.0
+    elif case == "one_bin":
+        nb, e = 1, [0.0, 180.0]
+    elif case == "one_narrow_bin":
+        nb, e = 1, [1.0, 1.001]
+    elif case == "far_bins":
+        nb, e = 3, [30.0, 31.0, 32.0, 33.0]
+    elif case == "linear_64_whole_range":
+        D, R, _, _ = synth.make_config(4, n_d=40_000, n_r=30_000)
+        nb, e, mode = 64, [0.0, 180.0], "linear"
+    elif case == "linear_300_fine":
+        nb, e, mode = 300, [0.0, 10.0], "linear"
+    elif case == "tiny":
+        D, R, e, cfg = synth.make_config(1, n_d=100, n_r=130)
+        nb = cfg.nbins
+    out = {}
+    for eng in ("exact64", "tensor"):
+        with T.Context(nb, e, mode) as c:
+            c.set_engine(eng)
+            if kw.get("window") is False:
+                c.set_window(False)
+            if "gs" in kw:
+                c.set_guard_scale(kw["gs"])
+            c.load("D", D)
+            c.load("R", R)
+            out[eng] = gpu_all(c)
+    for k in KINDS:
+        np.testing.assert_array_equal(out["tensor"][k], out["exact64"][k])
