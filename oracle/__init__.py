@@ -34,6 +34,13 @@ def lib() -> ctypes.CDLL:
         L.orc_count_cross.restype = i32
         L.orc_count_rows.argtypes = [vp, i64p, sz, sz, vp, sz, i32, vp, i32, vp, vp, vp]
         L.orc_count_rows.restype = i32
+        f64 = ctypes.c_double
+        L.orc_count_auto_xyz.argtypes = [vp, sz, sz, sz, vp, i32, f64, vp, vp]
+        L.orc_count_auto_xyz.restype = i32
+        L.orc_count_cross_xyz.argtypes = [vp, sz, sz, sz, vp, sz, vp, i32, f64, vp, vp]
+        L.orc_count_cross_xyz.restype = i32
+        L.orc_count_rows_xyz.argtypes = [vp, i64p, sz, sz, vp, sz, i32, vp, i32, f64, vp, vp]
+        L.orc_count_rows_xyz.restype = i32
         L.orc_estimate.argtypes = [vp, vp, vp, i32, ctypes.c_uint64, ctypes.c_uint64, vp]
         L.orc_estimate.restype = None
         _lib = L
@@ -165,3 +172,42 @@ def estimate(dd, dr, rr, n_d: int, n_r: int) -> np.ndarray:
     w = np.empty(dd.shape[0], dtype=np.float64)
     lib().orc_estimate(_ptr(dd), _ptr(dr), _ptr(rr), dd.shape[0], int(n_d), int(n_r), _ptr(w))
     return w
+
+
+# ---- 3-D variant: Euclidean separations of Cartesian rows, bins in r -------------------------------
+def count_auto_xyz(xyz: np.ndarray, r_edges, near_tol: float = -1.0, threads: int = 1) -> Counts:
+    """DD or RR of the 3-D variant: all unordered pairs i<j, r = |a - b| in fp64; near_tol >= 0 also fills `near`."""
+    xyz = np.ascontiguousarray(xyz, dtype=np.float64)
+    e = np.ascontiguousarray(r_edges, dtype=np.float64)
+    nb, n = e.shape[0] - 1, xyz.shape[0]
+    L = lib()
+    call = lambda a, b, h, nr, mm: L.orc_count_auto_xyz(_ptr(xyz), n, a, b, _ptr(e), nb, near_tol, _ptr(h), _ptr(nr))
+    return _run("auto_xyz", _triangle_spans(n, threads * 4 if threads > 1 else 1), call, nb, near_tol >= 0, threads)
+
+
+def count_cross_xyz(a: np.ndarray, b: np.ndarray, r_edges, near_tol: float = -1.0, threads: int = 1) -> Counts:
+    """DR of the 3-D variant: all N_a * N_b ordered pairs."""
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    b = np.ascontiguousarray(b, dtype=np.float64)
+    e = np.ascontiguousarray(r_edges, dtype=np.float64)
+    nb = e.shape[0] - 1
+    L = lib()
+    call = lambda i0, i1, h, nr, mm: L.orc_count_cross_xyz(_ptr(a), a.shape[0], i0, i1, _ptr(b), b.shape[0], _ptr(e), nb,
+                                                           near_tol, _ptr(h), _ptr(nr))
+    return _run("cross_xyz", _even_spans(a.shape[0], threads), call, nb, near_tol >= 0, threads)
+
+
+def count_rows_xyz(a: np.ndarray, rows, b: np.ndarray, exclude_self: bool, r_edges, near_tol: float = -1.0,
+                   threads: int = 1) -> Counts:
+    """Row-subset mode of the 3-D variant."""
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    b = np.ascontiguousarray(b, dtype=np.float64)
+    r = np.ascontiguousarray(rows, dtype=np.int64)
+    if r.size and (r.min() < 0 or r.max() >= a.shape[0]):
+        raise ValueError("row index out of range")
+    e = np.ascontiguousarray(r_edges, dtype=np.float64)
+    nb = e.shape[0] - 1
+    L = lib()
+    call = lambda r0, r1, h, nr, mm: L.orc_count_rows_xyz(_ptr(a), _ptr(r), r0, r1, _ptr(b), b.shape[0],
+                                                          1 if exclude_self else 0, _ptr(e), nb, near_tol, _ptr(h), _ptr(nr))
+    return _run("rows_xyz", _even_spans(r.shape[0], threads), call, nb, near_tol >= 0, threads)

@@ -19,7 +19,9 @@
  *
  * Pins (tests/test_oracle_pins.py, run with -m "not gpu"): hand catalogs P1, totals P2,
  * numpy.histogram of arccos of a Gram matrix P3, great-circle ring closed form P4, integer
- * identities P5, uniform-sphere closed form P6, null test P7, Eq. 1 hand case P8, acos-vs-asin P9.
+ * identities P5, uniform-sphere closed form P6, null test P7, Eq. 1 hand case P8, acos-vs-asin P9;
+ * 3-D variant (orc_count_*_xyz): cubic-lattice multiplicities X1, totals X2, unit-cube distance
+ * distribution X3, unit vectors with chord edges reproduce the angular histogram X4.
  * Unpinned: absolute w(theta) values on the MICE catalogs / Fig. 1 (data not available).
  *
  * Build: gcc -O2 -ffp-contract=off -fPIC -shared tpcf_oracle.c -o libtpcf_oracle.so -lm
@@ -164,4 +166,58 @@ void orc_estimate(const uint64_t *dd, const uint64_t *dr, const uint64_t *rr, in
         double fdd = (double)dd[k] / ndd, fdr = (double)dr[k] / ndr, frr = (double)rr[k] / nrr;
         w[k] = (fdd - 2.0 * fdr + frr) / frr;
     }
+}
+
+/*
+ * ---- 3-D variant ("results are extendible to the 3-dimensional variant as well") ----
+ * The spatial two-point function xi(r) needs the same three histograms with the Euclidean separation
+ * r = |a - b| of Cartesian positions in place of the angle.  Definition written out: r in fp64 by
+ * sqrt(dx^2 + dy^2 + dz^2), bins [e_k, e_{k+1}) in r, last bin closed (A5), under = r < e_0,
+ * over = r > e_n.  near[k] counts the pairs with |r - e_k| <= near_tol (the checker's tolerance for
+ * pairs a different rounding order may put on the other side of an edge).
+ */
+static inline void one_pair_xyz(const double *a, const double *b, const double *e, int n, double near_tol,
+                                uint64_t *hist, uint64_t *near)
+{
+    double dx = a[0] - b[0], dy = a[1] - b[1], dz = a[2] - b[2];
+    double r = sqrt(dx * dx + dy * dy + dz * dz);
+    ++hist[bin_slot(r, e, n)];
+    if (near)
+        for (int k = 0; k <= n; ++k)
+            if (fabs(r - e[k]) <= near_tol) ++near[k];
+}
+
+int orc_count_auto_xyz(const double *xyz, size_t npts, size_t i_begin, size_t i_end, const double *edges, int nbins,
+                       double near_tol, uint64_t *hist, uint64_t *near)
+{
+    if (nbins < 1 || nbins + 1 > MAX_EDGES) return -1;
+    for (size_t i = i_begin; i < i_end && i < npts; ++i)
+        for (size_t j = i + 1; j < npts; ++j)
+            one_pair_xyz(xyz + 3 * i, xyz + 3 * j, edges, nbins, near_tol, hist, near);
+    return 0;
+}
+
+int orc_count_cross_xyz(const double *a, size_t na, size_t i_begin, size_t i_end, const double *b, size_t nb,
+                        const double *edges, int nbins, double near_tol, uint64_t *hist, uint64_t *near)
+{
+    if (nbins < 1 || nbins + 1 > MAX_EDGES) return -1;
+    for (size_t i = i_begin; i < i_end && i < na; ++i)
+        for (size_t j = 0; j < nb; ++j)
+            one_pair_xyz(a + 3 * i, b + 3 * j, edges, nbins, near_tol, hist, near);
+    return 0;
+}
+
+int orc_count_rows_xyz(const double *a, const int64_t *rows, size_t r_begin, size_t r_end, const double *b, size_t nb,
+                       int exclude_self, const double *edges, int nbins, double near_tol, uint64_t *hist,
+                       uint64_t *near)
+{
+    if (nbins < 1 || nbins + 1 > MAX_EDGES) return -1;
+    for (size_t r = r_begin; r < r_end; ++r) {
+        size_t i = (size_t)rows[r];
+        for (size_t j = 0; j < nb; ++j) {
+            if (exclude_self && j == i) continue;
+            one_pair_xyz(a + 3 * i, b + 3 * j, edges, nbins, near_tol, hist, near);
+        }
+    }
+    return 0;
 }

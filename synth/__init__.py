@@ -19,4 +19,8 @@ from .catalogs import (  # noqa: F401
     great_circle_ring,
     edges,
     config_edges,
+    uniform_box,
+    clustered_box,
+    cubic_lattice,
+    make_box_config,
 )

@@ -284,3 +284,35 @@ def subset_rows(n: int, k: int = 2000, seed: int = 12345) -> np.ndarray:
     k = min(k, n)
     order = np.argsort(SplitMix(seed, 7).u64(n), kind="stable")
     return np.sort(order[:k]).astype(np.int64)
+
+
+# ---- 3-D boxes for the xi(r) variant; positions only, no distances are formed here ---------------
+def uniform_box(n: int, side: float, rng: SplitMix) -> np.ndarray:
+    """n rows (x, y, z) uniform in the cube [0, side)^3."""
+    return (rng.uniform(3 * n) * side).reshape(n, 3)
+
+
+def clustered_box(n: int, side: float, n_clumps: int, sigma: float, rng: SplitMix) -> np.ndarray:
+    """n rows in [0, side)^3: Gaussian clumps of width sigma around n_clumps uniform centres, emitted clump-major;
+    points that fall outside the cube are reflected back in (a stand-in for a clustered 3-D galaxy mock)."""
+    centres = rng.uniform(3 * n_clumps).reshape(n_clumps, 3) * side
+    pick = np.sort(rng.integers(n, n_clumps))
+    x = centres[pick] + sigma * rng.normal(3 * n).reshape(n, 3)
+    x = np.abs(x)
+    x = np.where(x >= side, 2.0 * side - x, x)
+    return np.clip(x, 0.0, np.nextafter(side, 0.0))
+
+
+def cubic_lattice(m: int) -> np.ndarray:
+    """The m^3 points of the integer lattice {0..m-1}^3 (hand-checkable pair multiplicities)."""
+    g = np.arange(m, dtype=np.float64)
+    return np.stack(np.meshgrid(g, g, g, indexing="ij"), axis=-1).reshape(-1, 3)
+
+
+def make_box_config(n_d: int = 430_000, n_r: int = 430_000, side: float = 1000.0, nbins: int = 40,
+                    r_min: float = 1.0, r_max: float = 200.0, mode: str = "log", seed: int = 31):
+    """3-D stand-in at paper scale: D clustered (n_d / 400 clumps of width side / 200), R uniform, in a cube of `side`
+    (think Mpc/h); `nbins` bins in r from r_min to r_max.  Returns (D, R, r_edges)."""
+    D = clustered_box(n_d, side, max(1, n_d // 400), side / 200.0, SplitMix(seed, 0))
+    R = uniform_box(n_r, side, SplitMix(seed, 1))
+    return D, R, edges(nbins, r_min, r_max, mode)

@@ -271,6 +271,19 @@ def test_p9_acos_vs_asin_chord(idx):
     assert oracle.count_cross(d, r, e, validate=True).mismatch == 0
 
 
+def test_p9_mismatch_counter_does_count():
+    """Positive pin of the O8 counter: two points 1e-7 deg apart on the equator.  In fp64 the dot product is
+    1 - 1.5e-18 = 1.0, so acos gives theta = 0 (under the first edge) while 2 asin(chord / 2) gives 1e-7 deg
+    (inside the bin): the two formulas disagree on exactly this pair and agree on the 1-degree pair."""
+    x = xyz_of([[10.0, 0.0], [10.0 + 1e-7, 0.0], [11.0, 0.0]])
+    c = oracle.count_auto(x, np.array([5e-8, 2e-7, 0.5, 2.0]), validate=True)
+    assert c.mismatch == 1
+    assert (c.under, list(c.hist), c.over) == (1, [0, 0, 2], 0)          # the acos path, as the paper computes it
+    # far from theta = 0 the same construction does not trip it
+    y = xyz_of([[10.0, 0.0], [10.0 + 1e-3, 0.0], [11.0, 0.0]])
+    assert oracle.count_auto(y, np.array([5e-4, 2e-3, 0.5, 2.0]), validate=True).mismatch == 0
+
+
 def test_o6_near_edge_counters_match_numpy():
     D, R, e, _ = synth.make_config(1, n_d=600, n_r=400)
     d, r = oracle.radec_to_xyz(D), oracle.radec_to_xyz(R)
@@ -280,3 +293,86 @@ def test_o6_near_edge_counters_match_numpy():
     got = oracle.count_cross(d, r, e, validate=True).near
     assert np.abs(got.astype(np.int64) - want).sum() <= 2      # BLAS-vs-loop rounding at the 1e-6 boundary
     assert got.sum() > 0                                       # the small log bins do sit within 1e-6 in cos
+
+
+# ------------------------------------------------------------------ 3-D variant: orc_count_*_xyz
+def _lattice_multiplicities(m):
+    """Unordered pairs of the m^3 integer lattice by squared distance, from the offset-vector count
+    (m - |dx|)(m - |dy|)(m - |dz|) per ordered offset -- no point-by-point loop."""
+    out = {}
+    rng = range(-(m - 1), m)
+    for dx in rng:
+        for dy in rng:
+            for dz in rng:
+                if (dx, dy, dz) == (0, 0, 0):
+                    continue
+                d2 = dx * dx + dy * dy + dz * dz
+                out[d2] = out.get(d2, 0) + (m - abs(dx)) * (m - abs(dy)) * (m - abs(dz))
+    return {d2: c // 2 for d2, c in out.items()}
+
+
+def test_x1_cubic_lattice_multiplicities():
+    """X1: 2x2x2 cube: 12 edges, 12 face diagonals, 4 space diagonals; 3x3x3: 54, 72, 32, 27, 72, 48, 18, 24, 4 pairs
+    at r^2 = 1, 2, 3, 4, 5, 6, 8, 9, 12 (hand-derived, total 351)."""
+    assert _lattice_multiplicities(2) == {1: 12, 2: 12, 3: 4}
+    hand3 = {1: 54, 2: 72, 3: 32, 4: 27, 5: 72, 6: 48, 8: 18, 9: 24, 12: 4}
+    assert _lattice_multiplicities(3) == hand3 and sum(hand3.values()) == 27 * 26 // 2
+    for m, want in ((2, {1: 12, 2: 12, 3: 4}), (3, hand3)):
+        x = synth.cubic_lattice(m) * 2.5 + np.array([7.0, -3.0, 11.0])          # scaled and shifted: r = 2.5 sqrt(d2)
+        d2s = sorted(want)
+        # one bin per distinct distance, edges half way between consecutive distances
+        r = 2.5 * np.sqrt(np.array(d2s, dtype=np.float64))
+        e = np.concatenate([[0.5 * r[0]], 0.5 * (r[:-1] + r[1:]), [r[-1] + 1.0]])
+        c = oracle.count_auto_xyz(x, e)
+        assert list(c.hist) == [want[d] for d in d2s] and c.under == 0 and c.over == 0
+        # edges exactly ON the distances 2.5 and 5.0 (exact in fp64): lower-inclusive bins, closed last bin
+        c = oracle.count_auto_xyz(x, np.array([2.5, 5.0]))
+        assert c.hist[0] == sum(v for d, v in want.items() if 1 <= d <= 4) and c.under == 0
+        assert c.over == sum(v for d, v in want.items() if d > 4)
+
+
+def test_x2_totals_and_identities_xyz():
+    a = synth.clustered_box(700, 50.0, 9, 2.0, synth.SplitMix(5, 0))
+    b = synth.uniform_box(500, 50.0, synth.SplitMix(5, 1))
+    e = synth.edges(12, 0.5, 40.0, "log")
+    ca, cb, cx = oracle.count_auto_xyz(a, e), oracle.count_auto_xyz(b, e), oracle.count_cross_xyz(a, b, e)
+    assert ca.total == 700 * 699 // 2 and cb.total == 500 * 499 // 2 and cx.total == 700 * 500
+    cu = oracle.count_auto_xyz(np.concatenate([a, b]), e)                          # DD(A u B) = DD(A) + DD(B) + DR(A, B)
+    assert np.array_equal(cu.hist, ca.hist + cb.hist + cx.hist) and cu.under == ca.under + cb.under + cx.under
+    rows = synth.subset_rows(700, 700, 3)                                          # a permutation: subset mode sums to 2 DD
+    cr = oracle.count_rows_xyz(a, rows, a, True, e)
+    assert np.array_equal(cr.hist, 2 * ca.hist) and cr.total == 700 * 699
+    assert np.array_equal(oracle.count_auto_xyz(a[::-1].copy(), e).hist, ca.hist)   # order invariance
+    assert np.array_equal(oracle.count_cross_xyz(a, b, e, threads=3).hist, cx.hist)
+
+
+def test_x3_unit_cube_distance_distribution():
+    """X3: two uniform points in the unit cube: P(r <= t) = 4 pi t^3/3 - 3 pi t^4/2 + 8 t^5/5 - t^6/6 for t <= 1
+    (the classical cube line-picking law); counts within 5 sigma per bin."""
+    n = 3000
+    x = synth.uniform_box(n, 1.0, synth.SplitMix(77, 0))
+    e = np.linspace(0.0, 1.0, 11)
+    F = lambda t: 4 * np.pi * t ** 3 / 3 - 1.5 * np.pi * t ** 4 + 1.6 * t ** 5 - t ** 6 / 6
+    c = oracle.count_auto_xyz(x, e, threads=oracle.host_threads())
+    npairs = n * (n - 1) // 2
+    exp = npairs * (F(e[1:]) - F(e[:-1]))
+    assert np.all(np.abs(c.hist - exp) <= 5 * np.sqrt(exp) + 1)
+    assert abs(c.over - npairs * (1 - F(1.0))) <= 5 * np.sqrt(npairs * (1 - F(1.0)))
+    assert abs(F(1.0) - 0.90966) < 1e-4                                             # the law's own checksum
+
+
+def test_x4_unit_vectors_with_chord_edges_reproduce_angular_histogram():
+    """X4: fed unit vectors and r-edges 2 sin(theta_k / 2), the 3-D counter is the angular counter."""
+    D, R, e, _ = synth.make_config(2, n_d=900, n_r=700)
+    d, r = oracle.radec_to_xyz(D), oracle.radec_to_xyz(R)
+    re = 2.0 * np.sin(np.radians(e) / 2.0)
+    for ang, xyz in ((oracle.count_auto(d, e, validate=True), oracle.count_auto_xyz(d, re)),
+                     (oracle.count_cross(d, r, e, validate=True), oracle.count_cross_xyz(d, r, re))):
+        diff = np.abs(ang.hist.astype(np.int64) - xyz.hist.astype(np.int64))
+        assert ang.total == xyz.total and np.all(diff <= ang.tol()) and diff.sum() <= 2
+
+
+def test_x_near_counter_xyz():
+    x = np.array([[0.0, 0, 0], [3.0, 4.0, 0], [3.0, 4.0, 1e-7]])                   # r = 5, 5 + 1e-15, 1e-7
+    c = oracle.count_auto_xyz(x, np.array([1.0, 5.0, 9.0]), near_tol=1e-9)
+    assert list(c.near) == [0, 2, 0] and c.under == 1 and list(c.hist) == [0, 2]
