@@ -54,7 +54,8 @@ struct tpcf_ctx {
     // device side
     bool cuda_ready = false;
     int sm_count = 0;
-    float2* d_lut = nullptr;
+    float* d_lut = nullptr;
+    int lut_multi = 0;
     uint16_t* d_slotmap = nullptr;
     float2 *d_band_mh = nullptr, *d_band_lh = nullptr;
     uint16_t *d_band_slot = nullptr, *d_cell_band = nullptr;
@@ -133,18 +134,19 @@ tpcf_status upload_tables(tpcf_ctx* ctx) {
     cudaFree(ctx->d_band_lh);
     cudaFree(ctx->d_band_slot);
     cudaFree(ctx->d_cell_band);
-    ctx->d_lut = ctx->d_band_mh = ctx->d_band_lh = nullptr;
+    ctx->d_lut = nullptr;
+    ctx->d_band_mh = ctx->d_band_lh = nullptr;
     ctx->d_slotmap = ctx->d_band_slot = ctx->d_cell_band = nullptr;
-    std::vector<float2> lut(t.ncells);
     std::vector<uint16_t> sm(2 * (size_t)t.ncells);
+    ctx->lut_multi = 0;
     for (int c = 0; c < t.ncells; ++c) {
-        lut[c] = make_float2(t.lo[c], t.hi[c]);
-        sm[2 * c] = t.slot0[c];
-        sm[2 * c + 1] = t.slot1[c];
+        if (t.tcell[c] != t.tcell[c]) ctx->lut_multi = 1;
+        sm[c] = t.slot0[c];
+        sm[(size_t)t.ncells + c] = t.slot1[c];
     }
-    CU(cudaMalloc(&ctx->d_lut, lut.size() * sizeof(float2)), "cudaMalloc lut");
+    CU(cudaMalloc(&ctx->d_lut, t.tcell.size() * sizeof(float)), "cudaMalloc lut");
     CU(cudaMalloc(&ctx->d_slotmap, sm.size() * sizeof(uint16_t)), "cudaMalloc slotmap");
-    CU(cudaMemcpy(ctx->d_lut, lut.data(), lut.size() * sizeof(float2), cudaMemcpyHostToDevice), "upload lut");
+    CU(cudaMemcpy(ctx->d_lut, t.tcell.data(), t.tcell.size() * sizeof(float), cudaMemcpyHostToDevice), "upload lut");
     CU(cudaMemcpy(ctx->d_slotmap, sm.data(), sm.size() * sizeof(uint16_t), cudaMemcpyHostToDevice), "upload slotmap");
     std::vector<float2> mh(t.nbands), lh(t.nbands);
     for (int b = 0; b < t.nbands; ++b) {
@@ -339,6 +341,8 @@ tpcf_status enqueue_count(tpcf_ctx* ctx, tpcf_kind kind, const int64_t* rows_hos
     p.shift = ctx->ft.shift;
     p.sqrt_scale = ctx->ft.sqrt_scale;
     p.sqrt_clamp = ctx->ft.sqrt_clamp;
+    p.guard_scale = (float)ctx->guard_scale;
+    p.lut_multi = ctx->lut_multi;
     p.thr = ctx->d_thr;
     p.nbins = nb;
     p.result = ctx->d_result;

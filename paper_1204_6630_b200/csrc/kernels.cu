@@ -24,7 +24,7 @@ namespace {
 
 constexpr int R = kIPerThread;
 constexpr uint32_t kSqrtMagic = 0x1FBD1DF5u;
-constexpr unsigned long long kFlushPairs = 3500000000ull;   // flush 32-bit partial counters before they can wrap
+constexpr unsigned long long kFlushPairs = 2000000000ull;   // flush the 32-bit partial counters before they can reach 2^31 (those of the lookup path are signed)
 
 // ---- small PTX wrappers (mbarrier + bulk async copy, the TMA 1-D path) ---------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -142,62 +142,163 @@ __device__ __forceinline__ void rq_drain(uint2* rq, unsigned& qn, SlowCtx* slow)
     __syncwarp();
 }
 
-// ---- work items -----------------------------------------------------------------------------------------
-template <int MAP>
-__device__ __forceinline__ uint32_t cell_byte_offset(float d2, int shift, float scale, float clamp) {
+// ---- cell-lookup path ("lookup" path) ---------------------------------------------------------------------------
+// One pair: fp32 squared chord q (difference form) -> cell -> the one threshold T whose guard band reaches into the
+// cell (one LDS.32) -> side of T -> shared-memory partial histogram indexed by (side, cell); a pair with |q - T| <= g is
+// not counted here but re-evaluated in fp64.  g = alpha Q + beta_r r sqrt(Q) + beta_0 bounds the fp32 error of every pair
+// of the (lane, subtile) block: Q bounds its squared chords, r is the sum of its bounding radii.
+struct Lookup {
+    const char* lut;        // ncells x fp32 threshold (+inf: none; NaN: several, every pair of the cell is ambiguous)
+    char* hist;             // 2 x ncells x u32: [0, ncells) pairs below the cell's threshold, [ncells, 2 ncells) at or above it
+    uint32_t lut_s;         // lut as a shared-window address
+    uint32_t above_off;     // ncells * 4
+    int shift;
+    float scale, clamp;
+    float alpha, beta_r, beta0;
+    int multi;              // some cell holds a NaN: the lazy detection of ambiguous pairs (a minimum) cannot be used
+};
+
+__device__ __forceinline__ Lookup make_lookup(const PairParams& p, unsigned char* lut, unsigned char* hist) {
+    Lookup lk;
+    lk.lut = reinterpret_cast<const char*>(lut);
+    lk.hist = reinterpret_cast<char*>(hist);
+    lk.lut_s = smem_u32(lut);
+    lk.above_off = (uint32_t)p.ncells * 4u;
+    lk.shift = p.shift;
+    lk.scale = p.sqrt_scale;
+    lk.clamp = p.sqrt_clamp;
+    lk.alpha = kLookupAlpha * p.guard_scale;
+    lk.beta_r = kLookupBetaR * p.guard_scale;
+    lk.beta0 = kLookupBeta0 * p.guard_scale;
+    lk.multi = p.lut_multi;
+    return lk;
+}
+
+// byte offset 4 * cell of the lookup cell of q; exactly FastTables::cell_of (tables.cpp)
+template <int MAP, bool CLAMP>
+__device__ __forceinline__ uint32_t cell_off4(float q, const Lookup& lk) {
     if (MAP == (int)CellMap::LogBits) {
-        return (__float_as_uint(d2) >> (shift - 3)) & ~7u;
+        return (__float_as_uint(q) >> (lk.shift - 2)) & ~3u;
     } else {
-        const float c = fminf(d2, clamp);
+        const float c = CLAMP ? fminf(q, lk.clamp) : q;
         const float key = __uint_as_float((__float_as_uint(c) >> 1) + kSqrtMagic);
-        const float t = fmaf(key, scale, 8388608.0f);
-        return (__float_as_uint(t) << 3) & 0x3FFFFF8u;
+        const float t = fmaf(key, lk.scale, 8388608.0f);
+        return __float_as_uint(t) & 0x7FFFFCu;
     }
 }
 
-// ---- coordinates ------------------------------------------------------------------------------------------------
-// Inside a (lane, subtile) block both points are taken relative to the subtile centre cs:
-//   s  = a' + (cq - cs)      the lane's i-point (a' = offset from its quad centre cq), formed per subtile in fp32
-//   b' = offset of the j-point from cs, stored as (-2 b', |b'|^2)
-// so |a - b|^2 = |s - b'|^2 = |s|^2 + |b'|^2 - 2 s.b'.  Every rounding is relative to |s| ~ chord or to the radii:
-// nothing is lost against the unit length of the vectors, which is what lets fp32 resolve the 0.01-degree bins.
+__device__ __forceinline__ float lookup_guard(const Lookup& lk, float rs, float hi) {
+    const float hi2 = __fmul_ru(hi, hi);
+    return fmaf(lk.alpha, hi2, fmaf(lk.beta_r * rs, hi * 1.0001f, lk.beta0));
+}
 
-// ---- per-pair cell-lookup path ("lookup" path) ---------------------------------------------------------------
-// One pair: fp32 squared chord (difference form) -> cell -> (lo, hi) of the cell's guard band -> shared-memory
-// partial histogram, or the fp64 recheck when lo <= d2 < hi.
-// Returns true when the pair is valid and fell inside a guard band (the caller then rechecks it in fp64); every other
-// valid pair is counted here.  No call and no branch in here, so the pairs of one j-row overlap in the pipes.
+// s - b' and its square, two i-rows at a time; b holds (-2 b', .) broadcast to both halves.  Only explicitly rounded
+// operations: the rescan of a j-row (lookup_rescan) must reproduce these values bit for bit.
+__device__ __forceinline__ f32x2 chord2_diff2(f32x2 sx, f32x2 sy, f32x2 sz, f32x2 bx, f32x2 by, f32x2 bz) {
+    const f32x2 half2 = pack2(0.5f, 0.5f);
+    const f32x2 dx = fma2(bx, half2, sx), dy = fma2(by, half2, sy), dz = fma2(bz, half2, sz);
+    return fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));
+}
+
+// generic form, one pair at a time (diagonal chunks, recounts of flagged lanes and rows, tables with NaN cells).
+// Returns true when the pair is valid and ambiguous (the caller then rechecks it in fp64); every other valid pair is
+// counted here.
 template <int MAP>
-__device__ __forceinline__ bool lookup_pair(float sx, float sy, float sz, const float4& b, const char* lut, char* hist,
-                                            bool valid, int shift, float scale, float clamp) {
+__device__ __forceinline__ bool lookup_pair(float sx, float sy, float sz, const float4& b, const Lookup& lk, float g, bool valid) {
     const float dx = fmaf(b.x, 0.5f, sx), dy = fmaf(b.y, 0.5f, sy), dz = fmaf(b.z, 0.5f, sz);     // s - b', one rounding each
-    const float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-    const uint32_t q8 = cell_byte_offset<MAP>(d2, shift, scale, clamp);
-    const float2 lh = *reinterpret_cast<const float2*>(lut + q8);
-    const bool above = d2 >= lh.x;
-    const bool amb = above && (d2 < lh.y);
-    if (valid && !amb) atomicAdd(reinterpret_cast<unsigned*>(hist + q8) + (above ? 1 : 0), 1u);
+    const float q = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+    const uint32_t off = cell_off4<MAP, true>(q, lk);
+    const float e = __fsub_rn(q, *reinterpret_cast<const float*>(lk.lut + off));
+    const bool amb = !(fabsf(e) > g);
+    if (valid && !amb) atomicAdd(reinterpret_cast<unsigned*>(lk.hist + off + (e < 0.f ? 0u : lk.above_off)), 1u);
     return valid && amb;
 }
 
-// One subtile against this lane's R points, every pair by cell lookup.  MASK: only pairs j > i (diagonal chunk).
-// Called by the whole warp; lanes with active == false count nothing.
+// fast form: count the pair on the side of T its fp32 value shows (one shared atomic, no branch); returns |q - T|.
+// A pair with |q - T| <= g is taken out again by lookup_rescan, which sees the same bits.
+__device__ __forceinline__ float lds_f32(uint32_t addr) {
+    float v;
+    asm("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr));
+    return v;
+}
+template <int MAP, bool CLAMP>
+__device__ __forceinline__ float lookup_count(float q, const Lookup& lk) {
+    const uint32_t off = cell_off4<MAP, CLAMP>(q, lk);
+    const float e = __fsub_rn(q, lds_f32(lk.lut_s + off));
+    atomicAdd(reinterpret_cast<unsigned*>(lk.hist + off + (e < 0.f ? 0u : lk.above_off)), 1u);
+    return fabsf(e);
+}
+
+// One subtile against this lane's R rows, every pair by cell lookup, generic form.  MASK: only pairs j > i (diagonal
+// chunk).  Called by the whole warp; lanes with active == false count nothing.
 template <int MAP, bool MASK>
 __device__ __forceinline__ void lookup_block(const float4* __restrict__ js, const float (&sx)[R], const float (&sy)[R],
-                                             const float (&sz)[R], bool active, const char* lut, char* hist, SlowCtx* slow,
-                                             uint2* rq, unsigned& qn, uint32_t i0, uint32_t j0, int shift, float scale,
-                                             float clamp) {
+                                             const float (&sz)[R], bool active, const Lookup& lk, float g, SlowCtx* slow,
+                                             uint2* rq, unsigned& qn, uint32_t i0, uint32_t j0) {
 #pragma unroll 2
     for (int jj = 0; jj < kSubJ; ++jj) {
         const float4 b = js[jj];                                  // one LDS.128, broadcast to the warp
         unsigned amb = 0;
 #pragma unroll
         for (int r = 0; r < R; ++r)
-            amb |= (lookup_pair<MAP>(sx[r], sy[r], sz[r], b, lut, hist, active && (!MASK || (j0 + jj > i0 + r)), shift, scale, clamp) ? 1u : 0u) << r;
-        if (__any_sync(0xffffffffu, amb != 0)) {                  // rare: pairs inside a guard band
-#pragma unroll 1
-            for (int r = 0; r < R; ++r) rq_push(rq, qn, (amb >> r) & 1u, i0 + r, j0 + jj, slow);
+            amb |= (lookup_pair<MAP>(sx[r], sy[r], sz[r], b, lk, g, active && (!MASK || (j0 + jj > i0 + r))) ? 1u : 0u) << r;
+        while (__any_sync(0xffffffffu, amb != 0)) {               // rare: pairs inside a guard band
+            const int r = __ffs(amb) - 1;
+            rq_push(rq, qn, amb != 0, i0 + r, j0 + jj, slow);
+            amb &= amb - 1;
         }
+    }
+}
+
+// The ambiguous pairs (|q - T| <= g) of one j-row, which lookup_block_fast counted like every other pair: found again
+// (same operations, same bits), taken out of the partial histogram and queued for the fp64 recheck.  The partial
+// counters of the lookup path are therefore signed 32-bit values (flush_slots), and a counter may be read as -1 for a
+// moment when a flush falls between the two atomics.
+template <int MAP, bool CLAMP>
+__device__ __noinline__ void lookup_rescan(const float4 b, const f32x2 (&sx2)[R / 2], const f32x2 (&sy2)[R / 2], const f32x2 (&sz2)[R / 2],
+                                           const Lookup& lk, float g, SlowCtx* slow, uint2* rq, unsigned& qn, uint32_t i0, uint32_t j) {
+    const f32x2 bx = pack2(b.x, b.x), by = pack2(b.y, b.y), bz = pack2(b.z, b.z);
+    unsigned amb = 0;
+#pragma unroll
+    for (int r = 0; r < R / 2; ++r) {
+        float q[2];
+        unpack2(chord2_diff2(sx2[r], sy2[r], sz2[r], bx, by, bz), q[0], q[1]);
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const uint32_t off = cell_off4<MAP, CLAMP>(q[h], lk);
+            const float e = __fsub_rn(q[h], lds_f32(lk.lut_s + off));
+            if (fabsf(e) <= g) {
+                atomicSub(reinterpret_cast<unsigned*>(lk.hist + off + (e < 0.f ? 0u : lk.above_off)), 1u);
+                amb |= 1u << (2 * r + h);
+            }
+        }
+    }
+    while (__any_sync(0xffffffffu, amb != 0)) {
+        const int r = __ffs(amb) - 1;
+        rq_push(rq, qn, amb != 0, i0 + r, j, slow);
+        amb &= amb - 1;
+    }
+}
+
+// One subtile against this lane's R rows, every pair by cell lookup, fast form (every lane active, no mask, no NaN
+// cells): per pair 3 packed FMA-pipe instructions for two squared chords, the cell offset, one LDS.32, one subtraction,
+// the side select and one shared atomic; ambiguous pairs are detected per j-row from the smallest |q - T|.
+template <int MAP, bool CLAMP>
+__device__ __forceinline__ void lookup_block_fast(const float4* __restrict__ js, const f32x2 (&sx2)[R / 2], const f32x2 (&sy2)[R / 2],
+                                                  const f32x2 (&sz2)[R / 2], const Lookup& lk, float g, SlowCtx* slow, uint2* rq,
+                                                  unsigned& qn, uint32_t i0, uint32_t j0) {
+#pragma unroll 2
+    for (int jj = 0; jj < kSubJ; ++jj) {
+        const float4 b = js[jj];
+        const f32x2 bx = pack2(b.x, b.x), by = pack2(b.y, b.y), bz = pack2(b.z, b.z);
+        float m = 3.0e38f;
+#pragma unroll
+        for (int r = 0; r < R / 2; ++r) {
+            float q0, q1;
+            unpack2(chord2_diff2(sx2[r], sy2[r], sz2[r], bx, by, bz), q0, q1);
+            m = fminf(m, fminf(lookup_count<MAP, CLAMP>(q0, lk), lookup_count<MAP, CLAMP>(q1, lk)));
+        }
+        if (__any_sync(0xffffffffu, m <= g)) lookup_rescan<MAP, CLAMP>(b, sx2, sy2, sz2, lk, g, slow, rq, qn, i0, j0 + jj);
     }
 }
 
@@ -284,10 +385,9 @@ struct WinTables {
 template <int MAP>
 __device__ __forceinline__ void subtile_pairs(const float4* __restrict__ js, const float4 sp, bool windows, bool mask,
                                               const f32x2 (&px2)[R / 2], const f32x2 (&py2)[R / 2], const f32x2 (&pz2)[R / 2], float cqx,
-                                              float cqy, float cqz, float ri, const WinTables& wt, const char* lut,
-                                              char* hist, SlowCtx* slow, uint2* rq, unsigned& qn, uint32_t i0, uint32_t n_i,
-                                              uint32_t j0, uint32_t n_j, int shift, float scale, float clamp,
-                                              unsigned (&npath)[6]) {
+                                              float cqy, float cqz, float ri, const WinTables& wt, const Lookup& lk,
+                                              SlowCtx* slow, uint2* rq, unsigned& qn, uint32_t i0, uint32_t n_i,
+                                              uint32_t j0, uint32_t n_j, unsigned (&npath)[6]) {
     const int lane = threadIdx.x & 31;
     // bounds on every TRUE chord of the block from the triangle inequality: |cq - cs| -/+ (ri + rj), made safe
     // against the fp32 evaluation (relative 4e-6 on the centre distance, 1e-7 absolute)
@@ -298,13 +398,14 @@ __device__ __forceinline__ void subtile_pairs(const float4* __restrict__ js, con
     const float rs = ri + sp.w;
     const float lo = fmaf(dc, 1.0f - 4.0e-6f, -rs) - 1.0e-7f;
     const float hi = fmaf(dc, 1.0f + 4.0e-6f, rs) + 1.0e-7f;
+    const float g = lookup_guard(lk, rs, hi);       // guard of the cell-lookup path for this block
     int mode = 4, k = 0;
     if (rs > kRCap) {
         mode = 5;
     } else if (windows && !mask && lo >= kFarKappa * rs) {
         const float lo2 = __fmul_rd(lo, lo), hi2 = __fmul_ru(hi, hi);
         // first band that is not wholly below the window, then how many bands the window reaches
-        k = wt.cell_band[cell_byte_offset<MAP>(lo2, shift, scale, clamp) >> 3];
+        k = wt.cell_band[cell_off4<MAP, true>(lo2, lk) >> 2];
         while (k < wt.nbands && wt.band_lh[k].y <= lo2) ++k;
         int e = 1;
         while (e <= kMaxWinEdges && k + e < wt.nbands && wt.band_lh[k + e].x <= hi2) ++e;
@@ -332,15 +433,25 @@ __device__ __forceinline__ void subtile_pairs(const float4* __restrict__ js, con
         }
     }
     if (wmode > kMaxWinEdges) {
-        const bool act = mode != 5;                 // lanes with mode 5 are counted below, by the whole warp, in fp64
+        // lanes with mode 5 are counted below, by the whole warp, in fp64; a quad wholly past the end of the catalog and a
+        // subtile of padding rows only (lo > 2.2: no chord between unit vectors exceeds 2) hold no pair at all
+        const bool act = mode != 5 && i0 < n_i && lo <= 2.2f;
         if (!act) {
+            const f32x2 z2 = pack2(0.f, 0.f);
 #pragma unroll
-            for (int r = 0; r < R; ++r) sx[r] = sy[r] = sz[r] = 0.f;      // keeps their (unused) cells inside the table
+            for (int r = 0; r < R / 2; ++r) sx2[r] = sy2[r] = sz2[r] = z2;      // keeps their (unused) cells inside the table
+#pragma unroll
+            for (int r = 0; r < R; ++r) sx[r] = sy[r] = sz[r] = 0.f;
         }
-        if (mask)
-            lookup_block<MAP, true>(js, sx, sy, sz, act, lut, hist, slow, rq, qn, i0, j0, shift, scale, clamp);
-        else
-            lookup_block<MAP, false>(js, sx, sy, sz, act, lut, hist, slow, rq, qn, i0, j0, shift, scale, clamp);
+        if (mask) {
+            lookup_block<MAP, true>(js, sx, sy, sz, act, lk, g, slow, rq, qn, i0, j0);
+        } else if (lk.multi || !__all_sync(0xffffffffu, act)) {
+            lookup_block<MAP, false>(js, sx, sy, sz, act, lk, g, slow, rq, qn, i0, j0);
+        } else if (MAP == (int)CellMap::SqrtLin && __any_sync(0xffffffffu, __fmul_ru(hi, hi) > lk.clamp)) {
+            lookup_block_fast<MAP, true>(js, sx2, sy2, sz2, lk, g, slow, rq, qn, i0, j0);
+        } else {
+            lookup_block_fast<MAP, false>(js, sx2, sy2, sz2, lk, g, slow, rq, qn, i0, j0);
+        }
         if (wmode == 5) exact_lanes(slow, __ballot_sync(0xffffffffu, mode == 5), i0 - lane * R, n_i, j0, n_j, mask);
         ++npath[wmode == 5 ? 5 : 3];
         return;
@@ -401,14 +512,14 @@ __device__ __forceinline__ void subtile_pairs(const float4* __restrict__ js, con
         const int src = __ffs(todo) - 1;
         todo &= todo - 1;
         const uint32_t isrc = i0 + (uint32_t)(src - lane) * R;
+        const float gsrc = __shfl_sync(0xffffffffu, g, src);
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const float ux = __shfl_sync(0xffffffffu, sx[r], src), uy = __shfl_sync(0xffffffffu, sy[r], src),
                         uz = __shfl_sync(0xffffffffu, sz[r], src);
 #pragma unroll
             for (int h = 0; h < kSubJ / 32; ++h)
-                rq_push(rq, qn, lookup_pair<MAP>(ux, uy, uz, js[h * 32 + lane], lut, hist, true, shift, scale, clamp), isrc + r,
-                        j0 + h * 32 + lane, slow);
+                rq_push(rq, qn, lookup_pair<MAP>(ux, uy, uz, js[h * 32 + lane], lk, gsrc, true), isrc + r, j0 + h * 32 + lane, slow);
         }
         ++npath[4];
     }
@@ -439,7 +550,7 @@ __host__ __device__ inline FastSmem fast_smem_layout(int ncells, int nbands, int
     FastSmem L;
     uint32_t o = 0;
     L.ring = o;       o += kWarpsPerCta * NRING * kSlotBytes;
-    L.lut = o;        o = up16(o + (uint32_t)ncells * 8);
+    L.lut = o;        o = up16(o + (uint32_t)ncells * 4);
     L.hist = o;       o = up16(o + (uint32_t)ncells * 8);
     L.band_mh = o;    o = up16(o + (uint32_t)nbands * 8);
     L.band_lh = o;    o = up16(o + (uint32_t)nbands * 8);
@@ -472,9 +583,9 @@ __device__ __forceinline__ uint32_t tri_row_of(const uint32_t* __restrict__ row_
 __device__ __forceinline__ void flush_slots(unsigned* hist, int nslots, const uint16_t* __restrict__ slotmap, unsigned* whist,
                                             int nres, unsigned long long* result, unsigned* nrecheck,
                                             unsigned long long* rechecked, int first, int stride) {
-    for (int s = first; s < nslots; s += stride) {
-        const unsigned v = hist[s] ? atomicExch(hist + s, 0u) : 0u;
-        if (v) atomicAdd(result + slotmap[s], (unsigned long long)v);
+    for (int s = first; s < nslots; s += stride) {       // signed: lookup_rescan takes ambiguous pairs out again
+        const int v = hist[s] ? (int)atomicExch(hist + s, 0u) : 0;
+        if (v) atomicAdd(result + slotmap[s], (unsigned long long)(long long)v);
     }
     for (int s = first; s < nres; s += stride) {
         const unsigned v = whist[s] ? atomicExch(whist + s, 0u) : 0u;
@@ -493,8 +604,8 @@ template <int MAP>
 __global__ void __launch_bounds__(kThreads, 2) pair_fast_kernel(const __grid_constant__ PairParams p) {
     extern __shared__ __align__(128) unsigned char smem[];
     const FastSmem L = fast_smem_layout(p.ncells, p.nbands, p.nbins);
-    char* lut = reinterpret_cast<char*>(smem + L.lut);
     unsigned* hist = reinterpret_cast<unsigned*>(smem + L.hist);
+    const Lookup lk = make_lookup(p, smem + L.lut, smem + L.hist);
     SlowCtx* slow = reinterpret_cast<SlowCtx*>(smem + L.slow);
     WinTables wt;
     wt.band_mh = reinterpret_cast<const float2*>(smem + L.band_mh);
@@ -508,9 +619,9 @@ __global__ void __launch_bounds__(kThreads, 2) pair_fast_kernel(const __grid_con
     unsigned char* ring = smem + L.ring + (size_t)warp * NRING * kSlotBytes;
     const uint32_t bar0 = smem_u32(smem + L.bars + (size_t)warp * NRING * 8);
     for (int c = tid; c < p.ncells; c += kThreads) {
-        reinterpret_cast<float2*>(lut)[c] = p.lut[c];
-        hist[2 * c] = 0;
-        hist[2 * c + 1] = 0;
+        reinterpret_cast<float*>(smem + L.lut)[c] = p.lut[c];
+        hist[c] = 0;
+        hist[p.ncells + c] = 0;
         reinterpret_cast<uint16_t*>(smem + L.cell_band)[c] = p.cell_band[c];
     }
     for (int b = tid; b < p.nbands; b += kThreads) {
@@ -602,9 +713,8 @@ __global__ void __launch_bounds__(kThreads, 2) pair_fast_kernel(const __grid_con
             const bool mask = p.tri && ch < dch_end;        // a chunk of the warp's own rows: pairs j > i only
 #pragma unroll 1
             for (int sub = 0; sub < kSubPerChunk; ++sub)
-                subtile_pairs<MAP>(jt + sub * kSubJ, jsph[sub], p.window != 0, mask, px2, py2, pz2, q4.x, q4.y, q4.z, q4.w, wt, lut,
-                                   reinterpret_cast<char*>(hist), slow, rq, qn, i0, p.n_i, ch * kChunkJ + sub * kSubJ, p.n_j, p.shift,
-                                   p.sqrt_scale, p.sqrt_clamp, npath);
+                subtile_pairs<MAP>(jt + sub * kSubJ, jsph[sub], p.window != 0, mask, px2, py2, pz2, q4.x, q4.y, q4.z, q4.w, wt, lk,
+                                   slow, rq, qn, i0, p.n_i, ch * kChunkJ + sub * kSubJ, p.n_j, npath);
             __syncwarp();
             pairs_since_flush += (unsigned long long)kWarpI * kChunkJ;
         }
@@ -661,8 +771,8 @@ __device__ __forceinline__ uint64_t umma_desc(uint32_t saddr, uint32_t lbo, uint
 
 // window of one (quad, subtile) block: mode 1..3 = edges of the window loop, 4 = cell lookup, 5 = fp64; k = first band
 template <int MAP>
-__device__ __forceinline__ void window_of(const float4 cq, const float4 sp, bool windows, const WinTables& wt, int shift, float scale,
-                                          float clamp, int& mode, int& k) {
+__device__ __forceinline__ void window_of(const float4 cq, const float4 sp, bool windows, const WinTables& wt, const Lookup& lk, int& mode,
+                                          int& k, float& g) {
     const float tx = __fsub_rn(cq.x, sp.x), ty = __fsub_rn(cq.y, sp.y), tz = __fsub_rn(cq.z, sp.z);
     const float dc2 = fmaf(tz, tz, fmaf(ty, ty, tx * tx));
     float dc;
@@ -670,13 +780,14 @@ __device__ __forceinline__ void window_of(const float4 cq, const float4 sp, bool
     const float rs = cq.w + sp.w;
     const float lo = fmaf(dc, 1.0f - 4.0e-6f, -rs) - 1.0e-7f;
     const float hi = fmaf(dc, 1.0f + 4.0e-6f, rs) + 1.0e-7f;
+    g = lookup_guard(lk, rs, hi);
     mode = 4;
     k = 0;
     if (rs > kRCap) {
         mode = 5;
     } else if (windows && lo >= kFarKappa * rs) {
         const float lo2 = __fmul_rd(lo, lo), hi2 = __fmul_ru(hi, hi);
-        k = wt.cell_band[cell_byte_offset<MAP>(lo2, shift, scale, clamp) >> 3];
+        k = wt.cell_band[cell_off4<MAP, true>(lo2, lk) >> 2];
         while (k < wt.nbands && wt.band_lh[k].y <= lo2) ++k;
         int e = 1;
         while (e <= kMaxWinEdges && k + e < wt.nbands && wt.band_lh[k + e].x <= hi2) ++e;
@@ -692,7 +803,7 @@ __host__ __device__ inline TcSmem tc_smem_layout(int ncells, int nbands, int nbi
     uint32_t o = 0;
     L.ring = o;       o += kTcRing * ((kTcSlotBytes + 127u) & ~127u);
     L.abuf = o;       o += kTcABytes;
-    L.lut = o;        o = up16(o + (uint32_t)ncells * 8);
+    L.lut = o;        o = up16(o + (uint32_t)ncells * 4);
     L.hist = o;       o = up16(o + (uint32_t)ncells * 8);
     L.band_mh = o;    o = up16(o + (uint32_t)nbands * 8);
     L.band_lh = o;    o = up16(o + (uint32_t)nbands * 8);
@@ -711,19 +822,20 @@ __host__ __device__ inline TcSmem tc_smem_layout(int ncells, int nbands, int nbi
 // rows of `todo` (one bit per lane = i-row) against the kTcSubJ j-rows at xs: every pair through the cell lookup, the warp
 // working together on one row at a time (lane l takes j-rows l, l + 32, ..)
 template <int MAP>
-__device__ __forceinline__ void tc_lookup_rows(unsigned todo, float sx, float sy, float sz, const float4* __restrict__ xs, const char* lut,
-                                               char* hist, SlowCtx* slow, uint2* rq, unsigned& qn, uint32_t iwarp, uint32_t j0, bool mask,
-                                               int shift, float scale, float clamp) {
+__device__ __forceinline__ void tc_lookup_rows(unsigned todo, float sx, float sy, float sz, float g, const float4* __restrict__ xs,
+                                               const Lookup& lk, SlowCtx* slow, uint2* rq, unsigned& qn, uint32_t iwarp, uint32_t j0,
+                                               bool mask) {
     const int lane = threadIdx.x & 31;
     while (todo) {
         const int src = __ffs(todo) - 1;
         todo &= todo - 1;
         const uint32_t i = iwarp + src;
         const float ux = __shfl_sync(0xffffffffu, sx, src), uy = __shfl_sync(0xffffffffu, sy, src), uz = __shfl_sync(0xffffffffu, sz, src);
+        const float gs = __shfl_sync(0xffffffffu, g, src);
 #pragma unroll
         for (int h = 0; h < kTcSubJ / 32; ++h) {
             const uint32_t j = j0 + h * 32 + lane;
-            rq_push(rq, qn, lookup_pair<MAP>(ux, uy, uz, xs[h * 32 + lane], lut, hist, !mask || j > i, shift, scale, clamp), i, j, slow);
+            rq_push(rq, qn, lookup_pair<MAP>(ux, uy, uz, xs[h * 32 + lane], lk, gs, !mask || j > i), i, j, slow);
         }
     }
 }
@@ -756,15 +868,15 @@ __device__ __noinline__ void tc_exact_rows(SlowCtx* s, unsigned todo, uint32_t i
 struct TcRow {
     float sx, sy, sz;           // the row relative to the tile centre (for the lookup recount)
     float dt1, dt2, hmax;       // mid_0 - mid_e of the further edges, largest band half width
+    float g;                    // guard of the cell-lookup path for this row's block
     int mode, k, we;            // this row's mode, first band, edges the warp runs
 };
 
 // Bin the kTcSubJ accumulators of this thread's row and count or recount the row.
 template <int MAP>
 __device__ __forceinline__ void tc_bin(const TcRow& pd, uint32_t taddr, const float4* __restrict__ xs, uint32_t j0, bool mask,
-                                       const WinTables& wt, const char* lut, char* hist, SlowCtx* slow, uint2* rq, unsigned& qn,
-                                       uint32_t iwarp, uint32_t n_i, uint32_t n_j, int shift, float scale, float clamp,
-                                       unsigned (&npath)[6]) {
+                                       const WinTables& wt, const Lookup& lk, SlowCtx* slow, uint2* rq, unsigned& qn,
+                                       uint32_t iwarp, uint32_t n_i, uint32_t n_j, unsigned (&npath)[6]) {
     const bool win = pd.mode <= kMaxWinEdges;
     bool flagged = false;
     if (pd.we <= kMaxWinEdges) {                    // warp-uniform
@@ -825,11 +937,11 @@ __device__ __forceinline__ void tc_bin(const TcRow& pd, uint32_t taddr, const fl
     } else {
         ++npath[3];
     }
-    const unsigned lk = __ballot_sync(0xffffffffu, (win && flagged) || pd.mode == 4);
+    const unsigned lkrows = __ballot_sync(0xffffffffu, (win && flagged) || pd.mode == 4);
     const unsigned ex = __ballot_sync(0xffffffffu, pd.mode == 5);
-    if (lk) {
-        tc_lookup_rows<MAP>(lk, pd.sx, pd.sy, pd.sz, xs, lut, hist, slow, rq, qn, iwarp, j0, mask, shift, scale, clamp);
-        npath[4] += __popc(lk);
+    if (lkrows) {
+        tc_lookup_rows<MAP>(lkrows, pd.sx, pd.sy, pd.sz, pd.g, xs, lk, slow, rq, qn, iwarp, j0, mask);
+        npath[4] += __popc(lkrows);
     }
     if (ex) {
         tc_exact_rows(slow, ex, iwarp, n_i, j0, n_j, mask);
@@ -841,8 +953,8 @@ template <int MAP>
 __global__ void __launch_bounds__(kTcThreads, 4) pair_tensor_kernel(const __grid_constant__ PairParams p) {
     extern __shared__ __align__(128) unsigned char smem[];
     const TcSmem L = tc_smem_layout(p.ncells, p.nbands, p.nbins);
-    char* lut = reinterpret_cast<char*>(smem + L.lut);
     unsigned* hist = reinterpret_cast<unsigned*>(smem + L.hist);
+    const Lookup lk = make_lookup(p, smem + L.lut, smem + L.hist);
     SlowCtx* slow = reinterpret_cast<SlowCtx*>(smem + L.slow);
     WinTables wt;
     wt.band_mh = reinterpret_cast<const float2*>(smem + L.band_mh);
@@ -858,9 +970,9 @@ __global__ void __launch_bounds__(kTcThreads, 4) pair_tensor_kernel(const __grid
     unsigned char* ring = smem + L.ring;
     const uint32_t ring_bar = smem_u32(smem + L.bars), full_bar = ring_bar + 8 * kTcRing;      // kTcRing slot barriers, "accumulators ready"
     for (int c = tid; c < p.ncells; c += kTcThreads) {
-        reinterpret_cast<float2*>(lut)[c] = p.lut[c];
-        hist[2 * c] = 0;
-        hist[2 * c + 1] = 0;
+        reinterpret_cast<float*>(smem + L.lut)[c] = p.lut[c];
+        hist[c] = 0;
+        hist[p.ncells + c] = 0;
         reinterpret_cast<uint16_t*>(smem + L.cell_band)[c] = p.cell_band[c];
     }
     for (int b = tid; b < p.nbands; b += kTcThreads) {
@@ -952,6 +1064,7 @@ __global__ void __launch_bounds__(kTcThreads, 4) pair_tensor_kernel(const __grid
             for (uint32_t n = 0; n < min(ntile, (uint32_t)kTcRing); ++n) fetch_tile(gch + n, ch + n);
 
         int bmode = 4, bk = 0;              // window of (this thread's quad, tile (lane & 7) of the current batch of 8)
+        float bg = 0.f;
         for (uint32_t t = 0; t < ntile; ++t) {
             const uint32_t n = gch + t, tabs = ch + t;
             unsigned char* slot = ring + (size_t)(n % kTcRing) * kSlotStride;
@@ -959,12 +1072,13 @@ __global__ void __launch_bounds__(kTcThreads, 4) pair_tensor_kernel(const __grid
             const bool mask = p.tri && tabs == dch;
             if (t == 0 || (tabs & 7u) == 0) {               // windows of 8 tiles at a time, one per lane of the quad
                 const uint32_t su = (tabs & ~7u) + (lane & 7);
-                window_of<MAP>(cq, p.ct[su], p.window != 0, wt, p.shift, p.sqrt_scale, p.sqrt_clamp, bmode, bk);
+                window_of<MAP>(cq, p.ct[su], p.window != 0, wt, lk, bmode, bk, bg);
             }
             const int owner = (lane & ~7) | (int)(tabs & 7u);
             TcRow rw;
             rw.mode = __shfl_sync(0xffffffffu, bmode, owner);
             rw.k = __shfl_sync(0xffffffffu, bk, owner);
+            rw.g = __shfl_sync(0xffffffffu, bg, owner);
             if (mask && rw.mode <= kMaxWinEdges) rw.mode = 4;
             const int wmax = __reduce_max_sync(0xffffffffu, rw.mode <= kMaxWinEdges ? rw.mode : 0);
             rw.we = wmax ? wmax : kMaxWinEdges + 1;
@@ -1016,8 +1130,8 @@ __global__ void __launch_bounds__(kTcThreads, 4) pair_tensor_kernel(const __grid
             }
             mbar_wait(full_bar, gs & 1);
             asm volatile("tcgen05.fence::after_thread_sync;");
-            tc_bin<MAP>(rw, tlane, reinterpret_cast<const float4*>(slot + kTcBBytes), tabs * kTcSubJ, mask, wt, lut, reinterpret_cast<char*>(hist),
-                        slow, rq, qn, ibase + warp * 32, p.n_i, p.n_j, p.shift, p.sqrt_scale, p.sqrt_clamp, npath);
+            tc_bin<MAP>(rw, tlane, reinterpret_cast<const float4*>(slot + kTcBBytes), tabs * kTcSubJ, mask, wt, lk, slow, rq, qn,
+                        ibase + warp * 32, p.n_i, p.n_j, npath);
             ++gs;
         }
         const uint32_t nchunks = ntile;

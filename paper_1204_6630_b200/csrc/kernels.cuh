@@ -34,10 +34,12 @@ struct PairParams {
     uint32_t jsplit;            // fast engine: a warp item covers 1/jsplit of its item's (single) j-tile; 1, 2, 4, 8 or 16,
                                 // > 1 only when chunk == 1 (small catalogs: more, shorter warp items for the tail)
     // fast engine tables
-    const float2* lut;          // ncells x (lo, hi)
-    const uint16_t* slotmap;    // 2 x ncells: result slot of (cell, d2 < lo) and (cell, d2 >= hi)
+    const float* lut;           // ncells x threshold of the cell (+inf: none, NaN: several)
+    const uint16_t* slotmap;    // 2 x ncells: result slots below the threshold of cell c [c] and at or above it [ncells + c]
     int ncells, shift;
     float sqrt_scale, sqrt_clamp;
+    float guard_scale;          // tpcf_set_guard_scale
+    int lut_multi;              // 1: some cell sees several thresholds (its lut entry is NaN)
     const float2* band_mh;      // nbands x (mid, half width)
     const float2* band_lh;      // nbands x (lo, hi)
     const uint16_t* band_slot;  // nbands + 1 result slots: below band b; [nbands] = above the last band

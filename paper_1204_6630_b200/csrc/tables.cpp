@@ -105,15 +105,19 @@ int FastTables::cell_of(float d2) const {
     float c = std::fmin(d2, sqrt_clamp);
     float key = u2f((f2u(c) >> 1) + kSqrtMagic);
     float t = std::fmaf(key, sqrt_scale, 8388608.0f);
-    return (int)(f2u(t) & 0x7FFFFFu);
+    return (int)((f2u(t) & 0x7FFFFFu) >> 2);
 }
 
 int FastTables::classify(float d2) const {
     int c = cell_of(d2);
     if (c < 0 || c >= ncells) return -2;
-    bool p0 = d2 >= lo[c];
-    if (p0 && d2 < hi[c]) return -1;
-    return p0 ? slot1[c] : slot0[c];
+    const float T = tcell[c];
+    if (T != T) return -1;
+    // the kernel's test with the widest block it admits (r = kRCap) and the tightest bound on the block's chords (q itself)
+    const float e = d2 - T;
+    const double g = guard_scale * ((double)kLookupAlpha * d2 + (double)kLookupBetaR * kRCap * std::sqrt((double)d2) + (double)kLookupBeta0);
+    if (!(std::fabs((double)e) > g)) return -1;
+    return e < 0.0f ? slot0[c] : slot1[c];
 }
 
 void FastTables::window(float lo2, float hi2, int& first_band, int& n_edges) const {
@@ -132,6 +136,8 @@ namespace {
 struct Band {
     float lo, hi;
     int below, above;
+    float t = 0.f;          // fp32 rounding of the threshold the band surrounds
+    bool merged = false;    // several overlapping bands in one: no single threshold
 };
 
 // first float (as bits) whose cell index is >= c; cell_of is monotone non-decreasing in d2 >= 0
@@ -149,8 +155,7 @@ uint32_t first_bits_of_cell(const FastTables& t, int c) {
 int fill(FastTables& t, const std::vector<Band>& bands, int lowest_slot) {
     const float inf = std::numeric_limits<float>::infinity();
     t.ncells = t.cell_of(u2f(kTopBits)) + 1;
-    t.lo.assign(t.ncells, inf);
-    t.hi.assign(t.ncells, inf);
+    t.tcell.assign(t.ncells, inf);
     t.slot0.assign(t.ncells, 0);
     t.slot1.assign(t.ncells, 0);
     t.cell_band.assign(t.ncells, 0);
@@ -174,11 +179,11 @@ int fill(FastTables& t, const std::vector<Band>& bands, int lowest_slot) {
         if (last == first) {
             t.slot0[c] = t.slot1[c] = (uint16_t)region;
         } else {
-            // More than one band in a cell: everything from the first band's lo to the last band's hi is
-            // treated as ambiguous (classified by the fp64 path), which is always correct, only slower.
+            // More than one band reaches into the cell (or one that stands for several merged ones): every pair of the
+            // cell is treated as ambiguous (classified by the fp64 path), which is always correct, only slower.
+            const bool multi = last - first > 1 || bands[first].merged;
             if (last - first > 1) ++bad;
-            t.lo[c] = bands[first].lo;
-            t.hi[c] = bands[last - 1].hi;
+            t.tcell[c] = multi ? std::numeric_limits<float>::quiet_NaN() : bands[first].t;
             t.slot0[c] = (uint16_t)bands[first].below;
             t.slot1[c] = (uint16_t)bands[last - 1].above;
         }
@@ -222,9 +227,11 @@ static int make_bands(const Binning& b, double gs, bool lookup, std::vector<Band
         bd.hi = float_up(T + g);
         bd.below = k;
         bd.above = k + 1;
+        bd.t = (float)T;
         if (!bands.empty() && bd.lo < bands.back().hi) {      // overlapping guard bands: one wider ambiguous band
             bands.back().hi = std::max(bands.back().hi, bd.hi);
             bands.back().above = bd.above;
+            bands.back().merged = true;
             ++overlapping;
         } else {
             bands.push_back(bd);
@@ -233,7 +240,7 @@ static int make_bands(const Binning& b, double gs, bool lookup, std::vector<Band
     const int lowest = b.drop_first ? 1 : 0;
     {   // everything at or above kDiscardFrom involves a padding row: zero-width band, never ambiguous
         Band d;
-        d.lo = d.hi = kDiscardFrom;
+        d.lo = d.hi = d.t = kDiscardFrom;
         d.below = bands.empty() ? lowest : bands.back().above;
         d.above = n + 2;
         if (!bands.empty() && bands.back().hi > kDiscardFrom) bands.back().hi = kDiscardFrom;
@@ -262,7 +269,8 @@ void build_fast_tables(const Binning& b, double gs, FastTables& out) {
     std::vector<Band> lookup_bands, window_bands;
     const int ov = make_bands(b, gs, true, lookup_bands);
     make_bands(b, gs, false, window_bands);
-    build_fast_tables_impl(b, lookup_bands, ov, out);      // cell map + (lo, hi, slots) per cell: the lookup path
+    build_fast_tables_impl(b, lookup_bands, ov, out);      // cell map + (threshold, slots) per cell: the lookup path
+    out.guard_scale = gs;
     export_bands(window_bands, out);                       // the bands the window loops compare against
     fill_cell_band(out, window_bands);
 }
@@ -288,7 +296,7 @@ static void build_fast_tables_impl(const Binning& b, const std::vector<Band>& ba
         for (int target = 512; target <= kMaxCells; target *= 2) {
             t.map = CellMap::SqrtLin;
             t.sqrt_clamp = clamp;
-            t.sqrt_scale = (float)((target - 2) / (double)keymax);
+            t.sqrt_scale = (float)(4.0 * (target - 2) / (double)keymax);
             if (fill(t, bands, lowest) == 0 && t.ncells <= kMaxCells) { out = t; return; }
         }
     }

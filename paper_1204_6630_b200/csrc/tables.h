@@ -17,6 +17,10 @@ constexpr int kPlanSMs = 148;          // B200 SM count the plan balances for
 constexpr float kPadCoord = 2.0f;      // padding rows are (2,2,2): 6.07 <= d2 <= 19.9 against any unit vector
 constexpr float kDiscardFrom = 5.0f;   // d2 >= 5 can only involve a padding row
 constexpr int kMaxCells = 8192;
+// guard of the cell-lookup path around the threshold of a cell: a pair with fp32 squared chord q is
+// decided in fp32 iff |q - T| > scale * (kLookupAlpha * Q + kLookupBetaR * r * sqrt(Q) + kLookupBeta0), Q >= q a bound on the
+// squared chords of the (lane, subtile) block and r the sum of its bounding radii; true error <= (9 q + 10 sqrt(q) r) 2^-24
+constexpr float kLookupAlpha = 7.5e-7f, kLookupBetaR = 8.0e-7f, kLookupBeta0 = 1.0e-13f;
 constexpr int kSubJ = 64;              // j-points per window subtile (one bounding sphere each)
 constexpr int kChunkJ = 128;           // j-points per bulk copy into a warp's shared-memory ring (= i-points per warp)
 constexpr int kWarpsPerCta = kThreads / 32;
@@ -31,11 +35,15 @@ enum class CellMap : int { LogBits = 0, SqrtLin = 1 };
 struct FastTables {
     CellMap map = CellMap::LogBits;
     int shift = 21;                 // LogBits: cell = bits(d2) >> shift
-    float sqrt_scale = 0.f;         // SqrtLin: cell = low 23 bits of fmaf(approx_sqrt(min(d2, sqrt_clamp)), sqrt_scale, 2^23)
+    float sqrt_scale = 0.f;         // SqrtLin: 4 * cell + 2 noise bits = low 23 bits of fmaf(approx_sqrt(min(d2, sqrt_clamp)), sqrt_scale, 2^23)
     float sqrt_clamp = 0.f;
     int ncells = 0;
     int merged_bands = 0;           // guard bands that had to be merged because they shared a cell (0 normally)
-    std::vector<float> lo, hi;      // per cell: below lo -> slot0, [lo, hi) -> ambiguous, >= hi -> slot1
+    double guard_scale = 1.0;       // tpcf_set_guard_scale: multiplies every guard width, in the tables and in the kernels
+    // per cell: the one threshold T (fp32 rounding of 4 sin^2(e_k/2)) whose guard band reaches into the cell:
+    //   d2 < T -> slot0, d2 >= T -> slot1, |d2 - T| <= guard -> ambiguous (fp64 recheck);
+    // +inf: no band reaches the cell (slot0 == slot1); NaN: several do, every pair of the cell is ambiguous
+    std::vector<float> tcell;
     std::vector<uint16_t> slot0, slot1;
     // The guard bands themselves, ascending and disjoint (the last one is the zero-width "discard" band at
     // kDiscardFrom).  The window path of the kernel compares against these directly: a pair whose fp32 squared chord
