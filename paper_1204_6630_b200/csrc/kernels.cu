@@ -120,7 +120,8 @@ __device__ __noinline__ void recheck_pair(SlowCtx* s, uint32_t i, uint32_t j) {
 // to its own recheck, they are queued per warp in shared memory and rechecked 32 at a time, one per lane.
 // rq holds kRecheckQueue entries (i, j); qn (warp-uniform, < 32 between calls) is the fill level.
 constexpr int kRecheckQueue = 64;
-constexpr int kMaxSlowLanes = 16;         // lookup / fp64 lanes a window block may carry (subtile_pairs)
+constexpr int kMaxSlowLanes = 8;          // lookup / fp64 lanes a window block may carry (subtile_pairs)
+constexpr float kMaxFlagExpect = 0.35f;   // a lane whose window block expects more ambiguous pairs than this takes the cell lookup
 __device__ __forceinline__ void rq_push(uint2* rq, unsigned& qn, bool has, uint32_t i, uint32_t j, SlowCtx* slow) {
     const int lane = threadIdx.x & 31;
     const unsigned bal = __ballot_sync(0xffffffffu, has);
@@ -235,7 +236,7 @@ template <int MAP, bool MASK>
 __device__ __forceinline__ void lookup_block(const float4* __restrict__ js, const float (&sx)[R], const float (&sy)[R],
                                              const float (&sz)[R], bool active, const Lookup& lk, float g, SlowCtx* slow,
                                              uint2* rq, unsigned& qn, uint32_t i0, uint32_t j0) {
-#pragma unroll 2
+#pragma unroll 1
     for (int jj = 0; jj < kSubJ; ++jj) {
         const float4 b = js[jj];                                  // one LDS.128, broadcast to the warp
         unsigned amb = 0;
@@ -255,24 +256,28 @@ __device__ __forceinline__ void lookup_block(const float4* __restrict__ js, cons
 // counters of the lookup path are therefore signed 32-bit values (flush_slots), and a counter may be read as -1 for a
 // moment when a flush falls between the two atomics.
 template <int MAP, bool CLAMP>
-__device__ __noinline__ void lookup_rescan(const float4 b, const f32x2 (&sx2)[R / 2], const f32x2 (&sy2)[R / 2], const f32x2 (&sz2)[R / 2],
-                                           const Lookup& lk, float g, SlowCtx* slow, uint2* rq, unsigned& qn, uint32_t i0, uint32_t j) {
-    const f32x2 bx = pack2(b.x, b.x), by = pack2(b.y, b.y), bz = pack2(b.z, b.z);
+__device__ __forceinline__ void lookup_rescan(const float4 b, float m, const f32x2 (&sx2)[R / 2], const f32x2 (&sy2)[R / 2],
+                                              const f32x2 (&sz2)[R / 2], const Lookup& lk, float g, SlowCtx* slow, uint2* rq, unsigned& qn,
+                                              uint32_t i0, uint32_t j) {
     unsigned amb = 0;
+    if (m <= g) {                                   // only the lanes that saw one walk their R pairs again
+        const f32x2 bx = pack2(b.x, b.x), by = pack2(b.y, b.y), bz = pack2(b.z, b.z);
 #pragma unroll
-    for (int r = 0; r < R / 2; ++r) {
-        float q[2];
-        unpack2(chord2_diff2(sx2[r], sy2[r], sz2[r], bx, by, bz), q[0], q[1]);
+        for (int r = 0; r < R / 2; ++r) {
+            float q[2];
+            unpack2(chord2_diff2(sx2[r], sy2[r], sz2[r], bx, by, bz), q[0], q[1]);
 #pragma unroll
-        for (int h = 0; h < 2; ++h) {
-            const uint32_t off = cell_off4<MAP, CLAMP>(q[h], lk);
-            const float e = __fsub_rn(q[h], lds_f32(lk.lut_s + off));
-            if (fabsf(e) <= g) {
-                atomicSub(reinterpret_cast<unsigned*>(lk.hist + off + (e < 0.f ? 0u : lk.above_off)), 1u);
-                amb |= 1u << (2 * r + h);
+            for (int h = 0; h < 2; ++h) {
+                const uint32_t off = cell_off4<MAP, CLAMP>(q[h], lk);
+                const float e = __fsub_rn(q[h], lds_f32(lk.lut_s + off));
+                if (fabsf(e) <= g) {
+                    atomicSub(reinterpret_cast<unsigned*>(lk.hist + off + (e < 0.f ? 0u : lk.above_off)), 1u);
+                    amb |= 1u << (2 * r + h);
+                }
             }
         }
     }
+    __syncwarp();
     while (__any_sync(0xffffffffu, amb != 0)) {
         const int r = __ffs(amb) - 1;
         rq_push(rq, qn, amb != 0, i0 + r, j, slow);
@@ -298,7 +303,7 @@ __device__ __forceinline__ void lookup_block_fast(const float4* __restrict__ js,
             unpack2(chord2_diff2(sx2[r], sy2[r], sz2[r], bx, by, bz), q0, q1);
             m = fminf(m, fminf(lookup_count<MAP, CLAMP>(q0, lk), lookup_count<MAP, CLAMP>(q1, lk)));
         }
-        if (__any_sync(0xffffffffu, m <= g)) lookup_rescan<MAP, CLAMP>(b, sx2, sy2, sz2, lk, g, slow, rq, qn, i0, j0 + jj);
+        if (__any_sync(0xffffffffu, m <= g)) lookup_rescan<MAP, CLAMP>(b, m, sx2, sy2, sz2, lk, g, slow, rq, qn, i0, j0 + jj);
     }
 }
 
@@ -410,6 +415,9 @@ __device__ __forceinline__ void subtile_pairs(const float4* __restrict__ js, con
         int e = 1;
         while (e <= kMaxWinEdges && k + e < wt.nbands && wt.band_lh[k + e].x <= hi2) ++e;
         mode = e;
+        // fine binnings: when the bands fill so much of the window that one of the block's kSubJ x R pairs is likely to
+        // fall inside one (chords spread evenly over the window), the window loop would only be followed by a recount
+        if (k < wt.nbands && (float)(2 * kSubJ * R) * (float)e * wt.band_mh[k].y > kMaxFlagExpect * (hi2 - lo2)) mode = 4;
     }
     // A few lanes that need the cell lookup (or fp64) do not drag the whole warp into lookup_block: the warp runs the
     // window loop of the other lanes, those lanes' counters are dropped and their pairs are recounted by the whole
