@@ -45,7 +45,7 @@ struct tpcf_ctx {
     FastTables ft;
     double guard_scale = 1.0;
     bool tables_dirty = true;
-    tpcf_engine engine = TPCF_ENGINE_FAST;
+    tpcf_engine engine = TPCF_ENGINE_TENSOR;
     bool window = true;
     cudaStream_t stream = nullptr;
     int part = 0, nparts = 1;
@@ -121,7 +121,7 @@ tpcf_status ensure_cuda(tpcf_ctx* ctx) {
 }
 
 void rebuild_tables(tpcf_ctx* ctx) {
-    build_fast_tables(ctx->bin, ctx->guard_scale, ctx->ft);
+    build_fast_tables(ctx->bin, ctx->guard_scale, ctx->engine == TPCF_ENGINE_TENSOR, ctx->ft);
     ctx->tables_dirty = true;
 }
 
@@ -621,7 +621,9 @@ tpcf_status tpcf_set_stream(tpcf_ctx* ctx, void* cuda_stream) {
 tpcf_status tpcf_set_engine(tpcf_ctx* ctx, tpcf_engine e) {
     if (!ctx) return TPCF_EINVAL;
     if (e != TPCF_ENGINE_FAST && e != TPCF_ENGINE_EXACT64 && e != TPCF_ENGINE_TENSOR) return fail(ctx, TPCF_EINVAL, "unknown engine");
+    const bool rebuild = (ctx->engine == TPCF_ENGINE_TENSOR) != (e == TPCF_ENGINE_TENSOR);
     ctx->engine = e;
+    if (rebuild) rebuild_tables(ctx);       // the tensor engine's window bands are wider
     return TPCF_OK;
 }
 

@@ -76,9 +76,14 @@ __device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) {
     return d;
 }
 
-// TF32 split of an fp32 value: hi = x with the low 13 mantissa bits cleared (exactly representable in TF32 whatever the
-// tensor core does with those bits), x - hi is exact in fp32
-__device__ __forceinline__ float tf32_hi(float x) { return __uint_as_float(__float_as_uint(x) & 0xFFFFE000u); }
+// TF32 split of an fp32 value: hi = x rounded to nearest (ties away) to TF32's 10 mantissa bits (cvt.rna: the low 13 bits
+// of the result are zero, so it is exactly representable whatever the tensor core does with those bits); x - hi is exact
+// in fp32 and |x - hi| <= 2^-11 |x|
+__device__ __forceinline__ float tf32_hi(float x) {
+    uint32_t r;
+    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(x));
+    return __uint_as_float(r);
+}
 
 // ---- exact classification (fp64), shared by the recheck path and the fp64 engine -----------------------
 __device__ __forceinline__ double chord2_f64(const double4& a, const double4& b) {

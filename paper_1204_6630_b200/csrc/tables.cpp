@@ -90,6 +90,10 @@ int exact_slot(double d2, const Binning& b) {
 //   expanded form (window path, d >= kFarKappa r = 2.5 r): 29.1 d^2 u          <= 1.74e-6 t
 // The constants below add margin (x1.67 on the sqrt term, x1.72 on the linear one).
 double guard_width(double t, double scale) { return scale * (1.0e-7 * std::sqrt(t) + 3.0e-6 * t + 1.0e-13); }
+// The tensor engine forms the same expanded form from 3xTF32 operands on the tensor core: inputs and norms 15.2 u, 3xTF32
+// split residual 13.4 u, the tensor core's truncating accumulation 13.1 u, further edges 2 u = 43.7 u max(d^2, mid) =
+// 2.61e-6 t (lemma T; the accumulation model is checked bit for bit on the GPU); margin x1.53.
+double guard_width_tensor(double t, double scale) { return scale * (1.0e-7 * std::sqrt(t) + 4.0e-6 * t + 1.0e-13); }
 // The cell-lookup path only ever evaluates the difference form: its bands need not cover the expanded form's error.
 // (9 d^2 + 10 d r) u <= 5.4e-7 t + 6.0e-8 sqrt(t); margins x1.85 and x1.67.
 double guard_width_lookup(double t, double scale) { return scale * (1.0e-7 * std::sqrt(t) + 1.0e-6 * t + 1.0e-13); }
@@ -215,13 +219,13 @@ static void export_bands(const std::vector<Band>& bands, FastTables& t) {
 
 // Guard bands around the droppable edges (ascending, overlapping ones merged) + the zero-width discard band.
 // Returns the number of merges.
-static int make_bands(const Binning& b, double gs, bool lookup, std::vector<Band>& bands) {
+static int make_bands(const Binning& b, double gs, int form /* 0 window, 1 lookup, 2 tensor window */, std::vector<Band>& bands) {
     const int n = b.nbins;
     int overlapping = 0;
     bands.clear();
     for (int k = 0; k <= n; ++k) {
         if ((k == 0 && b.drop_first) || (k == n && b.drop_last)) continue;
-        double T = b.thr[k], g = lookup ? guard_width_lookup(T, gs) : guard_width(T, gs);
+        double T = b.thr[k], g = form == 1 ? guard_width_lookup(T, gs) : form == 2 ? guard_width_tensor(T, gs) : guard_width(T, gs);
         Band bd;
         bd.lo = (T - g <= 0.0 || T < 1e-12) ? 0.0f : float_down(T - g);
         bd.hi = float_up(T + g);
@@ -265,10 +269,10 @@ static void fill_cell_band(FastTables& t, const std::vector<Band>& bands) {
 
 static void build_fast_tables_impl(const Binning& b, const std::vector<Band>& bands, int overlapping, FastTables& out);
 
-void build_fast_tables(const Binning& b, double gs, FastTables& out) {
+void build_fast_tables(const Binning& b, double gs, bool tensor, FastTables& out) {
     std::vector<Band> lookup_bands, window_bands;
-    const int ov = make_bands(b, gs, true, lookup_bands);
-    make_bands(b, gs, false, window_bands);
+    const int ov = make_bands(b, gs, 1, lookup_bands);
+    make_bands(b, gs, tensor ? 2 : 0, window_bands);
     build_fast_tables_impl(b, lookup_bands, ov, out);      // cell map + (threshold, slots) per cell: the lookup path
     out.guard_scale = gs;
     export_bands(window_bands, out);                       // the bands the window loops compare against

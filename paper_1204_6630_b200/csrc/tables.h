@@ -73,10 +73,13 @@ std::string make_binning(int nbins, const double* theta_deg, int mode, Binning& 
 
 // fp32 rounding bound of the fast engine's squared chord around the true value t.
 double guard_width(double t, double scale);
+// ... of the tensor engine's: the 3xTF32 split and the tensor core's truncating accumulation come on top
+double guard_width_tensor(double t, double scale);
 // ... and of the difference form alone (the bands of the cell-lookup tables)
 double guard_width_lookup(double t, double scale);
 
-void build_fast_tables(const Binning& b, double guard_scale, FastTables& out);
+// tensor: the window bands are those of the tensor engine (guard_width_tensor)
+void build_fast_tables(const Binning& b, double guard_scale, bool tensor, FastTables& out);
 
 // Exact classification used by the fp64 engine and the recheck path (host mirror of the device code).
 int exact_slot(double d2, const Binning& b);

@@ -28,6 +28,19 @@ W_TOL = 1e-6        # BASELINE.json: |w_gpu - w_oracle| <= 1e-6 absolute
 KINDS = ("DD", "DR", "RR")
 
 
+@pytest.fixture(autouse=True)
+def fast_engine_in_this_module(monkeypatch):
+    """The tests of this file pin TPCF_ENGINE_FAST (the FFMA2 kernel); tests/test_gpu_tensor.py repeats them for the
+    library's default engine, TPCF_ENGINE_TENSOR."""
+    init = T.Context.__init__
+
+    def init_fast(self, *a, **k):
+        init(self, *a, **k)
+        self.set_engine("fast")
+
+    monkeypatch.setattr(T.Context, "__init__", init_fast)
+
+
 def full(h, u, o):
     return np.concatenate([[u], np.asarray(h, dtype=np.int64), [o]]).astype(np.int64)
 
