@@ -31,7 +31,6 @@ import synth  # noqa: E402
 KINDS = ("DD", "DR", "RR")
 METRIC = "pair evals/sec (DD+DR+RR)"
 UNIT = "Gpairs/s"
-SM_COUNT = 148
 LANES_PER_CLK_PER_SM = 128      # 4 schedulers x 1 warp instruction x 32 lanes
 PAPER_CONTEXT = {"table2_row1_0.43e6_lines_seconds": {"cpu_2xE5520": 3.60e4, "gtx295": 3.01e2, "c1060": 2.91e2,
                                                       "c2050": 2.19e2}, "source": "PAPER.md:61 (other hardware; context, not target)"}
@@ -102,9 +101,7 @@ def profile_summary(cfg_idx: int, engine: str = "fast"):
     path = os.path.join(ROOT, "profiles", "inst_per_pair.json")
     try:
         d = json.load(open(path))
-        if engine == "tensor":
-            return d.get(f"cfg{cfg_idx}_tensor") or d.get("default_tensor") or {}
-        return d.get(f"cfg{cfg_idx}") or d["default"]
+        return d.get(f"cfg{cfg_idx}_{engine}") or {}        # no capture of this (config, kernel): the line prints null
     except Exception:
         return {}
 
@@ -173,6 +170,8 @@ def run_ours(args):
     torch.cuda.set_device(local)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        print(f"[bench] rank {rank}/{world}: communicator of {dist.get_world_size()} ranks, backend {dist.get_backend()}, "
+              f"device cuda:{local}", file=sys.stderr, flush=True)
     D, R, e, cfg = synth.make_config(args.config)
     nd, nr = D.shape[0], R.shape[0]
     pairs_step = total_pairs(nd, nr)
@@ -300,6 +299,7 @@ def run_ours(args):
         peak_src = "MEASURED_PEAKS.json sm_max_mhz"
     except Exception:
         sm_max, peak_src = 1965.0, "fallback 1965 MHz (B200_PROFILING.md nominal clocks.max.sm)"
+    SM_COUNT = torch.cuda.get_device_properties(local).multi_processor_count
     peak = SM_COUNT * LANES_PER_CLK_PER_SM * sm_max * 1e6 / 1e12          # T lane-operations/s
     # per launch: pairs of that histogram (this rank's share) / its own duration; the three launches repeat DD, DR, RR
     share = [w_ / world for w_ in want]
@@ -343,7 +343,7 @@ def run_ours(args):
                                   "fp64 recheck as in the fast engine)" if tensor_ran else
                                   "fast (fp32 squared chord by FFMA2 + fp64 recheck of guard-band pairs)"),
                        "parallelism": f"tile work items w % {world} == rank, one all-reduce of 3x{nb + 2} int64" if world > 1 else "1 GPU",
-                       "grid": stats["grid"], "block": stats["block"], "smem_bytes": stats["smem_bytes"], "cells": stats["cells"]},
+                       "comm_nranks": world, "grid": stats["grid"], "block": stats["block"], "smem_bytes": stats["smem_bytes"], "cells": stats["cells"]},
             "seconds_per_w_theta": ms_step * 1e-3,
             "e2e": {"value": pairs_step / e2e_s / 1e9, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "seconds_per_step": e2e_s, "steps": e2e_steps,

@@ -42,18 +42,21 @@ typedef enum { TPCF_F32 = 0, TPCF_F64 = 1 } tpcf_dtype;
 typedef enum { TPCF_DD = 0, TPCF_DR = 1, TPCF_RR = 2 } tpcf_kind;
 
 /* Which kernel family tpcf_count uses (tpcf_set_engine).
- *   TPCF_ENGINE_FAST    fp32 squared-chord evaluation, O(1) cell lookup against cos/chord-space
- *                       thresholds, privatised shared-memory histograms; every pair that lands within the
- *                       fp32 rounding guard band of a bin edge is re-evaluated in fp64 from the fp64
- *                       coordinates, so the histograms equal those of TPCF_ENGINE_EXACT64 (default).
+ *   TPCF_ENGINE_TENSOR  (default) blocks of 128 i-rows x 128 j-rows; for every (8-row group, j-tile) block whose bounding
+ *                       spheres leave at most 3 bin edges in reach, the window quantity q = |a-b|^2 - mid is formed by a
+ *                       3xTF32 tcgen05.mma (fp32 accumulators in tensor memory, one i-row per thread) and every pair is
+ *                       classified by 1..3 sign tests; a pair within the guard band of an edge (4.0e-6 T: 1.5 times the
+ *                       proven bound 43.7 x 2^-24 T of DESIGN.md section 4, which rests on the measured, bit-exactly
+ *                       reproduced accumulation model of tests/tc_model.py), near blocks and fine binnings go through the
+ *                       fp32 cell lookup of TPCF_ENGINE_FAST and, inside its guard band, the fp64 recheck: the
+ *                       histograms equal those of TPCF_ENGINE_EXACT64.  Binnings whose lookup tables leave room for
+ *                       fewer than 3 such CTAs per SM (config 5) run TPCF_ENGINE_FAST's kernel.
+ *   TPCF_ENGINE_FAST    the same windows with q formed by packed FP32 FMAs (FFMA2) on the CUDA cores, 8 i-rows per lane
+ *                       against 64-row j-subtiles (guard band 3.0e-6 T, proven bound 29.1 x 2^-24 T); otherwise an O(1)
+ *                       cell lookup against chord-space thresholds with privatised shared-memory histograms; every pair
+ *                       inside a guard band is re-evaluated in fp64.  Same histograms.
  *   TPCF_ENGINE_EXACT64 plain fp64 kernel: fp64 squared chord against fp64 thresholds 4 sin^2(e_k/2) by
- *                       binary search.  Slow; kept as the device-side cross-check of the fast engine.
- *   TPCF_ENGINE_TENSOR  the window quantity q of TPCF_ENGINE_FAST's far blocks is formed by a 3xTF32 tcgen05.mma
- *                       (fp32 accumulators in tensor memory, one i-row per thread) instead of the FFMA2 chain;
- *                       everything else (windows, guard bands, cell lookup, fp64 recheck) is the same, and so are the
- *                       histograms.  Faster on all but fine binnings (which run the FFMA2 kernel under this engine
- *                       too).  Not the default because the tensor core's accumulation error is measured (a factor 12
- *                       inside the guard band, tpcf_tensor_probe), not proven.
+ *                       binary search.  Slow; kept as the device-side cross-check of the other two.
  */
 typedef enum { TPCF_ENGINE_FAST = 0, TPCF_ENGINE_EXACT64 = 1, TPCF_ENGINE_TENSOR = 2 } tpcf_engine;
 
@@ -84,8 +87,9 @@ tpcf_status tpcf_get_edges(const tpcf_ctx* ctx, double* edges_out /* nbins+1 */)
  *   tpcf_count_async on another stream than cuda_stream / the context's stream is still reading them.
  *   cuda_stream: a cudaStream_t (or NULL for the context's stream) the copy and conversion are ordered on;
  *   the call returns after they completed.
- *   Errors: TPCF_EINVAL for n == 0, n > 2^31-1, |Dec| > 90 or a non-finite value in any row (checked on
- *   the device); TPCF_ENOMEM; TPCF_ECUDA.
+ *   Errors: TPCF_EINVAL for n == 0, n > 2^31-1, |Dec| > 90, |RA| > 1e6 or a non-finite value in any row
+ *   (checked on the device; RA is periodic, any value up to 1e6 degrees in magnitude is accepted); TPCF_ENOMEM; TPCF_ECUDA.
+ *   The context is bound to the CUDA device that is current at its first GPU call; later calls make that device current.
  */
 tpcf_status tpcf_load(tpcf_ctx* ctx, tpcf_cat which, const void* radec_deg, tpcf_dtype dt, size_t n, int on_device,
                       void* cuda_stream);
@@ -140,12 +144,12 @@ tpcf_status tpcf_set_engine(tpcf_ctx* ctx, tpcf_engine e);
  * give identical histograms; the tests use 2.0 and 8.0 to demonstrate that the band is wide enough.
  * scale <= 0 is TPCF_EINVAL. */
 tpcf_status tpcf_set_guard_scale(tpcf_ctx* ctx, double scale);
-/* Window path of the fast engine on (default) / off.  On: catalogs are held in Hilbert-curve order with a bounding
- * sphere per 32 rows; for every (lane = 4 consecutive i-rows, 32-row j-subtile) block the kernel bounds the chord
- * lengths by the triangle inequality, and when at most 3 bin edges can be reached it classifies each pair with that
- * many sign tests against the band midpoints (register counters, no shared-memory traffic per pair); otherwise, and
- * always when off, each pair goes through the cell lookup.  Every pair is evaluated either way; the histograms are
- * identical (tests). */
+/* Window path on (default) / off.  On: catalogs are held in Hilbert-curve order with a bounding sphere per 8-row group
+ * (i side) and per 64-row subtile / 128-row tile (j side); for every (group, subtile) block the kernel bounds the chord
+ * lengths by the triangle inequality, and when at most 3 bin edges can be reached it classifies each pair with that many
+ * sign tests against the band midpoints (register counters, no shared-memory traffic per pair); otherwise, and always
+ * when off, each pair goes through the cell lookup.  Every pair is evaluated either way; the histograms are identical
+ * (tests). */
 tpcf_status tpcf_set_window(tpcf_ctx* ctx, int enabled);
 /* Work partition for multi-process runs (one process per GPU): this context enumerates only the tile
  * work items w with w % nparts == part; summing the histograms of all parts gives the full count
@@ -167,7 +171,7 @@ typedef struct {
     int cells, cell_bits;    /* lookup cells of the fast engine and mantissa bits per octave */
     int hist_copies;         /* privatised copies of each partial-histogram slot per CTA */
     float kernel_ms;         /* device time of the last synchronous count (CUDA events) */
-    uint64_t win_blocks[6];  /* (warp of 128 i-rows, 32-row j-subtile) blocks of the last synchronous count by path:
+    uint64_t win_blocks[6];  /* (warp of 256 i-rows, 64-row j-subtile) blocks -- tensor engine: (warp of 32 i-rows, 128-row j-tile) -- of the last synchronous count by path:
                                 counted by the 1-, 2-, 3-edge window loops, by the per-pair cell lookup; [4] = lanes of
                                 window blocks recounted pair by pair because a pair came within a guard band;
                                 [5] = blocks classified wholly in fp64 (bounding radii too large for the fp32 bound) */

@@ -20,7 +20,7 @@ struct Catalog {                 // rows in Hilbert order (counts are order-inva
     double4* x64 = nullptr;
     uint32_t* inv = nullptr;     // caller row -> position in the sorted catalog (row-subset mode)
     float4 *xq = nullptr, *cq = nullptr;   // i-side role: rows as offsets from their 8-row group ("quad") centre; (centre, radius)
-    float4 *xs = nullptr, *cs = nullptr;   // j-side role: rows as (-2 offset, |offset|^2) from their 32-row subtile centre
+    float4 *xs = nullptr, *cs = nullptr;   // j-side role: rows as (-2 offset, |offset|^2) from their 64-row subtile centre
     float4 *xt = nullptr, *ct = nullptr;   // j-side role of the tensor engine: the same for 128-row tiles
     float* xb = nullptr;                   // ... and per tile a 128 x 16 TF32 operand block (kernels.cuh)
 };
@@ -53,7 +53,8 @@ struct tpcf_ctx {
     PlanCache plans[3];
     // device side
     bool cuda_ready = false;
-    int sm_count = 0;
+    int sm_count = kPlanSMs;    // replaced by cudaDevAttrMultiProcessorCount of the context's device at its first GPU call
+    int device = -1;            // the device the context is bound to (ensure_cuda)
     float* d_lut = nullptr;
     int lut_multi = 0;
     uint16_t* d_slotmap = nullptr;
@@ -68,6 +69,7 @@ struct tpcf_ctx {
     size_t arena_bytes = 0;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
     bool time_kernels = false;
+    int warp_items_per_item = 1;                // how the pair kernel that ran counts work items (pair_fast_kernel: per warp)
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> kev_pool, kev_used;
     // stored full counts for tpcf_estimate
     std::vector<uint64_t> counts[3];
@@ -94,7 +96,12 @@ tpcf_status cuda_fail(tpcf_ctx* c, cudaError_t e, const char* what) {
 
 // No CPU fallback: without a usable GPU every compute entry point fails with TPCF_ECUDA.
 tpcf_status ensure_cuda(tpcf_ctx* ctx) {
-    if (ctx->cuda_ready) return TPCF_OK;
+    if (ctx->cuda_ready) {
+        // the context lives on the device that was current at its first GPU call: make it current again for this call
+        int cur = -1;
+        if (cudaGetDevice(&cur) != cudaSuccess || cur != ctx->device) CU(cudaSetDevice(ctx->device), "cudaSetDevice");
+        return TPCF_OK;
+    }
     int n = 0;
     cudaError_t e = cudaGetDeviceCount(&n);
     if (e != cudaSuccess || n < 1) {
@@ -107,6 +114,7 @@ tpcf_status ensure_cuda(tpcf_ctx* ctx) {
     CU(cudaGetDeviceProperties(&prop, dev), "cudaGetDeviceProperties");
     if (prop.major < 10) return fail(ctx, TPCF_ECUDA, "libtpcf is built for sm_100a (B200) only");
     ctx->sm_count = prop.multiProcessorCount;
+    ctx->device = dev;
     const int nb = ctx->bin.nbins;
     CU(cudaMalloc(&ctx->d_thr, (nb + 1) * sizeof(double)), "cudaMalloc thresholds");
     CU(cudaMalloc(&ctx->d_result, (nb + 3) * sizeof(unsigned long long)), "cudaMalloc result");
@@ -278,7 +286,7 @@ tpcf_status enqueue_count(tpcf_ctx* ctx, tpcf_kind kind, const int64_t* rows_hos
         sc.release();
         if (e != cudaSuccess) return cuda_fail(ctx, e, "gather subset rows");
         if (bad) return fail(ctx, TPCF_EINVAL, "row index out of range");
-        make_plan(false, nrows, cj.n, subset_plan);
+        make_plan(false, nrows, cj.n, ctx->sm_count, subset_plan);
         plan = &subset_plan;
         p.xq = tmp->xq;
         p.cq = tmp->cq;
@@ -290,7 +298,7 @@ tpcf_status enqueue_count(tpcf_ctx* ctx, tpcf_kind kind, const int64_t* rows_hos
     } else {
         PlanCache& pc = ctx->plans[kind];
         if (!pc.valid) {
-            make_plan(sd.tri, ci.n, cj.n, pc.plan);
+            make_plan(sd.tri, ci.n, cj.n, ctx->sm_count, pc.plan);
             if (pc.d_row_start) cudaFree(pc.d_row_start);
             pc.d_row_start = nullptr;
             if (sd.tri) {
@@ -325,7 +333,7 @@ tpcf_status enqueue_count(tpcf_ctx* ctx, tpcf_kind kind, const int64_t* rows_hos
     // small catalogs: split the j-tile of every warp item until each resident warp gets ~32 of them
     p.jsplit = 1;
     while (p.chunk == 1 && p.jsplit < (uint32_t)(kTileJ / kChunkJ) &&
-           (uint64_t)p.n_items_part * kWarpsPerCta * p.jsplit < 32ull * kPlanSMs * 2 * kWarpsPerCta)
+           (uint64_t)p.n_items_part * kWarpsPerCta * p.jsplit < 32ull * (uint64_t)ctx->sm_count * 2 * kWarpsPerCta)
         p.jsplit *= 2;
     p.part = (uint32_t)ctx->part;
     p.nparts = (uint32_t)ctx->nparts;
@@ -362,12 +370,15 @@ tpcf_status enqueue_count(tpcf_ctx* ctx, tpcf_kind kind, const int64_t* rows_hos
         }
         CU(cudaEventRecord(kev.first, st), "cudaEventRecord");
     }
-    if (ctx->engine == TPCF_ENGINE_FAST)
-        CU(launch_pairs_fast(p, ctx->ft.map, ctx->sm_count, st, &li), "pair_fast_kernel launch");
-    else if (ctx->engine == TPCF_ENGINE_TENSOR)
-        CU(launch_pairs_tensor(p, ctx->ft.map, ctx->sm_count, st, &li), "pair_tensor_kernel launch");
-    else
-        CU(launch_pairs_exact64(p, ctx->sm_count, st, &li), "pair_exact64_kernel launch");
+    {
+        const cudaError_t le = ctx->engine == TPCF_ENGINE_FAST     ? launch_pairs_fast(p, ctx->ft.map, ctx->sm_count, st, &li)
+                               : ctx->engine == TPCF_ENGINE_TENSOR ? launch_pairs_tensor(p, ctx->ft.map, ctx->sm_count, st, &li)
+                                                                   : launch_pairs_exact64(p, ctx->sm_count, st, &li);
+        if (le != cudaSuccess) {
+            if (kev.first) ctx->kev_pool.push_back(kev);        // the event pair goes back to the pool
+            return cuda_fail(ctx, le, "pair kernel launch");
+        }
+    }
     if (kev.first) {
         CU(cudaEventRecord(kev.second, st), "cudaEventRecord");
         ctx->kev_used.push_back(kev);
@@ -377,6 +388,7 @@ tpcf_status enqueue_count(tpcf_ctx* ctx, tpcf_kind kind, const int64_t* rows_hos
     ctx->stats.launches += 2;
     ctx->stats.grid = li.grid;
     ctx->stats.block = li.block;
+    ctx->warp_items_per_item = (li.block == kThreads && ctx->engine != TPCF_ENGINE_EXACT64) ? kWarpsPerCta : 1;
     ctx->stats.smem_bytes = li.smem_bytes;
     ctx->stats.cells = ctx->ft.ncells;
     ctx->stats.cell_bits = (ctx->ft.map == CellMap::LogBits) ? 23 - ctx->ft.shift : -1;
@@ -504,7 +516,7 @@ tpcf_status tpcf_load(tpcf_ctx* ctx, tpcf_cat which, const void* radec_deg, tpcf
     }
     if (bad) {
         free_catalog(c);
-        return fail(ctx, TPCF_EINVAL, "catalog has a non-finite value or |Dec| > 90");
+        return fail(ctx, TPCF_EINVAL, "catalog has a non-finite value, |RA| > 1e6 or |Dec| > 90");
     }
     c.n = n;
     c.n_pad = n_pad;
@@ -542,8 +554,8 @@ tpcf_status tpcf_count(tpcf_ctx* ctx, tpcf_kind kind, uint64_t* hist_out, uint64
     ctx->stats.kernel_ms = ms;
     ctx->stats.pairs = pairs;
     ctx->stats.rechecked = ctr[1];
-    // the fast engine executes every plan item as kWarpsPerCta warp items
-    ctx->stats.work_items = (ctx->engine == TPCF_ENGINE_FAST) ? ctr[2] / kWarpsPerCta : ctr[2];
+    // pair_fast_kernel (also when the tensor engine falls back to it) executes every plan item as kWarpsPerCta warp items
+    ctx->stats.work_items = ctr[2] / ctx->warp_items_per_item;
     for (int k = 0; k < 6; ++k) ctx->stats.win_blocks[k] = ctr[3 + k];
     for (int k = 0; k < nb; ++k) hist_out[k] = host[k + 1];
     if (under_over_out) {
@@ -583,6 +595,7 @@ tpcf_status tpcf_estimate(tpcf_ctx* ctx, double* w_out) {
 void tpcf_destroy(tpcf_ctx* ctx) {
     if (!ctx) return;
     if (ctx->cuda_ready) {
+        cudaSetDevice(ctx->device);
         free_catalog(ctx->cat[0]);
         free_catalog(ctx->cat[1]);
         for (auto& pc : ctx->plans)
@@ -732,7 +745,7 @@ tpcf_status tpcf_plan(const tpcf_ctx* ctx, tpcf_kind kind, uint64_t n_d, uint64_
     if (!ctx || !n_items_out || n_d == 0 || n_r == 0) return TPCF_EINVAL;
     Plan p;
     const Sides sd = sides_of(kind);
-    make_plan(sd.tri, sd.ci == 0 ? n_d : n_r, sd.cj == 0 ? n_d : n_r, p);
+    make_plan(sd.tri, sd.ci == 0 ? n_d : n_r, sd.cj == 0 ? n_d : n_r, ctx->sm_count, p);
     *n_items_out = p.n_items;
     return TPCF_OK;
 }
@@ -742,7 +755,7 @@ tpcf_status tpcf_plan_item_pairs(const tpcf_ctx* ctx, tpcf_kind kind, uint64_t n
     if (!ctx || !pairs_out || n_d == 0 || n_r == 0) return TPCF_EINVAL;
     Plan p;
     const Sides sd = sides_of(kind);
-    make_plan(sd.tri, sd.ci == 0 ? n_d : n_r, sd.cj == 0 ? n_d : n_r, p);
+    make_plan(sd.tri, sd.ci == 0 ? n_d : n_r, sd.cj == 0 ? n_d : n_r, ctx->sm_count, p);
     if (w >= p.n_items) return TPCF_EINVAL;
     *pairs_out = p.item_pairs(w);
     return TPCF_OK;

@@ -1301,8 +1301,8 @@ __global__ void __launch_bounds__(kThreads) pair_exact64_kernel(const __grid_con
             }
         }
         ++items_done;
-        // at most kMaxChunk * 2^20 pairs per item and slot; flush well before 2^32
-        if ((items_done & 255) == 0) {
+        // at most kMaxChunk * kTileI * kTileJ = 2^25 pairs per item and slot: 32 items stay below 2^31
+        if ((items_done & 31) == 0) {
             __syncthreads();
             for (int k = tid; k < nslots; k += kThreads) {
                 if (hist[k]) atomicAdd(p.result + k, (unsigned long long)hist[k]);

@@ -12,7 +12,7 @@ struct PairParams {
     // i side: rows as fp32 offsets from the centre of their 8-row group ("quad"), and the groups' (centre, radius)
     const float4* xq;
     const float4* cq;
-    // j side: rows as (-2 offset, |offset|^2) from the centre of their 32-row subtile, and the subtiles' (centre, radius)
+    // j side: rows as (-2 offset, |offset|^2) from the centre of their 64-row subtile, and the subtiles' (centre, radius)
     const float4* xs;
     const float4* cs;
     // j side, tensor engine: the same roles for kTcSubJ = 128-row tiles (rows xt, spheres ct), and per tile a
@@ -76,7 +76,7 @@ cudaError_t launch_permute(const double4* x64_rows, const uint32_t* order, uint6
                            uint32_t* inv, cudaStream_t st);
 // i-side role: per kIPerThread-row group ("quad") its (centre, radius) and the rows as fp32 offsets from the centre
 cudaError_t launch_quads(const double4* x64, uint64_t n_pad, float4* xq, float4* cq, cudaStream_t st);
-// j-side role: per 32-row subtile its (centre, radius) and the rows as (-2 offset, |offset|^2)
+// j-side role: per 64-row subtile its (centre, radius) and the rows as (-2 offset, |offset|^2)
 cudaError_t launch_subtiles(const double4* x64, uint64_t n_pad, float4* xs, float4* cs, float4* xt, float4* ct, float* xb,
                             cudaStream_t st);
 // subset mode: caller rows -> positions in the sorted catalog (keys for the sort) with range check

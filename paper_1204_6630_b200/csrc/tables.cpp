@@ -316,7 +316,7 @@ static void build_fast_tables_impl(const Binning& b, const std::vector<Band>& ba
 // Work plan: the N_D x N_R rectangle (DR) or the i<j triangle (DD, RR) cut into items of one kTileI-row
 // i-block times up to `chunk` kTileJ-column j-tiles (north_star "triangular tiles").
 // --------------------------------------------------------------------------------------------------
-void make_plan(bool tri, uint64_t n_i, uint64_t n_j, Plan& p) {
+void make_plan(bool tri, uint64_t n_i, uint64_t n_j, int sm_count, Plan& p) {
     p = Plan();
     p.tri = tri;
     p.n_i = n_i;
@@ -324,7 +324,7 @@ void make_plan(bool tri, uint64_t n_i, uint64_t n_j, Plan& p) {
     p.blocks_i = (uint32_t)((n_i + kTileI - 1) / kTileI);
     p.tiles_j = (uint32_t)((p.n_j + kTileJ - 1) / kTileJ);
     uint64_t tiles = tri ? (uint64_t)p.blocks_i * (p.blocks_i + 1) / 2 : (uint64_t)p.blocks_i * p.tiles_j;
-    uint64_t c = tiles / (160ull * kPlanSMs);
+    uint64_t c = tiles / (160ull * (uint64_t)std::max(sm_count, 1));
     p.chunk = (uint32_t)std::min<uint64_t>(std::max<uint64_t>(c, 1), kMaxChunk);
     if (tri) {
         p.row_start.resize((size_t)p.blocks_i + 1);

@@ -13,7 +13,7 @@ constexpr int kIPerThread = 8;         // i-points held in registers per thread 
 constexpr int kTileI = kThreads * kIPerThread;   // 2048 i-points per plan item
 constexpr int kTileJ = kTileI;         // j-points per plan tile (the triangle plan needs kTileJ == kTileI)
 constexpr int kMaxChunk = 8;           // j-tiles per work item, at most
-constexpr int kPlanSMs = 148;          // B200 SM count the plan balances for
+constexpr int kPlanSMs = 148;          // SM count the plan balances for until the context has seen its device (B200: 148)
 constexpr float kPadCoord = 2.0f;      // padding rows are (2,2,2): 6.07 <= d2 <= 19.9 against any unit vector
 constexpr float kDiscardFrom = 5.0f;   // d2 >= 5 can only involve a padding row
 constexpr int kMaxCells = 8192;
@@ -95,7 +95,7 @@ struct Plan {
     void item(uint64_t w, uint32_t& I, uint32_t& tile0, uint32_t& ntiles) const;
     uint64_t item_pairs(uint64_t w) const;
 };
-void make_plan(bool tri, uint64_t n_i, uint64_t n_j, Plan& out);
+void make_plan(bool tri, uint64_t n_i, uint64_t n_j, int sm_count, Plan& out);
 
 void estimate(const uint64_t* dd, const uint64_t* dr, const uint64_t* rr, int nbins, uint64_t n_d, uint64_t n_r,
               double* w);

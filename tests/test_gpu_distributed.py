@@ -1,0 +1,90 @@
+"""NEXT-1 ("multi-GPU solution", "full-blown multi-GPU implementation") with the
+real kernels in real processes: two ranks (both on cuda:0 -- this pool has one GPU per box; their kernels never wait on
+one another), each loading both catalogs, taking its share of the tile work plan (tpcf_set_partition), counting DD, DR
+and RR with the CUDA kernels, one all-reduce of the integer histograms (gloo here, NCCL in bench.py --gpus N), then the
+estimator on the summed counts.  The sum must equal the single-process histograms bit for bit and match the oracle."""
+import os
+import socket
+
+import numpy as np
+import pytest
+import torch.multiprocessing as mp
+
+import oracle
+import paper_1204_6630_b200 as T
+import synth
+from test_gpu_parity import KINDS, assert_parity, assert_w, full, oracle_all, totals
+
+pytestmark = pytest.mark.gpu
+ND, NR = 20_000, 17_777
+
+
+def _free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def _worker(rank, world, port, engine, q):
+    import torch
+    import torch.distributed as dist
+
+    import paper_1204_6630_b200 as TT
+    from paper_1204_6630_b200 import dist as tdist
+
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    torch.cuda.set_device(0)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        D, R, e, cfg = synth.make_config(2, n_d=ND, n_r=NR)
+        with TT.Context(cfg.nbins, e, "explicit") as c:
+            c.set_engine(engine)
+            c.load("D", D)
+            c.load("R", R)
+            assert tdist.apply_partition(c) == (rank, world)
+            mine, pairs = [], []
+            for k in KINDS:
+                h, u, o = c.count(k)
+                mine.append(np.concatenate([[u], h.astype(np.int64), [o]]))
+                pairs.append(c.stats()["pairs"])
+            mine = np.stack(mine)
+            summed = tdist.allreduce_counts(mine.copy())
+            w = TT.tpcf_estimate_from(summed[0][1:-1], summed[1][1:-1], summed[2][1:-1], ND, NR)
+            q.put((rank, mine.tolist(), pairs, summed.tolist(), w.tolist(), c.stats()["block"]))
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("engine", ["tensor", "fast"])
+def test_two_processes_count_their_partitions_and_allreduce(engine, oracle_threads):
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_worker, args=(r, 2, port, engine, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    got = sorted(q.get(timeout=600) for _ in procs)
+    for p in procs:
+        p.join(timeout=120)
+        assert p.exitcode == 0
+    D, R, e, cfg = synth.make_config(2, n_d=ND, n_r=NR)
+    with T.Context(cfg.nbins, e, "explicit") as c:
+        c.set_engine(engine)
+        c.load("D", D)
+        c.load("R", R)
+        single = np.stack([full(*c.count(k)) for k in KINDS])
+        w1 = c.estimate()
+    part0, part1 = np.asarray(got[0][1]), np.asarray(got[1][1])
+    want = totals(ND, NR)
+    for i, k in enumerate(KINDS):
+        assert got[0][2][i] + got[1][2][i] == want[k]                      # the partition covers every pair once
+        assert int(part0[i].sum()) == got[0][2][i] and int(part1[i].sum()) == got[1][2][i]
+        assert min(got[0][2][i], got[1][2][i]) > 0.3 * want[k]             # and both ranks really worked
+    for rank in range(2):
+        np.testing.assert_array_equal(np.asarray(got[rank][3]), single)    # all-reduced sum == single process, on both ranks
+        np.testing.assert_array_equal(np.asarray(got[rank][4]), w1)
+    np.testing.assert_array_equal(part0 + part1, single)
+    o = oracle_all(D, R, e, oracle_threads)
+    for i, k in enumerate(KINDS):
+        assert_parity(single[i], o[k], want[k])
+    assert_w(w1, oracle.estimate(o["DD"].hist, o["DR"].hist, o["RR"].hist, ND, NR))
