@@ -45,6 +45,40 @@ def workload_name(idx: int, cfg, nd: int, nr: int) -> str:
             f"{cfg.theta_min}-{cfg.theta_max} deg, {total_pairs(nd, nr):.4g} pairs per step")
 
 
+class Workload:
+    """The catalogs, edges and names of one bench workload: BASELINE.json configs 1-5 (angular), or 6 = the 3-D variant of
+    the paper-scale case: 430k clustered + 430k uniform rows in a 1000-box, 40 log bins
+    in r from 1 to 200."""
+
+    def __init__(self, idx: int):
+        self.idx, self.spatial = idx, idx == 6
+        if self.spatial:
+            self.D, self.R, self.e = synth.make_box_config()
+            self.nbins, self.max_abs = len(self.e) - 1, 1000.0
+            self.name = (f"3-D variant (PAPER.md:18) of the paper-scale case: N_D={len(self.D)} clustered, N_R={len(self.R)} uniform rows "
+                         f"(x, y, z) in a 1000-box, 40 log bins in r 1-200, {total_pairs(len(self.D), len(self.R)):.4g} pairs per step")
+        else:
+            self.D, self.R, self.e, cfg = synth.make_config(idx)
+            self.nbins, self.max_abs = cfg.nbins, None
+            self.name = workload_name(idx, cfg, len(self.D), len(self.R))
+
+    def context(self, T):
+        return T.Context(self.nbins, self.e, "explicit", max_abs_coord=self.max_abs)
+
+    def oracle_rows(self, oracle, rows_per_hist: int, threads: int):
+        """(pairs, seconds) of the oracle on a seeded row subset of each of DD, DR, RR"""
+        if self.spatial:
+            d, r = self.D, self.R
+            cnt = lambda a, rows, b, ex: oracle.count_rows_xyz(a, rows, b, ex, self.e, threads=threads)
+        else:
+            d, r = oracle.radec_to_xyz(self.D), oracle.radec_to_xyz(self.R)
+            cnt = lambda a, rows, b, ex: oracle.count_rows(a, rows, b, ex, self.e, threads=threads)
+        rd, rr = synth.subset_rows(len(d), rows_per_hist, 777), synth.subset_rows(len(r), rows_per_hist, 778)
+        t0 = time.perf_counter()
+        tot = cnt(d, rd, d, True).total + cnt(d, rd, r, False).total + cnt(r, rr, r, True).total
+        return tot, time.perf_counter() - t0
+
+
 class ClockSampler:
     """nvidia-smi SM clock / throttle reasons every 200 ms while the timed region runs."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
@@ -107,18 +141,10 @@ def profile_summary(cfg_idx: int, engine: str = "fast"):
 
 
 # ------------------------------------------------------------------------------------------------ oracle legs
-def oracle_sample_rate(D, R, e, rows_per_hist: int, threads: int):
+def oracle_sample_rate(wl, rows_per_hist: int, threads: int):
     """Time the oracle (as it stands) on a seeded row subset of each of DD, DR, RR; returns (pairs, seconds)."""
     import oracle
-    d, r = oracle.radec_to_xyz(D), oracle.radec_to_xyz(R)
-    nd, nr = d.shape[0], r.shape[0]
-    rd, rr = synth.subset_rows(nd, rows_per_hist, 777), synth.subset_rows(nr, rows_per_hist, 778)
-    t0 = time.perf_counter()
-    a = oracle.count_rows(d, rd, d, True, e, threads=threads)
-    b = oracle.count_rows(d, rd, r, False, e, threads=threads)
-    c = oracle.count_rows(r, rr, r, True, e, threads=threads)
-    dt = time.perf_counter() - t0
-    return a.total + b.total + c.total, dt
+    return wl.oracle_rows(oracle, rows_per_hist, threads)
 
 
 def run_reference(args):
@@ -127,18 +153,18 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
-    D, R, e, cfg = synth.make_config(args.config)
-    nd, nr = D.shape[0], R.shape[0]
+    wl = Workload(args.config)
+    nd, nr = wl.D.shape[0], wl.R.shape[0]
     threads = oracle.host_threads()
-    pairs, dt = oracle_sample_rate(D, R, e, 16, threads)          # probe to size the sample
+    pairs, dt = oracle_sample_rate(wl, 16, threads)          # probe to size the sample
     rate = pairs / dt
     budget = 150.0 / (args.steps + args.warmup)                   # whole run within a few minutes
     rows = int(max(16, min(2000, rate * min(budget, 20.0) / (nd + nr + nr))))
     for _ in range(args.warmup):
-        oracle_sample_rate(D, R, e, rows, threads)
+        oracle_sample_rate(wl, rows, threads)
     t_tot, p_tot = 0.0, 0
     for _ in range(args.steps):
-        p, t = oracle_sample_rate(D, R, e, rows, threads)
+        p, t = oracle_sample_rate(wl, rows, threads)
         p_tot += p
         t_tot += t
     val = p_tot / t_tot / 1e9
@@ -146,7 +172,7 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * t_tot / args.steps, "higher_is_better": True, "scaling": "strong",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": workload_name(args.config, cfg, nd, nr), "sample": sample},
+            "config": {"workload": wl.name, "sample": sample},
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "full_workload_seconds_extrapolated": total_pairs(nd, nr) / (val * 1e9)}
@@ -172,16 +198,19 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
         print(f"[bench] rank {rank}/{world}: communicator of {dist.get_world_size()} ranks, backend {dist.get_backend()}, "
               f"device cuda:{local}", file=sys.stderr, flush=True)
-    D, R, e, cfg = synth.make_config(args.config)
+    wl = Workload(args.config)
+    D, R, e = wl.D, wl.R, wl.e
     nd, nr = D.shape[0], R.shape[0]
     pairs_step = total_pairs(nd, nr)
-    nb = cfg.nbins
+    nb = wl.nbins
 
     st = torch.cuda.Stream()
-    ctx = T.Context(nb, e, "explicit")
+    ctx = wl.context(T)
     ctx.set_stream(st.cuda_stream)
     if args.engine != "default":
         ctx.set_engine(args.engine)
+    if args.pruning:
+        ctx.set_pruning(True)
     ctx.load("D", D, stream=st.cuda_stream)
     ctx.load("R", R, stream=st.cuda_stream)
     tdist.apply_partition(ctx)
@@ -233,7 +262,7 @@ def run_ours(args):
 
     # the other engine on the same resident catalogs, a few steps, for the record (its histograms must be the same integers)
     other = None
-    if world == 1 and args.engine in ("default", "tensor"):
+    if world == 1 and args.engine in ("default", "tensor") and not args.pruning:
         ctx.set_engine("fast")
         out2 = torch.zeros_like(out)
         def step2():
@@ -327,17 +356,19 @@ def run_ours(args):
     if world == 1 and not args.no_cpu_baseline:
         import oracle
         threads = oracle.host_threads()
-        p0, t0_ = oracle_sample_rate(D, R, e, 16, threads)
+        p0, t0_ = oracle_sample_rate(wl, 16, threads)
         rows = int(max(16, min(2000, (p0 / t0_) * 15.0 / (nd + nr + nr))))
-        p1, t1_ = oracle_sample_rate(D, R, e, rows, threads)
+        p1, t1_ = oracle_sample_rate(wl, rows, threads)
         cpu = {"value": p1 / t1_ / 1e9, "unit": UNIT, "cores": threads, "kind": "oracle",
                "sample": f"{rows} seeded rows of each of DD, DR, RR against all j = {p1:.4g} pairs in {t1_:.1f} s",
                "full_workload_seconds_extrapolated": pairs_step / (p1 / t1_)}
 
-    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+    metric = METRIC if not args.pruning else \
+        "pairs COUNTED/sec (DD+DR+RR) in pruning mode: blocks without a bin edge in reach are added wholesale, NOT evaluated (SURVEY.md NEXT-3); not BASELINE.json's metric"
+    line = {"metric": metric, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f32",
             "data": "synthetic",
-            "config": {"workload": workload_name(args.config, cfg, nd, nr),
+            "config": {"workload": wl.name,
                        "l2": "256 MiB write between steps (inside the timed region); catalogs (28 MB each) are L2-resident by design",
                        "engine": ("tensor (window quantity by 3xTF32 tcgen05.mma into TMEM + tcgen05.ld read-back; guard bands, cell lookup and "
                                   "fp64 recheck as in the fast engine)" if tensor_ran else
@@ -347,7 +378,7 @@ def run_ours(args):
             "seconds_per_w_theta": ms_step * 1e-3,
             "e2e": {"value": pairs_step / e2e_s / 1e9, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "seconds_per_step": e2e_s, "steps": e2e_steps,
-                    "path": "tpcf_load(D), tpcf_load(R) from pinned host rows + tpcf_count x3 + tpcf_estimate"},
+                    "path": ("tpcf_load_xyz" if wl.spatial else "tpcf_load") + "(D), (R) from pinned host rows + tpcf_count x3 + tpcf_estimate"},
             "gpu_launches": args.steps * 6,
             "gpu_launches_note": f"per step: 3 x ({'pair_tensor_kernel' if tensor_ran else 'pair_fast_kernel'} + finalize_kernel); memsets are driver memset nodes; the e2e leg adds 2 x 29 load kernels per step",
             "other_engine": other,
@@ -363,9 +394,12 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4, 5, 6],
+                    help="BASELINE.json configs 1-5; 6 = the 3-D variant (Cartesian rows, bins in r) of the paper-scale case")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--pruning", action="store_true",
+                    help="time the separately named pruning mode (tpcf_set_pruning; not the brute-force count, not the headline)")
     ap.add_argument("--engine", default="default", choices=["default", "tensor", "fast"],
                     help="pair kernel family (include/tpcf.h tpcf_engine); default = the library's default (tensor); both give the same histograms")
     args = ap.parse_args()

@@ -132,6 +132,30 @@ tpcf_status tpcf_estimate(tpcf_ctx* ctx, double* w_out /* nbins */);
 tpcf_status tpcf_estimate_from(const uint64_t* dd, const uint64_t* dr, const uint64_t* rr, int nbins, uint64_t n_d,
                                uint64_t n_r, double* w_out /* nbins */);
 
+/*
+ * 3-D variant (Section 2: "our results are extendible to the 3-dimensional variant as well"): the same three
+ * histograms DD, DR, RR over the Euclidean separation r = |a - b| of Cartesian positions, and the same estimator on
+ * them (the spatial two-point function xi(r)).  Everything else -- tpcf_count, tpcf_count_async, tpcf_estimate, the
+ * controls, row-subset mode -- is shared with the angular contexts.
+ *
+ * tpcf_create_r -- fix the separation binning: r_edges as theta_deg in tpcf_create (LINEAR / LOG: {min, max}, min >= 0,
+ *   LOG: min > 0; EXPLICIT: nbins+1 strictly increasing values >= 0), in the units of the coordinates.  Bin k =
+ *   [e_k, e_{k+1}) in r, last bin closed, under = r < e_0, over = r > e_n.
+ *   max_abs_coord: a bound the caller guarantees for |x|, |y|, |z| of every row of both catalogs (> 0).  Positions are
+ *   multiplied by the power of two that brings them inside the unit ball (exact in binary floating point) and bins are
+ *   compared in squared separation, (e_k * scale)^2, so the fp64 engine's decision differs from sqrt(dx^2+dy^2+dz^2)
+ *   against e_k only for pairs within fp64 rounding of an edge.  e_n may not exceed the largest separation the bound
+ *   allows (2 / scale >= 2 sqrt(3) max_abs_coord): TPCF_EINVAL, as for any other violated condition.
+ * tpcf_load_xyz -- load catalog D or R: n rows of (x, y, z), row-major n x 3, dtype F32 or F64, host or device memory
+ *   as in tpcf_load.  The rows are sorted along a 3-D Hilbert curve and stored as fp32 offsets from group centres
+ *   exactly as the angular rows are (DESIGN.md section 4 uses nothing of the unit sphere but d^2 <= 4).
+ *   Errors: TPCF_ESTATE on a context made by tpcf_create (and tpcf_load on one made by tpcf_create_r); TPCF_EINVAL for
+ *   n == 0, n > 2^31-1, a non-finite coordinate or one beyond max_abs_coord; TPCF_ENOMEM; TPCF_ECUDA.
+ */
+tpcf_status tpcf_create_r(tpcf_ctx** out, int nbins, const double* r_edges, tpcf_binning mode, double max_abs_coord);
+tpcf_status tpcf_load_xyz(tpcf_ctx* ctx, tpcf_cat which, const void* xyz, tpcf_dtype dt, size_t n, int on_device,
+                          void* cuda_stream);
+
 void tpcf_destroy(tpcf_ctx* ctx);
 const char* tpcf_last_error(const tpcf_ctx* ctx);
 
@@ -151,6 +175,13 @@ tpcf_status tpcf_set_guard_scale(tpcf_ctx* ctx, double scale);
  * when off, each pair goes through the cell lookup.  Every pair is evaluated either way; the histograms are identical
  * (tests). */
 tpcf_status tpcf_set_window(tpcf_ctx* ctx, int enabled);
+/* Pruning mode, off by default (PAPER.md:29-31 k-trees, "coding the k-trees" as future
+ * work).  On: a (256 i-rows, 64 j-rows) block none of whose 32 (8-row group, subtile) windows reaches a bin edge is added
+ * to the histogram wholesale -- its pairs are NOT evaluated.  The histograms are the same integers (the windows bound
+ * every true separation, tests), but this is the dual-tree idea at block granularity, not the brute-force count the
+ * paper and BASELINE.json's metric are about: "pair evaluations per second" loses its meaning, so bench.py reports it as
+ * a separate line (--pruning) and never as the headline.  Runs the FFMA2 kernel whatever the engine. */
+tpcf_status tpcf_set_pruning(tpcf_ctx* ctx, int enabled);
 /* Work partition for multi-process runs (one process per GPU): this context enumerates only the tile
  * work items w with w % nparts == part; summing the histograms of all parts gives the full count
  * (integer, order-independent).  Default (0, 1). */
@@ -175,6 +206,11 @@ typedef struct {
                                 counted by the 1-, 2-, 3-edge window loops, by the per-pair cell lookup; [4] = lanes of
                                 window blocks recounted pair by pair because a pair came within a guard band;
                                 [5] = blocks classified wholly in fp64 (bounding radii too large for the fp32 bound) */
+    uint64_t pruned_blocks;  /* pruning mode: (warp, subtile) blocks added wholesale by the last synchronous count */
+    float lookup_share;      /* TPCF_ENGINE_TENSOR: estimated share of the pairs in blocks the tensor kernel would count pair by
+                                pair (near blocks, more than 3 edges in reach); above 0.04 the engine launches the FFMA2 kernel */
+    float tile_radius, extent;  /* what that estimate used: median bounding radius of the j catalog's 128-row tiles and the
+                                larger extent of the two catalogs (chords of the unit sphere / scaled lengths) */
 } tpcf_stats;
 tpcf_status tpcf_get_stats(const tpcf_ctx* ctx, tpcf_stats* out);
 
@@ -206,6 +242,11 @@ tpcf_status tpcf_window_host(const tpcf_ctx* ctx, float lo2, float hi2, int* fir
  * 3xTF32 tcgen05.mma of pair_tensor_kernel forms it (same operand split, same instruction, same read-back).  What the tests
  * measure the tensor core's accumulation error with.  TPCF_EINVAL for NULL pointers or ntiles == 0 or > 65535. */
 tpcf_status tpcf_tensor_probe(tpcf_ctx* ctx, const float* s_rows, const float* b_rows, size_t ntiles, float* q_out);
+
+/* The estimate behind TPCF_ENGINE_TENSOR's choice of kernel (tpcf_stats.lookup_share): share of the pairs in blocks the
+ * tensor kernel would count pair by pair, for typical bounding radii summing to r and catalogs of extent `extent` (both
+ * as chords of the unit sphere, or scaled lengths in a 3-D context). */
+tpcf_status tpcf_lookup_share(const tpcf_ctx* ctx, double r, double extent, double* share_out);
 
 /* Number of tile work items of a full count of `kind` for catalog sizes (n_d, n_r), and the number of
  * pairs in item w: the partition arithmetic of tpcf_set_partition, testable without a GPU. */

@@ -32,7 +32,7 @@ EXPORTS = (
     "tpcf_estimate_from", "tpcf_destroy", "tpcf_last_error", "tpcf_set_stream", "tpcf_set_engine",
     "tpcf_set_guard_scale", "tpcf_set_partition", "tpcf_get_stats", "tpcf_get_thresholds", "tpcf_classify_fast",
     "tpcf_plan", "tpcf_plan_item_pairs", "tpcf_set_kernel_timing", "tpcf_get_kernel_times", "tpcf_set_window",
-    "tpcf_get_bands", "tpcf_window_host", "tpcf_tensor_probe",
+    "tpcf_get_bands", "tpcf_window_host", "tpcf_tensor_probe", "tpcf_create_r", "tpcf_load_xyz", "tpcf_lookup_share", "tpcf_set_pruning",
 )
 
 
@@ -46,7 +46,8 @@ class tpcf_stats(ctypes.Structure):
     _fields_ = [("pairs", ctypes.c_uint64), ("rechecked", ctypes.c_uint64), ("work_items", ctypes.c_uint64),
                 ("launches", ctypes.c_int), ("grid", ctypes.c_int), ("block", ctypes.c_int),
                 ("smem_bytes", ctypes.c_int), ("cells", ctypes.c_int), ("cell_bits", ctypes.c_int),
-                ("hist_copies", ctypes.c_int), ("kernel_ms", ctypes.c_float), ("win_blocks", ctypes.c_uint64 * 6)]
+                ("hist_copies", ctypes.c_int), ("kernel_ms", ctypes.c_float), ("win_blocks", ctypes.c_uint64 * 6),
+                ("pruned_blocks", ctypes.c_uint64), ("lookup_share", ctypes.c_float), ("tile_radius", ctypes.c_float), ("extent", ctypes.c_float)]
 
     def as_dict(self):
         d = {k: getattr(self, k) for k, _ in self._fields_}
@@ -68,6 +69,8 @@ def lib() -> ctypes.CDLL:
         vp, i32, sz, u64, dbl = ctypes.c_void_p, ctypes.c_int, ctypes.c_size_t, ctypes.c_uint64, ctypes.c_double
         sig = {
             "tpcf_create": [ctypes.POINTER(vp), i32, vp, i32],
+            "tpcf_create_r": [ctypes.POINTER(vp), i32, vp, i32, dbl],
+            "tpcf_load_xyz": [vp, i32, vp, i32, sz, i32, vp],
             "tpcf_get_edges": [vp, vp],
             "tpcf_load": [vp, i32, vp, i32, sz, i32, vp],
             "tpcf_count": [vp, i32, vp, vp, vp, sz],
@@ -78,6 +81,7 @@ def lib() -> ctypes.CDLL:
             "tpcf_set_engine": [vp, i32],
             "tpcf_set_guard_scale": [vp, dbl],
             "tpcf_set_window": [vp, i32],
+            "tpcf_set_pruning": [vp, i32],
             "tpcf_get_bands": [vp, i32, vp, vp, vp, ctypes.POINTER(i32)],
             "tpcf_window_host": [vp, ctypes.c_float, ctypes.c_float, ctypes.POINTER(i32), ctypes.POINTER(i32)],
             "tpcf_tensor_probe": [vp, vp, vp, ctypes.c_size_t, vp],
@@ -87,6 +91,7 @@ def lib() -> ctypes.CDLL:
             "tpcf_get_kernel_times": [vp, vp, i32, ctypes.POINTER(i32)],
             "tpcf_get_thresholds": [vp, vp],
             "tpcf_classify_fast": [vp, ctypes.c_float, ctypes.POINTER(i32)],
+            "tpcf_lookup_share": [vp, dbl, dbl, ctypes.POINTER(dbl)],
             "tpcf_plan": [vp, i32, u64, u64, ctypes.POINTER(u64)],
             "tpcf_plan_item_pairs": [vp, i32, u64, u64, u64, ctypes.POINTER(u64)],
         }
@@ -130,6 +135,19 @@ def tpcf_create(nbins: int, theta_deg, mode) -> ctypes.c_void_p:
     return ctx
 
 
+def tpcf_create_r(nbins: int, r_edges, mode, max_abs_coord: float) -> ctypes.c_void_p:
+    mode = _MODES.get(mode, mode)
+    e = np.ascontiguousarray(r_edges, dtype=np.float64)
+    need = nbins + 1 if mode == TPCF_EXPLICIT else 2
+    if e.ndim != 1 or e.shape[0] != need:
+        raise TpcfError(TPCF_EINVAL, f"r_edges must hold {need} values")
+    ctx = ctypes.c_void_p()
+    st = lib().tpcf_create_r(ctypes.byref(ctx), int(nbins), _np_ptr(e), int(mode), float(max_abs_coord))
+    if st != TPCF_OK:
+        raise TpcfError(st, "tpcf_create_r rejected the binning")
+    return ctx
+
+
 def tpcf_destroy(ctx) -> None:
     lib().tpcf_destroy(ctx)
 
@@ -146,12 +164,17 @@ def tpcf_get_thresholds(ctx, nbins: int) -> np.ndarray:
     return t
 
 
-def tpcf_load(ctx, which: int, radec_deg, stream: int = 0) -> int:
+def tpcf_load_xyz(ctx, which: int, xyz, stream: int = 0) -> int:
+    """xyz: (n, 3) float32/float64 numpy array, CPU torch tensor (pinned or not) or CUDA torch tensor."""
+    return tpcf_load(ctx, which, xyz, stream, cols=3)
+
+
+def tpcf_load(ctx, which: int, radec_deg, stream: int = 0, cols: int = 2) -> int:
     """radec_deg: (n, 2) float32/float64 numpy array, CPU torch tensor (pinned or not) or CUDA torch tensor."""
     if _is_torch(radec_deg):
         t = radec_deg
-        if t.dim() != 2 or t.shape[1] != 2 or not t.is_contiguous():
-            raise TpcfError(TPCF_EINVAL, "catalog must be a contiguous (n, 2) tensor")
+        if t.dim() != 2 or t.shape[1] != cols or not t.is_contiguous():
+            raise TpcfError(TPCF_EINVAL, f"catalog must be a contiguous (n, {cols}) tensor")
         dt = {"torch.float32": TPCF_F32, "torch.float64": TPCF_F64}.get(str(t.dtype))
         if dt is None:
             raise TpcfError(TPCF_EINVAL, "catalog dtype must be float32 or float64")
@@ -162,11 +185,12 @@ def tpcf_load(ctx, which: int, radec_deg, stream: int = 0) -> int:
         if a.dtype not in (np.float32, np.float64):
             raise TpcfError(TPCF_EINVAL, "catalog dtype must be float32 or float64")
         a = np.ascontiguousarray(a)
-        if a.ndim != 2 or a.shape[1] != 2:
-            raise TpcfError(TPCF_EINVAL, "catalog must be an (n, 2) array")
+        if a.ndim != 2 or a.shape[1] != cols:
+            raise TpcfError(TPCF_EINVAL, f"catalog must be an (n, {cols}) array")
         dt = TPCF_F32 if a.dtype == np.float32 else TPCF_F64
         n, ptr, on_dev, keep = a.shape[0], _np_ptr(a), 0, a
-    _check(ctx, lib().tpcf_load(ctx, int(which), ptr, dt, n, on_dev, ctypes.c_void_p(stream)))
+    fn = lib().tpcf_load_xyz if cols == 3 else lib().tpcf_load
+    _check(ctx, fn(ctx, int(which), ptr, dt, n, on_dev, ctypes.c_void_p(stream)))
     del keep
     return n
 
@@ -218,6 +242,10 @@ def tpcf_set_guard_scale(ctx, scale: float) -> None:
 
 def tpcf_set_window(ctx, enabled: bool) -> None:
     _check(ctx, lib().tpcf_set_window(ctx, int(bool(enabled))))
+
+
+def tpcf_set_pruning(ctx, enabled: bool) -> None:
+    _check(ctx, lib().tpcf_set_pruning(ctx, int(bool(enabled))))
 
 
 def tpcf_get_bands(ctx):
@@ -275,6 +303,12 @@ def tpcf_classify_fast(ctx, d2: float) -> int:
     return out.value
 
 
+def tpcf_lookup_share(ctx, r: float, extent: float) -> float:
+    out = ctypes.c_double()
+    _check(ctx, lib().tpcf_lookup_share(ctx, float(r), float(extent), ctypes.byref(out)))
+    return out.value
+
+
 def tpcf_plan(ctx, kind: int, n_d: int, n_r: int) -> int:
     out = ctypes.c_uint64()
     _check(ctx, lib().tpcf_plan(ctx, int(kind), int(n_d), int(n_r), ctypes.byref(out)))
@@ -290,9 +324,11 @@ def tpcf_plan_item_pairs(ctx, kind: int, n_d: int, n_r: int, w: int) -> int:
 class Context:
     """Owns one tpcf_ctx.  Convenience wrapper over the functions above; holds no arithmetic."""
 
-    def __init__(self, nbins: int, theta_deg, mode="explicit"):
+    def __init__(self, nbins: int, theta_deg, mode="explicit", max_abs_coord: Optional[float] = None):
+        """Angular context (tpcf_create); with max_abs_coord a 3-D context (tpcf_create_r: theta_deg holds r edges)."""
         self.nbins = int(nbins)
-        self._ctx = tpcf_create(nbins, theta_deg, mode)
+        self.spatial = max_abs_coord is not None
+        self._ctx = tpcf_create_r(nbins, theta_deg, mode, max_abs_coord) if self.spatial else tpcf_create(nbins, theta_deg, mode)
         self.n = {TPCF_D: 0, TPCF_R: 0}
 
     def close(self):
@@ -320,7 +356,7 @@ class Context:
 
     def load(self, which, radec_deg, stream: int = 0):
         which = {"D": TPCF_D, "R": TPCF_R}.get(which, which)
-        self.n[which] = tpcf_load(self._ctx, which, radec_deg, stream)
+        self.n[which] = tpcf_load(self._ctx, which, radec_deg, stream, cols=3 if self.spatial else 2)
 
     def count(self, kind, rows=None):
         return tpcf_count(self._ctx, _KINDS.get(kind, kind), self.nbins, rows)
@@ -346,6 +382,9 @@ class Context:
 
     def set_window(self, enabled: bool):
         tpcf_set_window(self._ctx, enabled)
+
+    def set_pruning(self, enabled: bool):
+        tpcf_set_pruning(self._ctx, enabled)
 
     def bands(self):
         return tpcf_get_bands(self._ctx)

@@ -1,6 +1,7 @@
 // api.cu -- the C ABI of libtpcf (include/tpcf.h): context, argument checking, device memory, launches.
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -23,6 +24,7 @@ struct Catalog {                 // rows in Hilbert order (counts are order-inva
     float4 *xs = nullptr, *cs = nullptr;   // j-side role: rows as (-2 offset, |offset|^2) from their 64-row subtile centre
     float4 *xt = nullptr, *ct = nullptr;   // j-side role of the tensor engine: the same for 128-row tiles
     float* xb = nullptr;                   // ... and per tile a 128 x 16 TF32 operand block (kernels.cuh)
+    double r_tile = 0.0, extent = 0.0;     // typical bounding radius of a 128-row tile and extent of the catalog (chord units)
 };
 // scratch of one spatial sort: (key, idx) ping-pong buffers and the digit counts
 struct SortScratch {
@@ -47,6 +49,7 @@ struct tpcf_ctx {
     bool tables_dirty = true;
     tpcf_engine engine = TPCF_ENGINE_TENSOR;
     bool window = true;
+    bool prune = false;
     cudaStream_t stream = nullptr;
     int part = 0, nparts = 1;
     Catalog cat[2];
@@ -340,6 +343,7 @@ tpcf_status enqueue_count(tpcf_ctx* ctx, tpcf_kind kind, const int64_t* rows_hos
     p.lut = ctx->d_lut;
     p.slotmap = ctx->d_slotmap;
     p.window = (ctx->window && ctx->ft.nbands >= 1) ? 1 : 0;
+    p.prune = (ctx->prune && p.window) ? 1 : 0;
     p.band_mh = ctx->d_band_mh;
     p.band_lh = ctx->d_band_lh;
     p.band_slot = ctx->d_band_slot;
@@ -371,7 +375,20 @@ tpcf_status enqueue_count(tpcf_ctx* ctx, tpcf_kind kind, const int64_t* rows_hos
         CU(cudaEventRecord(kev.first, st), "cudaEventRecord");
     }
     {
-        const cudaError_t le = ctx->engine == TPCF_ENGINE_FAST     ? launch_pairs_fast(p, ctx->ft.map, ctx->sm_count, st, &li)
+        // TPCF_ENGINE_TENSOR runs the FFMA2 kernel where too many pairs would take the tensor kernel's slow rows
+        // (fine binnings, catalogs whose tiles are large against the scales binned: tables.h lookup_pair_share)
+        bool tensor_kernel = ctx->engine == TPCF_ENGINE_TENSOR && !p.prune;      // pruning lives in the FFMA2 kernel
+        if (tensor_kernel) {
+            const int dim = ctx->bin.spatial ? 3 : 2;
+            const double r = cj.r_tile * (1.0 + std::pow((double)kIPerThread / kTcSubJ, 1.0 / dim));     // tile + 8-row group
+            ctx->stats.lookup_share = (float)lookup_pair_share(ctx->bin, r, std::max(ci.extent, cj.extent), dim);
+            ctx->stats.tile_radius = (float)cj.r_tile;
+            ctx->stats.extent = (float)std::max(ci.extent, cj.extent);
+            tensor_kernel = ctx->stats.lookup_share <= 0.04f;
+        }
+        if (ctx->engine == TPCF_ENGINE_EXACT64) p.prune = 0;
+        const cudaError_t le = ctx->engine == TPCF_ENGINE_FAST || (ctx->engine == TPCF_ENGINE_TENSOR && !tensor_kernel)
+                                   ? launch_pairs_fast(p, ctx->ft.map, ctx->sm_count, st, &li)
                                : ctx->engine == TPCF_ENGINE_TENSOR ? launch_pairs_tensor(p, ctx->ft.map, ctx->sm_count, st, &li)
                                                                    : launch_pairs_exact64(p, ctx->sm_count, st, &li);
         if (le != cudaSuccess) {
@@ -430,6 +447,27 @@ tpcf_status tpcf_create(tpcf_ctx** out, int nbins, const double* theta_deg, tpcf
     return TPCF_OK;
 }
 
+tpcf_status tpcf_create_r(tpcf_ctx** out, int nbins, const double* r_edges, tpcf_binning mode, double max_abs_coord) {
+    if (!out) return TPCF_EINVAL;
+    *out = nullptr;
+    tpcf_ctx* ctx = new (std::nothrow) tpcf_ctx();
+    if (!ctx) return TPCF_ENOMEM;
+    std::string why;
+    try {
+        why = make_binning_r(nbins, r_edges, (int)mode, max_abs_coord, ctx->bin);
+        if (why.empty()) rebuild_tables(ctx);
+    } catch (const std::bad_alloc&) {
+        delete ctx;
+        return TPCF_ENOMEM;
+    }
+    if (!why.empty()) {
+        delete ctx;
+        return TPCF_EINVAL;
+    }
+    *out = ctx;
+    return TPCF_OK;
+}
+
 tpcf_status tpcf_get_edges(const tpcf_ctx* ctx, double* edges_out) {
     if (!ctx || !edges_out) return TPCF_EINVAL;
     std::memcpy(edges_out, ctx->bin.edges.data(), ctx->bin.edges.size() * sizeof(double));
@@ -442,9 +480,12 @@ tpcf_status tpcf_get_thresholds(const tpcf_ctx* ctx, double* t_out) {
     return TPCF_OK;
 }
 
-tpcf_status tpcf_load(tpcf_ctx* ctx, tpcf_cat which, const void* radec_deg, tpcf_dtype dt, size_t n, int on_device,
-                      void* cuda_stream) {
+static tpcf_status load_catalog(tpcf_ctx* ctx, tpcf_cat which, const void* radec_deg, tpcf_dtype dt, size_t n, int on_device,
+                                void* cuda_stream, bool spatial) {
     if (!ctx) return TPCF_EINVAL;
+    if (ctx->bin.spatial != spatial)
+        return fail(ctx, TPCF_ESTATE, spatial ? "tpcf_load_xyz needs a context made by tpcf_create_r" : "tpcf_load needs a context made by tpcf_create");
+    const int cols = spatial ? 3 : 2;       // values per row
     if (which != TPCF_D && which != TPCF_R) return fail(ctx, TPCF_EINVAL, "which must be TPCF_D or TPCF_R");
     if (dt != TPCF_F32 && dt != TPCF_F64) return fail(ctx, TPCF_EINVAL, "dtype must be TPCF_F32 or TPCF_F64");
     if (!radec_deg || n == 0) return fail(ctx, TPCF_EINVAL, "empty catalog");
@@ -480,7 +521,7 @@ tpcf_status tpcf_load(tpcf_ctx* ctx, tpcf_cat which, const void* radec_deg, tpcf
     }
     const uint64_t nblk = (n + kSortChunk - 1) / kSortChunk;
     const size_t need = n * sizeof(double4) + 2 * n * sizeof(uint64_t) + 2 * n * sizeof(uint32_t) + 256 * nblk * sizeof(uint32_t) +
-                        (on_device ? 0 : n * 2 * esz) + 8 * 256;
+                        (on_device ? 0 : n * cols * esz) + 8 * 256;
     s = arena_reserve(ctx, need);
     if (s) { free_catalog(c); return s; }
     Carver cv{static_cast<char*>(ctx->arena)};
@@ -494,14 +535,16 @@ tpcf_status tpcf_load(tpcf_ctx* ctx, tpcf_cat which, const void* radec_deg, tpcf
     cudaError_t e = cudaSuccess;
     const void* src = radec_deg;
     if (!on_device) {
-        void* staged = cv.take<char>(n * 2 * esz);
-        e = cudaMemcpyAsync(staged, radec_deg, n * 2 * esz, cudaMemcpyHostToDevice, st);
+        void* staged = cv.take<char>(n * cols * esz);
+        e = cudaMemcpyAsync(staged, radec_deg, n * cols * esz, cudaMemcpyHostToDevice, st);
         if (e != cudaSuccess) { free_catalog(c); return cuda_fail(ctx, e, "copy catalog to device"); }
         src = staged;
     }
     // convert (fp64 unit vectors + sort keys) -> sort -> sorted fp64 rows + row map -> quad and subtile roles
     e = cudaMemsetAsync(ctx->d_bad, 0, sizeof(int), st);
-    if (e == cudaSuccess) e = launch_convert(src, dt == TPCF_F64, n, rows64, sc.ka, sc.ia, ctx->d_bad, st);
+    if (e == cudaSuccess)
+        e = spatial ? launch_convert_xyz(src, dt == TPCF_F64, n, ctx->bin.scale, ctx->bin.max_abs, rows64, sc.ka, sc.ia, ctx->d_bad, st)
+                    : launch_convert(src, dt == TPCF_F64, n, rows64, sc.ka, sc.ia, ctx->d_bad, st);
     bool in_a = true;
     if (e == cudaSuccess) e = launch_sort_pairs(sc.ka, sc.kb, sc.ia, sc.ib, sc.counts, (uint32_t)n, 63, st, &in_a);
     if (e == cudaSuccess) e = launch_permute(rows64, in_a ? sc.ia : sc.ib, n, n_pad, c.x64, c.inv, st);
@@ -516,11 +559,44 @@ tpcf_status tpcf_load(tpcf_ctx* ctx, tpcf_cat which, const void* radec_deg, tpcf
     }
     if (bad) {
         free_catalog(c);
-        return fail(ctx, TPCF_EINVAL, "catalog has a non-finite value, |RA| > 1e6 or |Dec| > 90");
+        return fail(ctx, TPCF_EINVAL, spatial ? "catalog has a non-finite coordinate or one beyond max_abs_coord"
+                                              : "catalog has a non-finite value, |RA| > 1e6 or |Dec| > 90");
     }
     c.n = n;
     c.n_pad = n_pad;
+    {   // typical tile radius and extent of the catalog, from the 128-row tiles' bounding spheres (choice of the pair
+        // kernel under TPCF_ENGINE_TENSOR; a heuristic: it never changes a count)
+        const size_t nt = n_pad / kTcSubJ;
+        std::vector<float4> ct(nt);
+        CU(cudaMemcpyAsync(ct.data(), c.ct, nt * sizeof(float4), cudaMemcpyDeviceToHost, st), "copy tile spheres");
+        CU(cudaStreamSynchronize(st), "copy tile spheres");
+        std::vector<float> rad;
+        double mx = 0, my = 0, mz = 0;
+        auto real = [](const float4& t) {               // not a tile of padding rows (centre (2,2,2)) or one that holds some
+            return t.w <= 1.0f && t.x * t.x + t.y * t.y + t.z * t.z <= 1.05f;
+        };
+        for (const float4& t : ct)
+            if (real(t)) { rad.push_back(t.w); mx += t.x; my += t.y; mz += t.z; }
+        c.r_tile = 0.0;
+        c.extent = 0.0;
+        if (!rad.empty()) {
+            std::nth_element(rad.begin(), rad.begin() + rad.size() / 2, rad.end());
+            c.r_tile = rad[rad.size() / 2];
+            mx /= rad.size(); my /= rad.size(); mz /= rad.size();
+            for (const float4& t : ct)
+                if (real(t)) c.extent = std::max(c.extent, std::sqrt((t.x - mx) * (t.x - mx) + (t.y - my) * (t.y - my) + (t.z - mz) * (t.z - mz)) + t.w);
+        }
+    }
     return TPCF_OK;
+}
+
+tpcf_status tpcf_load(tpcf_ctx* ctx, tpcf_cat which, const void* radec_deg, tpcf_dtype dt, size_t n, int on_device,
+                      void* cuda_stream) {
+    return load_catalog(ctx, which, radec_deg, dt, n, on_device, cuda_stream, false);
+}
+
+tpcf_status tpcf_load_xyz(tpcf_ctx* ctx, tpcf_cat which, const void* xyz, tpcf_dtype dt, size_t n, int on_device, void* cuda_stream) {
+    return load_catalog(ctx, which, xyz, dt, n, on_device, cuda_stream, true);
 }
 
 tpcf_status tpcf_count(tpcf_ctx* ctx, tpcf_kind kind, uint64_t* hist_out, uint64_t* under_over_out, const int64_t* rows,
@@ -557,6 +633,7 @@ tpcf_status tpcf_count(tpcf_ctx* ctx, tpcf_kind kind, uint64_t* hist_out, uint64
     // pair_fast_kernel (also when the tensor engine falls back to it) executes every plan item as kWarpsPerCta warp items
     ctx->stats.work_items = ctr[2] / ctx->warp_items_per_item;
     for (int k = 0; k < 6; ++k) ctx->stats.win_blocks[k] = ctr[3 + k];
+    ctx->stats.pruned_blocks = ctr[9];
     for (int k = 0; k < nb; ++k) hist_out[k] = host[k + 1];
     if (under_over_out) {
         under_over_out[0] = host[0];
@@ -643,6 +720,12 @@ tpcf_status tpcf_set_engine(tpcf_ctx* ctx, tpcf_engine e) {
 tpcf_status tpcf_set_window(tpcf_ctx* ctx, int enabled) {
     if (!ctx) return TPCF_EINVAL;
     ctx->window = enabled != 0;
+    return TPCF_OK;
+}
+
+tpcf_status tpcf_set_pruning(tpcf_ctx* ctx, int enabled) {
+    if (!ctx) return TPCF_EINVAL;
+    ctx->prune = enabled != 0;
     return TPCF_OK;
 }
 
@@ -738,6 +821,12 @@ tpcf_status tpcf_get_bands(const tpcf_ctx* ctx, int capacity, float* lo_out, flo
         if (hi_out) hi_out[b] = t.band_hi[b];
         if (slot_below_out) slot_below_out[b] = t.band_slot[b];
     }
+    return TPCF_OK;
+}
+
+tpcf_status tpcf_lookup_share(const tpcf_ctx* ctx, double r, double extent, double* share_out) {
+    if (!ctx || !share_out || !(r >= 0.0) || !(extent >= 0.0)) return TPCF_EINVAL;
+    *share_out = lookup_pair_share(ctx->bin, r, extent, ctx->bin.spatial ? 3 : 2);
     return TPCF_OK;
 }
 

@@ -393,11 +393,11 @@ struct WinTables {
 // Every lane chooses the cheapest loop that is valid for its block; the warp runs the most general of them.
 //   1..3  window loop with that many edges      4  cell lookup      5  fp64
 template <int MAP>
-__device__ __forceinline__ void subtile_pairs(const float4* __restrict__ js, const float4 sp, bool windows, bool mask,
+__device__ __forceinline__ void subtile_pairs(const float4* __restrict__ js, const float4 sp, bool windows, bool prune, bool mask,
                                               const f32x2 (&px2)[R / 2], const f32x2 (&py2)[R / 2], const f32x2 (&pz2)[R / 2], float cqx,
                                               float cqy, float cqz, float ri, const WinTables& wt, const Lookup& lk,
                                               SlowCtx* slow, uint2* rq, unsigned& qn, uint32_t i0, uint32_t n_i,
-                                              uint32_t j0, uint32_t n_j, unsigned (&npath)[6]) {
+                                              uint32_t j0, uint32_t n_j, unsigned (&npath)[7]) {
     const int lane = threadIdx.x & 31;
     // bounds on every TRUE chord of the block from the triangle inequality: |cq - cs| -/+ (ri + rj), made safe
     // against the fp32 evaluation (relative 4e-6 on the centre distance, 1e-7 absolute)
@@ -423,6 +423,17 @@ __device__ __forceinline__ void subtile_pairs(const float4* __restrict__ js, con
         // fine binnings: when the bands fill so much of the window that one of the block's kSubJ x R pairs is likely to
         // fall inside one (chords spread evenly over the window), the window loop would only be followed by a recount
         if (k < wt.nbands && (float)(2 * kSubJ * R) * (float)e * wt.band_mh[k].y > kMaxFlagExpect * (hi2 - lo2)) mode = 4;
+    }
+    // Pruning mode (tpcf_set_pruning: the dual-tree idea of PAPER.md:29 at block granularity; NOT the
+    // brute-force count): when no lane's window reaches a band, every pair of a lane's block lies in one result slot and
+    // the kSubJ x R pairs are added wholesale, unevaluated.
+    if (prune) {
+        const bool empty = mode == 1 && (k >= wt.nbands || wt.band_lh[k].x > __fmul_ru(hi, hi));
+        if (__all_sync(0xffffffffu, empty)) {
+            atomicAdd(wt.whist + wt.band_slot[min(k, wt.nbands)], (unsigned)(kSubJ * R));
+            ++npath[6];
+            return;
+        }
     }
     // A few lanes that need the cell lookup (or fp64) do not drag the whole warp into lookup_block: the warp runs the
     // window loop of the other lanes, those lanes' counters are dropped and their pairs are recounted by the whole
@@ -674,7 +685,7 @@ __global__ void __launch_bounds__(kThreads, 2) pair_fast_kernel(const __grid_con
     unsigned qn = 0;                        // fill level of this warp's recheck queue
     uint32_t g = 0;                         // chunks this warp consumed so far: selects ring slot and mbarrier parity
     unsigned long long pairs_since_flush = 0, witems_done = 0;
-    unsigned npath[6] = {0, 0, 0, 0, 0, 0};
+    unsigned npath[7] = {0, 0, 0, 0, 0, 0, 0};
     for (;;) {
         unsigned long long c = 0;
         if (lane == 0) c = atomicAdd(p.counters, 1ull);
@@ -726,7 +737,7 @@ __global__ void __launch_bounds__(kThreads, 2) pair_fast_kernel(const __grid_con
             const bool mask = p.tri && ch < dch_end;        // a chunk of the warp's own rows: pairs j > i only
 #pragma unroll 1
             for (int sub = 0; sub < kSubPerChunk; ++sub)
-                subtile_pairs<MAP>(jt + sub * kSubJ, jsph[sub], p.window != 0, mask, px2, py2, pz2, q4.x, q4.y, q4.z, q4.w, wt, lk,
+                subtile_pairs<MAP>(jt + sub * kSubJ, jsph[sub], p.window != 0, p.prune != 0, mask, px2, py2, pz2, q4.x, q4.y, q4.z, q4.w, wt, lk,
                                    slow, rq, qn, i0, p.n_i, ch * kChunkJ + sub * kSubJ, p.n_j, npath);
             __syncwarp();
             pairs_since_flush += (unsigned long long)kWarpI * kChunkJ;
@@ -743,7 +754,7 @@ __global__ void __launch_bounds__(kThreads, 2) pair_fast_kernel(const __grid_con
     if (lane == 0) {
         if (witems_done) atomicAdd(p.counters + 2, witems_done);
 #pragma unroll
-        for (int k = 0; k < 6; ++k)
+        for (int k = 0; k < 7; ++k)
             if (npath[k]) atomicAdd(p.counters + 3 + k, (unsigned long long)npath[k]);
     }
 }
@@ -889,7 +900,7 @@ struct TcRow {
 template <int MAP>
 __device__ __forceinline__ void tc_bin(const TcRow& pd, uint32_t taddr, const float4* __restrict__ xs, uint32_t j0, bool mask,
                                        const WinTables& wt, const Lookup& lk, SlowCtx* slow, uint2* rq, unsigned& qn,
-                                       uint32_t iwarp, uint32_t n_i, uint32_t n_j, unsigned (&npath)[6]) {
+                                       uint32_t iwarp, uint32_t n_i, uint32_t n_j, unsigned (&npath)[7]) {
     const bool win = pd.mode <= kMaxWinEdges;
     bool flagged = false;
     if (pd.we <= kMaxWinEdges) {                    // warp-uniform
@@ -1037,7 +1048,7 @@ __global__ void __launch_bounds__(kTcThreads, 4) pair_tensor_kernel(const __grid
     unsigned qn = 0;
     uint32_t gch = 0, gs = 0;               // j-tiles fetched / multiplied so far: ring slot and mbarrier parities
     unsigned long long pairs_since_flush = 0, items_done = 0;
-    unsigned npath[6] = {0, 0, 0, 0, 0, 0};
+    unsigned npath[7] = {0, 0, 0, 0, 0, 0, 0};
     for (;;) {
         if (tid == 0) {
             const unsigned long long c = atomicAdd(p.counters, 1ull);
@@ -1166,7 +1177,7 @@ __global__ void __launch_bounds__(kTcThreads, 4) pair_tensor_kernel(const __grid
     if (tid == 0 && items_done) atomicAdd(p.counters + 2, items_done);
     if (lane == 0) {
 #pragma unroll
-        for (int k = 0; k < 6; ++k)
+        for (int k = 0; k < 7; ++k)
             if (npath[k]) atomicAdd(p.counters + 3 + k, (unsigned long long)npath[k]);
     }
 }
@@ -1374,6 +1385,63 @@ __global__ void convert_kernel(const T* __restrict__ radec, uint64_t n, double4*
     }
 }
 
+// 3-D variant: sort key of a position inside the unit ball = its index along a 3-D Hilbert curve of the cube [-1, 1)^3,
+// 21 bits per axis (Skilling's transpose algorithm: inverse undo, Gray encode, then the bits of the three axes
+// interleaved).  As above only the ORDER matters: consecutive rows of the sorted catalog are neighbours in space.
+__device__ inline unsigned long long hilbert_key3(double x, double y, double z) {
+    constexpr int B = 21;
+    const double scale = (double)(1u << (B - 1));
+    uint32_t X[3];
+    X[0] = (uint32_t)fmin(fmax((x + 1.0) * scale, 0.0), (double)((1u << B) - 1));
+    X[1] = (uint32_t)fmin(fmax((y + 1.0) * scale, 0.0), (double)((1u << B) - 1));
+    X[2] = (uint32_t)fmin(fmax((z + 1.0) * scale, 0.0), (double)((1u << B) - 1));
+    const uint32_t M = 1u << (B - 1);
+    for (uint32_t Q = M; Q > 1; Q >>= 1) {
+        const uint32_t P = Q - 1;
+#pragma unroll
+        for (int i = 0; i < 3; ++i) {
+            if (X[i] & Q) {
+                X[0] ^= P;
+            } else {
+                const uint32_t t = (X[0] ^ X[i]) & P;
+                X[0] ^= t;
+                X[i] ^= t;
+            }
+        }
+    }
+    X[1] ^= X[0];
+    X[2] ^= X[1];
+    uint32_t t = 0;
+    for (uint32_t Q = M; Q > 1; Q >>= 1)
+        if (X[2] & Q) t ^= Q - 1;
+    X[0] ^= t;
+    X[1] ^= t;
+    X[2] ^= t;
+    unsigned long long d = 0;
+    for (int bit = B - 1; bit >= 0; --bit)
+#pragma unroll
+        for (int i = 0; i < 3; ++i) d = (d << 1) | ((X[i] >> bit) & 1u);
+    return d;
+}
+
+// 3-D variant of convert_kernel: rows (x, y, z) in the caller's units -> position * scale (a power of two: exact) inside
+// the unit ball, in the caller's row order.  A row with a non-finite coordinate or |coordinate| > max_abs sets *bad.
+template <typename T>
+__global__ void convert_xyz_kernel(const T* __restrict__ xyz, uint64_t n, double scale, double max_abs, double4* __restrict__ x64_rows,
+                                   unsigned long long* __restrict__ keys, uint32_t* __restrict__ idx, int* __restrict__ bad) {
+    for (uint64_t k = blockIdx.x * (uint64_t)blockDim.x + threadIdx.x; k < n; k += (uint64_t)gridDim.x * blockDim.x) {
+        const double x = (double)xyz[3 * k], y = (double)xyz[3 * k + 1], z = (double)xyz[3 * k + 2];
+        double4 v = make_double4(0.0, 0.0, 0.0, 0.0);
+        if (!(fabs(x) <= max_abs) || !(fabs(y) <= max_abs) || !(fabs(z) <= max_abs))      // also catches NaN and inf
+            *bad = 1;
+        else
+            v = make_double4(x * scale, y * scale, z * scale, 0.0);
+        x64_rows[k] = v;
+        keys[k] = hilbert_key3(v.x, v.y, v.z);
+        idx[k] = (uint32_t)k;
+    }
+}
+
 // ---- stable LSD radix sort of (key, idx) pairs, 8 bits per pass ----------------------------------------------
 // Block b owns elements [b * kSortChunk, (b+1) * kSortChunk).  counts is digit-major: counts[d * nblk + b].
 __global__ void radix_hist_kernel(const unsigned long long* __restrict__ keys, uint32_t n, int shift,
@@ -1572,6 +1640,17 @@ cudaError_t launch_convert(const void* radec, int is_f64, uint64_t n, double4* x
         convert_kernel<double><<<grid, block, 0, st>>>(static_cast<const double*>(radec), n, x64_rows, k, idx, bad_flag);
     else
         convert_kernel<float><<<grid, block, 0, st>>>(static_cast<const float*>(radec), n, x64_rows, k, idx, bad_flag);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_convert_xyz(const void* xyz, int is_f64, uint64_t n, double scale, double max_abs, double4* x64_rows, uint64_t* keys,
+                               uint32_t* idx, int* bad_flag, cudaStream_t st) {
+    const int block = 256, grid = grid_for(n, block);
+    auto* k = reinterpret_cast<unsigned long long*>(keys);
+    if (is_f64)
+        convert_xyz_kernel<double><<<grid, block, 0, st>>>(static_cast<const double*>(xyz), n, scale, max_abs, x64_rows, k, idx, bad_flag);
+    else
+        convert_xyz_kernel<float><<<grid, block, 0, st>>>(static_cast<const float*>(xyz), n, scale, max_abs, x64_rows, k, idx, bad_flag);
     return cudaGetLastError();
 }
 

@@ -27,6 +27,7 @@ struct PairParams {
     uint32_t n_i, n_j;          // real (unpadded) sizes
     int tri;                    // 1: i and j are the same catalog and only pairs i<j are enumerated
     int window;                 // 1: window loops enabled (tpcf_set_window)
+    int prune;                  // 1: pruning mode (tpcf_set_pruning): blocks whose window reaches no band are added wholesale
     uint32_t blocks_i, tiles_j, chunk;
     uint32_t n_items_part;      // items this launch executes (after the partition)
     const uint32_t* row_start;  // tri: first item of i-block I (blocks_i + 1 entries)
@@ -51,7 +52,8 @@ struct PairParams {
     unsigned long long* result; // nbins + 3: under, bins, over, discard
     // [0] next work item (fast engine: next warp item), [1] pairs rechecked in fp64, [2] items done,
     // [3..6] (lane-quad x subtile) warp blocks counted by the 1-, 2-, 3-edge window loops and by the cell-lookup loop,
-    // [7] lanes of window blocks recounted because a pair came within a guard band, [8] warp blocks sent to the fp64 loop
+    // [7] lanes of window blocks recounted because a pair came within a guard band, [8] warp blocks sent to the fp64 loop,
+    // [9] warp blocks added wholesale in pruning mode
     unsigned long long* counters;
 };
 
@@ -67,6 +69,9 @@ constexpr int kSortChunk = 2048;        // elements per block of the radix sort
 // RA/Dec rows -> fp64 unit vectors (caller order) + 63-bit Hilbert keys + identity index
 cudaError_t launch_convert(const void* radec, int is_f64, uint64_t n, double4* x64_rows, uint64_t* keys, uint32_t* idx,
                            int* bad_flag, cudaStream_t st);
+// 3-D variant: Cartesian rows * scale (a power of two) -> positions inside the unit ball + 63-bit 3-D Hilbert keys
+cudaError_t launch_convert_xyz(const void* xyz, int is_f64, uint64_t n, double scale, double max_abs, double4* x64_rows, uint64_t* keys,
+                               uint32_t* idx, int* bad_flag, cudaStream_t st);
 // Stable LSD radix sort of (key, idx) pairs on the low `nbits` bits; buffers A hold the input, the sorted
 // result ends in A or B (*in_a).  counts: 256 * ceil(n / kSortChunk) words of scratch.
 cudaError_t launch_sort_pairs(uint64_t* keys_a, uint64_t* keys_b, uint32_t* idx_a, uint32_t* idx_b, uint32_t* counts,

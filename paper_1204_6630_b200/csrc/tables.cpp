@@ -70,6 +70,56 @@ std::string make_binning(int nbins, const double* theta, int mode, Binning& out)
     return "";
 }
 
+// 3-D variant ("results are extendible to the 3-dimensional variant as well"): the same histograms over the
+// Euclidean separation r = |a - b| of Cartesian positions.  Positions are scaled by a power of two (exact in binary
+// floating point) into the unit ball, so that everything the kernels assume about squared chords of unit vectors holds
+// (d^2 <= 4, padding rows at (2,2,2) are farther than 6 from every row); thresholds T_k = (e_k * scale)^2.
+std::string make_binning_r(int nbins, const double* r, int mode, double max_abs, Binning& out) {
+    if (nbins < 1 || nbins > 4096) return "nbins must be in [1, 4096]";
+    if (!r) return "r_edges is NULL";
+    if (!(max_abs > 0.0) || !(max_abs < 1.0e300)) return "max_abs_coord must be positive and finite";
+    int ex = 0;
+    std::frexp(max_abs * 1.7320508075688774, &ex);          // 2^ex > sqrt(3) max_abs >= |p|
+    const double scale = std::ldexp(1.0, -ex);
+    std::vector<double> e((size_t)nbins + 1);
+    if (mode == 0 || mode == 1) {
+        const double lo = r[0], hi = r[1];
+        if (!(lo == lo) || !(hi == hi)) return "NaN edge";
+        if (!(lo >= 0.0 && lo < hi) || !(hi < 1.0e300)) return "need 0 <= min < max";
+        if (mode == 1 && !(lo > 0.0)) return "LOG binning needs min > 0";
+        for (int k = 0; k <= nbins; ++k)
+            e[k] = (mode == 0) ? lo + k * ((hi - lo) / nbins) : lo * std::pow(hi / lo, (double)k / nbins);
+        e[0] = lo;
+        e[nbins] = hi;
+    } else if (mode == 2) {
+        for (int k = 0; k <= nbins; ++k) {
+            if (!(r[k] == r[k])) return "NaN edge";
+            e[k] = r[k];
+        }
+    } else {
+        return "unknown binning mode";
+    }
+    if (!(e[0] >= 0.0)) return "edges must be >= 0";
+    for (int k = 0; k < nbins; ++k)
+        if (!(e[k] < e[k + 1])) return "edges must be strictly increasing";
+    out = Binning();
+    out.nbins = nbins;
+    out.edges = e;
+    out.spatial = true;
+    out.scale = scale;
+    out.max_abs = max_abs;
+    out.thr.resize((size_t)nbins + 1);
+    for (int k = 0; k <= nbins; ++k) {
+        const double es = e[k] * scale;                     // exact
+        out.thr[k] = std::min(es * es, 4.5);                // no two scaled rows are farther apart than 2
+    }
+    out.drop_first = (e[0] == 0.0);
+    out.drop_last = false;
+    for (int k = 0; k < nbins; ++k)
+        if (!(out.thr[k] < out.thr[k + 1]) || out.thr[k + 1] > 4.0) return "edges beyond the largest possible separation, or closer than fp64 can separate";
+    return "";
+}
+
 int exact_slot(double d2, const Binning& b) {
     const int n = b.nbins;
     if (d2 > 4.0) d2 = 4.0;                 // the oracle clamps the dot product to [-1, 1] (reading A7)
@@ -369,6 +419,39 @@ uint64_t Plan::item_pairs(uint64_t w) const {
         total += (tri && t == I) ? rows * (rows - 1) / 2 : rows * cols;
     }
     return total;
+}
+
+double lookup_pair_share(const Binning& b, double r, double extent, int dim) {
+    if (!(r > 0.0) || !(extent > 0.0)) return 0.0;
+    const int n = b.nbins;
+    auto weight = [&](double lo, double hi) {          // pairs with separation in [lo, hi] ~ hi^dim - lo^dim, cut at the extent
+        lo = std::min(lo, extent);
+        hi = std::min(hi, extent);
+        return std::pow(hi, dim) - std::pow(lo, dim);
+    };
+    double slow = 0.0;
+    const double total = std::pow(extent, dim);
+    // below the first edge, the bins, above the last edge: separations as chords sqrt(T)
+    std::vector<double> c((size_t)n + 1);
+    for (int k = 0; k <= n; ++k) c[k] = std::sqrt(b.thr[k]);
+    for (int k = -1; k <= n; ++k) {
+        const double lo = k < 0 ? 0.0 : c[k], hi = k >= n ? std::max(extent, c[n]) : c[k + 1];
+        if (!(hi > lo)) continue;
+        // a few block centre distances across the bin: a block is slow when it is near or sees more than kMaxWinEdges edges
+        const int steps = 8;
+        for (int s = 0; s < steps; ++s) {
+            const double a = lo + (hi - lo) * s / steps, z = lo + (hi - lo) * (s + 1) / steps, D = 0.5 * (a + z);
+            bool is_slow = D - r < kFarKappa * r;
+            if (!is_slow) {
+                const double w0 = (D - r) * (D - r), w1 = (D + r) * (D + r);
+                int edges = 0;
+                for (int e = 0; e <= n; ++e) edges += (b.thr[e] >= w0 && b.thr[e] <= w1) ? 1 : 0;
+                is_slow = edges > kMaxWinEdges;
+            }
+            if (is_slow) slow += weight(a, z);
+        }
+    }
+    return std::min(1.0, slow / total);
 }
 
 // PAPER.md:20-25 Eq. 1 in the pair-count-normalised reading A1 (BASELINE.json north_star).

@@ -62,14 +62,20 @@ struct FastTables {
 
 struct Binning {
     int nbins = 0;
-    std::vector<double> edges;      // degrees, nbins+1
-    std::vector<double> thr;        // T_k = 4 sin^2(e_k/2), nbins+1
+    std::vector<double> edges;      // degrees (angular contexts) or lengths (3-D contexts), nbins+1
+    std::vector<double> thr;        // angular: T_k = 4 sin^2(e_k/2); 3-D: T_k = (e_k * scale)^2; nbins+1
+    bool spatial = false;           // 3-D context (tpcf_create_r): rows are Cartesian positions, bins are in |a - b|
+    double scale = 1.0;             // 3-D: positions are multiplied by this power of two (exact) so that |p * scale| <= 1
+    double max_abs = 0.0;           // 3-D: the largest |coordinate| the caller promised
     bool drop_first = false;        // e_0 == 0: nothing can be "under"
     bool drop_last = false;         // e_n == 180: nothing can be "over"
 };
 
 // Returns "" on success, else the reason (-> TPCF_EINVAL).
 std::string make_binning(int nbins, const double* theta_deg, int mode, Binning& out);
+// 3-D variant: edges are separations r >= 0 in the units of the coordinates; every coordinate of every row
+// will satisfy |x| <= max_abs_coord.
+std::string make_binning_r(int nbins, const double* r_edges, int mode, double max_abs_coord, Binning& out);
 
 // fp32 rounding bound of the fast engine's squared chord around the true value t.
 double guard_width(double t, double scale);
@@ -96,6 +102,14 @@ struct Plan {
     uint64_t item_pairs(uint64_t w) const;
 };
 void make_plan(bool tri, uint64_t n_i, uint64_t n_j, int sm_count, Plan& out);
+
+// Which pair kernel TPCF_ENGINE_TENSOR launches.  The tensor kernel classifies a (row, 128-row j-tile)
+// block on the tensor core only when its window reaches at most kMaxWinEdges edges and its chords exceed kFarKappa r;
+// its other rows go pair by pair through the cell lookup, which the FFMA2 kernel does ~2x faster (8 rows per lane,
+// 64-row subtiles).  Estimate of the share of pairs in such blocks for catalogs whose pairs fill a dim-dimensional region
+// of extent `extent` evenly: blocks are taken at the separations of the bin centres and beyond the last edge, r = sum of
+// the typical bounding radii (chord units), weights ~ D^(dim-1) dD.
+double lookup_pair_share(const Binning& b, double r, double extent, int dim);
 
 void estimate(const uint64_t* dd, const uint64_t* dr, const uint64_t* rr, int nbins, uint64_t n_d, uint64_t n_r,
               double* w);

@@ -208,6 +208,31 @@ def test_every_kernel_path_gives_the_same_histogram(idx, nd, nr):
             np.testing.assert_array_equal(full(*c.count(k)), win[k])
 
 
+@pytest.mark.parametrize("idx,nd,nr", [(3, 60_000, 50_000), (2, 30_000, 30_000), (5, 40_000, 30_000), (4, 50_000, 70_000)])
+def test_pruning_mode_gives_the_same_histograms(idx, nd, nr):
+    """SURVEY.md NEXT-3 (the k-tree idea, at block granularity, as a separately named mode): blocks whose
+    windows reach no bin edge are added wholesale.  Same integers as the brute-force count; the statistics show that
+    blocks really were skipped."""
+    D, R, e, cfg = synth.make_config(idx, n_d=nd, n_r=nr)
+    with T.Context(cfg.nbins, e, "explicit") as c:
+        c.load("D", D)
+        c.load("R", R)
+        brute = {k: full(*c.count(k)) for k in KINDS}
+        assert c.stats()["pruned_blocks"] == 0
+        c.set_pruning(True)
+        pruned = 0
+        for k in KINDS:
+            np.testing.assert_array_equal(full(*c.count(k)), brute[k])
+            st = c.stats()
+            pruned += st["pruned_blocks"]
+            assert st["pairs"] == totals(nd, nr)[k]
+        assert pruned > 0                    # on config 5 only the blocks of padding rows: its bins are finer than any block
+        rows = synth.subset_rows(nd, 500)
+        a = full(*c.count("DD", rows))
+        c.set_pruning(False)
+        np.testing.assert_array_equal(full(*c.count("DD", rows)), a)
+
+
 def test_sparse_catalogs_fall_back_to_fp64_blocks(oracle_threads):
     """A few hundred points on the whole sky: every bounding radius exceeds the cap of the fp32 error bound, so all
     blocks are classified from the fp64 coordinates -- and still match the oracle."""

@@ -63,6 +63,26 @@ def test_edges_match_the_input_recipe_and_thresholds_closed_form(idx):
     np.testing.assert_allclose(thr[big], 2.0 - 2.0 * np.cos(np.radians(ref[big])), rtol=1e-13)
 
 
+def test_create_r_binning_of_the_3d_variant():
+    """tpcf_create_r: thresholds are (e_k * scale)^2 with scale the power of two that brings every
+    position inside the unit ball; edges beyond the largest possible separation and bad edges are rejected."""
+    with T.Context(40, [1.0, 200.0], "log", max_abs_coord=1000.0) as c:
+        e = c.edges()
+        np.testing.assert_allclose(e, synth.edges(40, 1.0, 200.0, "log"), rtol=1e-14)
+        thr = c.thresholds()
+        scale = 2.0 ** -11                                   # 2^11 = 2048 > sqrt(3) * 1000
+        np.testing.assert_array_equal(thr, (e * scale) ** 2)
+        assert c.classify_fast(float(np.float32(thr[10] * 1.01))) == 11 and c.classify_fast(5.5) == 42
+    with T.Context(8, [0.0, 4096.0], "linear", max_abs_coord=1000.0) as c:      # up to 2 / scale = 4096 is allowed
+        assert c.thresholds()[0] == 0.0 and c.thresholds()[-1] == 4.0
+    for nbins, th, mode, mx in [(8, [0.0, 4097.0], "linear", 1000.0), (4, [0.0, 1.0], "log", 10.0), (4, [-1.0, 1.0], "linear", 10.0),
+                                (4, [1.0, 2.0], "linear", 0.0), (4, [1.0, 2.0], "linear", float("inf")),
+                                (2, [0.0, 1.0, 1.0], "explicit", 10.0), (2, [0.0, float("nan"), 1.0], "explicit", 10.0)]:
+        with pytest.raises(T.TpcfError) as ei:
+            T.tpcf_create_r(nbins, th, mode, mx)
+        assert ei.value.status == T.TPCF_EINVAL
+
+
 def expected_slot(v, thr, nbins):
     if v >= 5.0:
         return nbins + 2
