@@ -119,6 +119,19 @@ tpcf_status tpcf_count(tpcf_ctx* ctx, tpcf_kind kind, uint64_t* hist_out, uint64
 tpcf_status tpcf_count_async(tpcf_ctx* ctx, tpcf_kind kind, uint64_t* hist_dev /* device, nbins+2 */);
 
 /*
+ * tpcf_count_all / tpcf_count_all_async -- the three full histograms of one w(theta) in one call: DD, DR and RR are put
+ *   in flight together (DR on the context's stream, DD and RR on two internal streams forked from it and joined back), so
+ *   that the persistent grids of the three pair kernels fill each other's ramp and tail instead of running back to back;
+ *   the results are those of three tpcf_count calls.
+ *   tpcf_count_all: hist_out = 3 x nbins uint64 (host) in the order DD, DR, RR; under_over_out = NULL or 3 x 2 uint64; the
+ *   counts are stored for tpcf_estimate (unless a partition is set).  tpcf_count_all_async: hist_dev = 3 x (nbins+2)
+ *   uint64 on the DEVICE, {under, bins, over} per kind in the same order, valid once the context's stream has passed the
+ *   call; nothing is stored.  Errors as tpcf_count.
+ */
+tpcf_status tpcf_count_all(tpcf_ctx* ctx, uint64_t* hist_out /* 3 x nbins */, uint64_t* under_over_out /* 3 x 2, nullable */);
+tpcf_status tpcf_count_all_async(tpcf_ctx* ctx, uint64_t* hist_dev /* device, 3 x (nbins+2) */);
+
+/*
  * tpcf_estimate -- Landy-Szalay w(theta) in the pair-count-normalised form (Eq. 1, whose
  *   extraction lost the square on N_random/N_real; form fixed by BASELINE.json north_star, reading A1):
  *     w_k = (DD_k/nDD - 2 DR_k/nDR + RR_k/nRR) / (RR_k/nRR),
@@ -189,7 +202,8 @@ tpcf_status tpcf_set_partition(tpcf_ctx* ctx, int part, int nparts);
 
 /* Per-kernel device timing: when enabled, every later count records a CUDA event pair around its pair
  * kernel on the context's stream (up to 64 outstanding).  tpcf_get_kernel_times waits for them, writes the
- * durations in milliseconds, oldest first, and clears the list.  Used by bench.py for the roofline line. */
+ * durations in milliseconds, oldest first, and clears the list.  tpcf_count_all(_async) records ONE pair around its three
+ * kernels (they overlap).  Used by bench.py for the roofline line. */
 tpcf_status tpcf_set_kernel_timing(tpcf_ctx* ctx, int enabled);
 tpcf_status tpcf_get_kernel_times(tpcf_ctx* ctx, float* ms_out, int capacity, int* n_out);
 

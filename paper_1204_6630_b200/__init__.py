@@ -32,7 +32,7 @@ EXPORTS = (
     "tpcf_estimate_from", "tpcf_destroy", "tpcf_last_error", "tpcf_set_stream", "tpcf_set_engine",
     "tpcf_set_guard_scale", "tpcf_set_partition", "tpcf_get_stats", "tpcf_get_thresholds", "tpcf_classify_fast",
     "tpcf_plan", "tpcf_plan_item_pairs", "tpcf_set_kernel_timing", "tpcf_get_kernel_times", "tpcf_set_window",
-    "tpcf_get_bands", "tpcf_window_host", "tpcf_tensor_probe", "tpcf_create_r", "tpcf_load_xyz", "tpcf_lookup_share", "tpcf_set_pruning",
+    "tpcf_get_bands", "tpcf_window_host", "tpcf_tensor_probe", "tpcf_create_r", "tpcf_load_xyz", "tpcf_lookup_share", "tpcf_set_pruning", "tpcf_count_all", "tpcf_count_all_async",
 )
 
 
@@ -75,6 +75,8 @@ def lib() -> ctypes.CDLL:
             "tpcf_load": [vp, i32, vp, i32, sz, i32, vp],
             "tpcf_count": [vp, i32, vp, vp, vp, sz],
             "tpcf_count_async": [vp, i32, vp],
+            "tpcf_count_all": [vp, vp, vp],
+            "tpcf_count_all_async": [vp, vp],
             "tpcf_estimate": [vp, vp],
             "tpcf_estimate_from": [vp, vp, vp, i32, u64, u64, vp],
             "tpcf_set_stream": [vp, vp],
@@ -209,6 +211,18 @@ def tpcf_count(ctx, kind: int, nbins: int, rows=None) -> Tuple[np.ndarray, int, 
 
 def tpcf_count_async(ctx, kind: int, hist_dev_ptr: int) -> None:
     _check(ctx, lib().tpcf_count_async(ctx, int(kind), ctypes.c_void_p(hist_dev_ptr)))
+
+
+def tpcf_count_all(ctx, nbins: int):
+    """{"DD": (hist, under, over), "DR": ..., "RR": ...} of one call that has the three counts in flight together."""
+    hist = np.zeros((3, nbins), dtype=np.uint64)
+    uo = np.zeros((3, 2), dtype=np.uint64)
+    _check(ctx, lib().tpcf_count_all(ctx, _np_ptr(hist), _np_ptr(uo)))
+    return {k: (hist[i].copy(), int(uo[i, 0]), int(uo[i, 1])) for k, i in _KINDS.items()}
+
+
+def tpcf_count_all_async(ctx, hist_dev_ptr: int) -> None:
+    _check(ctx, lib().tpcf_count_all_async(ctx, ctypes.c_void_p(hist_dev_ptr)))
 
 
 def tpcf_estimate(ctx, nbins: int) -> np.ndarray:
@@ -367,6 +381,16 @@ class Context:
                 and out.element_size() == 8):
             raise TpcfError(TPCF_EINVAL, "out must be a contiguous CUDA 64-bit tensor of nbins+2 elements")
         tpcf_count_async(self._ctx, _KINDS.get(kind, kind), out.data_ptr())
+
+    def count_all(self):
+        return tpcf_count_all(self._ctx, self.nbins)
+
+    def count_all_async(self, out):
+        """out: contiguous CUDA 64-bit tensor of 3 x (nbins+2) elements: {under, bins..., over} of DD, DR, RR."""
+        if not (_is_torch(out) and out.is_cuda and out.is_contiguous() and out.numel() >= 3 * (self.nbins + 2)
+                and out.element_size() == 8):
+            raise TpcfError(TPCF_EINVAL, "out must be a contiguous CUDA 64-bit tensor of 3 x (nbins+2) elements")
+        tpcf_count_all_async(self._ctx, out.data_ptr())
 
     def estimate(self):
         return tpcf_estimate(self._ctx, self.nbins)

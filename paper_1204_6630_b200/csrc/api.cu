@@ -64,9 +64,12 @@ struct tpcf_ctx {
     float2 *d_band_mh = nullptr, *d_band_lh = nullptr;
     uint16_t *d_band_slot = nullptr, *d_cell_band = nullptr;
     double* d_thr = nullptr;
-    unsigned long long* d_result = nullptr;     // nbins + 3
-    unsigned long long* d_counters = nullptr;   // kNumCounters
-    unsigned long long* d_out = nullptr;        // nbins + 2
+    // one set per kind: tpcf_count_all_async has the three pair kernels in flight together
+    unsigned long long* d_result3 = nullptr;    // 3 x (nbins + 3)
+    unsigned long long* d_counters3 = nullptr;  // 3 x kNumCounters
+    unsigned long long* d_out3 = nullptr;       // 3 x (nbins + 2)
+    cudaStream_t side[2] = {nullptr, nullptr};  // streams of the second and third count of tpcf_count_all_async
+    cudaEvent_t fork = nullptr, join[2] = {nullptr, nullptr};
     int* d_bad = nullptr;
     void* arena = nullptr;                      // scratch of tpcf_load, grown on demand, kept until destroy
     size_t arena_bytes = 0;
@@ -120,9 +123,14 @@ tpcf_status ensure_cuda(tpcf_ctx* ctx) {
     ctx->device = dev;
     const int nb = ctx->bin.nbins;
     CU(cudaMalloc(&ctx->d_thr, (nb + 1) * sizeof(double)), "cudaMalloc thresholds");
-    CU(cudaMalloc(&ctx->d_result, (nb + 3) * sizeof(unsigned long long)), "cudaMalloc result");
-    CU(cudaMalloc(&ctx->d_out, (nb + 2) * sizeof(unsigned long long)), "cudaMalloc out");
-    CU(cudaMalloc(&ctx->d_counters, kNumCounters * sizeof(unsigned long long)), "cudaMalloc counters");
+    CU(cudaMalloc(&ctx->d_result3, 3 * (nb + 3) * sizeof(unsigned long long)), "cudaMalloc result");
+    CU(cudaMalloc(&ctx->d_out3, 3 * (nb + 2) * sizeof(unsigned long long)), "cudaMalloc out");
+    CU(cudaMalloc(&ctx->d_counters3, 3 * kNumCounters * sizeof(unsigned long long)), "cudaMalloc counters");
+    for (int k = 0; k < 2; ++k) {
+        CU(cudaStreamCreateWithFlags(&ctx->side[k], cudaStreamNonBlocking), "cudaStreamCreate");
+        CU(cudaEventCreateWithFlags(&ctx->join[k], cudaEventDisableTiming), "cudaEventCreate");
+    }
+    CU(cudaEventCreateWithFlags(&ctx->fork, cudaEventDisableTiming), "cudaEventCreate");
     CU(cudaMalloc(&ctx->d_bad, sizeof(int)), "cudaMalloc flag");
     CU(cudaMemcpy(ctx->d_thr, ctx->bin.thr.data(), (nb + 1) * sizeof(double), cudaMemcpyHostToDevice), "upload thresholds");
     CU(cudaEventCreate(&ctx->ev0), "cudaEventCreate");
@@ -240,9 +248,9 @@ uint32_t items_of_part(uint64_t n_items, int part, int nparts) {
     return (uint32_t)((n_items - part + nparts - 1) / nparts);
 }
 
-// Enqueue one count on ctx->stream; the nbins+2 result lands in d_out_dev.  rows_dev == nullptr: full count.
+// Enqueue one count on stream st (nullptr entry: ctx->stream); the nbins+2 result lands in out_dev.  rows_host == nullptr: full count.
 tpcf_status enqueue_count(tpcf_ctx* ctx, tpcf_kind kind, const int64_t* rows_host, size_t nrows, unsigned long long* out_dev,
-                          Catalog* tmp, int64_t** tmp_rows, uint64_t* pairs_out) {
+                          Catalog* tmp, int64_t** tmp_rows, uint64_t* pairs_out, cudaStream_t* on_stream = nullptr) {
     tpcf_status s = ensure_cuda(ctx);
     if (s) return s;
     if (kind != TPCF_DD && kind != TPCF_DR && kind != TPCF_RR) return fail(ctx, TPCF_EINVAL, "unknown kind");
@@ -254,8 +262,10 @@ tpcf_status enqueue_count(tpcf_ctx* ctx, tpcf_kind kind, const int64_t* rows_hos
         s = upload_tables(ctx);
         if (s) return s;
     }
-    cudaStream_t st = ctx->stream;
+    cudaStream_t st = on_stream ? *on_stream : ctx->stream;
     const int nb = ctx->bin.nbins;
+    unsigned long long* d_result = ctx->d_result3 + (size_t)kind * (nb + 3);
+    unsigned long long* d_counters = ctx->d_counters3 + (size_t)kind * kNumCounters;
 
     PairParams p{};
     Plan subset_plan;
@@ -357,11 +367,11 @@ tpcf_status enqueue_count(tpcf_ctx* ctx, tpcf_kind kind, const int64_t* rows_hos
     p.lut_multi = ctx->lut_multi;
     p.thr = ctx->d_thr;
     p.nbins = nb;
-    p.result = ctx->d_result;
-    p.counters = ctx->d_counters;
+    p.result = d_result;
+    p.counters = d_counters;
 
-    CU(cudaMemsetAsync(ctx->d_result, 0, (nb + 3) * sizeof(unsigned long long), st), "memset result");
-    CU(cudaMemsetAsync(ctx->d_counters, 0, kNumCounters * sizeof(unsigned long long), st), "memset counters");
+    CU(cudaMemsetAsync(d_result, 0, (nb + 3) * sizeof(unsigned long long), st), "memset result");
+    CU(cudaMemsetAsync(d_counters, 0, kNumCounters * sizeof(unsigned long long), st), "memset counters");
     LaunchInfo li{};
     std::pair<cudaEvent_t, cudaEvent_t> kev{nullptr, nullptr};
     if (ctx->time_kernels && ctx->kev_used.size() < 64) {
@@ -401,7 +411,7 @@ tpcf_status enqueue_count(tpcf_ctx* ctx, tpcf_kind kind, const int64_t* rows_hos
         ctx->kev_used.push_back(kev);
     }
     const int zero_slot = (ctx->bin.thr[0] > 0.0) ? 0 : 1;
-    CU(launch_finalize(ctx->d_result, nb, zero_slot, self_pairs, out_dev, st), "finalize launch");
+    CU(launch_finalize(d_result, nb, zero_slot, self_pairs, out_dev, st), "finalize launch");
     ctx->stats.launches += 2;
     ctx->stats.grid = li.grid;
     ctx->stats.block = li.block;
@@ -521,7 +531,7 @@ static tpcf_status load_catalog(tpcf_ctx* ctx, tpcf_cat which, const void* radec
     }
     const uint64_t nblk = (n + kSortChunk - 1) / kSortChunk;
     const size_t need = n * sizeof(double4) + 2 * n * sizeof(uint64_t) + 2 * n * sizeof(uint32_t) + 256 * nblk * sizeof(uint32_t) +
-                        (on_device ? 0 : n * cols * esz) + 8 * 256;
+                        (on_device ? 0 : n * cols * esz) + 10 * 256;
     s = arena_reserve(ctx, need);
     if (s) { free_catalog(c); return s; }
     Carver cv{static_cast<char*>(ctx->arena)};
@@ -532,6 +542,7 @@ static tpcf_status load_catalog(tpcf_ctx* ctx, tpcf_cat which, const void* radec
     sc.ia = cv.take<uint32_t>(n);
     sc.ib = cv.take<uint32_t>(n);
     sc.counts = cv.take<uint32_t>(256 * nblk);
+    uint64_t* bounds = cv.take<uint64_t>(32);
     cudaError_t e = cudaSuccess;
     const void* src = radec_deg;
     if (!on_device) {
@@ -543,8 +554,8 @@ static tpcf_status load_catalog(tpcf_ctx* ctx, tpcf_cat which, const void* radec
     // convert (fp64 unit vectors + sort keys) -> sort -> sorted fp64 rows + row map -> quad and subtile roles
     e = cudaMemsetAsync(ctx->d_bad, 0, sizeof(int), st);
     if (e == cudaSuccess)
-        e = spatial ? launch_convert_xyz(src, dt == TPCF_F64, n, ctx->bin.scale, ctx->bin.max_abs, rows64, sc.ka, sc.ia, ctx->d_bad, st)
-                    : launch_convert(src, dt == TPCF_F64, n, rows64, sc.ka, sc.ia, ctx->d_bad, st);
+        e = spatial ? launch_convert_xyz(src, dt == TPCF_F64, n, ctx->bin.scale, ctx->bin.max_abs, rows64, sc.ka, sc.ia, ctx->d_bad, bounds, st)
+                    : launch_convert(src, dt == TPCF_F64, n, rows64, sc.ka, sc.ia, ctx->d_bad, bounds, st);
     bool in_a = true;
     if (e == cudaSuccess) e = launch_sort_pairs(sc.ka, sc.kb, sc.ia, sc.ib, sc.counts, (uint32_t)n, 63, st, &in_a);
     if (e == cudaSuccess) e = launch_permute(rows64, in_a ? sc.ia : sc.ib, n, n_pad, c.x64, c.inv, st);
@@ -613,12 +624,13 @@ tpcf_status tpcf_count(tpcf_ctx* ctx, tpcf_kind kind, uint64_t* hist_out, uint64
     const int nb = ctx->bin.nbins;
     std::vector<unsigned long long> host(nb + 2), ctr(kNumCounters);
     cudaError_t e = cudaEventRecord(ctx->ev0, st);
-    s = (e == cudaSuccess) ? enqueue_count(ctx, kind, rows, nrows, ctx->d_out, &tmp, &tmp_rows, &pairs)
+    unsigned long long* d_out = ctx->d_out3 + (size_t)kind * (nb + 2);
+    s = (e == cudaSuccess) ? enqueue_count(ctx, kind, rows, nrows, d_out, &tmp, &tmp_rows, &pairs)
                            : cuda_fail(ctx, e, "cudaEventRecord");
     if (s == TPCF_OK) {
         e = cudaEventRecord(ctx->ev1, st);
-        if (e == cudaSuccess) e = cudaMemcpyAsync(host.data(), ctx->d_out, (nb + 2) * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st);
-        if (e == cudaSuccess) e = cudaMemcpyAsync(ctr.data(), ctx->d_counters, kNumCounters * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(host.data(), d_out, (nb + 2) * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(ctr.data(), ctx->d_counters3 + (size_t)kind * kNumCounters, kNumCounters * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st);
         if (e == cudaSuccess) e = cudaStreamSynchronize(st);
         if (e != cudaSuccess) s = cuda_fail(ctx, e, "pair count");
     }
@@ -650,6 +662,93 @@ tpcf_status tpcf_count_async(tpcf_ctx* ctx, tpcf_kind kind, uint64_t* hist_dev) 
     if (!ctx) return TPCF_EINVAL;
     if (!hist_dev) return fail(ctx, TPCF_EINVAL, "hist_dev is NULL");
     return enqueue_count(ctx, kind, nullptr, 0, reinterpret_cast<unsigned long long*>(hist_dev), nullptr, nullptr, nullptr);
+}
+
+// DD, DR and RR of one w(theta) in flight together: DR (twice the pairs) on the context's stream, DD and RR on two side
+// streams forked from it and joined back, so that the persistent grids of the three pair kernels fill each other's ramps
+// and tails.  Results land in hist_dev[kind].
+static tpcf_status enqueue_count_all(tpcf_ctx* ctx, unsigned long long* hist_dev, uint64_t* pairs_out /* 3, nullable */) {
+    tpcf_status s = ensure_cuda(ctx);
+    if (s) return s;
+    const int nb = ctx->bin.nbins;
+    cudaStream_t st = ctx->stream;
+    const bool timing = ctx->time_kernels;
+    std::pair<cudaEvent_t, cudaEvent_t> kev{nullptr, nullptr};
+    if (timing && ctx->kev_used.size() < 64) {      // one event pair around the whole group, on the context's stream
+        if (ctx->kev_pool.empty()) {
+            CU(cudaEventCreate(&kev.first), "cudaEventCreate");
+            CU(cudaEventCreate(&kev.second), "cudaEventCreate");
+        } else {
+            kev = ctx->kev_pool.back();
+            ctx->kev_pool.pop_back();
+        }
+        CU(cudaEventRecord(kev.first, st), "cudaEventRecord");
+    }
+    ctx->time_kernels = false;
+    CU(cudaEventRecord(ctx->fork, st), "cudaEventRecord");
+    const tpcf_kind order[3] = {TPCF_DR, TPCF_DD, TPCF_RR};
+    for (int k = 0; k < 3 && s == TPCF_OK; ++k) {
+        cudaStream_t on = k == 0 ? st : ctx->side[k - 1];
+        if (k > 0) {
+            cudaError_t e = cudaStreamWaitEvent(on, ctx->fork, 0);
+            if (e != cudaSuccess) { s = cuda_fail(ctx, e, "cudaStreamWaitEvent"); break; }
+        }
+        s = enqueue_count(ctx, order[k], nullptr, 0, hist_dev + (size_t)order[k] * (nb + 2), nullptr, nullptr,
+                          pairs_out ? pairs_out + order[k] : nullptr, &on);
+        if (s == TPCF_OK && k > 0) {
+            cudaError_t e = cudaEventRecord(ctx->join[k - 1], on);
+            if (e == cudaSuccess) e = cudaStreamWaitEvent(st, ctx->join[k - 1], 0);
+            if (e != cudaSuccess) s = cuda_fail(ctx, e, "join side stream");
+        }
+    }
+    ctx->time_kernels = timing;
+    if (kev.first) {
+        if (s == TPCF_OK && cudaEventRecord(kev.second, st) == cudaSuccess)
+            ctx->kev_used.push_back(kev);
+        else
+            ctx->kev_pool.push_back(kev);
+    }
+    return s;
+}
+
+tpcf_status tpcf_count_all_async(tpcf_ctx* ctx, uint64_t* hist_dev) {
+    if (!ctx) return TPCF_EINVAL;
+    if (!hist_dev) return fail(ctx, TPCF_EINVAL, "hist_dev is NULL");
+    return enqueue_count_all(ctx, reinterpret_cast<unsigned long long*>(hist_dev), nullptr);
+}
+
+tpcf_status tpcf_count_all(tpcf_ctx* ctx, uint64_t* hist_out, uint64_t* under_over_out) {
+    if (!ctx) return TPCF_EINVAL;
+    if (!hist_out) return fail(ctx, TPCF_EINVAL, "hist_out is NULL");
+    tpcf_status s = ensure_cuda(ctx);
+    if (s) return s;
+    const int nb = ctx->bin.nbins;
+    std::vector<unsigned long long> host(3 * (size_t)(nb + 2));
+    uint64_t pairs[3] = {0, 0, 0};
+    cudaError_t e = cudaEventRecord(ctx->ev0, ctx->stream);
+    s = (e == cudaSuccess) ? enqueue_count_all(ctx, ctx->d_out3, pairs) : cuda_fail(ctx, e, "cudaEventRecord");
+    if (s) return s;
+    e = cudaEventRecord(ctx->ev1, ctx->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(host.data(), ctx->d_out3, host.size() * sizeof(unsigned long long), cudaMemcpyDeviceToHost, ctx->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "pair counts");
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, ctx->ev0, ctx->ev1);
+    ctx->stats.kernel_ms = ms;
+    ctx->stats.pairs = pairs[0] + pairs[1] + pairs[2];
+    for (int k = 0; k < 3; ++k) {
+        const unsigned long long* h = host.data() + (size_t)k * (nb + 2);
+        for (int b = 0; b < nb; ++b) hist_out[(size_t)k * nb + b] = h[b + 1];
+        if (under_over_out) {
+            under_over_out[2 * k] = h[0];
+            under_over_out[2 * k + 1] = h[nb + 1];
+        }
+        if (ctx->nparts == 1) {
+            ctx->counts[k].assign(hist_out + (size_t)k * nb, hist_out + (size_t)(k + 1) * nb);
+            ctx->have[k] = true;
+        }
+    }
+    return TPCF_OK;
 }
 
 tpcf_status tpcf_estimate_from(const uint64_t* dd, const uint64_t* dr, const uint64_t* rr, int nbins, uint64_t n_d,
@@ -684,9 +783,14 @@ void tpcf_destroy(tpcf_ctx* ctx) {
         cudaFree(ctx->d_band_slot);
         cudaFree(ctx->d_cell_band);
         cudaFree(ctx->d_thr);
-        cudaFree(ctx->d_result);
-        cudaFree(ctx->d_out);
-        cudaFree(ctx->d_counters);
+        cudaFree(ctx->d_result3);
+        cudaFree(ctx->d_out3);
+        cudaFree(ctx->d_counters3);
+        for (int k = 0; k < 2; ++k) {
+            if (ctx->side[k]) cudaStreamDestroy(ctx->side[k]);
+            if (ctx->join[k]) cudaEventDestroy(ctx->join[k]);
+        }
+        if (ctx->fork) cudaEventDestroy(ctx->fork);
         cudaFree(ctx->d_bad);
         cudaFree(ctx->arena);
         if (ctx->ev0) cudaEventDestroy(ctx->ev0);

@@ -1329,22 +1329,61 @@ __global__ void __launch_bounds__(kThreads) pair_exact64_kernel(const __grid_con
 }
 
 // ---- load / convert / spatial sort (step a1) -------------------------------------------------------------------
-// Sort key of a unit vector: the face of the circumscribed cube it projects onto (3 bits) followed by the 56-bit
-// index of its projection along a 2-D Hilbert curve of that face (28 bits per axis).  Only the ORDER it induces is
-// used: the curve is continuous on each face, so consecutive rows of the sorted catalog are neighbours on the sky
-// (except at the <= 5 face changes), which is what keeps the bounding spheres of quads and subtiles small.  Counts
-// do not depend on it.
-__device__ inline unsigned long long hilbert_key(double x, double y, double z) {
-    constexpr int B = 28;
+// Bounding boxes of a catalog for the sort keys, as order-preserving 64-bit images of doubles (atomicMin / atomicMax):
+// angular: per cube face f the gnomonic coordinates' [4f] u_min, [4f+1] u_max, [4f+2] v_min, [4f+3] v_max; 3-D: [0..5] =
+// x_min, x_max, y_min, y_max, z_min, z_max.
+constexpr int kBoundWords = 24;
+__device__ __forceinline__ unsigned long long ordered_bits(double x) {
+    const long long b = __double_as_longlong(x);
+    return (unsigned long long)(b ^ ((b >> 63) | (long long)0x8000000000000000ull));
+}
+__device__ __forceinline__ double from_ordered_bits(unsigned long long o) {
+    const long long b = (long long)o;
+    return __longlong_as_double(b ^ ((~b >> 63) | (long long)0x8000000000000000ull));
+}
+__device__ __forceinline__ void face_uv(double x, double y, double z, int& face, double& u, double& v) {
     const double ax = fabs(x), ay = fabs(y), az = fabs(z);
-    int face;
-    double u, v, m;
+    double m;
     if (ax >= ay && ax >= az) { face = x >= 0 ? 0 : 1; u = y; v = z; m = ax; }
     else if (ay >= az)        { face = y >= 0 ? 2 : 3; u = z; v = x; m = ay; }
     else                      { face = z >= 0 ? 4 : 5; u = x; v = y; m = az; }
-    const double scale = (double)(1u << (B - 1));
-    uint32_t X = (uint32_t)fmin(fmax((u / m + 1.0) * scale, 0.0), (double)((1u << B) - 1));
-    uint32_t Y = (uint32_t)fmin(fmax((v / m + 1.0) * scale, 0.0), (double)((1u << B) - 1));
+    u /= m;
+    v /= m;
+}
+// the warp's minimum / maximum of a value into the bound slots (one atomic pair per warp and slot pair)
+__device__ __forceinline__ void bound_update(unsigned long long* b, int slot_min, bool valid, double x) {
+    unsigned long long lo = valid ? ordered_bits(x) : ~0ull, hi = valid ? ordered_bits(x) : 0ull;
+#pragma unroll
+    for (int off = 16; off; off >>= 1) {
+        lo = min(lo, __shfl_xor_sync(0xffffffffu, lo, off));
+        hi = max(hi, __shfl_xor_sync(0xffffffffu, hi, off));
+    }
+    if ((threadIdx.x & 31) == 0 && lo <= hi) {
+        atomicMin(b + slot_min, lo);
+        atomicMax(b + slot_min + 1, hi);
+    }
+}
+__global__ void bounds_init_kernel(unsigned long long* b) {
+    if (threadIdx.x < kBoundWords) b[threadIdx.x] = (threadIdx.x & 1) ? 0ull : ~0ull;
+}
+
+// Sort key of a unit vector: the face of the circumscribed cube it projects onto (3 bits) followed by the 56-bit
+// index of its projection along a 2-D Hilbert curve (28 bits per axis) of the smallest square of that face, anchored at
+// the corner (u_min, v_min), that holds every row of the catalog on the face: the curve then stays inside the populated
+// region, so consecutive rows of the sorted catalog are neighbours on the sky (except at the <= 5 face changes), which is
+// what keeps the bounding spheres of quads and subtiles small.  Only the ORDER the key induces is used: counts do not
+// depend on it.
+__device__ inline unsigned long long hilbert_key(double x, double y, double z, const unsigned long long* __restrict__ bounds) {
+    constexpr int B = 28;
+    int face;
+    double u, v;
+    face_uv(x, y, z, face, u, v);
+    const double u0 = from_ordered_bits(bounds[4 * face]), u1 = from_ordered_bits(bounds[4 * face + 1]);
+    const double v0 = from_ordered_bits(bounds[4 * face + 2]), v1 = from_ordered_bits(bounds[4 * face + 3]);
+    const double side = fmax(fmax(u1 - u0, v1 - v0), 1.0e-300);
+    const double scale = (double)((1u << B) - 1) / side;
+    uint32_t X = (uint32_t)fmin(fmax((u - u0) * scale, 0.0), (double)((1u << B) - 1));
+    uint32_t Y = (uint32_t)fmin(fmax((v - v0) * scale, 0.0), (double)((1u << B) - 1));
     unsigned long long d = 0;
     for (uint32_t s = 1u << (B - 1); s > 0; s >>= 1) {
         const uint32_t rx = (X & s) ? 1u : 0u, ry = (Y & s) ? 1u : 0u;
@@ -1365,36 +1404,54 @@ __device__ inline unsigned long long hilbert_key(double x, double y, double z) {
 // x = cos(dec) cos(ra), y = cos(dec) sin(ra), z = sin(dec) in fp64 (reading A8), in the caller's row order.
 template <typename T>
 __global__ void convert_kernel(const T* __restrict__ radec, uint64_t n, double4* __restrict__ x64_rows,
-                               unsigned long long* __restrict__ keys, uint32_t* __restrict__ idx, int* __restrict__ bad) {
+                               unsigned long long* __restrict__ bounds, uint32_t* __restrict__ idx, int* __restrict__ bad) {
     const double kPi = 3.14159265358979323846;
-    for (uint64_t k = blockIdx.x * (uint64_t)blockDim.x + threadIdx.x; k < n; k += (uint64_t)gridDim.x * blockDim.x) {
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    for (uint64_t k0 = blockIdx.x * (uint64_t)blockDim.x; k0 < n; k0 += stride) {      // whole warps walk together (shuffles below)
+        const uint64_t k = k0 + threadIdx.x;
+        const bool valid = k < n;
         double4 v = make_double4(1.0, 0.0, 0.0, 0.0);
-        const double ra = (double)radec[2 * k], dec = (double)radec[2 * k + 1];
-        if (!(fabs(ra) <= 1.0e6) || !(fabs(dec) <= 90.0)) {      // also catches NaN and inf
-            *bad = 1;
-        } else {
-            const double alpha = ra * kPi / 180.0, delta = dec * kPi / 180.0;
-            double sa, ca, sd, cd;
-            sincos(alpha, &sa, &ca);
-            sincos(delta, &sd, &cd);
-            v = make_double4(cd * ca, cd * sa, sd, 0.0);
+        if (valid) {
+            const double ra = (double)radec[2 * k], dec = (double)radec[2 * k + 1];
+            if (!(fabs(ra) <= 1.0e6) || !(fabs(dec) <= 90.0)) {      // also catches NaN and inf
+                *bad = 1;
+            } else {
+                const double alpha = ra * kPi / 180.0, delta = dec * kPi / 180.0;
+                double sa, ca, sd, cd;
+                sincos(alpha, &sa, &ca);
+                sincos(delta, &sd, &cd);
+                v = make_double4(cd * ca, cd * sa, sd, 0.0);
+            }
+            x64_rows[k] = v;
+            idx[k] = (uint32_t)k;
         }
-        x64_rows[k] = v;
-        keys[k] = hilbert_key(v.x, v.y, v.z);
-        idx[k] = (uint32_t)k;
+        int face;
+        double fu, fv;
+        face_uv(v.x, v.y, v.z, face, fu, fv);
+        __syncwarp();
+        for (int f = 0; f < 6; ++f) {
+            bound_update(bounds, 4 * f, valid && face == f, fu);
+            bound_update(bounds, 4 * f + 2, valid && face == f, fv);
+        }
     }
 }
 
-// 3-D variant: sort key of a position inside the unit ball = its index along a 3-D Hilbert curve of the cube [-1, 1)^3,
-// 21 bits per axis (Skilling's transpose algorithm: inverse undo, Gray encode, then the bits of the three axes
-// interleaved).  As above only the ORDER matters: consecutive rows of the sorted catalog are neighbours in space.
-__device__ inline unsigned long long hilbert_key3(double x, double y, double z) {
+// second pass of the load: the sort keys, once the bounding boxes are known
+__global__ void keys_kernel(const double4* __restrict__ x64_rows, uint64_t n, const unsigned long long* __restrict__ bounds, int spatial,
+                            unsigned long long* __restrict__ keys);
+
+// 3-D variant: sort key of a position = its index along a 3-D Hilbert curve (21 bits per axis; Skilling's transpose
+// algorithm: inverse undo, Gray encode, then the bits of the three axes interleaved) of the smallest cube anchored at
+// (x_min, y_min, z_min) that holds the catalog.  As above only the ORDER matters.
+__device__ inline unsigned long long hilbert_key3(double x, double y, double z, const unsigned long long* __restrict__ bounds) {
     constexpr int B = 21;
-    const double scale = (double)(1u << (B - 1));
+    const double x0 = from_ordered_bits(bounds[0]), y0 = from_ordered_bits(bounds[2]), z0 = from_ordered_bits(bounds[4]);
+    const double side = fmax(fmax(fmax(from_ordered_bits(bounds[1]) - x0, from_ordered_bits(bounds[3]) - y0), from_ordered_bits(bounds[5]) - z0), 1.0e-300);
+    const double scale = (double)((1u << B) - 1) / side;
     uint32_t X[3];
-    X[0] = (uint32_t)fmin(fmax((x + 1.0) * scale, 0.0), (double)((1u << B) - 1));
-    X[1] = (uint32_t)fmin(fmax((y + 1.0) * scale, 0.0), (double)((1u << B) - 1));
-    X[2] = (uint32_t)fmin(fmax((z + 1.0) * scale, 0.0), (double)((1u << B) - 1));
+    X[0] = (uint32_t)fmin(fmax((x - x0) * scale, 0.0), (double)((1u << B) - 1));
+    X[1] = (uint32_t)fmin(fmax((y - y0) * scale, 0.0), (double)((1u << B) - 1));
+    X[2] = (uint32_t)fmin(fmax((z - z0) * scale, 0.0), (double)((1u << B) - 1));
     const uint32_t M = 1u << (B - 1);
     for (uint32_t Q = M; Q > 1; Q >>= 1) {
         const uint32_t P = Q - 1;
@@ -1428,17 +1485,36 @@ __device__ inline unsigned long long hilbert_key3(double x, double y, double z) 
 // the unit ball, in the caller's row order.  A row with a non-finite coordinate or |coordinate| > max_abs sets *bad.
 template <typename T>
 __global__ void convert_xyz_kernel(const T* __restrict__ xyz, uint64_t n, double scale, double max_abs, double4* __restrict__ x64_rows,
-                                   unsigned long long* __restrict__ keys, uint32_t* __restrict__ idx, int* __restrict__ bad) {
-    for (uint64_t k = blockIdx.x * (uint64_t)blockDim.x + threadIdx.x; k < n; k += (uint64_t)gridDim.x * blockDim.x) {
-        const double x = (double)xyz[3 * k], y = (double)xyz[3 * k + 1], z = (double)xyz[3 * k + 2];
+                                   unsigned long long* __restrict__ bounds, uint32_t* __restrict__ idx, int* __restrict__ bad) {
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    for (uint64_t k0 = blockIdx.x * (uint64_t)blockDim.x; k0 < n; k0 += stride) {
+        const uint64_t k = k0 + threadIdx.x;
+        const bool valid = k < n;
         double4 v = make_double4(0.0, 0.0, 0.0, 0.0);
-        if (!(fabs(x) <= max_abs) || !(fabs(y) <= max_abs) || !(fabs(z) <= max_abs))      // also catches NaN and inf
-            *bad = 1;
-        else
-            v = make_double4(x * scale, y * scale, z * scale, 0.0);
-        x64_rows[k] = v;
-        keys[k] = hilbert_key3(v.x, v.y, v.z);
-        idx[k] = (uint32_t)k;
+        bool good = false;
+        if (valid) {
+            const double x = (double)xyz[3 * k], y = (double)xyz[3 * k + 1], z = (double)xyz[3 * k + 2];
+            if (!(fabs(x) <= max_abs) || !(fabs(y) <= max_abs) || !(fabs(z) <= max_abs)) {      // also catches NaN and inf
+                *bad = 1;
+            } else {
+                v = make_double4(x * scale, y * scale, z * scale, 0.0);
+                good = true;
+            }
+            x64_rows[k] = v;
+            idx[k] = (uint32_t)k;
+        }
+        __syncwarp();
+        bound_update(bounds, 0, good, v.x);
+        bound_update(bounds, 2, good, v.y);
+        bound_update(bounds, 4, good, v.z);
+    }
+}
+
+__global__ void keys_kernel(const double4* __restrict__ x64_rows, uint64_t n, const unsigned long long* __restrict__ bounds, int spatial,
+                            unsigned long long* __restrict__ keys) {
+    for (uint64_t k = blockIdx.x * (uint64_t)blockDim.x + threadIdx.x; k < n; k += (uint64_t)gridDim.x * blockDim.x) {
+        const double4 v = x64_rows[k];
+        keys[k] = spatial ? hilbert_key3(v.x, v.y, v.z, bounds) : hilbert_key(v.x, v.y, v.z, bounds);
     }
 }
 
@@ -1633,24 +1709,30 @@ __global__ void finalize_kernel(const unsigned long long* __restrict__ result, i
 static int grid_for(uint64_t n, int block) { return (int)std::max<uint64_t>(1, std::min<uint64_t>((n + block - 1) / block, 148ull * 16)); }
 
 cudaError_t launch_convert(const void* radec, int is_f64, uint64_t n, double4* x64_rows, uint64_t* keys, uint32_t* idx,
-                           int* bad_flag, cudaStream_t st) {
+                           int* bad_flag, uint64_t* bounds, cudaStream_t st) {
     const int block = 256, grid = grid_for(n, block);
     auto* k = reinterpret_cast<unsigned long long*>(keys);
+    auto* b = reinterpret_cast<unsigned long long*>(bounds);
+    bounds_init_kernel<<<1, 32, 0, st>>>(b);
     if (is_f64)
-        convert_kernel<double><<<grid, block, 0, st>>>(static_cast<const double*>(radec), n, x64_rows, k, idx, bad_flag);
+        convert_kernel<double><<<grid, block, 0, st>>>(static_cast<const double*>(radec), n, x64_rows, b, idx, bad_flag);
     else
-        convert_kernel<float><<<grid, block, 0, st>>>(static_cast<const float*>(radec), n, x64_rows, k, idx, bad_flag);
+        convert_kernel<float><<<grid, block, 0, st>>>(static_cast<const float*>(radec), n, x64_rows, b, idx, bad_flag);
+    keys_kernel<<<grid, block, 0, st>>>(x64_rows, n, b, 0, k);
     return cudaGetLastError();
 }
 
 cudaError_t launch_convert_xyz(const void* xyz, int is_f64, uint64_t n, double scale, double max_abs, double4* x64_rows, uint64_t* keys,
-                               uint32_t* idx, int* bad_flag, cudaStream_t st) {
+                               uint32_t* idx, int* bad_flag, uint64_t* bounds, cudaStream_t st) {
     const int block = 256, grid = grid_for(n, block);
     auto* k = reinterpret_cast<unsigned long long*>(keys);
+    auto* b = reinterpret_cast<unsigned long long*>(bounds);
+    bounds_init_kernel<<<1, 32, 0, st>>>(b);
     if (is_f64)
-        convert_xyz_kernel<double><<<grid, block, 0, st>>>(static_cast<const double*>(xyz), n, scale, max_abs, x64_rows, k, idx, bad_flag);
+        convert_xyz_kernel<double><<<grid, block, 0, st>>>(static_cast<const double*>(xyz), n, scale, max_abs, x64_rows, b, idx, bad_flag);
     else
-        convert_xyz_kernel<float><<<grid, block, 0, st>>>(static_cast<const float*>(xyz), n, scale, max_abs, x64_rows, k, idx, bad_flag);
+        convert_xyz_kernel<float><<<grid, block, 0, st>>>(static_cast<const float*>(xyz), n, scale, max_abs, x64_rows, b, idx, bad_flag);
+    keys_kernel<<<grid, block, 0, st>>>(x64_rows, n, b, 1, k);
     return cudaGetLastError();
 }
 

@@ -67,11 +67,12 @@ constexpr int kTcK = 16;               // K of the tensor engine's operand tiles
 constexpr int kSortChunk = 2048;        // elements per block of the radix sort
 
 // RA/Dec rows -> fp64 unit vectors (caller order) + 63-bit Hilbert keys + identity index
+// (bounds: 24 words of scratch for the catalog's bounding boxes, which the keys are taken relative to)
 cudaError_t launch_convert(const void* radec, int is_f64, uint64_t n, double4* x64_rows, uint64_t* keys, uint32_t* idx,
-                           int* bad_flag, cudaStream_t st);
+                           int* bad_flag, uint64_t* bounds, cudaStream_t st);
 // 3-D variant: Cartesian rows * scale (a power of two) -> positions inside the unit ball + 63-bit 3-D Hilbert keys
 cudaError_t launch_convert_xyz(const void* xyz, int is_f64, uint64_t n, double scale, double max_abs, double4* x64_rows, uint64_t* keys,
-                               uint32_t* idx, int* bad_flag, cudaStream_t st);
+                               uint32_t* idx, int* bad_flag, uint64_t* bounds, cudaStream_t st);
 // Stable LSD radix sort of (key, idx) pairs on the low `nbits` bits; buffers A hold the input, the sorted
 // result ends in A or B (*in_a).  counts: 256 * ceil(n / kSortChunk) words of scratch.
 cudaError_t launch_sort_pairs(uint64_t* keys_a, uint64_t* keys_b, uint32_t* idx_a, uint32_t* idx_b, uint32_t* counts,

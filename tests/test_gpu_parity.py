@@ -233,6 +233,39 @@ def test_pruning_mode_gives_the_same_histograms(idx, nd, nr):
         np.testing.assert_array_equal(full(*c.count("DD", rows)), a)
 
 
+@pytest.mark.parametrize("engine", ["fast", "tensor"])
+def test_count_all_equals_three_counts(engine):
+    """tpcf_count_all / tpcf_count_all_async (the three pair kernels in flight together on three streams) against three
+    tpcf_count calls: same integers, stored for tpcf_estimate, repeatable, and after a catalog was replaced."""
+    import torch
+    D, R, e, cfg = synth.make_config(2, n_d=30_000, n_r=25_000)
+    with T.Context(cfg.nbins, e, "explicit") as c:
+        c.set_engine(engine)
+        c.load("D", D)
+        c.load("R", R)
+        one = {k: c.count(k) for k in KINDS}
+        w1 = c.estimate()
+        for _ in range(2):
+            al = c.count_all()
+            for k in KINDS:
+                np.testing.assert_array_equal(al[k][0], one[k][0])
+                assert al[k][1:] == one[k][1:]
+        np.testing.assert_array_equal(c.estimate(), w1)
+        out = torch.zeros(3, cfg.nbins + 2, dtype=torch.int64, device="cuda")
+        st = torch.cuda.Stream()
+        c.set_stream(st.cuda_stream)
+        for _ in range(3):
+            c.count_all_async(out)
+        st.synchronize()
+        for i, k in enumerate(KINDS):
+            np.testing.assert_array_equal(out[i].cpu().numpy(), full(*one[k]))
+        c.load("D", R[:20_000], stream=st.cuda_stream)      # replace D: the next count_all sees the new catalog
+        al = c.count_all()
+        assert int(al["DD"][0].sum()) + al["DD"][1] + al["DD"][2] == 20_000 * 19_999 // 2
+        np.testing.assert_array_equal(al["RR"][0], one["RR"][0])
+        c.set_stream(0)
+
+
 def test_sparse_catalogs_fall_back_to_fp64_blocks(oracle_threads):
     """A few hundred points on the whole sky: every bounding radius exceeds the cap of the fp32 error bound, so all
     blocks are classified from the fp64 coordinates -- and still match the oracle."""
