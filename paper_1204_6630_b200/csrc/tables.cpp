@@ -144,9 +144,10 @@ double guard_width(double t, double scale) { return scale * (1.0e-7 * std::sqrt(
 // split residual 13.4 u, the tensor core's truncating accumulation 13.1 u, further edges 2 u = 43.7 u max(d^2, mid) =
 // 2.61e-6 t (lemma T; the accumulation model is checked bit for bit on the GPU); margin x1.53.
 double guard_width_tensor(double t, double scale) { return scale * (1.0e-7 * std::sqrt(t) + 4.0e-6 * t + 1.0e-13); }
-// The cell-lookup path only ever evaluates the difference form: its bands need not cover the expanded form's error.
-// (9 d^2 + 10 d r) u <= 5.4e-7 t + 6.0e-8 sqrt(t); margins x1.85 and x1.67.
-double guard_width_lookup(double t, double scale) { return scale * (1.0e-7 * std::sqrt(t) + 1.0e-6 * t + 1.0e-13); }
+// The cell-lookup path only ever evaluates the difference form: (9 d^2 + 10 d r) u with r <= kRCap = 0.25, i.e.
+// 5.4e-7 t + 1.5e-7 sqrt(t); margins x1.85 and x1.67.  This width decides which cells SEE a threshold (tables.h
+// FastTables::tcell); whether a pair is ambiguous is decided in the kernel from the radii of its own block.
+double guard_width_lookup(double t, double scale) { return scale * (2.5e-7 * std::sqrt(t) + 1.0e-6 * t + 1.0e-13); }
 
 // --------------------------------------------------------------------------------------------------
 // Cell maps.  Both are integer/IEEE arithmetic on the float's bit pattern, reproduced exactly on the device.

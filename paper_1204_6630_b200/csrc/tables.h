@@ -25,7 +25,7 @@ constexpr int kSubJ = 64;              // j-points per window subtile (one bound
 constexpr int kChunkJ = 128;           // j-points per bulk copy into a warp's shared-memory ring (= i-points per warp)
 constexpr int kWarpsPerCta = kThreads / 32;
 constexpr int kWarpI = 32 * kIPerThread;   // i-points per warp work item
-constexpr float kRCap = 0.1f;          // blocks whose bounding radii sum to more go to the fp64 path (guard_width assumes it)
+constexpr float kRCap = 0.25f;         // blocks whose bounding radii sum to more go to the fp64 path (guard_width_lookup assumes it)
 constexpr float kFarKappa = 2.5f;      // the expanded-form window loops need  min chord >= kFarKappa * (ri + rj)
 constexpr int kMaxWinEdges = 3;        // a (lane, subtile) window that sees more guard bands goes to the cell-lookup path
 
