@@ -50,7 +50,7 @@ class Workload:
     the paper-scale case: 430k clustered + 430k uniform rows in a 1000-box, 40 log bins
     in r from 1 to 200."""
 
-    def __init__(self, idx: int):
+    def __init__(self, idx: int, shuffle_d: bool = False):
         self.idx, self.spatial = idx, idx == 6
         if self.spatial:
             self.D, self.R, self.e = synth.make_box_config()
@@ -58,9 +58,9 @@ class Workload:
             self.name = (f"3-D variant (PAPER.md:18) of the paper-scale case: N_D={len(self.D)} clustered, N_R={len(self.R)} uniform rows "
                          f"(x, y, z) in a 1000-box, 40 log bins in r 1-200, {total_pairs(len(self.D), len(self.R)):.4g} pairs per step")
         else:
-            self.D, self.R, self.e, cfg = synth.make_config(idx)
+            self.D, self.R, self.e, cfg = synth.make_config(idx, shuffle_d=shuffle_d)
             self.nbins, self.max_abs = cfg.nbins, None
-            self.name = workload_name(idx, cfg, len(self.D), len(self.R))
+            self.name = workload_name(idx, cfg, len(self.D), len(self.R)) + (" (rows of D in a seeded random order, SURVEY.md A16)" if shuffle_d else "")
 
     def context(self, T):
         return T.Context(self.nbins, self.e, "explicit", max_abs_coord=self.max_abs)
@@ -153,7 +153,7 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
-    wl = Workload(args.config)
+    wl = Workload(args.config, args.shuffle_d)
     nd, nr = wl.D.shape[0], wl.R.shape[0]
     threads = oracle.host_threads()
     pairs, dt = oracle_sample_rate(wl, 16, threads)          # probe to size the sample
@@ -198,7 +198,7 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
         print(f"[bench] rank {rank}/{world}: communicator of {dist.get_world_size()} ranks, backend {dist.get_backend()}, "
               f"device cuda:{local}", file=sys.stderr, flush=True)
-    wl = Workload(args.config)
+    wl = Workload(args.config, args.shuffle_d)
     D, R, e = wl.D, wl.R, wl.e
     nd, nr = D.shape[0], R.shape[0]
     pairs_step = total_pairs(nd, nr)
@@ -398,6 +398,7 @@ def main():
                     help="BASELINE.json configs 1-5; 6 = the 3-D variant (Cartesian rows, bins in r) of the paper-scale case")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--shuffle-d", action="store_true", help="configs 1-5: rows of D in a seeded random order instead of generation order (SURVEY.md A16)")
     ap.add_argument("--pruning", action="store_true",
                     help="time the separately named pruning mode (tpcf_set_pruning; not the brute-force count, not the headline)")
     ap.add_argument("--engine", default="default", choices=["default", "tensor", "fast"],

@@ -221,10 +221,9 @@ typedef struct {
                                 window blocks recounted pair by pair because a pair came within a guard band;
                                 [5] = blocks classified wholly in fp64 (bounding radii too large for the fp32 bound) */
     uint64_t pruned_blocks;  /* pruning mode: (warp, subtile) blocks added wholesale by the last synchronous count */
-    float lookup_share;      /* TPCF_ENGINE_TENSOR: estimated share of the pairs in blocks the tensor kernel would count pair by
-                                pair (near blocks, more than 3 edges in reach); above 0.04 the engine launches the FFMA2 kernel */
-    float tile_radius, extent;  /* what that estimate used: median bounding radius of the j catalog's 128-row tiles and the
-                                larger extent of the two catalogs (chords of the unit sphere / scaled lengths) */
+    float lookup_share;      /* TPCF_ENGINE_TENSOR: share of the (8-row group, 128-row tile) blocks the tensor kernel would count pair
+                                by pair (near blocks, more than 3 edges in reach, radii beyond the cap), sampled on 65536 blocks once per
+                                catalog pair; above 0.025 the engine launches the FFMA2 kernel (the histograms are the same) */
 } tpcf_stats;
 tpcf_status tpcf_get_stats(const tpcf_ctx* ctx, tpcf_stats* out);
 
@@ -256,11 +255,6 @@ tpcf_status tpcf_window_host(const tpcf_ctx* ctx, float lo2, float hi2, int* fir
  * 3xTF32 tcgen05.mma of pair_tensor_kernel forms it (same operand split, same instruction, same read-back).  What the tests
  * measure the tensor core's accumulation error with.  TPCF_EINVAL for NULL pointers or ntiles == 0 or > 65535. */
 tpcf_status tpcf_tensor_probe(tpcf_ctx* ctx, const float* s_rows, const float* b_rows, size_t ntiles, float* q_out);
-
-/* The estimate behind TPCF_ENGINE_TENSOR's choice of kernel (tpcf_stats.lookup_share): share of the pairs in blocks the
- * tensor kernel would count pair by pair, for typical bounding radii summing to r and catalogs of extent `extent` (both
- * as chords of the unit sphere, or scaled lengths in a 3-D context). */
-tpcf_status tpcf_lookup_share(const tpcf_ctx* ctx, double r, double extent, double* share_out);
 
 /* Number of tile work items of a full count of `kind` for catalog sizes (n_d, n_r), and the number of
  * pairs in item w: the partition arithmetic of tpcf_set_partition, testable without a GPU. */

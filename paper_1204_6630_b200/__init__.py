@@ -32,7 +32,7 @@ EXPORTS = (
     "tpcf_estimate_from", "tpcf_destroy", "tpcf_last_error", "tpcf_set_stream", "tpcf_set_engine",
     "tpcf_set_guard_scale", "tpcf_set_partition", "tpcf_get_stats", "tpcf_get_thresholds", "tpcf_classify_fast",
     "tpcf_plan", "tpcf_plan_item_pairs", "tpcf_set_kernel_timing", "tpcf_get_kernel_times", "tpcf_set_window",
-    "tpcf_get_bands", "tpcf_window_host", "tpcf_tensor_probe", "tpcf_create_r", "tpcf_load_xyz", "tpcf_lookup_share", "tpcf_set_pruning", "tpcf_count_all", "tpcf_count_all_async",
+    "tpcf_get_bands", "tpcf_window_host", "tpcf_tensor_probe", "tpcf_create_r", "tpcf_load_xyz", "tpcf_set_pruning", "tpcf_count_all", "tpcf_count_all_async",
 )
 
 
@@ -47,7 +47,7 @@ class tpcf_stats(ctypes.Structure):
                 ("launches", ctypes.c_int), ("grid", ctypes.c_int), ("block", ctypes.c_int),
                 ("smem_bytes", ctypes.c_int), ("cells", ctypes.c_int), ("cell_bits", ctypes.c_int),
                 ("hist_copies", ctypes.c_int), ("kernel_ms", ctypes.c_float), ("win_blocks", ctypes.c_uint64 * 6),
-                ("pruned_blocks", ctypes.c_uint64), ("lookup_share", ctypes.c_float), ("tile_radius", ctypes.c_float), ("extent", ctypes.c_float)]
+                ("pruned_blocks", ctypes.c_uint64), ("lookup_share", ctypes.c_float)]
 
     def as_dict(self):
         d = {k: getattr(self, k) for k, _ in self._fields_}
@@ -93,7 +93,6 @@ def lib() -> ctypes.CDLL:
             "tpcf_get_kernel_times": [vp, vp, i32, ctypes.POINTER(i32)],
             "tpcf_get_thresholds": [vp, vp],
             "tpcf_classify_fast": [vp, ctypes.c_float, ctypes.POINTER(i32)],
-            "tpcf_lookup_share": [vp, dbl, dbl, ctypes.POINTER(dbl)],
             "tpcf_plan": [vp, i32, u64, u64, ctypes.POINTER(u64)],
             "tpcf_plan_item_pairs": [vp, i32, u64, u64, u64, ctypes.POINTER(u64)],
         }
@@ -314,12 +313,6 @@ def tpcf_tensor_probe(ctx, s_rows: np.ndarray, b_rows: np.ndarray) -> np.ndarray
 def tpcf_classify_fast(ctx, d2: float) -> int:
     out = ctypes.c_int()
     _check(ctx, lib().tpcf_classify_fast(ctx, ctypes.c_float(d2), ctypes.byref(out)))
-    return out.value
-
-
-def tpcf_lookup_share(ctx, r: float, extent: float) -> float:
-    out = ctypes.c_double()
-    _check(ctx, lib().tpcf_lookup_share(ctx, float(r), float(extent), ctypes.byref(out)))
     return out.value
 
 

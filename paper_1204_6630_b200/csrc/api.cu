@@ -24,7 +24,6 @@ struct Catalog {                 // rows in Hilbert order (counts are order-inva
     float4 *xs = nullptr, *cs = nullptr;   // j-side role: rows as (-2 offset, |offset|^2) from their 64-row subtile centre
     float4 *xt = nullptr, *ct = nullptr;   // j-side role of the tensor engine: the same for 128-row tiles
     float* xb = nullptr;                   // ... and per tile a 128 x 16 TF32 operand block (kernels.cuh)
-    double r_tile = 0.0, extent = 0.0;     // typical bounding radius of a 128-row tile and extent of the catalog (chord units)
 };
 // scratch of one spatial sort: (key, idx) ping-pong buffers and the digit counts
 struct SortScratch {
@@ -35,8 +34,10 @@ struct SortScratch {
         *this = SortScratch();
     }
 };
+constexpr float kTensorMaxSlowShare = 0.025f;   // above this share of pair-by-pair blocks TPCF_ENGINE_TENSOR launches pair_fast_kernel
 struct PlanCache {
     bool valid = false;
+    float share = -1.f;          // sampled share of (group, tile) blocks the tensor kernel would count pair by pair; < 0: not sampled yet
     Plan plan;
     uint32_t* d_row_start = nullptr;
 };
@@ -140,6 +141,7 @@ tpcf_status ensure_cuda(tpcf_ctx* ctx) {
 }
 
 void rebuild_tables(tpcf_ctx* ctx) {
+    for (auto& pc : ctx->plans) pc.share = -1.f;
     build_fast_tables(ctx->bin, ctx->guard_scale, ctx->engine == TPCF_ENGINE_TENSOR, ctx->ft);
     ctx->tables_dirty = true;
 }
@@ -387,14 +389,26 @@ tpcf_status enqueue_count(tpcf_ctx* ctx, tpcf_kind kind, const int64_t* rows_hos
     {
         // TPCF_ENGINE_TENSOR runs the FFMA2 kernel where too many pairs would take the tensor kernel's slow rows
         // (fine binnings, catalogs whose tiles are large against the scales binned: tables.h lookup_pair_share)
+        // TPCF_ENGINE_TENSOR runs the FFMA2 kernel where too many pairs would take the tensor kernel's pair-by-pair rows
+        // (fine binnings, catalogs whose tiles are large against the scales binned): the share of such (8-row group, 128-row
+        // tile) blocks is SAMPLED once per (kind, catalogs, tables) and kept with the plan
         bool tensor_kernel = ctx->engine == TPCF_ENGINE_TENSOR && !p.prune;      // pruning lives in the FFMA2 kernel
         if (tensor_kernel) {
-            const int dim = ctx->bin.spatial ? 3 : 2;
-            const double r = cj.r_tile * (1.0 + std::pow((double)kIPerThread / kTcSubJ, 1.0 / dim));     // tile + 8-row group
-            ctx->stats.lookup_share = (float)lookup_pair_share(ctx->bin, r, std::max(ci.extent, cj.extent), dim);
-            ctx->stats.tile_radius = (float)cj.r_tile;
-            ctx->stats.extent = (float)std::max(ci.extent, cj.extent);
-            tensor_kernel = ctx->stats.lookup_share <= 0.04f;
+            float share = -1.f;
+            PlanCache* pc = rows_host ? nullptr : &ctx->plans[kind];
+            if (pc && pc->share >= 0.f) share = pc->share;
+            if (share < 0.f) {
+                unsigned long long h[2] = {0, 0};
+                CU(cudaMemsetAsync(d_counters, 0, 2 * sizeof(unsigned long long), st), "memset counters");
+                CU(launch_sample_modes(p, ctx->ft.map, 1u << 16, d_counters, st), "sample_modes_kernel launch");
+                CU(cudaMemcpyAsync(h, d_counters, sizeof(h), cudaMemcpyDeviceToHost, st), "copy sample");
+                CU(cudaStreamSynchronize(st), "sample block modes");
+                CU(cudaMemsetAsync(d_counters, 0, kNumCounters * sizeof(unsigned long long), st), "memset counters");
+                share = h[1] ? (float)((double)h[0] / (double)h[1]) : 0.f;
+                if (pc) pc->share = share;
+            }
+            ctx->stats.lookup_share = share;
+            tensor_kernel = share <= kTensorMaxSlowShare;
         }
         if (ctx->engine == TPCF_ENGINE_EXACT64) p.prune = 0;
         const cudaError_t le = ctx->engine == TPCF_ENGINE_FAST || (ctx->engine == TPCF_ENGINE_TENSOR && !tensor_kernel)
@@ -511,6 +525,7 @@ static tpcf_status load_catalog(tpcf_ctx* ctx, tpcf_cat which, const void* radec
         if (sd.ci == (int)which || sd.cj == (int)which) {
             ctx->have[k] = false;
             ctx->plans[k].valid = false;
+            ctx->plans[k].share = -1.f;
         }
     }
     const uint64_t n_pad = pad_to(n, kTileI);
@@ -575,29 +590,6 @@ static tpcf_status load_catalog(tpcf_ctx* ctx, tpcf_cat which, const void* radec
     }
     c.n = n;
     c.n_pad = n_pad;
-    {   // typical tile radius and extent of the catalog, from the 128-row tiles' bounding spheres (choice of the pair
-        // kernel under TPCF_ENGINE_TENSOR; a heuristic: it never changes a count)
-        const size_t nt = n_pad / kTcSubJ;
-        std::vector<float4> ct(nt);
-        CU(cudaMemcpyAsync(ct.data(), c.ct, nt * sizeof(float4), cudaMemcpyDeviceToHost, st), "copy tile spheres");
-        CU(cudaStreamSynchronize(st), "copy tile spheres");
-        std::vector<float> rad;
-        double mx = 0, my = 0, mz = 0;
-        auto real = [](const float4& t) {               // not a tile of padding rows (centre (2,2,2)) or one that holds some
-            return t.w <= 1.0f && t.x * t.x + t.y * t.y + t.z * t.z <= 1.05f;
-        };
-        for (const float4& t : ct)
-            if (real(t)) { rad.push_back(t.w); mx += t.x; my += t.y; mz += t.z; }
-        c.r_tile = 0.0;
-        c.extent = 0.0;
-        if (!rad.empty()) {
-            std::nth_element(rad.begin(), rad.begin() + rad.size() / 2, rad.end());
-            c.r_tile = rad[rad.size() / 2];
-            mx /= rad.size(); my /= rad.size(); mz /= rad.size();
-            for (const float4& t : ct)
-                if (real(t)) c.extent = std::max(c.extent, std::sqrt((t.x - mx) * (t.x - mx) + (t.y - my) * (t.y - my) + (t.z - mz) * (t.z - mz)) + t.w);
-        }
-    }
     return TPCF_OK;
 }
 
@@ -925,12 +917,6 @@ tpcf_status tpcf_get_bands(const tpcf_ctx* ctx, int capacity, float* lo_out, flo
         if (hi_out) hi_out[b] = t.band_hi[b];
         if (slot_below_out) slot_below_out[b] = t.band_slot[b];
     }
-    return TPCF_OK;
-}
-
-tpcf_status tpcf_lookup_share(const tpcf_ctx* ctx, double r, double extent, double* share_out) {
-    if (!ctx || !share_out || !(r >= 0.0) || !(extent >= 0.0)) return TPCF_EINVAL;
-    *share_out = lookup_pair_share(ctx->bin, r, extent, ctx->bin.spatial ? 3 : 2);
     return TPCF_OK;
 }
 

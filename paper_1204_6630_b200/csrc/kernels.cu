@@ -819,6 +819,42 @@ __device__ __forceinline__ void window_of(const float4 cq, const float4 sp, bool
     }
 }
 
+// Which kernel TPCF_ENGINE_TENSOR launches: the modes of nsamples pseudo-random (8-row group of the i side, 128-row tile of
+// the j side) blocks; out[0] += blocks that would be counted pair by pair (cell lookup or fp64), out[1] += blocks sampled.
+template <int MAP>
+__global__ void sample_modes_kernel(const __grid_constant__ PairParams p, uint32_t nsamples, unsigned long long* __restrict__ out) {
+    const uint32_t t = blockIdx.x * blockDim.x + threadIdx.x;
+    const Lookup lk = make_lookup(p, nullptr, nullptr);
+    WinTables wt;
+    wt.band_mh = p.band_mh;
+    wt.band_lh = p.band_lh;
+    wt.band_slot = p.band_slot;
+    wt.cell_band = p.cell_band;
+    wt.whist = nullptr;
+    wt.nbands = p.nbands;
+    const uint32_t nq = (p.n_i + R - 1) / R, nt = (p.n_j + kTcSubJ - 1) / kTcSubJ;
+    uint32_t h = t * 2654435761u + 0x9E3779B9u;             // two multiplicative hashes of the sample number
+    h ^= h >> 15;
+    h *= 2246822519u;
+    h ^= h >> 13;
+    const uint32_t qi = (uint32_t)(((unsigned long long)h * nq) >> 32);
+    h = h * 3266489917u + 0x85EBCA6Bu;
+    h ^= h >> 16;
+    const uint32_t tj = (uint32_t)(((unsigned long long)h * nt) >> 32);
+    int mode = 0, k = 0;
+    float g;
+    bool slow = false;
+    if (t < nsamples) {
+        window_of<MAP>(p.cq[qi], p.ct[tj], p.window != 0, wt, lk, mode, k, g);
+        slow = mode > kMaxWinEdges;
+    }
+    const unsigned ns = __popc(__ballot_sync(0xffffffffu, slow)), nn = __popc(__ballot_sync(0xffffffffu, t < nsamples));
+    if ((threadIdx.x & 31) == 0 && nn) {
+        atomicAdd(out, (unsigned long long)ns);
+        atomicAdd(out + 1, (unsigned long long)nn);
+    }
+}
+
 struct TcSmem {
     uint32_t ring, abuf, lut, hist, band_mh, band_lh, thr, whist, cell_band, band_slot, bars, slow, rq, misc, total;
 };
@@ -1834,6 +1870,15 @@ cudaError_t launch_pairs_tensor(const PairParams& p, CellMap map, int sm_count, 
     int grid = (int)std::min<uint64_t>((uint64_t)sm_count * per_sm, std::max<uint64_t>(citems, 1));
     kern<<<grid, kTcThreads, smem, st>>>(p);
     if (info) *info = LaunchInfo{grid, kTcThreads, (int)smem, 1};
+    return cudaGetLastError();
+}
+
+cudaError_t launch_sample_modes(const PairParams& p, CellMap map, uint32_t nsamples, unsigned long long* out, cudaStream_t st) {
+    const int block = 256, grid = (int)((nsamples + block - 1) / block);
+    if (map == CellMap::LogBits)
+        sample_modes_kernel<(int)CellMap::LogBits><<<grid, block, 0, st>>>(p, nsamples, out);
+    else
+        sample_modes_kernel<(int)CellMap::SqrtLin><<<grid, block, 0, st>>>(p, nsamples, out);
     return cudaGetLastError();
 }
 

@@ -93,6 +93,8 @@ cudaError_t launch_gather(const double4* src64, const uint64_t* pos, uint64_t nr
                           cudaStream_t st);
 cudaError_t launch_pairs_fast(const PairParams& p, CellMap map, int sm_count, cudaStream_t st, LaunchInfo* info);
 cudaError_t launch_pairs_tensor(const PairParams& p, CellMap map, int sm_count, cudaStream_t st, LaunchInfo* info);
+// out[0] += sampled (8-row group, 128-row tile) blocks the tensor kernel would count pair by pair, out[1] += blocks sampled
+cudaError_t launch_sample_modes(const PairParams& p, CellMap map, uint32_t nsamples, unsigned long long* out, cudaStream_t st);
 // ntiles x (128 x 128) accumulator tiles of the tensor engine's MMA for given operand rows (device pointers)
 cudaError_t launch_tensor_probe(const float4* srows, const float4* brows, float* q, uint32_t ntiles, cudaStream_t st);
 cudaError_t launch_pairs_exact64(const PairParams& p, int sm_count, cudaStream_t st, LaunchInfo* info);

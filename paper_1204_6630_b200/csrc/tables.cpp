@@ -422,39 +422,6 @@ uint64_t Plan::item_pairs(uint64_t w) const {
     return total;
 }
 
-double lookup_pair_share(const Binning& b, double r, double extent, int dim) {
-    if (!(r > 0.0) || !(extent > 0.0)) return 0.0;
-    const int n = b.nbins;
-    auto weight = [&](double lo, double hi) {          // pairs with separation in [lo, hi] ~ hi^dim - lo^dim, cut at the extent
-        lo = std::min(lo, extent);
-        hi = std::min(hi, extent);
-        return std::pow(hi, dim) - std::pow(lo, dim);
-    };
-    double slow = 0.0;
-    const double total = std::pow(extent, dim);
-    // below the first edge, the bins, above the last edge: separations as chords sqrt(T)
-    std::vector<double> c((size_t)n + 1);
-    for (int k = 0; k <= n; ++k) c[k] = std::sqrt(b.thr[k]);
-    for (int k = -1; k <= n; ++k) {
-        const double lo = k < 0 ? 0.0 : c[k], hi = k >= n ? std::max(extent, c[n]) : c[k + 1];
-        if (!(hi > lo)) continue;
-        // a few block centre distances across the bin: a block is slow when it is near or sees more than kMaxWinEdges edges
-        const int steps = 8;
-        for (int s = 0; s < steps; ++s) {
-            const double a = lo + (hi - lo) * s / steps, z = lo + (hi - lo) * (s + 1) / steps, D = 0.5 * (a + z);
-            bool is_slow = D - r < kFarKappa * r;
-            if (!is_slow) {
-                const double w0 = (D - r) * (D - r), w1 = (D + r) * (D + r);
-                int edges = 0;
-                for (int e = 0; e <= n; ++e) edges += (b.thr[e] >= w0 && b.thr[e] <= w1) ? 1 : 0;
-                is_slow = edges > kMaxWinEdges;
-            }
-            if (is_slow) slow += weight(a, z);
-        }
-    }
-    return std::min(1.0, slow / total);
-}
-
 // PAPER.md:20-25 Eq. 1 in the pair-count-normalised reading A1 (BASELINE.json north_star).
 void estimate(const uint64_t* dd, const uint64_t* dr, const uint64_t* rr, int nbins, uint64_t n_d, uint64_t n_r,
               double* w) {

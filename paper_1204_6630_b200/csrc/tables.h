@@ -103,14 +103,6 @@ struct Plan {
 };
 void make_plan(bool tri, uint64_t n_i, uint64_t n_j, int sm_count, Plan& out);
 
-// Which pair kernel TPCF_ENGINE_TENSOR launches.  The tensor kernel classifies a (row, 128-row j-tile)
-// block on the tensor core only when its window reaches at most kMaxWinEdges edges and its chords exceed kFarKappa r;
-// its other rows go pair by pair through the cell lookup, which the FFMA2 kernel does ~2x faster (8 rows per lane,
-// 64-row subtiles).  Estimate of the share of pairs in such blocks for catalogs whose pairs fill a dim-dimensional region
-// of extent `extent` evenly: blocks are taken at the separations of the bin centres and beyond the last edge, r = sum of
-// the typical bounding radii (chord units), weights ~ D^(dim-1) dD.
-double lookup_pair_share(const Binning& b, double r, double extent, int dim);
-
 void estimate(const uint64_t* dd, const uint64_t* dr, const uint64_t* rr, int nbins, uint64_t n_d, uint64_t n_r,
               double* w);
 

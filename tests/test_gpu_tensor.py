@@ -56,7 +56,10 @@ def test_tensor_engine_full_size_equals_fast_engine(idx):
             c.load("R", R)
             res[eng] = gpu_all(c)
             if eng == "tensor":
-                assert c.stats()["block"] == 128              # the tensor kernel really ran (4-warp CTAs)
+                st = c.stats()
+                # configs 3 and 4: the tensor kernel really ran (4-warp CTAs); config 2 has 5 % of its blocks nearer than
+                # the windows allow, so the engine launches the FFMA2 kernel there (tpcf_stats.lookup_share)
+                assert st["block"] == (128 if idx != 2 else 256) and (st["lookup_share"] <= 0.025) == (idx != 2)
     for k in KINDS:
         assert int(res["tensor"][k].sum()) == totals(nd, nr)[k]
         np.testing.assert_array_equal(res["tensor"][k], res["fast"][k])
