@@ -351,6 +351,10 @@ def run_ours(args):
                 "peak_source": f"{SM_COUNT} SMs x {LANES_PER_CLK_PER_SM} FP32 lanes/clk x {sm_max:.0f} MHz ({peak_src}); DESIGN.md section 7",
                 "frac_at_sampled_clock": (achieved / (SM_COUNT * LANES_PER_CLK_PER_SM * clocks["sm_mhz"] * 1e6 / 1e12)) if clocks.get("sm_mhz") else None}
 
+    if args.pruning:        # blocks are added wholesale: pairs per second is not work per second, no roofline applies
+        roofline.update({"achieved": None, "frac": None, "frac_at_sampled_clock": None,
+                         "note": "pruning mode: unevaluated blocks make pairs/s incomparable with the brute-force roofline"})
+
     # ---- the oracle timed beside it (rank 0, N = 1 only) --------------------------------------------------------
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
