@@ -41,6 +41,10 @@ def lib() -> ctypes.CDLL:
         L.orc_count_cross_xyz.restype = i32
         L.orc_count_rows_xyz.argtypes = [vp, i64p, sz, sz, vp, sz, i32, vp, i32, f64, vp, vp]
         L.orc_count_rows_xyz.restype = i32
+        L.orc_wsum_auto.argtypes = [vp, vp, sz, sz, sz, vp, i32, vp, vp]
+        L.orc_wsum_auto.restype = i32
+        L.orc_wsum_cross.argtypes = [vp, vp, sz, sz, sz, vp, vp, sz, vp, i32, vp, vp]
+        L.orc_wsum_cross.restype = i32
         L.orc_estimate.argtypes = [vp, vp, vp, i32, ctypes.c_uint64, ctypes.c_uint64, vp]
         L.orc_estimate.restype = None
         _lib = L
@@ -211,3 +215,55 @@ def count_rows_xyz(a: np.ndarray, rows, b: np.ndarray, exclude_self: bool, r_edg
     call = lambda r0, r1, h, nr, mm: L.orc_count_rows_xyz(_ptr(a), _ptr(r), r0, r1, _ptr(b), b.shape[0],
                                                           1 if exclude_self else 0, _ptr(e), nb, near_tol, _ptr(h), _ptr(nr))
     return _run("rows_xyz", _even_spans(r.shape[0], threads), call, nb, near_tol >= 0, threads)
+
+
+# ---- weighted counts (oracle/tpcf_oracle.c orc_wsum_*): sum of w_i * w_j per bin --------------------------------------
+@dataclass
+class WeightedSums:
+    """Per theta bin the fp64 sum of w_i * w_j over its pairs, plus the out-of-range sums and the sums of |w_i * w_j|."""
+    hist: np.ndarray          # float64[nbins]
+    under: float
+    over: float
+    abs_hist: np.ndarray      # float64[nbins + 2]: sum |w_i w_j| for {under, bins, over}: the scale of the tolerance
+
+
+def _run_w(spans, call, nbins: int, threads: int) -> WeightedSums:
+    def one(span):
+        h, a = np.zeros(nbins + 2), np.zeros(nbins + 2)
+        if call(span[0], span[1], h, a) != 0:
+            raise ValueError("oracle weighted sums: bad arguments")
+        return h, a
+
+    if threads <= 1 or len(spans) == 1:
+        parts = [one(s) for s in spans]
+    else:
+        with ThreadPoolExecutor(max_workers=threads) as ex:
+            parts = list(ex.map(one, spans))
+    h = np.sum([p[0] for p in parts], axis=0)
+    a = np.sum([p[1] for p in parts], axis=0)
+    return WeightedSums(h[1:-1].copy(), float(h[0]), float(h[-1]), a)
+
+
+def wsum_auto(xyz: np.ndarray, w, edges, threads: int = 1) -> WeightedSums:
+    L = lib()
+    xyz = np.ascontiguousarray(xyz, dtype=np.float64)
+    w = np.ascontiguousarray(w, dtype=np.float64)
+    e = np.ascontiguousarray(edges, dtype=np.float64)
+    nb, n = e.shape[0] - 1, xyz.shape[0]
+    assert w.shape == (n,)
+    call = lambda a, b, h, ab: L.orc_wsum_auto(_ptr(xyz), _ptr(w), n, a, b, _ptr(e), nb, _ptr(h), _ptr(ab))
+    return _run_w(_triangle_spans(n, threads * 4 if threads > 1 else 1), call, nb, threads)
+
+
+def wsum_cross(a: np.ndarray, wa, b: np.ndarray, wb, edges, threads: int = 1) -> WeightedSums:
+    L = lib()
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    b = np.ascontiguousarray(b, dtype=np.float64)
+    wa = np.ascontiguousarray(wa, dtype=np.float64)
+    wb = np.ascontiguousarray(wb, dtype=np.float64)
+    e = np.ascontiguousarray(edges, dtype=np.float64)
+    nb = e.shape[0] - 1
+    assert wa.shape == (a.shape[0],) and wb.shape == (b.shape[0],)
+    call = lambda i0, i1, h, ab: L.orc_wsum_cross(_ptr(a), _ptr(wa), a.shape[0], i0, i1, _ptr(b), _ptr(wb), b.shape[0], _ptr(e), nb,
+                                                  _ptr(h), _ptr(ab))
+    return _run_w(_even_spans(a.shape[0], threads), call, nb, threads)

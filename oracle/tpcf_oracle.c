@@ -221,3 +221,49 @@ int orc_count_rows_xyz(const double *a, const int64_t *rows, size_t r_begin, siz
     }
     return 0;
 }
+
+/*
+ * ---- weighted counts (cross-correlations of galaxy positions with weighted quantities such as shear;
+ * extensions named as future work) ----
+ * Every object carries a weight; the histogram holds, per theta bin, the sum over the pairs of w_i * w_j instead of the
+ * number of pairs.  Definition written out: the pair's bin exactly as in one_pair (dot -> clamp -> acos -> degrees ->
+ * bin_slot), the product w_i * w_j in fp64, added to the bin's fp64 sum in the loop's order (i ascending, j ascending).
+ * wsum has n+2 slots {under, bins, over} and is ACCUMULATED into; asum, if not NULL, accumulates |w_i * w_j| the same way
+ * (the scale of the checker's tolerance: a different summation order changes a sum of m terms by at most
+ * (m - 1) 2^-53 sum |terms|).
+ */
+int orc_wsum_auto(const double *xyz, const double *w, size_t npts, size_t i_begin, size_t i_end, const double *edges,
+                  int nbins, double *wsum, double *asum)
+{
+    if (nbins < 1 || nbins + 1 > MAX_EDGES) return -1;
+    for (size_t i = i_begin; i < i_end && i < npts; ++i)
+        for (size_t j = i + 1; j < npts; ++j) {
+            const double *a = xyz + 3 * i, *b = xyz + 3 * j;
+            double s = a[0] * b[0] + a[1] * b[1] + a[2] * b[2];
+            if (s > 1.0) s = 1.0;
+            if (s < -1.0) s = -1.0;
+            int slot = bin_slot(acos(s) * 180.0 / M_PI, edges, nbins);
+            double t = w[i] * w[j];
+            wsum[slot] += t;
+            if (asum) asum[slot] += fabs(t);
+        }
+    return 0;
+}
+
+int orc_wsum_cross(const double *a, const double *wa, size_t na, size_t i_begin, size_t i_end, const double *b,
+                   const double *wb, size_t nb, const double *edges, int nbins, double *wsum, double *asum)
+{
+    if (nbins < 1 || nbins + 1 > MAX_EDGES) return -1;
+    for (size_t i = i_begin; i < i_end && i < na; ++i)
+        for (size_t j = 0; j < nb; ++j) {
+            const double *p = a + 3 * i, *q = b + 3 * j;
+            double s = p[0] * q[0] + p[1] * q[1] + p[2] * q[2];
+            if (s > 1.0) s = 1.0;
+            if (s < -1.0) s = -1.0;
+            int slot = bin_slot(acos(s) * 180.0 / M_PI, edges, nbins);
+            double t = wa[i] * wb[j];
+            wsum[slot] += t;
+            if (asum) asum[slot] += fabs(t);
+        }
+    return 0;
+}

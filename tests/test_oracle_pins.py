@@ -376,3 +376,43 @@ def test_x_near_counter_xyz():
     x = np.array([[0.0, 0, 0], [3.0, 4.0, 0], [3.0, 4.0, 1e-7]])                   # r = 5, 5 + 1e-15, 1e-7
     c = oracle.count_auto_xyz(x, np.array([1.0, 5.0, 9.0]), near_tol=1e-9)
     assert list(c.near) == [0, 2, 0] and c.under == 1 and list(c.hist) == [0, 2]
+
+
+# ------------------------------------------------------------------ weighted sums: orc_wsum_*
+def test_w1_hand_case_and_unit_weights():
+    """W1: three points on the equator at RA 0, 1, 3 deg with weights 2, 3, 5: separations 1, 2, 3 deg carry the products
+    6, 15, 10; and with unit weights the weighted sums ARE the pair counts (integers, exact in fp64)."""
+    v = xyz_of([[0, 0], [1, 0], [3, 0]])
+    c = oracle.wsum_auto(v, [2.0, 3.0, 5.0], np.array([0.5, 1.5, 2.5, 3.5]))
+    assert list(c.hist) == [6.0, 15.0, 10.0] and c.under == 0.0 and c.over == 0.0
+    x = oracle.wsum_cross(v[:1], [2.0], v[1:], [3.0, -5.0], np.array([0.5, 1.5, 2.5, 3.5]))
+    assert list(x.hist) == [6.0, 0.0, -10.0] and list(x.abs_hist) == [0.0, 6.0, 0.0, 10.0, 0.0]
+    D, R, e, _ = synth.make_config(1, n_d=700, n_r=500)
+    d, r = oracle.radec_to_xyz(D), oracle.radec_to_xyz(R)
+    ca, cx = oracle.count_auto(d, e), oracle.count_cross(d, r, e)
+    wa, wx = oracle.wsum_auto(d, np.ones(700), e), oracle.wsum_cross(d, np.ones(700), r, np.ones(500), e)
+    assert np.array_equal(wa.hist, ca.hist.astype(np.float64)) and (wa.under, wa.over) == (ca.under, ca.over)
+    assert np.array_equal(wx.hist, cx.hist.astype(np.float64)) and (wx.under, wx.over) == (cx.under, cx.over)
+
+
+def test_w2_masks_bilinearity_and_numpy():
+    """W2: 0/1 weights select a sub-catalog (its counts, exactly); scaling the weights of one side by 4 scales every sum
+    by 4 exactly; general weights against numpy's weighted histogram of arccos(Gram) within the reordering bound."""
+    D, R, e, _ = synth.make_config(1, n_d=600, n_r=400)
+    d, r = oracle.radec_to_xyz(D), oracle.radec_to_xyz(R)
+    rng = synth.SplitMix(41)
+    mask = (rng.uniform(600) < 0.4).astype(np.float64)
+    sub = d[mask > 0]
+    assert np.array_equal(oracle.wsum_auto(d, mask, e).hist, oracle.count_auto(sub, e).hist.astype(np.float64))
+    wd, wr = 0.5 + rng.uniform(600), rng.normal(400)
+    x1, x4 = oracle.wsum_cross(d, wd, r, wr, e), oracle.wsum_cross(d, 4.0 * wd, r, wr, e)
+    assert np.array_equal(4.0 * x1.hist, x4.hist) and 4.0 * x1.over == x4.over
+    assert np.array_equal(oracle.wsum_cross(d, wd, r, wr, e, threads=3).abs_hist.round(6), x1.abs_hist.round(6))
+    th = np.degrees(np.arccos(np.clip(d @ r.T, -1.0, 1.0)))
+    ref, _ = np.histogram(th.ravel(), bins=e, weights=np.outer(wd, wr).ravel())
+    assert np.all(np.abs(ref - x1.hist) <= 600 * 400 * 2.0 ** -53 * x1.abs_hist[1:-1] + 1e-300)
+    a = oracle.wsum_auto(d, wd, e)
+    tri = np.triu_indices(600, 1)
+    tha = np.degrees(np.arccos(np.clip(d @ d.T, -1.0, 1.0)))[tri]
+    refa, _ = np.histogram(tha, bins=e, weights=np.outer(wd, wd)[tri])
+    assert np.all(np.abs(refa - a.hist) <= 600 * 600 * 2.0 ** -53 * a.abs_hist[1:-1] + 1e-300)
