@@ -37,9 +37,9 @@ typedef struct tpcf_ctx tpcf_ctx;
 
 typedef enum { TPCF_OK = 0, TPCF_EINVAL = 1, TPCF_ENOMEM = 2, TPCF_ECUDA = 3, TPCF_ESTATE = 4 } tpcf_status;
 typedef enum { TPCF_LINEAR = 0, TPCF_LOG = 1, TPCF_EXPLICIT = 2 } tpcf_binning;
-typedef enum { TPCF_D = 0, TPCF_R = 1 } tpcf_cat;
+typedef enum { TPCF_D = 0, TPCF_R = 1, TPCF_D2 = 2 } tpcf_cat;     /* D2: a second data catalog (cross-correlations) */
 typedef enum { TPCF_F32 = 0, TPCF_F64 = 1 } tpcf_dtype;
-typedef enum { TPCF_DD = 0, TPCF_DR = 1, TPCF_RR = 2 } tpcf_kind;
+typedef enum { TPCF_DD = 0, TPCF_DR = 1, TPCF_RR = 2, TPCF_D1D2 = 3, TPCF_D2R = 4 } tpcf_kind;
 
 /* Which kernel family tpcf_count uses (tpcf_set_engine).
  *   TPCF_ENGINE_TENSOR  (default) blocks of 128 i-rows x 128 j-rows; for every (8-row group, j-tile) block whose bounding
@@ -168,6 +168,31 @@ tpcf_status tpcf_estimate_from(const uint64_t* dd, const uint64_t* dr, const uin
 tpcf_status tpcf_create_r(tpcf_ctx** out, int nbins, const double* r_edges, tpcf_binning mode, double max_abs_coord);
 tpcf_status tpcf_load_xyz(tpcf_ctx* ctx, tpcf_cat which, const void* xyz, tpcf_dtype dt, size_t n, int on_device,
                           void* cuda_stream);
+
+/*
+ * Cross-catalog and weighted counts (PAPER.md:16 cross-correlations of galaxy positions with other
+ * quantities, PAPER.md:83, 89 extensions named as future work).
+ *
+ * A third catalog slot TPCF_D2 (tpcf_load / tpcf_load_xyz with which = TPCF_D2) and two more kinds for tpcf_count and
+ * tpcf_count_async: TPCF_D1D2 = all N_D x N_D2 pairs of D with D2, TPCF_D2R = all N_D2 x N_R pairs (row subsets index
+ * D for D1D2 and D2 for D2R).  The same kernels count them.
+ * tpcf_estimate_cross -- the Landy-Szalay cross-correlation of D and D2 in the pair-count-normalised form,
+ *     w12_k = (D1D2_k/(N_D N_D2) - DR_k/(N_D N_R) - D2R_k/(N_D2 N_R) + RR_k/nRR) / (RR_k/nRR);
+ *   needs full D1D2, DR, D2R and RR counts by tpcf_count on the current catalogs, else TPCF_ESTATE.
+ *
+ * tpcf_set_weights -- one fp64 weight per row of a loaded catalog, in the caller's row order (n must equal the
+ *   catalog's size; a later tpcf_load of that slot drops them).  Errors: TPCF_ESTATE before the load, TPCF_EINVAL for a
+ *   wrong n or a non-finite weight.
+ * tpcf_count_weighted -- per bin the sum over the pairs of `kind` of w_i * w_j (under_over_out: the two out-of-range
+ *   sums), in fp64 throughout: fp64 separations against the fp64 thresholds (the bins are those of
+ *   TPCF_ENGINE_EXACT64) and fp64 sums.  The order of the additions is not fixed (fp64 atomics), so a sum of m terms is
+ *   reproducible only up to (m - 1) 2^-53 sum |w_i w_j|; partial sums hold at most 2^25 terms.
+ *   A first, correct path on the fp64 kernel's plan: about 50 times slower than the unweighted counts.
+ *   Errors: TPCF_ESTATE without catalogs or weights; TPCF_ECUDA.
+ */
+tpcf_status tpcf_estimate_cross(tpcf_ctx* ctx, double* w_out /* nbins */);
+tpcf_status tpcf_set_weights(tpcf_ctx* ctx, tpcf_cat which, const double* w, size_t n);
+tpcf_status tpcf_count_weighted(tpcf_ctx* ctx, tpcf_kind kind, double* wsum_out /* nbins */, double* under_over_out /* 2, nullable */);
 
 void tpcf_destroy(tpcf_ctx* ctx);
 const char* tpcf_last_error(const tpcf_ctx* ctx);

@@ -18,13 +18,15 @@ from . import build as _build
 
 TPCF_OK, TPCF_EINVAL, TPCF_ENOMEM, TPCF_ECUDA, TPCF_ESTATE = 0, 1, 2, 3, 4
 TPCF_LINEAR, TPCF_LOG, TPCF_EXPLICIT = 0, 1, 2
-TPCF_D, TPCF_R = 0, 1
+TPCF_D, TPCF_R, TPCF_D2 = 0, 1, 2
 TPCF_F32, TPCF_F64 = 0, 1
-TPCF_DD, TPCF_DR, TPCF_RR = 0, 1, 2
+TPCF_DD, TPCF_DR, TPCF_RR, TPCF_D1D2, TPCF_D2R = 0, 1, 2, 3, 4
 TPCF_ENGINE_FAST, TPCF_ENGINE_EXACT64, TPCF_ENGINE_TENSOR = 0, 1, 2
 _STATUS = {0: "TPCF_OK", 1: "TPCF_EINVAL", 2: "TPCF_ENOMEM", 3: "TPCF_ECUDA", 4: "TPCF_ESTATE"}
 _MODES = {"linear": TPCF_LINEAR, "log": TPCF_LOG, "explicit": TPCF_EXPLICIT}
 _KINDS = {"DD": TPCF_DD, "DR": TPCF_DR, "RR": TPCF_RR}
+_ALL_KINDS = dict(_KINDS, D1D2=TPCF_D1D2, D2R=TPCF_D2R)
+_CATS = {"D": TPCF_D, "R": TPCF_R, "D2": TPCF_D2}
 
 # every symbol include/tpcf.h declares (tests check that the library exports them all)
 EXPORTS = (
@@ -33,6 +35,7 @@ EXPORTS = (
     "tpcf_set_guard_scale", "tpcf_set_partition", "tpcf_get_stats", "tpcf_get_thresholds", "tpcf_classify_fast",
     "tpcf_plan", "tpcf_plan_item_pairs", "tpcf_set_kernel_timing", "tpcf_get_kernel_times", "tpcf_set_window",
     "tpcf_get_bands", "tpcf_window_host", "tpcf_tensor_probe", "tpcf_create_r", "tpcf_load_xyz", "tpcf_set_pruning", "tpcf_count_all", "tpcf_count_all_async",
+    "tpcf_estimate_cross", "tpcf_set_weights", "tpcf_count_weighted",
 )
 
 
@@ -78,6 +81,9 @@ def lib() -> ctypes.CDLL:
             "tpcf_count_all": [vp, vp, vp],
             "tpcf_count_all_async": [vp, vp],
             "tpcf_estimate": [vp, vp],
+            "tpcf_estimate_cross": [vp, vp],
+            "tpcf_set_weights": [vp, i32, vp, sz],
+            "tpcf_count_weighted": [vp, i32, vp, vp],
             "tpcf_estimate_from": [vp, vp, vp, i32, u64, u64, vp],
             "tpcf_set_stream": [vp, vp],
             "tpcf_set_engine": [vp, i32],
@@ -230,6 +236,26 @@ def tpcf_estimate(ctx, nbins: int) -> np.ndarray:
     return w
 
 
+def tpcf_estimate_cross(ctx, nbins: int) -> np.ndarray:
+    w = np.empty(nbins, dtype=np.float64)
+    _check(ctx, lib().tpcf_estimate_cross(ctx, _np_ptr(w)))
+    return w
+
+
+def tpcf_set_weights(ctx, which: int, w) -> None:
+    w = np.ascontiguousarray(w, dtype=np.float64)
+    if w.ndim != 1:
+        raise TpcfError(TPCF_EINVAL, "weights must be a 1-D array")
+    _check(ctx, lib().tpcf_set_weights(ctx, int(which), _np_ptr(w), w.shape[0]))
+
+
+def tpcf_count_weighted(ctx, kind: int, nbins: int) -> Tuple[np.ndarray, float, float]:
+    h = np.zeros(nbins, dtype=np.float64)
+    uo = np.zeros(2, dtype=np.float64)
+    _check(ctx, lib().tpcf_count_weighted(ctx, int(kind), _np_ptr(h), _np_ptr(uo)))
+    return h, float(uo[0]), float(uo[1])
+
+
 def tpcf_estimate_from(dd, dr, rr, n_d: int, n_r: int) -> np.ndarray:
     dd = np.ascontiguousarray(dd, dtype=np.uint64)
     dr = np.ascontiguousarray(dr, dtype=np.uint64)
@@ -336,7 +362,7 @@ class Context:
         self.nbins = int(nbins)
         self.spatial = max_abs_coord is not None
         self._ctx = tpcf_create_r(nbins, theta_deg, mode, max_abs_coord) if self.spatial else tpcf_create(nbins, theta_deg, mode)
-        self.n = {TPCF_D: 0, TPCF_R: 0}
+        self.n = {TPCF_D: 0, TPCF_R: 0, TPCF_D2: 0}
 
     def close(self):
         if getattr(self, "_ctx", None):
@@ -362,18 +388,18 @@ class Context:
         return tpcf_get_thresholds(self._ctx, self.nbins)
 
     def load(self, which, radec_deg, stream: int = 0):
-        which = {"D": TPCF_D, "R": TPCF_R}.get(which, which)
+        which = _CATS.get(which, which)
         self.n[which] = tpcf_load(self._ctx, which, radec_deg, stream, cols=3 if self.spatial else 2)
 
     def count(self, kind, rows=None):
-        return tpcf_count(self._ctx, _KINDS.get(kind, kind), self.nbins, rows)
+        return tpcf_count(self._ctx, _ALL_KINDS.get(kind, kind), self.nbins, rows)
 
     def count_async(self, kind, out):
         """out: CUDA uint64/int64 tensor with nbins+2 elements, written {under, bins..., over} on the stream."""
         if not (_is_torch(out) and out.is_cuda and out.is_contiguous() and out.numel() >= self.nbins + 2
                 and out.element_size() == 8):
             raise TpcfError(TPCF_EINVAL, "out must be a contiguous CUDA 64-bit tensor of nbins+2 elements")
-        tpcf_count_async(self._ctx, _KINDS.get(kind, kind), out.data_ptr())
+        tpcf_count_async(self._ctx, _ALL_KINDS.get(kind, kind), out.data_ptr())
 
     def count_all(self):
         return tpcf_count_all(self._ctx, self.nbins)
@@ -387,6 +413,15 @@ class Context:
 
     def estimate(self):
         return tpcf_estimate(self._ctx, self.nbins)
+
+    def estimate_cross(self):
+        return tpcf_estimate_cross(self._ctx, self.nbins)
+
+    def set_weights(self, which, w):
+        tpcf_set_weights(self._ctx, _CATS.get(which, which), w)
+
+    def count_weighted(self, kind):
+        return tpcf_count_weighted(self._ctx, _ALL_KINDS.get(kind, kind), self.nbins)
 
     def set_stream(self, stream: int):
         tpcf_set_stream(self._ctx, stream)

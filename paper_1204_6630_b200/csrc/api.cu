@@ -24,6 +24,7 @@ struct Catalog {                 // rows in Hilbert order (counts are order-inva
     float4 *xs = nullptr, *cs = nullptr;   // j-side role: rows as (-2 offset, |offset|^2) from their 64-row subtile centre
     float4 *xt = nullptr, *ct = nullptr;   // j-side role of the tensor engine: the same for 128-row tiles
     float* xb = nullptr;                   // ... and per tile a 128 x 16 TF32 operand block (kernels.cuh)
+    double* w64 = nullptr;                 // per-object weights in sorted order, n_pad entries, 0 for padding (tpcf_set_weights)
 };
 // scratch of one spatial sort: (key, idx) ping-pong buffers and the digit counts
 struct SortScratch {
@@ -34,6 +35,7 @@ struct SortScratch {
         *this = SortScratch();
     }
 };
+constexpr int kNumKinds = 5;                    // DD, DR, RR, D1D2, D2R
 constexpr float kTensorMaxSlowShare = 0.025f;   // above this share of pair-by-pair blocks TPCF_ENGINE_TENSOR launches pair_fast_kernel
 struct PlanCache {
     bool valid = false;
@@ -53,8 +55,8 @@ struct tpcf_ctx {
     bool prune = false;
     cudaStream_t stream = nullptr;
     int part = 0, nparts = 1;
-    Catalog cat[2];
-    PlanCache plans[3];
+    Catalog cat[3];              // D, R, D2
+    PlanCache plans[kNumKinds];
     // device side
     bool cuda_ready = false;
     int sm_count = kPlanSMs;    // replaced by cudaDevAttrMultiProcessorCount of the context's device at its first GPU call
@@ -66,9 +68,10 @@ struct tpcf_ctx {
     uint16_t *d_band_slot = nullptr, *d_cell_band = nullptr;
     double* d_thr = nullptr;
     // one set per kind: tpcf_count_all_async has the three pair kernels in flight together
-    unsigned long long* d_result3 = nullptr;    // 3 x (nbins + 3)
-    unsigned long long* d_counters3 = nullptr;  // 3 x kNumCounters
-    unsigned long long* d_out3 = nullptr;       // 3 x (nbins + 2)
+    unsigned long long* d_result3 = nullptr;    // kNumKinds x (nbins + 3)
+    unsigned long long* d_counters3 = nullptr;  // kNumKinds x kNumCounters
+    unsigned long long* d_out3 = nullptr;       // kNumKinds x (nbins + 2)
+    double* d_wresult = nullptr;                // nbins + 3 weighted sums (tpcf_count_weighted)
     cudaStream_t side[2] = {nullptr, nullptr};  // streams of the second and third count of tpcf_count_all_async
     cudaEvent_t fork = nullptr, join[2] = {nullptr, nullptr};
     int* d_bad = nullptr;
@@ -79,8 +82,8 @@ struct tpcf_ctx {
     int warp_items_per_item = 1;                // how the pair kernel that ran counts work items (pair_fast_kernel: per warp)
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> kev_pool, kev_used;
     // stored full counts for tpcf_estimate
-    std::vector<uint64_t> counts[3];
-    bool have[3] = {false, false, false};
+    std::vector<uint64_t> counts[kNumKinds];
+    bool have[kNumKinds] = {false, false, false, false, false};
     tpcf_stats stats{};
     std::string err;
 };
@@ -124,15 +127,16 @@ tpcf_status ensure_cuda(tpcf_ctx* ctx) {
     ctx->device = dev;
     const int nb = ctx->bin.nbins;
     CU(cudaMalloc(&ctx->d_thr, (nb + 1) * sizeof(double)), "cudaMalloc thresholds");
-    CU(cudaMalloc(&ctx->d_result3, 3 * (nb + 3) * sizeof(unsigned long long)), "cudaMalloc result");
-    CU(cudaMalloc(&ctx->d_out3, 3 * (nb + 2) * sizeof(unsigned long long)), "cudaMalloc out");
-    CU(cudaMalloc(&ctx->d_counters3, 3 * kNumCounters * sizeof(unsigned long long)), "cudaMalloc counters");
+    CU(cudaMalloc(&ctx->d_result3, kNumKinds * (nb + 3) * sizeof(unsigned long long)), "cudaMalloc result");
+    CU(cudaMalloc(&ctx->d_out3, kNumKinds * (nb + 2) * sizeof(unsigned long long)), "cudaMalloc out");
+    CU(cudaMalloc(&ctx->d_counters3, kNumKinds * kNumCounters * sizeof(unsigned long long)), "cudaMalloc counters");
     for (int k = 0; k < 2; ++k) {
         CU(cudaStreamCreateWithFlags(&ctx->side[k], cudaStreamNonBlocking), "cudaStreamCreate");
         CU(cudaEventCreateWithFlags(&ctx->join[k], cudaEventDisableTiming), "cudaEventCreate");
     }
     CU(cudaEventCreateWithFlags(&ctx->fork, cudaEventDisableTiming), "cudaEventCreate");
     CU(cudaMalloc(&ctx->d_bad, sizeof(int)), "cudaMalloc flag");
+    CU(cudaMalloc(&ctx->d_wresult, (nb + 3) * sizeof(double)), "cudaMalloc weighted result");
     CU(cudaMemcpy(ctx->d_thr, ctx->bin.thr.data(), (nb + 1) * sizeof(double), cudaMemcpyHostToDevice), "upload thresholds");
     CU(cudaEventCreate(&ctx->ev0), "cudaEventCreate");
     CU(cudaEventCreate(&ctx->ev1), "cudaEventCreate");
@@ -196,6 +200,7 @@ void free_catalog(Catalog& c) {
     cudaFree(c.xb);
     cudaFree(c.xt);
     cudaFree(c.ct);
+    cudaFree(c.w64);
     c = Catalog();
 }
 
@@ -241,6 +246,8 @@ Sides sides_of(tpcf_kind k) {
     switch (k) {
         case TPCF_DD: return {0, 0, true};
         case TPCF_RR: return {1, 1, true};
+        case TPCF_D1D2: return {0, 2, false};
+        case TPCF_D2R: return {2, 1, false};
         default: return {0, 1, false};
     }
 }
@@ -255,7 +262,7 @@ tpcf_status enqueue_count(tpcf_ctx* ctx, tpcf_kind kind, const int64_t* rows_hos
                           Catalog* tmp, int64_t** tmp_rows, uint64_t* pairs_out, cudaStream_t* on_stream = nullptr) {
     tpcf_status s = ensure_cuda(ctx);
     if (s) return s;
-    if (kind != TPCF_DD && kind != TPCF_DR && kind != TPCF_RR) return fail(ctx, TPCF_EINVAL, "unknown kind");
+    if ((int)kind < 0 || (int)kind >= kNumKinds) return fail(ctx, TPCF_EINVAL, "unknown kind");
     const Sides sd = sides_of(kind);
     const Catalog& ci = ctx->cat[sd.ci];
     const Catalog& cj = ctx->cat[sd.cj];
@@ -510,7 +517,7 @@ static tpcf_status load_catalog(tpcf_ctx* ctx, tpcf_cat which, const void* radec
     if (ctx->bin.spatial != spatial)
         return fail(ctx, TPCF_ESTATE, spatial ? "tpcf_load_xyz needs a context made by tpcf_create_r" : "tpcf_load needs a context made by tpcf_create");
     const int cols = spatial ? 3 : 2;       // values per row
-    if (which != TPCF_D && which != TPCF_R) return fail(ctx, TPCF_EINVAL, "which must be TPCF_D or TPCF_R");
+    if (which != TPCF_D && which != TPCF_R && which != TPCF_D2) return fail(ctx, TPCF_EINVAL, "which must be TPCF_D, TPCF_R or TPCF_D2");
     if (dt != TPCF_F32 && dt != TPCF_F64) return fail(ctx, TPCF_EINVAL, "dtype must be TPCF_F32 or TPCF_F64");
     if (!radec_deg || n == 0) return fail(ctx, TPCF_EINVAL, "empty catalog");
     if (n > 0x7FFFFFFFull) return fail(ctx, TPCF_EINVAL, "more than 2^31-1 rows");
@@ -520,7 +527,7 @@ static tpcf_status load_catalog(tpcf_ctx* ctx, tpcf_cat which, const void* radec
     Catalog& c = ctx->cat[which];
     // the arrays of the catalog being replaced may still be read by counts enqueued on the context's stream
     if (st != ctx->stream) CU(cudaStreamSynchronize(ctx->stream), "cudaStreamSynchronize");
-    for (int k = 0; k < 3; ++k) {           // DR depends on both catalogs
+    for (int k = 0; k < kNumKinds; ++k) {   // DR depends on both catalogs
         const Sides sd = sides_of((tpcf_kind)k);
         if (sd.ci == (int)which || sd.cj == (int)which) {
             ctx->have[k] = false;
@@ -530,6 +537,10 @@ static tpcf_status load_catalog(tpcf_ctx* ctx, tpcf_cat which, const void* radec
     }
     const uint64_t n_pad = pad_to(n, kTileI);
     const size_t esz = (dt == TPCF_F64) ? 8 : 4;
+    if (c.w64) {                                // weights belong to the rows they were set for
+        cudaFree(c.w64);
+        c.w64 = nullptr;
+    }
     if (c.x64 && c.n_pad == n_pad && c.n == n) {
         c.n = 0;                                // same shape as the catalog it replaces: keep the device arrays
     } else {
@@ -743,6 +754,103 @@ tpcf_status tpcf_count_all(tpcf_ctx* ctx, uint64_t* hist_out, uint64_t* under_ov
     return TPCF_OK;
 }
 
+tpcf_status tpcf_set_weights(tpcf_ctx* ctx, tpcf_cat which, const double* w, size_t n) {
+    if (!ctx) return TPCF_EINVAL;
+    if (which != TPCF_D && which != TPCF_R && which != TPCF_D2) return fail(ctx, TPCF_EINVAL, "which must be TPCF_D, TPCF_R or TPCF_D2");
+    tpcf_status s = ensure_cuda(ctx);
+    if (s) return s;
+    Catalog& c = ctx->cat[which];
+    if (!c.n) return fail(ctx, TPCF_ESTATE, "tpcf_set_weights before the catalog was loaded");
+    if (!w || n != c.n) return fail(ctx, TPCF_EINVAL, "weights must hold one value per row of the loaded catalog");
+    for (size_t k = 0; k < n; ++k)
+        if (!(std::fabs(w[k]) <= 1.0e150)) return fail(ctx, TPCF_EINVAL, "non-finite weight");
+    cudaStream_t st = ctx->stream;
+    if (!c.w64) CU(cudaMalloc(&c.w64, c.n_pad * sizeof(double)), "cudaMalloc weights");
+    s = arena_reserve(ctx, n * sizeof(double));
+    if (s) return s;
+    double* staged = static_cast<double*>(ctx->arena);
+    CU(cudaMemcpyAsync(staged, w, n * sizeof(double), cudaMemcpyHostToDevice, st), "copy weights");
+    CU(launch_scatter_weights(staged, c.inv, n, c.n_pad, c.w64, st), "scatter_weights_kernel launch");
+    CU(cudaStreamSynchronize(st), "set weights");
+    return TPCF_OK;
+}
+
+tpcf_status tpcf_count_weighted(tpcf_ctx* ctx, tpcf_kind kind, double* wsum_out, double* under_over_out) {
+    if (!ctx) return TPCF_EINVAL;
+    if (!wsum_out) return fail(ctx, TPCF_EINVAL, "wsum_out is NULL");
+    if ((int)kind < 0 || (int)kind >= kNumKinds) return fail(ctx, TPCF_EINVAL, "unknown kind");
+    tpcf_status s = ensure_cuda(ctx);
+    if (s) return s;
+    const Sides sd = sides_of(kind);
+    const Catalog& ci = ctx->cat[sd.ci];
+    const Catalog& cj = ctx->cat[sd.cj];
+    if (!ci.n || !cj.n) return fail(ctx, TPCF_ESTATE, "count before the needed catalog(s) were loaded");
+    if (!ci.w64 || !cj.w64) return fail(ctx, TPCF_ESTATE, "tpcf_count_weighted needs tpcf_set_weights on the catalog(s) it pairs");
+    cudaStream_t st = ctx->stream;
+    const int nb = ctx->bin.nbins;
+    Plan plan;
+    make_plan(sd.tri, ci.n, cj.n, ctx->sm_count, plan);
+    if (plan.n_items > 0xFFFFFFFFull) return fail(ctx, TPCF_EINVAL, "catalogs too large for the 32-bit work-item index");
+    uint32_t* d_row_start = nullptr;
+    if (sd.tri) {
+        CU(cudaMalloc(&d_row_start, plan.row_start.size() * sizeof(uint32_t)), "cudaMalloc plan");
+        cudaError_t e = cudaMemcpy(d_row_start, plan.row_start.data(), plan.row_start.size() * sizeof(uint32_t), cudaMemcpyHostToDevice);
+        if (e != cudaSuccess) { cudaFree(d_row_start); return cuda_fail(ctx, e, "upload plan"); }
+    }
+    PairParams p{};
+    p.xi64 = ci.x64;
+    p.xj64 = cj.x64;
+    p.n_i = (uint32_t)ci.n;
+    p.n_j = (uint32_t)cj.n;
+    p.tri = sd.tri ? 1 : 0;
+    p.blocks_i = plan.blocks_i;
+    p.tiles_j = plan.tiles_j;
+    p.chunk = plan.chunk;
+    p.n_items_part = items_of_part(plan.n_items, ctx->part, ctx->nparts);
+    p.row_start = d_row_start;
+    p.part = (uint32_t)ctx->part;
+    p.nparts = (uint32_t)ctx->nparts;
+    p.thr = ctx->d_thr;
+    p.nbins = nb;
+    p.counters = ctx->d_counters3 + (size_t)kind * kNumCounters;
+    std::vector<double> host(nb + 3);
+    cudaError_t e = cudaMemsetAsync(ctx->d_wresult, 0, (nb + 3) * sizeof(double), st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(p.counters, 0, kNumCounters * sizeof(unsigned long long), st);
+    if (e == cudaSuccess) e = cudaEventRecord(ctx->ev0, st);
+    if (e == cudaSuccess) e = launch_pairs_weighted64(p, ci.w64, cj.w64, ctx->d_wresult, ctx->sm_count, st);
+    if (e == cudaSuccess) e = cudaEventRecord(ctx->ev1, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(host.data(), ctx->d_wresult, (nb + 3) * sizeof(double), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    cudaFree(d_row_start);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "weighted pair sums");
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, ctx->ev0, ctx->ev1);
+    ctx->stats.kernel_ms = ms;
+    for (int k = 0; k < nb; ++k) wsum_out[k] = host[k + 1];
+    if (under_over_out) {
+        under_over_out[0] = host[0];
+        under_over_out[1] = host[nb + 1];
+    }
+    return TPCF_OK;
+}
+
+tpcf_status tpcf_estimate_cross(tpcf_ctx* ctx, double* w_out) {
+    if (!ctx) return TPCF_EINVAL;
+    if (!w_out) return fail(ctx, TPCF_EINVAL, "w_out is NULL");
+    if (!ctx->have[TPCF_D1D2] || !ctx->have[TPCF_DR] || !ctx->have[TPCF_D2R] || !ctx->have[TPCF_RR])
+        return fail(ctx, TPCF_ESTATE, "the cross estimate needs full D1D2, DR, D2R and RR counts on the current catalogs");
+    const double n1 = (double)ctx->cat[0].n, n2 = (double)ctx->cat[2].n, nr = (double)ctx->cat[1].n;
+    const double n12 = n1 * n2, n1r = n1 * nr, n2r = n2 * nr, nrr = 0.5 * nr * (nr - 1.0);
+    for (int k = 0; k < ctx->bin.nbins; ++k) {
+        const double rr = (double)ctx->counts[TPCF_RR][k];
+        if (rr == 0.0) { w_out[k] = std::nan(""); continue; }
+        const double frr = rr / nrr;
+        w_out[k] = ((double)ctx->counts[TPCF_D1D2][k] / n12 - (double)ctx->counts[TPCF_DR][k] / n1r -
+                    (double)ctx->counts[TPCF_D2R][k] / n2r + frr) / frr;
+    }
+    return TPCF_OK;
+}
+
 tpcf_status tpcf_estimate_from(const uint64_t* dd, const uint64_t* dr, const uint64_t* rr, int nbins, uint64_t n_d,
                                uint64_t n_r, double* w_out) {
     if (!dd || !dr || !rr || !w_out || nbins < 1) return TPCF_EINVAL;
@@ -764,8 +872,7 @@ void tpcf_destroy(tpcf_ctx* ctx) {
     if (!ctx) return;
     if (ctx->cuda_ready) {
         cudaSetDevice(ctx->device);
-        free_catalog(ctx->cat[0]);
-        free_catalog(ctx->cat[1]);
+        for (auto& c : ctx->cat) free_catalog(c);
         for (auto& pc : ctx->plans)
             if (pc.d_row_start) cudaFree(pc.d_row_start);
         cudaFree(ctx->d_lut);
@@ -778,6 +885,7 @@ void tpcf_destroy(tpcf_ctx* ctx) {
         cudaFree(ctx->d_result3);
         cudaFree(ctx->d_out3);
         cudaFree(ctx->d_counters3);
+        cudaFree(ctx->d_wresult);
         for (int k = 0; k < 2; ++k) {
             if (ctx->side[k]) cudaStreamDestroy(ctx->side[k]);
             if (ctx->join[k]) cudaEventDestroy(ctx->join[k]);

@@ -1364,6 +1364,62 @@ __global__ void __launch_bounds__(kThreads) pair_exact64_kernel(const __grid_con
     if (tid == 0 && items_done) atomicAdd(p.counters + 2, items_done);
 }
 
+// ---- weighted sums: sum of w_i w_j per bin, fp64 throughout -------------------------
+// The same plan and the same fp64 classification as pair_exact64_kernel; the CTA's partial sums are fp64 shared-memory
+// atomics, added to the global fp64 sums after every work item (at most 2^25 terms per partial: DESIGN.md section 14).
+__global__ void __launch_bounds__(kThreads) pair_weighted64_kernel(const __grid_constant__ PairParams p, const double* __restrict__ wi,
+                                                                   const double* __restrict__ wj, double* __restrict__ wresult) {
+    extern __shared__ __align__(128) unsigned char smem[];
+    double* thr = reinterpret_cast<double*>(smem);
+    double* sums = thr + p.nbins + 1;
+    __shared__ Item s_item;
+    const int tid = threadIdx.x, nslots = p.nbins + 3;
+    for (int k = tid; k <= p.nbins; k += kThreads) thr[k] = p.thr[k];
+    for (int k = tid; k < nslots; k += kThreads) sums[k] = 0.0;
+    __syncthreads();
+    for (;;) {
+        if (tid == 0) {
+            const unsigned long long c = atomicAdd(p.counters, 1ull);
+            Item it;
+            it.valid = 0;
+            if (c < p.n_items_part) it = decode_item(p, (uint32_t)c * p.nparts + p.part);
+            s_item = it;
+        }
+        __syncthreads();
+        const Item it = s_item;
+        __syncthreads();
+        if (!it.valid) break;
+        const uint32_t i0 = it.I * kTileI + tid * R;
+        for (int r = 0; r < R; ++r) {
+            const uint32_t i = i0 + r;
+            if (i >= p.n_i) continue;
+            const double4 a = p.xi64[i];
+            const double w = wi[i];
+            const uint32_t jbeg = it.tile0 * kTileJ, jend = min(p.n_j, (it.tile0 + it.ntiles) * kTileJ);
+            for (uint32_t j = jbeg; j < jend; ++j) {
+                if (p.tri && j <= i) continue;
+                const int slot = exact_slot_dev(chord2_f64(a, p.xj64[j]), thr, p.nbins);
+                atomicAdd(sums + slot, w * wj[j]);
+            }
+        }
+        __syncthreads();
+        for (int k = tid; k < nslots; k += kThreads) {
+            if (sums[k] != 0.0) atomicAdd(wresult + k, sums[k]);
+            sums[k] = 0.0;
+        }
+        __syncthreads();
+    }
+}
+
+// weights in the caller's row order -> sorted order (inv: caller row -> sorted position), 0 for the padding rows
+__global__ void scatter_weights_kernel(const double* __restrict__ w, const uint32_t* __restrict__ inv, uint64_t n, uint64_t n_pad,
+                                       double* __restrict__ out) {
+    for (uint64_t k = blockIdx.x * (uint64_t)blockDim.x + threadIdx.x; k < n_pad; k += (uint64_t)gridDim.x * blockDim.x) {
+        if (k < n) out[inv[k]] = w[k];
+        else out[k] = 0.0;
+    }
+}
+
 // ---- load / convert / spatial sort (step a1) -------------------------------------------------------------------
 // Bounding boxes of a catalog for the sort keys, as order-preserving 64-bit images of doubles (atomicMin / atomicMax):
 // angular: per cube face f the gnomonic coordinates' [4f] u_min, [4f+1] u_max, [4f+2] v_min, [4f+3] v_max; 3-D: [0..5] =
@@ -1896,6 +1952,23 @@ cudaError_t launch_pairs_exact64(const PairParams& p, int sm_count, cudaStream_t
     int grid = (int)std::min<uint64_t>((uint64_t)sm_count * per_sm, std::max<uint32_t>(p.n_items_part, 1));
     pair_exact64_kernel<<<grid, kThreads, smem, st>>>(p);
     if (info) *info = LaunchInfo{grid, kThreads, (int)smem, 1};
+    return cudaGetLastError();
+}
+
+cudaError_t launch_pairs_weighted64(const PairParams& p, const double* wi, const double* wj, double* wresult, int sm_count, cudaStream_t st) {
+    const size_t smem = (size_t)(p.nbins + 1) * 8 + (size_t)(p.nbins + 3) * 8;
+    int per_sm = 0;
+    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, pair_weighted64_kernel, kThreads, smem);
+    if (e != cudaSuccess) return e;
+    if (per_sm < 1) return cudaErrorLaunchOutOfResources;
+    const int grid = (int)std::min<uint64_t>((uint64_t)sm_count * per_sm, std::max<uint32_t>(p.n_items_part, 1));
+    pair_weighted64_kernel<<<grid, kThreads, smem, st>>>(p, wi, wj, wresult);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_scatter_weights(const double* w, const uint32_t* inv, uint64_t n, uint64_t n_pad, double* out, cudaStream_t st) {
+    const int block = 256;
+    scatter_weights_kernel<<<grid_for(n_pad, block), block, 0, st>>>(w, inv, n, n_pad, out);
     return cudaGetLastError();
 }
 

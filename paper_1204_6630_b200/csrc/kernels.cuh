@@ -98,6 +98,9 @@ cudaError_t launch_sample_modes(const PairParams& p, CellMap map, uint32_t nsamp
 // ntiles x (128 x 128) accumulator tiles of the tensor engine's MMA for given operand rows (device pointers)
 cudaError_t launch_tensor_probe(const float4* srows, const float4* brows, float* q, uint32_t ntiles, cudaStream_t st);
 cudaError_t launch_pairs_exact64(const PairParams& p, int sm_count, cudaStream_t st, LaunchInfo* info);
+// weighted sums: wresult[0 .. nbins+2] += sum of wi[i] * wj[j] per result slot, fp64 (weights in sorted order)
+cudaError_t launch_pairs_weighted64(const PairParams& p, const double* wi, const double* wj, double* wresult, int sm_count, cudaStream_t st);
+cudaError_t launch_scatter_weights(const double* w, const uint32_t* inv, uint64_t n, uint64_t n_pad, double* out, cudaStream_t st);
 // result[0 .. nbins+1] -> out (device), subtracting `self_pairs` from the slot that holds theta = 0
 cudaError_t launch_finalize(const unsigned long long* result, int nbins, int zero_slot, unsigned long long self_pairs,
                             unsigned long long* out, cudaStream_t st);
