@@ -193,9 +193,13 @@ def run_ours(args):
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device: libtpcf has no CPU fallback")
+    local = local % torch.cuda.device_count()      # one rank per GPU; on a box with fewer GPUs than ranks (tests) ranks share
     torch.cuda.set_device(local)
     if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        if args.backend == "nccl":
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        else:
+            dist.init_process_group(args.backend)
         print(f"[bench] rank {rank}/{world}: communicator of {dist.get_world_size()} ranks, backend {dist.get_backend()}, "
               f"device cuda:{local}", file=sys.stderr, flush=True)
     wl = Workload(args.config, args.shuffle_d)
@@ -402,6 +406,8 @@ def main():
                     help="BASELINE.json configs 1-5; 6 = the 3-D variant (Cartesian rows, bins in r) of the paper-scale case")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--backend", default="nccl", choices=["nccl", "gloo"],
+                    help="torch.distributed backend of the N > 1 run (gloo: smoke test of that path on a box with one GPU)")
     ap.add_argument("--shuffle-d", action="store_true", help="configs 1-5: rows of D in a seeded random order instead of generation order (SURVEY.md A16)")
     ap.add_argument("--pruning", action="store_true",
                     help="time the separately named pruning mode (tpcf_set_pruning; not the brute-force count, not the headline)")
