@@ -274,18 +274,20 @@ tpcf_status tpcf_get_bands(const tpcf_ctx* ctx, int capacity, float* lo_out, flo
  * cell-lookup path).  0 <= lo2 <= hi2 < 64. */
 tpcf_status tpcf_window_host(const tpcf_ctx* ctx, float lo2, float hi2, int* first_band_out, int* n_edges_out);
 
-/* The tensor engine's arithmetic on its own (DESIGN.md section 6): ntiles tiles of 128 i-rows x 128 j-rows.  s_rows: ntiles x
- * 128 x 4 floats (s_x, s_y, s_z, |s|^2 - mid) and b_rows: ntiles x 128 x 4 floats (-2 b'_x, -2 b'_y, -2 b'_z, |b'|^2), host
- * memory; q_out: ntiles x 128 x 128 floats, row-major per tile, host memory: q[i][j] = s_w[i] + b_w[j] + s[i] . b[j] as the
- * 3xTF32 tcgen05.mma of pair_tensor_kernel forms it (same operand split, same instruction, same read-back).  What the tests
- * measure the tensor core's accumulation error with.  TPCF_EINVAL for NULL pointers or ntiles == 0 or > 65535. */
-tpcf_status tpcf_tensor_probe(tpcf_ctx* ctx, const float* s_rows, const float* b_rows, size_t ntiles, float* q_out);
-
 /* Number of tile work items of a full count of `kind` for catalog sizes (n_d, n_r), and the number of
  * pairs in item w: the partition arithmetic of tpcf_set_partition, testable without a GPU. */
 tpcf_status tpcf_plan(const tpcf_ctx* ctx, tpcf_kind kind, uint64_t n_d, uint64_t n_r, uint64_t* n_items_out);
 tpcf_status tpcf_plan_item_pairs(const tpcf_ctx* ctx, tpcf_kind kind, uint64_t n_d, uint64_t n_r, uint64_t w,
                                  uint64_t* pairs_out);
+
+/* ---- diagnostics (not part of the counting path; needs the GPU) ------------------------------------------ */
+
+/* The tensor engine's arithmetic on its own (DESIGN.md section 4): ntiles tiles of 128 i-rows x 128 j-rows.  s_rows: ntiles x
+ * 128 x 4 floats (s_x, s_y, s_z, |s|^2 - mid) and b_rows: ntiles x 128 x 4 floats (-2 b'_x, -2 b'_y, -2 b'_z, |b'|^2), host
+ * memory; q_out: ntiles x 128 x 128 floats, row-major per tile, host memory: q[i][j] = s_w[i] + b_w[j] + s[i] . b[j] as the
+ * 3xTF32 tcgen05.mma of pair_tensor_kernel forms it (same operand split, same instruction, same read-back).  What the tests
+ * measure the tensor core's accumulation error with.  TPCF_EINVAL for NULL pointers or ntiles == 0 or > 65535. */
+tpcf_status tpcf_tensor_probe(tpcf_ctx* ctx, const float* s_rows, const float* b_rows, size_t ntiles, float* q_out);
 
 #ifdef __cplusplus
 }
