@@ -213,6 +213,10 @@ tpcf_status tpcf_set_guard_scale(tpcf_ctx* ctx, double scale);
  * when off, each pair goes through the cell lookup.  Every pair is evaluated either way; the histograms are identical
  * (tests). */
 tpcf_status tpcf_set_window(tpcf_ctx* ctx, int enabled);
+/* TPCF_ENGINE_TENSOR launches the tensor kernel when the sampled share of pair-by-pair blocks (tpcf_stats.lookup_share) is at
+ * most `limit` (default 0.025), else the FFMA2 kernel.  0 = always the FFMA2 kernel; 1 = always the tensor kernel (what the
+ * tests use to exercise it on small catalogs).  The histograms do not depend on it. */
+tpcf_status tpcf_set_tensor_share_limit(tpcf_ctx* ctx, double limit);
 /* Pruning mode, off by default (PAPER.md:29-31 k-trees, "coding the k-trees" as future
  * work).  On: a (256 i-rows, 64 j-rows) block none of whose 32 (8-row group, subtile) windows reaches a bin edge is added
  * to the histogram wholesale -- its pairs are NOT evaluated.  The histograms are the same integers (the windows bound

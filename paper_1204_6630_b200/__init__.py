@@ -35,7 +35,7 @@ EXPORTS = (
     "tpcf_set_guard_scale", "tpcf_set_partition", "tpcf_get_stats", "tpcf_get_thresholds", "tpcf_classify_fast",
     "tpcf_plan", "tpcf_plan_item_pairs", "tpcf_set_kernel_timing", "tpcf_get_kernel_times", "tpcf_set_window",
     "tpcf_get_bands", "tpcf_window_host", "tpcf_tensor_probe", "tpcf_create_r", "tpcf_load_xyz", "tpcf_set_pruning", "tpcf_count_all", "tpcf_count_all_async",
-    "tpcf_estimate_cross", "tpcf_set_weights", "tpcf_count_weighted",
+    "tpcf_estimate_cross", "tpcf_set_weights", "tpcf_count_weighted", "tpcf_set_tensor_share_limit",
 )
 
 
@@ -88,6 +88,7 @@ def lib() -> ctypes.CDLL:
             "tpcf_set_stream": [vp, vp],
             "tpcf_set_engine": [vp, i32],
             "tpcf_set_guard_scale": [vp, dbl],
+            "tpcf_set_tensor_share_limit": [vp, dbl],
             "tpcf_set_window": [vp, i32],
             "tpcf_set_pruning": [vp, i32],
             "tpcf_get_bands": [vp, i32, vp, vp, vp, ctypes.POINTER(i32)],
@@ -283,6 +284,10 @@ def tpcf_set_window(ctx, enabled: bool) -> None:
     _check(ctx, lib().tpcf_set_window(ctx, int(bool(enabled))))
 
 
+def tpcf_set_tensor_share_limit(ctx, limit: float) -> None:
+    _check(ctx, lib().tpcf_set_tensor_share_limit(ctx, float(limit)))
+
+
 def tpcf_set_pruning(ctx, enabled: bool) -> None:
     _check(ctx, lib().tpcf_set_pruning(ctx, int(bool(enabled))))
 
@@ -434,6 +439,9 @@ class Context:
 
     def set_window(self, enabled: bool):
         tpcf_set_window(self._ctx, enabled)
+
+    def set_tensor_share_limit(self, limit: float):
+        tpcf_set_tensor_share_limit(self._ctx, limit)
 
     def set_pruning(self, enabled: bool):
         tpcf_set_pruning(self._ctx, enabled)

@@ -53,6 +53,7 @@ struct tpcf_ctx {
     tpcf_engine engine = TPCF_ENGINE_TENSOR;
     bool window = true;
     bool prune = false;
+    float tensor_share_limit = kTensorMaxSlowShare;
     cudaStream_t stream = nullptr;
     int part = 0, nparts = 1;
     Catalog cat[3];              // D, R, D2
@@ -415,7 +416,7 @@ tpcf_status enqueue_count(tpcf_ctx* ctx, tpcf_kind kind, const int64_t* rows_hos
                 if (pc) pc->share = share;
             }
             ctx->stats.lookup_share = share;
-            tensor_kernel = share <= kTensorMaxSlowShare;
+            tensor_kernel = share <= ctx->tensor_share_limit;
         }
         if (ctx->engine == TPCF_ENGINE_EXACT64) p.prune = 0;
         const cudaError_t le = ctx->engine == TPCF_ENGINE_FAST || (ctx->engine == TPCF_ENGINE_TENSOR && !tensor_kernel)
@@ -924,6 +925,13 @@ tpcf_status tpcf_set_engine(tpcf_ctx* ctx, tpcf_engine e) {
 tpcf_status tpcf_set_window(tpcf_ctx* ctx, int enabled) {
     if (!ctx) return TPCF_EINVAL;
     ctx->window = enabled != 0;
+    return TPCF_OK;
+}
+
+tpcf_status tpcf_set_tensor_share_limit(tpcf_ctx* ctx, double limit) {
+    if (!ctx) return TPCF_EINVAL;
+    if (!(limit >= 0.0) || !(limit <= 1.0)) return fail(ctx, TPCF_EINVAL, "the share limit must be in [0, 1]");
+    ctx->tensor_share_limit = (float)limit;
     return TPCF_OK;
 }
 

@@ -39,6 +39,7 @@ def _worker(rank, world, port, engine, q):
         D, R, e, cfg = synth.make_config(2, n_d=ND, n_r=NR)
         with TT.Context(cfg.nbins, e, "explicit") as c:
             c.set_engine(engine)
+            c.set_tensor_share_limit(1.0)          # "tensor" means pair_tensor_kernel here, whatever the block mix
             c.load("D", D)
             c.load("R", R)
             assert tdist.apply_partition(c) == (rank, world)
@@ -70,6 +71,7 @@ def test_two_processes_count_their_partitions_and_allreduce(engine, oracle_threa
     D, R, e, cfg = synth.make_config(2, n_d=ND, n_r=NR)
     with T.Context(cfg.nbins, e, "explicit") as c:
         c.set_engine(engine)
+        c.set_tensor_share_limit(1.0)
         c.load("D", D)
         c.load("R", R)
         single = np.stack([full(*c.count(k)) for k in KINDS])

@@ -17,6 +17,7 @@ pytestmark = pytest.mark.gpu
 def tensor_ctx(nbins, e):
     c = T.Context(nbins, e, "explicit")
     c.set_engine("tensor")
+    c.set_tensor_share_limit(1.0)       # always pair_tensor_kernel, also where the engine on its own would pick the FFMA2 kernel
     return c
 
 
@@ -230,6 +231,7 @@ def test_tensor_engine_equals_fp64_engine_on_unusual_binnings_and_settings(case)
     for eng in ("exact64", "tensor"):
         with T.Context(nb, e, mode) as c:
             c.set_engine(eng)
+            c.set_tensor_share_limit(1.0)
             if kw.get("window") is False:
                 c.set_window(False)
             if "gs" in kw:
@@ -239,3 +241,24 @@ def test_tensor_engine_equals_fp64_engine_on_unusual_binnings_and_settings(case)
             out[eng] = gpu_all(c)
     for k in KINDS:
         np.testing.assert_array_equal(out["tensor"][k], out["exact64"][k])
+
+
+def test_engine_chooses_its_kernel_from_the_sampled_block_mix():
+    """TPCF_ENGINE_TENSOR samples the share of pair-by-pair blocks and launches pair_fast_kernel above the limit
+    (tpcf_set_tensor_share_limit); either way the same integers."""
+    D, R, e, cfg = synth.make_config(5, n_d=40_000, n_r=30_000)         # fine bins: every block is pair by pair
+    with T.Context(cfg.nbins, e, "explicit") as c:
+        c.load("D", D)
+        c.load("R", R)
+        a = full(*c.count("DR"))
+        st = c.stats()
+        assert st["lookup_share"] > 0.9 and st["block"] == 256
+        c.set_tensor_share_limit(1.0)
+        b = full(*c.count("DR"))
+        assert c.stats()["block"] == 128
+        np.testing.assert_array_equal(a, b)
+        c.set_tensor_share_limit(0.0)
+        np.testing.assert_array_equal(full(*c.count("DR")), a)
+        assert c.stats()["block"] == 256
+        with pytest.raises(T.TpcfError):
+            c.set_tensor_share_limit(1.5)

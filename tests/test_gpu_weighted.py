@@ -33,6 +33,7 @@ def test_cross_catalog_counts_and_estimator(engine, oracle_threads):
     want = {"D1D2": nd * n2, "DR": nd * nr, "D2R": n2 * nr, "RR": nr * (nr - 1) // 2}
     with T.Context(cfg.nbins, e, "explicit") as c:
         c.set_engine(engine)
+        c.set_tensor_share_limit(1.0)
         with pytest.raises(T.TpcfError) as ei:
             c.count("D1D2")
         assert ei.value.status == T.TPCF_ESTATE                       # D2 not loaded yet

@@ -18,6 +18,7 @@ ENGINES = ("tensor", "fast", "exact64")
 def box_ctx(nbins, edges, max_abs, engine="tensor", mode="explicit"):
     c = T.Context(nbins, edges, mode, max_abs_coord=max_abs)
     c.set_engine(engine)
+    c.set_tensor_share_limit(1.0)          # "tensor" means pair_tensor_kernel here, whatever the block mix
     return c
 
 
