@@ -76,13 +76,13 @@ __device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) {
     return d;
 }
 
-// TF32 split of an fp32 value: hi = x rounded to nearest (ties away) to TF32's 10 mantissa bits (cvt.rna: the low 13 bits
-// of the result are zero, so it is exactly representable whatever the tensor core does with those bits); x - hi is exact
-// in fp32 and |x - hi| <= 2^-11 |x|
+// TF32 split of an fp32 value: hi = x rounded to nearest to TF32's 11-bit significand by Veltkamp's splitting,
+// c = fl(x (2^13 + 1)), hi = fl(c - fl(c - x)): three FMA-pipe instructions (that pipe idles in the tensor kernel, while the
+// integer form of the rounding would load the ALU pipe, its busiest); the low 13 bits of hi are zero, so it is exactly
+// representable whatever the tensor core does with those bits; x - hi is exact in fp32 and |x - hi| <= 2^-11 |x|
 __device__ __forceinline__ float tf32_hi(float x) {
-    uint32_t r;
-    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(x));
-    return __uint_as_float(r);
+    const float c = __fmul_rn(x, 8193.0f);
+    return __fsub_rn(c, __fsub_rn(c, x));
 }
 
 // ---- exact classification (fp64), shared by the recheck path and the fp64 engine -----------------------
@@ -928,7 +928,6 @@ __device__ __noinline__ void tc_exact_rows(SlowCtx* s, unsigned todo, uint32_t i
 struct TcRow {
     float sx, sy, sz;           // the row relative to the tile centre (for the lookup recount)
     float dt1, dt2, hmax;       // mid_0 - mid_e of the further edges, largest band half width
-    float g;                    // guard of the cell-lookup path for this row's block
     int mode, k, we;            // this row's mode, first band, edges the warp runs
 };
 
@@ -936,10 +935,38 @@ struct TcRow {
 template <int MAP>
 __device__ __forceinline__ void tc_bin(const TcRow& pd, uint32_t taddr, const float4* __restrict__ xs, uint32_t j0, bool mask,
                                        const WinTables& wt, const Lookup& lk, SlowCtx* slow, uint2* rq, unsigned& qn,
-                                       uint32_t iwarp, uint32_t n_i, uint32_t n_j, unsigned (&npath)[7]) {
+                                       uint32_t iwarp, uint32_t n_i, uint32_t n_j, float bg, int owner, unsigned (&npath)[7]) {
     const bool win = pd.mode <= kMaxWinEdges;
     bool flagged = false;
-    if (pd.we <= kMaxWinEdges) {                    // warp-uniform
+    if (pd.we == 1) {                               // warp-uniform; 95 % of the blocks: the leanest path
+        unsigned c0 = 0;
+        float m = 3.0e38f;
+#pragma unroll 1
+        for (int half = 0; half < kTcSubJ / 64; ++half) {
+            uint32_t v[64];
+            TPCF_TMEM_LD32(v, 0, taddr + half * 64);
+            TPCF_TMEM_LD32(v, 32, taddr + half * 64 + 32);
+            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+            unsigned ca = 0, cb = 0;                // independent chains
+            float ma = 3.0e38f, mb = 3.0e38f;
+#pragma unroll
+            for (int j = 0; j < 64; j += 4) {
+                ca += v[j] >> 31;
+                cb += v[j + 1] >> 31;
+                ca += v[j + 2] >> 31;
+                cb += v[j + 3] >> 31;
+                ma = fminf(ma, fminf(fabsf(__uint_as_float(v[j])), fabsf(__uint_as_float(v[j + 1]))));
+                mb = fminf(mb, fminf(fabsf(__uint_as_float(v[j + 2])), fabsf(__uint_as_float(v[j + 3]))));
+            }
+            c0 += ca + cb;
+            m = fminf(m, fminf(ma, mb));
+        }
+        flagged = m <= pd.hmax;
+        if (win && !flagged) {                      // c0 pairs below the edge, the rest of the kTcSubJ above it
+            if (c0) atomicAdd(wt.whist + wt.band_slot[pd.k], c0);
+            if (c0 != kTcSubJ) atomicAdd(wt.whist + wt.band_slot[pd.k + 1], kTcSubJ - c0);
+        }
+    } else if (pd.we <= kMaxWinEdges) {             // warp-uniform
         unsigned c0 = 0, c1 = 0, c2 = 0;
         float m = 3.0e38f;
 #pragma unroll 1
@@ -948,21 +975,7 @@ __device__ __forceinline__ void tc_bin(const TcRow& pd, uint32_t taddr, const fl
             TPCF_TMEM_LD32(v, 0, taddr + half * 64);
             TPCF_TMEM_LD32(v, 32, taddr + half * 64 + 32);
             asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-            if (pd.we == 1) {
-                unsigned ca = 0, cb = 0;                // independent chains
-                float ma = 3.0e38f, mb = 3.0e38f;
-#pragma unroll
-                for (int j = 0; j < 64; j += 4) {
-                    ca += v[j] >> 31;
-                    cb += v[j + 1] >> 31;
-                    ca += v[j + 2] >> 31;
-                    cb += v[j + 3] >> 31;
-                    ma = fminf(ma, fminf(fabsf(__uint_as_float(v[j])), fabsf(__uint_as_float(v[j + 1]))));
-                    mb = fminf(mb, fminf(fabsf(__uint_as_float(v[j + 2])), fabsf(__uint_as_float(v[j + 3]))));
-                }
-                c0 += ca + cb;
-                m = fminf(m, fminf(ma, mb));
-            } else if (pd.we == 2) {
+            if (pd.we == 2) {
 #pragma unroll
                 for (int j = 0; j < 64; ++j) {
                     const float q = __uint_as_float(v[j]), q1 = __fadd_rn(q, pd.dt1);
@@ -985,27 +998,29 @@ __device__ __forceinline__ void tc_bin(const TcRow& pd, uint32_t taddr, const fl
         if (win && !flagged) {
             // c_e = pairs below edge e (e < we); the rest of the kTcSubJ lies above the last edge
             const unsigned T = kTcSubJ;
-            const unsigned n0 = c0, n1 = (pd.we >= 2 ? c1 : T) - c0, n2 = pd.we >= 2 ? (pd.we >= 3 ? c2 : T) - c1 : 0u, n3 = pd.we >= 3 ? T - c2 : 0u;
+            const unsigned n0 = c0, n1 = c1 - c0, n2 = (pd.we >= 3 ? c2 : T) - c1, n3 = pd.we >= 3 ? T - c2 : 0u;
             if (n0) atomicAdd(wt.whist + wt.band_slot[pd.k], n0);
             if (n1) atomicAdd(wt.whist + wt.band_slot[pd.k + 1], n1);
             if (n2) atomicAdd(wt.whist + wt.band_slot[pd.k + 2], n2);
             if (n3) atomicAdd(wt.whist + wt.band_slot[pd.k + 3], n3);
         }
-        npath[0] += pd.we == 1;
-        npath[1] += pd.we == 2;
-        npath[2] += pd.we == 3;
+        ++npath[pd.we == 2 ? 1 : 2];
     } else {
         ++npath[3];
     }
-    const unsigned lkrows = __ballot_sync(0xffffffffu, (win && flagged) || pd.mode == 4);
-    const unsigned ex = __ballot_sync(0xffffffffu, pd.mode == 5);
-    if (lkrows) {
-        tc_lookup_rows<MAP>(lkrows, pd.sx, pd.sy, pd.sz, pd.g, xs, lk, slow, rq, qn, iwarp, j0, mask);
-        npath[4] += __popc(lkrows);
-    }
-    if (ex) {
-        tc_exact_rows(slow, ex, iwarp, n_i, j0, n_j, mask);
-        ++npath[5];
+    // rows that saw a pair inside a band, rows whose block needs the cell lookup or fp64: rare, one vote in the common case
+    if (__any_sync(0xffffffffu, (win && flagged) || pd.mode > kMaxWinEdges)) {
+        const unsigned lkrows = __ballot_sync(0xffffffffu, (win && flagged) || pd.mode == 4);
+        const unsigned ex = __ballot_sync(0xffffffffu, pd.mode == 5);
+        if (lkrows) {
+            const float g = __shfl_sync(0xffffffffu, bg, owner);        // the lookup guard of this row's block: only needed here
+            tc_lookup_rows<MAP>(lkrows, pd.sx, pd.sy, pd.sz, g, xs, lk, slow, rq, qn, iwarp, j0, mask);
+            npath[4] += __popc(lkrows);
+        }
+        if (ex) {
+            tc_exact_rows(slow, ex, iwarp, n_i, j0, n_j, mask);
+            ++npath[5];
+        }
     }
 }
 
@@ -1123,7 +1138,9 @@ __global__ void __launch_bounds__(kTcThreads, 4) pair_tensor_kernel(const __grid
         if (tid == 0)
             for (uint32_t n = 0; n < min(ntile, (uint32_t)kTcRing); ++n) fetch_tile(gch + n, ch + n);
 
-        int bmode = 4, bk = 0;              // window of (this thread's quad, tile (lane & 7) of the current batch of 8)
+        // window of (this thread's quad, tile (lane & 7) of the current batch of 8), packed: mode | edges the warp runs << 3 |
+        // first band << 6; the lookup guard beside it
+        int bpack = 4 | (4 << 3);
         float bg = 0.f;
         for (uint32_t t = 0; t < ntile; ++t) {
             const uint32_t n = gch + t, tabs = ch + t;
@@ -1132,17 +1149,26 @@ __global__ void __launch_bounds__(kTcThreads, 4) pair_tensor_kernel(const __grid
             const bool mask = p.tri && tabs == dch;
             if (t == 0 || (tabs & 7u) == 0) {               // windows of 8 tiles at a time, one per lane of the quad
                 const uint32_t su = (tabs & ~7u) + (lane & 7);
+                int bmode, bk;
                 window_of<MAP>(cq, p.ct[su], p.window != 0, wt, lk, bmode, bk, bg);
+                // the warp runs, per tile, the largest window loop one of its four quads needs (none: all rows pair by pair)
+                int wm = bmode <= kMaxWinEdges ? bmode : 0;
+                wm = max(wm, __shfl_xor_sync(0xffffffffu, wm, 8));
+                wm = max(wm, __shfl_xor_sync(0xffffffffu, wm, 16));
+                const int bwe = wm ? wm : kMaxWinEdges + 1;
+                bpack = bmode | (bwe << 3) | ((bmode > kMaxWinEdges ? 0 : min(bk, p.nbands - bwe)) << 6);
             }
             const int owner = (lane & ~7) | (int)(tabs & 7u);
+            const int pk = __shfl_sync(0xffffffffu, bpack, owner);
             TcRow rw;
-            rw.mode = __shfl_sync(0xffffffffu, bmode, owner);
-            rw.k = __shfl_sync(0xffffffffu, bk, owner);
-            rw.g = __shfl_sync(0xffffffffu, bg, owner);
-            if (mask && rw.mode <= kMaxWinEdges) rw.mode = 4;
-            const int wmax = __reduce_max_sync(0xffffffffu, rw.mode <= kMaxWinEdges ? rw.mode : 0);
-            rw.we = wmax ? wmax : kMaxWinEdges + 1;
-            rw.k = rw.mode > kMaxWinEdges ? 0 : min(rw.k, p.nbands - rw.we);
+            rw.mode = pk & 7;
+            rw.we = (pk >> 3) & 7;
+            rw.k = pk >> 6;
+            if (mask) {                                     // the diagonal tile: every row pair by pair (pairs j > i)
+                rw.mode = max(rw.mode, 4);
+                rw.we = kMaxWinEdges + 1;
+                rw.k = 0;
+            }
             const float4 sp = *reinterpret_cast<const float4*>(slot + kTcBBytes + kTcRowBytes);
             const float tx = __fsub_rn(cq.x, sp.x), ty = __fsub_rn(cq.y, sp.y), tz = __fsub_rn(cq.z, sp.z);
             rw.sx = __fadd_rn(a.x, tx);
@@ -1191,7 +1217,7 @@ __global__ void __launch_bounds__(kTcThreads, 4) pair_tensor_kernel(const __grid
             mbar_wait(full_bar, gs & 1);
             asm volatile("tcgen05.fence::after_thread_sync;");
             tc_bin<MAP>(rw, tlane, reinterpret_cast<const float4*>(slot + kTcBBytes), tabs * kTcSubJ, mask, wt, lk, slow, rq, qn,
-                        ibase + warp * 32, p.n_i, p.n_j, npath);
+                        ibase + warp * 32, p.n_i, p.n_j, bg, owner, npath);
             ++gs;
         }
         const uint32_t nchunks = ntile;
@@ -1212,6 +1238,7 @@ __global__ void __launch_bounds__(kTcThreads, 4) pair_tensor_kernel(const __grid
     if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(kTcCols));
     if (tid == 0 && items_done) atomicAdd(p.counters + 2, items_done);
     if (lane == 0) {
+        npath[0] = gs - npath[1] - npath[2] - npath[3];      // the one-edge blocks are not counted one by one
 #pragma unroll
         for (int k = 0; k < 7; ++k)
             if (npath[k]) atomicAdd(p.counters + 3 + k, (unsigned long long)npath[k]);

@@ -23,9 +23,11 @@ KEEP_BITS = 25          # addends are kept down to 2^(e_max - KEEP_BITS)
 
 
 def rna_tf32(x):
-    """cvt.rna.tf32.f32: round to nearest, ties away from zero, to 10 mantissa bits (the low 13 bits end up zero)."""
-    b = np.ascontiguousarray(x, dtype=np.float32).view(np.uint32)
-    return ((b + np.uint32(0x1000)) & np.uint32(0xFFFFE000)).view(np.float32)
+    """The kernels' tf32_hi: Veltkamp's splitting c = fl(x (2^13 + 1)), hi = fl(c - fl(c - x)) in fp32 -- x rounded to nearest
+    to an 11-bit significand (the low 13 bits end up zero), |x - hi| <= 2^-11 |x|."""
+    x = np.ascontiguousarray(x, dtype=np.float32)
+    c = (x * np.float32(8193.0)).astype(np.float32)
+    return (c - (c - x).astype(np.float32)).astype(np.float32)
 
 
 def split2(x):
