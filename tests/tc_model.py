@@ -22,7 +22,7 @@ U = 2.0 ** -24
 KEEP_BITS = 25          # addends are kept down to 2^(e_max - KEEP_BITS)
 
 
-def rna_tf32(x):
+def rn11_tf32(x):
     """The kernels' tf32_hi: Veltkamp's splitting c = fl(x (2^13 + 1)), hi = fl(c - fl(c - x)) in fp32 -- x rounded to nearest
     to an 11-bit significand (the low 13 bits end up zero), |x - hi| <= 2^-11 |x|."""
     x = np.ascontiguousarray(x, dtype=np.float32)
@@ -32,16 +32,16 @@ def rna_tf32(x):
 
 def split2(x):
     x = np.asarray(x, dtype=np.float32)
-    hi = rna_tf32(x)
-    return hi, rna_tf32((x - hi).astype(np.float32))
+    hi = rn11_tf32(x)
+    return hi, rn11_tf32((x - hi).astype(np.float32))
 
 
 def split3(x):
     x = np.asarray(x, dtype=np.float32)
-    hi = rna_tf32(x)
+    hi = rn11_tf32(x)
     r = (x - hi).astype(np.float32)
-    mid = rna_tf32(r)
-    return hi, mid, rna_tf32((r - mid).astype(np.float32))
+    mid = rn11_tf32(r)
+    return hi, mid, rn11_tf32((r - mid).astype(np.float32))
 
 
 def _exponent(t):

@@ -7,7 +7,7 @@ import tc_model as M
 U = M.U
 
 
-def test_rna_split_is_exact_and_small():
+def test_tf32_split_is_exact_and_small():
     rng = np.random.default_rng(1)
     x = (rng.normal(size=200_000) * np.exp2(rng.integers(-20, 3, 200_000))).astype(np.float32)
     hi, lo = M.split2(x)
