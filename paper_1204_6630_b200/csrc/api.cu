@@ -401,7 +401,8 @@ tpcf_status enqueue_count(tpcf_ctx* ctx, tpcf_kind kind, const int64_t* rows_hos
         // (fine binnings, catalogs whose tiles are large against the scales binned): the share of such (8-row group, 128-row
         // tile) blocks is SAMPLED once per (kind, catalogs, tables) and kept with the plan
         bool tensor_kernel = ctx->engine == TPCF_ENGINE_TENSOR && !p.prune;      // pruning lives in the FFMA2 kernel
-        if (tensor_kernel) {
+        bool lookup_heavy = false;
+        if (ctx->engine != TPCF_ENGINE_EXACT64) {
             float share = -1.f;
             PlanCache* pc = rows_host ? nullptr : &ctx->plans[kind];
             if (pc && pc->share >= 0.f) share = pc->share;
@@ -416,11 +417,12 @@ tpcf_status enqueue_count(tpcf_ctx* ctx, tpcf_kind kind, const int64_t* rows_hos
                 if (pc) pc->share = share;
             }
             ctx->stats.lookup_share = share;
-            tensor_kernel = share <= ctx->tensor_share_limit;
+            tensor_kernel = tensor_kernel && share <= ctx->tensor_share_limit;
+            lookup_heavy = share >= 0.8f && !p.prune;       // the FFMA2 kernel's variant for 3 CTAs per SM (kernels.cu)
         }
         if (ctx->engine == TPCF_ENGINE_EXACT64) p.prune = 0;
         const cudaError_t le = ctx->engine == TPCF_ENGINE_FAST || (ctx->engine == TPCF_ENGINE_TENSOR && !tensor_kernel)
-                                   ? launch_pairs_fast(p, ctx->ft.map, ctx->sm_count, st, &li)
+                                   ? launch_pairs_fast(p, ctx->ft.map, ctx->sm_count, st, &li, lookup_heavy)
                                : ctx->engine == TPCF_ENGINE_TENSOR ? launch_pairs_tensor(p, ctx->ft.map, ctx->sm_count, st, &li)
                                                                    : launch_pairs_exact64(p, ctx->sm_count, st, &li);
         if (le != cudaSuccess) {

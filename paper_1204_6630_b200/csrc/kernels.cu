@@ -624,8 +624,11 @@ __device__ __forceinline__ void flush_slots(unsigned* hist, int nslots, const ui
 // The pair kernel.  Persistent CTAs of 8 independent warps.  A warp item = kWarpI = 256 consecutive i-rows (one 8-row group per lane)
 // against the j-rows of one plan item; the warp streams those j-rows through its own 2-slot shared-memory ring in
 // 128-row chunks (TMA bulk copies behind mbarriers, issued by lane 0), so no CTA-wide barrier sits in the loop.
-template <int MAP>
-__global__ void __launch_bounds__(kThreads, 2) pair_fast_kernel(const __grid_constant__ PairParams p) {
+// MINB = resident CTAs per SM the register budget is cut for: 2 (128 registers: the window loops need them) or, for launches
+// whose blocks almost all take the per-pair cell lookup (fine binnings), 3 (80 registers, the window loops spill, the lookup
+// loop gets 24 warps per SM to hide its LDS -> ATOMS chains: config 5 -4 %).
+template <int MAP, int MINB>
+__global__ void __launch_bounds__(kThreads, MINB) pair_fast_kernel(const __grid_constant__ PairParams p) {
     extern __shared__ __align__(128) unsigned char smem[];
     const FastSmem L = fast_smem_layout(p.ncells, p.nbands, p.nbins);
     unsigned* hist = reinterpret_cast<unsigned*>(smem + L.hist);
@@ -1910,9 +1913,10 @@ cudaError_t launch_gather(const double4* src64, const uint64_t* pos, uint64_t nr
     return cudaGetLastError();
 }
 
-cudaError_t launch_pairs_fast(const PairParams& p, CellMap map, int sm_count, cudaStream_t st, LaunchInfo* info) {
+cudaError_t launch_pairs_fast(const PairParams& p, CellMap map, int sm_count, cudaStream_t st, LaunchInfo* info, bool lookup_heavy) {
     const size_t smem = fast_smem_layout(p.ncells, p.nbands, p.nbins).total;
-    auto kern = (map == CellMap::LogBits) ? pair_fast_kernel<(int)CellMap::LogBits> : pair_fast_kernel<(int)CellMap::SqrtLin>;
+    auto kern = lookup_heavy ? ((map == CellMap::LogBits) ? pair_fast_kernel<(int)CellMap::LogBits, 3> : pair_fast_kernel<(int)CellMap::SqrtLin, 3>)
+                             : ((map == CellMap::LogBits) ? pair_fast_kernel<(int)CellMap::LogBits, 2> : pair_fast_kernel<(int)CellMap::SqrtLin, 2>);
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     int per_sm = 0;
@@ -1948,7 +1952,7 @@ cudaError_t launch_pairs_tensor(const PairParams& p, CellMap map, int sm_count, 
     per_sm = std::min(per_sm, (int)(512 / kTcCols));
     // fine binnings (thousands of lookup cells: config 5) leave room for fewer than 3 such CTAs per SM, i.e. too few
     // warps to hide the step-by-step MMA pipeline: those run the FFMA2 kernel
-    if (per_sm < 3) return launch_pairs_fast(p, map, sm_count, st, info);
+    if (per_sm < 3) return launch_pairs_fast(p, map, sm_count, st, info, false);
     const uint64_t citems = (uint64_t)p.n_items_part * (kTileI / kTcThreads) * p.jsplit;
     int grid = (int)std::min<uint64_t>((uint64_t)sm_count * per_sm, std::max<uint64_t>(citems, 1));
     kern<<<grid, kTcThreads, smem, st>>>(p);

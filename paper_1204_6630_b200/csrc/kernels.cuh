@@ -91,7 +91,8 @@ cudaError_t launch_row_keys(const int64_t* rows, uint64_t nrows, uint64_t n_src,
 // dst[k] = src[pos[k]] for k < nrows, padding point after
 cudaError_t launch_gather(const double4* src64, const uint64_t* pos, uint64_t nrows, uint64_t nrows_pad, double4* dst64,
                           cudaStream_t st);
-cudaError_t launch_pairs_fast(const PairParams& p, CellMap map, int sm_count, cudaStream_t st, LaunchInfo* info);
+// lookup_heavy: almost every block takes the per-pair cell lookup: the variant compiled for 3 CTAs per SM
+cudaError_t launch_pairs_fast(const PairParams& p, CellMap map, int sm_count, cudaStream_t st, LaunchInfo* info, bool lookup_heavy);
 cudaError_t launch_pairs_tensor(const PairParams& p, CellMap map, int sm_count, cudaStream_t st, LaunchInfo* info);
 // out[0] += sampled (8-row group, 128-row tile) blocks the tensor kernel would count pair by pair, out[1] += blocks sampled
 cudaError_t launch_sample_modes(const PairParams& p, CellMap map, uint32_t nsamples, unsigned long long* out, cudaStream_t st);
