@@ -395,8 +395,6 @@ tpcf_status enqueue_count(tpcf_ctx* ctx, tpcf_kind kind, const int64_t* rows_hos
         CU(cudaEventRecord(kev.first, st), "cudaEventRecord");
     }
     {
-        // TPCF_ENGINE_TENSOR runs the FFMA2 kernel where too many pairs would take the tensor kernel's slow rows
-        // (fine binnings, catalogs whose tiles are large against the scales binned: tables.h lookup_pair_share)
         // TPCF_ENGINE_TENSOR runs the FFMA2 kernel where too many pairs would take the tensor kernel's pair-by-pair rows
         // (fine binnings, catalogs whose tiles are large against the scales binned): the share of such (8-row group, 128-row
         // tile) blocks is SAMPLED once per (kind, catalogs, tables) and kept with the plan
