@@ -415,7 +415,10 @@ tpcf_status enqueue_count(tpcf_ctx* ctx, tpcf_kind kind, const int64_t* rows_hos
                 if (pc) pc->share = share;
             }
             ctx->stats.lookup_share = share;
-            tensor_kernel = tensor_kernel && share <= ctx->tensor_share_limit;
+            // ... unless the catalogs are so small that pair_fast_kernel's 2048-row plan items cannot fill the GPU: the
+            // tensor kernel's CTAs take 128 rows each (config 1: 48 CTAs against 512)
+            const bool tiny = (uint64_t)p.n_items_part * p.jsplit < 2ull * (uint64_t)ctx->sm_count && ctx->tensor_share_limit > 0.f;
+            tensor_kernel = tensor_kernel && (share <= ctx->tensor_share_limit || tiny);
             lookup_heavy = share >= 0.8f && !p.prune;       // the FFMA2 kernel's variant for 3 CTAs per SM (kernels.cu)
         }
         if (ctx->engine == TPCF_ENGINE_EXACT64) p.prune = 0;

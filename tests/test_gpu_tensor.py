@@ -246,7 +246,7 @@ def test_tensor_engine_equals_fp64_engine_on_unusual_binnings_and_settings(case)
 def test_engine_chooses_its_kernel_from_the_sampled_block_mix():
     """TPCF_ENGINE_TENSOR samples the share of pair-by-pair blocks and launches pair_fast_kernel above the limit
     (tpcf_set_tensor_share_limit); either way the same integers."""
-    D, R, e, cfg = synth.make_config(5, n_d=40_000, n_r=30_000)         # fine bins: every block is pair by pair
+    D, R, e, cfg = synth.make_config(5, n_d=400_000, n_r=30_000)        # fine bins: every block is pair by pair
     with T.Context(cfg.nbins, e, "explicit") as c:
         c.load("D", D)
         c.load("R", R)
