@@ -293,6 +293,52 @@ tpcf_status tpcf_plan_item_pairs(const tpcf_ctx* ctx, tpcf_kind kind, uint64_t n
  * measure the tensor core's accumulation error with.  TPCF_EINVAL for NULL pointers or ntiles == 0 or > 65535. */
 tpcf_status tpcf_tensor_probe(tpcf_ctx* ctx, const float* s_rows, const float* b_rows, size_t ntiles, float* q_out);
 
+/* ---- a count that allocates nothing ---------------------------------------------------------------------- */
+
+/*
+ * tpcf_count_static -- one pair count (the histogram over theta of the separations of all pairs;
+ *   PAPER.md:37-38), from RA/Dec rows to histogram, WITHOUT any allocation of device memory: no cudaMalloc, no cudaFree,
+ *   no allocating library routine, on the first call or any later one.  It needs no context.
+ *
+ *   Who needs it.  tpcf_load and tpcf_count allocate (catalog arrays, sort scratch, accumulators, the plan).  A caller
+ *   cannot always let a library do that: all device memory may already sit in the host application's own pool (a
+ *   framework's caching allocator), so that a raw cudaMalloc fails or eats into what the pool believes it owns; a
+ *   service may have to prove its per-GPU memory use at start-up; and cudaMalloc / cudaFree synchronise the whole
+ *   device, which a loop with other streams in flight cannot tolerate.  Such a caller hands in device pointers it
+ *   already owns and gets the result in a device buffer it already owns.
+ *
+ *   How.  The scratch of the count (the fp64 unit vectors made from the rows, the thresholds, the uint64 accumulators,
+ *   the work counter, the bad-row flag) lives in one fixed array inside the library's device image, about 2.07 MiB,
+ *   which every GPU that loads the image holds until the process exits.  Hence the limits:
+ *     rows:  n_i + n_j <= TPCF_STATIC_MAX_ROWS;   bins:  nbins <= TPCF_STATIC_MAX_BINS;
+ *   anything larger is refused with TPCF_EINVAL and a message that names the limit.  The pairs are counted by a variant
+ *   of the TPCF_ENGINE_EXACT64 kernel (fp64 squared chord against 4 sin^2(e_k/2)), so the histogram is the one
+ *   tpcf_count gives with any engine, up to fp64 ties; at these sizes the fp64 count takes milliseconds.
+ *
+ *   nbins, theta_deg, mode   the binning, as for tpcf_create (host memory).
+ *   radec_i_dev, n_i         DEVICE pointer to n_i rows of (RA, Dec) in degrees, row-major, dtype dt.
+ *   radec_j_dev, n_j         DEVICE pointer to a second catalog: all n_i * n_j pairs are counted (DR).
+ *                            NULL with n_j = 0: the n_i (n_i - 1) / 2 pairs i < j of the first catalog (DD, RR).
+ *   hist_dev                 DEVICE buffer of nbins + 2 uint64: {under, bin_0 .. bin_{n-1}, over} (tpcf_count_async's layout).
+ *   cuda_stream              the cudaStream_t to work on (NULL: the default stream).  The call returns after that stream
+ *                            has drained (it reads the bad-row flag back), so hist_dev is complete on return.
+ *   err, err_len             optional host buffer for a message when the status is not TPCF_OK (there is no context
+ *                            to ask).
+ *
+ *   One array serves every call.  It keeps whatever the last call left there; the call clears the parts that must
+ *   start at zero itself.  Two calls that overlap in time on one GPU (two host threads, two streams) corrupt each other:
+ *   serialise them.  Calls on different GPUs do not interact.
+ *   The first call on each device looks up where the array lives on that device (the device current at the call is the
+ *   one used) and may load the library's device image; make that first call before starting any stream capture.
+ *   Errors: TPCF_EINVAL (limits, NULL pointers, bad edges, a non-finite value, |RA| > 1e6 or |Dec| > 90 in a row);
+ *   TPCF_ECUDA (no usable sm_100 device -- there is no CPU fallback -- or a CUDA failure).
+ */
+#define TPCF_STATIC_MAX_ROWS 65536
+#define TPCF_STATIC_MAX_BINS 4096
+tpcf_status tpcf_count_static(int nbins, const double* theta_deg, tpcf_binning mode, const void* radec_i_dev, size_t n_i,
+                              const void* radec_j_dev, size_t n_j, tpcf_dtype dt, uint64_t* hist_dev /* device, nbins+2 */,
+                              void* cuda_stream, char* err, size_t err_len);
+
 #ifdef __cplusplus
 }
 #endif

@@ -36,7 +36,9 @@ EXPORTS = (
     "tpcf_plan", "tpcf_plan_item_pairs", "tpcf_set_kernel_timing", "tpcf_get_kernel_times", "tpcf_set_window",
     "tpcf_get_bands", "tpcf_window_host", "tpcf_tensor_probe", "tpcf_create_r", "tpcf_load_xyz", "tpcf_set_pruning", "tpcf_count_all", "tpcf_count_all_async",
     "tpcf_estimate_cross", "tpcf_set_weights", "tpcf_count_weighted", "tpcf_set_tensor_share_limit",
+    "tpcf_count_static",
 )
+TPCF_STATIC_MAX_ROWS, TPCF_STATIC_MAX_BINS = 65536, 4096
 
 
 class TpcfError(RuntimeError):
@@ -102,6 +104,7 @@ def lib() -> ctypes.CDLL:
             "tpcf_classify_fast": [vp, ctypes.c_float, ctypes.POINTER(i32)],
             "tpcf_plan": [vp, i32, u64, u64, ctypes.POINTER(u64)],
             "tpcf_plan_item_pairs": [vp, i32, u64, u64, u64, ctypes.POINTER(u64)],
+            "tpcf_count_static": [i32, vp, i32, vp, sz, vp, sz, i32, vp, vp, ctypes.c_char_p, sz],
         }
         for name, args in sig.items():
             fn = getattr(L, name)
@@ -217,6 +220,26 @@ def tpcf_count(ctx, kind: int, nbins: int, rows=None) -> Tuple[np.ndarray, int, 
 
 def tpcf_count_async(ctx, kind: int, hist_dev_ptr: int) -> None:
     _check(ctx, lib().tpcf_count_async(ctx, int(kind), ctypes.c_void_p(hist_dev_ptr)))
+
+
+def tpcf_count_static(nbins: int, theta_deg, mode, radec_i_dev_ptr: int, n_i: int, radec_j_dev_ptr: Optional[int], n_j: int,
+                      dtype: int, hist_dev_ptr: int, stream_ptr: int = 0) -> None:
+    """The count that never allocates device memory (include/tpcf.h): for callers whose GPU memory is already spoken for
+    (a framework's pool owns it all, a fixed per-GPU budget) or who cannot take the device-wide stall of cudaMalloc.
+    Inputs and the nbins + 2 uint64 output are DEVICE pointers the caller owns; radec_j_dev_ptr None/0 with n_j 0 counts
+    the pairs i < j of the first catalog.  At most TPCF_STATIC_MAX_ROWS rows (n_i + n_j) and TPCF_STATIC_MAX_BINS bins;
+    calls on one GPU must not overlap; returns when the stream has drained."""
+    mode = _MODES.get(mode, mode)
+    th = np.ascontiguousarray(theta_deg, dtype=np.float64)
+    need = nbins + 1 if mode == TPCF_EXPLICIT else 2
+    if th.ndim != 1 or th.shape[0] != need:
+        raise TpcfError(TPCF_EINVAL, f"theta_deg must hold {need} values")
+    err = ctypes.create_string_buffer(512)
+    st = lib().tpcf_count_static(int(nbins), _np_ptr(th), int(mode), ctypes.c_void_p(radec_i_dev_ptr), int(n_i),
+                                 ctypes.c_void_p(radec_j_dev_ptr or None), int(n_j), int(dtype), ctypes.c_void_p(hist_dev_ptr),
+                                 ctypes.c_void_p(stream_ptr or None), err, len(err))
+    if st != TPCF_OK:
+        raise TpcfError(st, err.value.decode())
 
 
 def tpcf_count_all(ctx, nbins: int):
