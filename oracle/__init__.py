@@ -47,6 +47,8 @@ def lib() -> ctypes.CDLL:
         L.orc_wsum_cross.restype = i32
         L.orc_estimate.argtypes = [vp, vp, vp, i32, ctypes.c_uint64, ctypes.c_uint64, vp]
         L.orc_estimate.restype = None
+        L.orc_estimate_cross.argtypes = [vp, vp, vp, vp, i32, ctypes.c_uint64, ctypes.c_uint64, ctypes.c_uint64, vp]
+        L.orc_estimate_cross.restype = None
         _lib = L
     return _lib
 
@@ -175,6 +177,14 @@ def estimate(dd, dr, rr, n_d: int, n_r: int) -> np.ndarray:
     rr = np.ascontiguousarray(rr, dtype=np.uint64)
     w = np.empty(dd.shape[0], dtype=np.float64)
     lib().orc_estimate(_ptr(dd), _ptr(dr), _ptr(rr), dd.shape[0], int(n_d), int(n_r), _ptr(w))
+    return w
+
+
+def estimate_cross(d1d2, d1r, d2r, rr, n_1: int, n_2: int, n_r: int) -> np.ndarray:
+    """Cross-correlation estimator w12_k = (D1D2/n12 - D1R/n1r - D2R/n2r + RR/nrr) / (RR/nrr) (orc_estimate_cross)."""
+    a = [np.ascontiguousarray(x, dtype=np.uint64) for x in (d1d2, d1r, d2r, rr)]
+    w = np.empty(a[0].shape[0], dtype=np.float64)
+    lib().orc_estimate_cross(_ptr(a[0]), _ptr(a[1]), _ptr(a[2]), _ptr(a[3]), a[0].shape[0], int(n_1), int(n_2), int(n_r), _ptr(w))
     return w
 
 

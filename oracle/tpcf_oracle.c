@@ -19,7 +19,8 @@
  *
  * Pins (tests/test_oracle_pins.py, run with -m "not gpu"): hand catalogs P1, totals P2,
  * numpy.histogram of arccos of a Gram matrix P3, great-circle ring closed form P4, integer
- * identities P5, uniform-sphere closed form P6, null test P7, Eq. 1 hand case P8, acos-vs-asin P9;
+ * identities P5, uniform-sphere closed form P6, null test P7, Eq. 1 hand case P8 (cross estimator: hand case 3/4,
+ * w12 = 1/N identity and null test, P8x), acos-vs-asin P9;
  * 3-D variant (orc_count_*_xyz): cubic-lattice multiplicities X1, totals X2, unit-cube distance
  * distribution X3, unit vectors with chord edges reproduce the angular histogram X4.
  * Unpinned: absolute w(theta) values on the MICE catalogs / Fig. 1 (data not available).
@@ -165,6 +166,29 @@ void orc_estimate(const uint64_t *dd, const uint64_t *dr, const uint64_t *rr, in
         if (rr[k] == 0) { w[k] = NAN; continue; }
         double fdd = (double)dd[k] / ndd, fdr = (double)dr[k] / ndr, frr = (double)rr[k] / nrr;
         w[k] = (fdd - 2.0 * fdr + frr) / frr;
+    }
+}
+
+/*
+ * Cross-correlation of two data catalogs D1, D2 against one random catalog R (PAPER.md:16
+ * "cross-correlation"; the form of Eq. 1, with the data-data term split over the two catalogs):
+ *   w12_k = (D1D2_k/n12 - D1R_k/n1r - D2R_k/n2r + RR_k/nrr) / (RR_k/nrr),
+ *   n12 = N_1 N_2, n1r = N_1 N_R, n2r = N_2 N_R (all ordered pairs), nrr = N_R(N_R-1)/2;  RR_k = 0 -> NaN (A14).
+ * With D2 = D1 = D this is NOT orc_estimate (D1D2 would count ordered pairs and self-pairs); it is its own definition.
+ * Pins: hand case 3/4, null test, sign test of each cross term (tests/test_oracle_pins.py).
+ */
+void orc_estimate_cross(const uint64_t *d1d2, const uint64_t *d1r, const uint64_t *d2r, const uint64_t *rr, int nbins,
+                        uint64_t n_1, uint64_t n_2, uint64_t n_r, double *w)
+{
+    double n12 = (double)n_1 * (double)n_2;
+    double n1r = (double)n_1 * (double)n_r;
+    double n2r = (double)n_2 * (double)n_r;
+    double nrr = 0.5 * (double)n_r * ((double)n_r - 1.0);
+    for (int k = 0; k < nbins; ++k) {
+        if (rr[k] == 0) { w[k] = NAN; continue; }
+        double f12 = (double)d1d2[k] / n12, f1r = (double)d1r[k] / n1r, f2r = (double)d2r[k] / n2r;
+        double frr = (double)rr[k] / nrr;
+        w[k] = (f12 - f1r - f2r + frr) / frr;
     }
 }
 

@@ -262,6 +262,35 @@ def test_p8_eq1_hand_case_and_same_catalog():
     np.testing.assert_allclose(w[ok], 2.0 / 500, rtol=0, atol=1e-12)
 
 
+def test_p8x_cross_estimator_hand_case_identity_and_null():
+    """orc_estimate_cross (the form of PAPER.md:20-25 Eq. 1 with the data term split over two catalogs).
+    Hand case: N_1 = 3, N_2 = 2, N_R = 4, one bin, D1D2 = 4, D1R = 5, D2R = 3, RR = 3 -> n12 = 6, n1r = 12, n2r = 8, nrr = 6:
+    (4/6 - 5/12 - 3/8 + 3/6) / (3/6) = (3/8) / (1/2) = 3/4.  Each term moved on its own changes w by a hand-computed step,
+    so a swapped or mis-signed term fails."""
+    w = oracle.estimate_cross([4], [5], [3], [3], 3, 2, 4)
+    assert abs(w[0] - 0.75) < 1e-15
+    assert abs(oracle.estimate_cross([5], [5], [3], [3], 3, 2, 4)[0] - (0.75 + (1 / 6) / 0.5)) < 1e-15      # +1 pair in D1D2
+    assert abs(oracle.estimate_cross([4], [6], [3], [3], 3, 2, 4)[0] - (0.75 - (1 / 12) / 0.5)) < 1e-15     # +1 pair in D1R
+    assert abs(oracle.estimate_cross([4], [5], [4], [3], 3, 2, 4)[0] - (0.75 - (1 / 8) / 0.5)) < 1e-15      # +1 pair in D2R
+    assert math.isnan(oracle.estimate_cross([1], [1], [1], [0], 5, 5, 5)[0])
+    # the same N rows as D1, D2 and R: the three cross counts are 2 DD_k and RR_k = DD_k in bins without theta = 0
+    #   => w12_k = 1 - 2 nrr / N^2 = 1/N exactly
+    D, _, e, _ = synth.make_config(1, n_d=400, n_r=8)
+    d = oracle.radec_to_xyz(D)
+    dd, x = oracle.count_auto(d, e), oracle.count_cross(d, d, e)
+    w = oracle.estimate_cross(x.hist, x.hist, x.hist, dd.hist, 400, 400, 400)
+    np.testing.assert_allclose(w[dd.hist > 0], 1.0 / 400, rtol=0, atol=1e-12)
+    # null test: three independent uniform catalogs on one footprint => w12 consistent with 0 (a wrong sign gives +-2, +-1)
+    patch = (0.0, 20.0, -10.0, 10.0)
+    a, b, r = (xyz_of(synth.uniform_patch(n, patch, synth.SplitMix(s))) for n, s in ((4000, 31), (3000, 32), (6000, 33)))
+    e = synth.edges(8, 0.5, 10.0, "log")
+    t = oracle.host_threads()
+    ab, ar, br, rr = (oracle.count_cross(a, b, e, threads=t), oracle.count_cross(a, r, e, threads=t),
+                      oracle.count_cross(b, r, e, threads=t), oracle.count_auto(r, e, threads=t))
+    w = oracle.estimate_cross(ab.hist, ar.hist, br.hist, rr.hist, 4000, 3000, 6000)
+    assert np.all(np.abs(w) <= 5.0 / np.sqrt(np.minimum(ab.hist, rr.hist)))
+
+
 # ------------------------------------------------------------------ P9 two independent angle formulas, O6
 @pytest.mark.parametrize("idx", [1, 2, 5])
 def test_p9_acos_vs_asin_chord(idx):
