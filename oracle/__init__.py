@@ -47,6 +47,8 @@ def lib() -> ctypes.CDLL:
         L.orc_wsum_cross.restype = i32
         L.orc_estimate.argtypes = [vp, vp, vp, i32, ctypes.c_uint64, ctypes.c_uint64, vp]
         L.orc_estimate.restype = None
+        L.orc_count_triples.argtypes = [vp, sz, sz, sz, vp, i32, vp]
+        L.orc_count_triples.restype = i32
         L.orc_estimate_cross.argtypes = [vp, vp, vp, vp, i32, ctypes.c_uint64, ctypes.c_uint64, ctypes.c_uint64, vp]
         L.orc_estimate_cross.restype = None
         _lib = L
@@ -178,6 +180,31 @@ def estimate(dd, dr, rr, n_d: int, n_r: int) -> np.ndarray:
     w = np.empty(dd.shape[0], dtype=np.float64)
     lib().orc_estimate(_ptr(dd), _ptr(dr), _ptr(rr), dd.shape[0], int(n_d), int(n_r), _ptr(w))
     return w
+
+
+def count_triples(xyz: np.ndarray, edges, threads: int = 1) -> np.ndarray:
+    """Three-point counts of one catalog (orc_count_triples): dense uint64 array [nbins+2]^3 over the ascending slots
+    (a <= b <= c; 0 = under, 1..nbins = bins, nbins+1 = over) of the three sides of every triple i<j<k."""
+    xyz = np.ascontiguousarray(xyz, dtype=np.float64)
+    e = np.ascontiguousarray(edges, dtype=np.float64)
+    nb, n = e.shape[0] - 1, xyz.shape[0]
+    m = nb + 2
+    L = lib()
+    # rows [0, c) hold about (c/n)-dependent shares of the triples; many short spans balance the threads well enough
+    spans = _even_spans(n, threads * 16 if threads > 1 else 1)
+
+    def one(span):
+        h = np.zeros(m * m * m, dtype=np.uint64)
+        if L.orc_count_triples(_ptr(xyz), n, span[0], span[1], _ptr(e), nb, _ptr(h)) != 0:
+            raise ValueError("oracle triples: bad arguments")
+        return h
+
+    if threads <= 1 or len(spans) == 1:
+        parts = [one(sp) for sp in spans]
+    else:
+        with ThreadPoolExecutor(max_workers=threads) as ex:
+            parts = list(ex.map(one, spans))
+    return np.sum(parts, axis=0, dtype=np.uint64).reshape(m, m, m)
 
 
 def estimate_cross(d1d2, d1r, d2r, rr, n_1: int, n_2: int, n_r: int) -> np.ndarray:

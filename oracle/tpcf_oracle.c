@@ -23,6 +23,8 @@
  * w12 = 1/N identity and null test, P8x), acos-vs-asin P9;
  * 3-D variant (orc_count_*_xyz): cubic-lattice multiplicities X1, totals X2, unit-cube distance
  * distribution X3, unit vectors with chord edges reproduce the angular histogram X4.
+ * Three-point counts (orc_count_triples): octahedron and equator hand triples, total C(N,3), row permutation,
+ * side-marginal identity against orc_count_auto, brute-force numpy on 40 points (T1-T5).
  * Unpinned: absolute w(theta) values on the MICE catalogs / Fig. 1 (data not available).
  *
  * Build: gcc -O2 -ffp-contract=off -fPIC -shared tpcf_oracle.c -o libtpcf_oracle.so -lm
@@ -146,6 +148,44 @@ int orc_count_rows(const double *a, const int64_t *rows, size_t r_begin, size_t 
             one_pair(a + 3 * i, b + 3 * j, edges, cose, nbins, hist, near, mismatch);
         }
     }
+    return 0;
+}
+
+/*
+ * Three-point counts ("extending the work to higher order correlation functions",
+ * PAPER.md:89).  The paper names the extension and gives no formula; the plain definition used here (DESIGN.md
+ * section 15): every unordered triple i<j<k of one catalog is a spherical triangle with the three side angles
+ * theta_ij, theta_ik, theta_jk, each computed exactly as a pair is (O4: dot, clamp, acos) and put in a slot exactly as a
+ * pair is (O5: slot 0 = under, 1..n = bins, n+1 = over).  The triple is counted once, in cell (a, b, c) of a dense
+ * (n+2)^3 array, a <= b <= c the three slots in ascending order: hist3[(a*(n+2) + b)*(n+2) + c].  Hence
+ *   sum(hist3) = N(N-1)(N-2)/6 exactly, and
+ *   for every slot s:  sum over cells of hist3[a,b,c] * ([a==s] + [b==s] + [c==s]) = (N-2) * (pairs in slot s),
+ * because every pair is a side of exactly N-2 triples.  i runs over [i_begin, i_end) so that callers can split the work;
+ * hist3 is ACCUMULATED into.  No blocking, no pair-slot table: each side is recomputed from its two points.
+ */
+int orc_count_triples(const double *xyz, size_t npts, size_t i_begin, size_t i_end, const double *edges, int nbins,
+                      uint64_t *hist3)
+{
+    if (nbins < 1 || nbins + 1 > MAX_EDGES) return -1;
+    const size_t m = (size_t)nbins + 2;
+    for (size_t i = i_begin; i < i_end && i < npts; ++i)
+        for (size_t j = i + 1; j < npts; ++j)
+            for (size_t k = j + 1; k < npts; ++k) {
+                const double *p[3] = {xyz + 3 * i, xyz + 3 * j, xyz + 3 * k};
+                int slot[3];
+                for (int side = 0; side < 3; ++side) {          /* sides ij, ik, jk */
+                    const double *a = p[side == 2 ? 1 : 0], *b = p[side == 0 ? 1 : 2];
+                    double s = a[0] * b[0] + a[1] * b[1] + a[2] * b[2];
+                    if (s > 1.0) s = 1.0;
+                    if (s < -1.0) s = -1.0;
+                    slot[side] = bin_slot(acos(s) * 180.0 / M_PI, edges, nbins);
+                }
+                /* ascending order of the three slots */
+                if (slot[0] > slot[1]) { int t = slot[0]; slot[0] = slot[1]; slot[1] = t; }
+                if (slot[1] > slot[2]) { int t = slot[1]; slot[1] = slot[2]; slot[2] = t; }
+                if (slot[0] > slot[1]) { int t = slot[0]; slot[0] = slot[1]; slot[1] = t; }
+                ++hist3[((size_t)slot[0] * m + (size_t)slot[1]) * m + (size_t)slot[2]];
+            }
     return 0;
 }
 
