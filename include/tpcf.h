@@ -49,8 +49,9 @@ typedef enum { TPCF_DD = 0, TPCF_DR = 1, TPCF_RR = 2, TPCF_D1D2 = 3, TPCF_D2R = 
  *                       proven bound 43.7 x 2^-24 T of DESIGN.md section 4, which rests on the measured, bit-exactly
  *                       reproduced accumulation model of tests/tc_model.py), near blocks and fine binnings go through the
  *                       fp32 cell lookup of TPCF_ENGINE_FAST and, inside its guard band, the fp64 recheck: the
- *                       histograms equal those of TPCF_ENGINE_EXACT64.  Binnings whose lookup tables leave room for
- *                       fewer than 3 such CTAs per SM (config 5) run TPCF_ENGINE_FAST's kernel.
+ *                       histograms equal those of TPCF_ENGINE_EXACT64.  Launches in which more than a small share of the
+ *                       blocks would take that pair-by-pair path (fine binnings such as config 5; the share is sampled,
+ *                       see tpcf_set_tensor_share_limit) run TPCF_ENGINE_FAST's kernel instead.
  *   TPCF_ENGINE_FAST    the same windows with q formed by packed FP32 FMAs (FFMA2) on the CUDA cores, 8 i-rows per lane
  *                       against 64-row j-subtiles (guard band 3.0e-6 T, proven bound 29.1 x 2^-24 T); otherwise an O(1)
  *                       cell lookup against chord-space thresholds with privatised shared-memory histograms; every pair
@@ -115,6 +116,10 @@ tpcf_status tpcf_count(tpcf_ctx* ctx, tpcf_kind kind, uint64_t* hist_out, uint64
  *   context's stream (tpcf_set_stream) and writes nbins+2 uint64 {under, bin_0..bin_{n-1}, over} to the
  *   DEVICE buffer hist_dev when they complete.  The count is not stored for tpcf_estimate.  This is the
  *   entry point timed with CUDA events when the catalogs are already resident.
+ *   One exception to "without host synchronisation": the FIRST count of a kind after tpcf_load, tpcf_set_engine or
+ *   tpcf_set_guard_scale (engines other than EXACT64) samples the block mix that picks the kernel variant, reads two
+ *   words back and waits for the stream once; it may also allocate (plan, tables).  Later calls on the same catalogs
+ *   neither wait nor allocate.  The same holds for tpcf_count_all_async.
  */
 tpcf_status tpcf_count_async(tpcf_ctx* ctx, tpcf_kind kind, uint64_t* hist_dev /* device, nbins+2 */);
 
@@ -226,7 +231,9 @@ tpcf_status tpcf_set_tensor_share_limit(tpcf_ctx* ctx, double limit);
 tpcf_status tpcf_set_pruning(tpcf_ctx* ctx, int enabled);
 /* Work partition for multi-process runs (one process per GPU): this context enumerates only the tile
  * work items w with w % nparts == part; summing the histograms of all parts gives the full count
- * (integer, order-independent).  Default (0, 1). */
+ * (integer, order-independent).  Default (0, 1).  Every part must number the same items: with nparts > 1 the plan's
+ * chunking is fixed (balanced for 148 SMs) and does not depend on the GPU a rank runs on; all ranks must load the same
+ * catalogs (same sizes) and use the same nparts. */
 tpcf_status tpcf_set_partition(tpcf_ctx* ctx, int part, int nparts);
 
 /* Per-kernel device timing: when enabled, every later count records a CUDA event pair around its pair
@@ -243,7 +250,6 @@ typedef struct {
     int launches;            /* kernels launched by the last count */
     int grid, block, smem_bytes;   /* geometry of the pair kernel */
     int cells, cell_bits;    /* lookup cells of the fast engine and mantissa bits per octave */
-    int hist_copies;         /* privatised copies of each partial-histogram slot per CTA */
     float kernel_ms;         /* device time of the last synchronous count (CUDA events) */
     uint64_t win_blocks[6];  /* (warp of 256 i-rows, 64-row j-subtile) blocks -- tensor engine: (warp of 32 i-rows, 128-row j-tile) -- of the last synchronous count by path:
                                 counted by the 1-, 2-, 3-edge window loops, by the per-pair cell lookup; [4] = lanes of
@@ -278,8 +284,10 @@ tpcf_status tpcf_get_bands(const tpcf_ctx* ctx, int capacity, float* lo_out, flo
  * cell-lookup path).  0 <= lo2 <= hi2 < 64. */
 tpcf_status tpcf_window_host(const tpcf_ctx* ctx, float lo2, float hi2, int* first_band_out, int* n_edges_out);
 
-/* Number of tile work items of a full count of `kind` for catalog sizes (n_d, n_r), and the number of
- * pairs in item w: the partition arithmetic of tpcf_set_partition, testable without a GPU. */
+/* Number of tile work items of a full count of `kind` (TPCF_DD, TPCF_DR or TPCF_RR; the D2 kinds have a third size and
+ * are refused with TPCF_EINVAL) for catalog sizes (n_d, n_r), and the number of pairs in item w: the partition arithmetic
+ * of tpcf_set_partition, testable without a GPU.  With nparts > 1 set on the context the numbering is the fixed one every
+ * rank uses; with nparts == 1 it is the one this context's own counts use (balanced for its device once it has seen one). */
 tpcf_status tpcf_plan(const tpcf_ctx* ctx, tpcf_kind kind, uint64_t n_d, uint64_t n_r, uint64_t* n_items_out);
 tpcf_status tpcf_plan_item_pairs(const tpcf_ctx* ctx, tpcf_kind kind, uint64_t n_d, uint64_t n_r, uint64_t w,
                                  uint64_t* pairs_out);
@@ -292,6 +300,25 @@ tpcf_status tpcf_plan_item_pairs(const tpcf_ctx* ctx, tpcf_kind kind, uint64_t n
  * 3xTF32 tcgen05.mma of pair_tensor_kernel forms it (same operand split, same instruction, same read-back).  What the tests
  * measure the tensor core's accumulation error with.  TPCF_EINVAL for NULL pointers or ntiles == 0 or > 65535. */
 tpcf_status tpcf_tensor_probe(tpcf_ctx* ctx, const float* s_rows, const float* b_rows, size_t ntiles, float* q_out);
+
+/* ---- three-point counts ------------------------------------------------------------------------------------ */
+
+/*
+ * tpcf_count3 -- three-point counts of one loaded catalog ("extending the work to higher
+ *   order correlation functions"; the paper names the extension and gives no formula -- the definition is
+ *   DESIGN.md section 15's).  Every unordered triple i<j<k of the catalog is a triangle with three sides; each side gets
+ *   the result slot a pair gets (0 = under, 1..nbins = bin_0..bin_{n-1}, nbins+1 = over; same edges, same conventions as
+ *   tpcf_count), and the triple is counted once in the cell of its three slots in ascending order a <= b <= c:
+ *     hist3_out[(a * m + b) * m + c],  m = nbins + 2,  host memory, m^3 uint64 (cells that are not ascending stay 0).
+ *   sum(hist3_out) = N(N-1)(N-2)/6 exactly.  Brute force: every triple is enumerated (O(N^3) byte operations after one
+ *   O(N^2) fp64 classification of the pairs).  Angular and 3-D contexts alike.  Not part of the w(theta) headline.
+ *   Limits: N <= TPCF_COUNT3_MAX_ROWS (the N x N byte matrix of pair slots is scratch), nbins <= TPCF_COUNT3_MAX_BINS
+ *   (the m^3 partial histogram lives in shared memory); beyond them TPCF_EINVAL.  TPCF_ESTATE before the catalog is loaded.
+ *   tpcf_get_stats afterwards: kernel_ms of the two kernels, pairs = number of triples.
+ */
+#define TPCF_COUNT3_MAX_ROWS 16384
+#define TPCF_COUNT3_MAX_BINS 30
+tpcf_status tpcf_count3(tpcf_ctx* ctx, tpcf_cat which, uint64_t* hist3_out /* (nbins+2)^3 */);
 
 /* ---- a count that allocates nothing ---------------------------------------------------------------------- */
 

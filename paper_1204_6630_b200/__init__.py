@@ -36,9 +36,10 @@ EXPORTS = (
     "tpcf_plan", "tpcf_plan_item_pairs", "tpcf_set_kernel_timing", "tpcf_get_kernel_times", "tpcf_set_window",
     "tpcf_get_bands", "tpcf_window_host", "tpcf_tensor_probe", "tpcf_create_r", "tpcf_load_xyz", "tpcf_set_pruning", "tpcf_count_all", "tpcf_count_all_async",
     "tpcf_estimate_cross", "tpcf_set_weights", "tpcf_count_weighted", "tpcf_set_tensor_share_limit",
-    "tpcf_count_static",
+    "tpcf_count_static", "tpcf_count3",
 )
 TPCF_STATIC_MAX_ROWS, TPCF_STATIC_MAX_BINS = 65536, 4096
+TPCF_COUNT3_MAX_ROWS, TPCF_COUNT3_MAX_BINS = 16384, 30
 
 
 class TpcfError(RuntimeError):
@@ -51,7 +52,7 @@ class tpcf_stats(ctypes.Structure):
     _fields_ = [("pairs", ctypes.c_uint64), ("rechecked", ctypes.c_uint64), ("work_items", ctypes.c_uint64),
                 ("launches", ctypes.c_int), ("grid", ctypes.c_int), ("block", ctypes.c_int),
                 ("smem_bytes", ctypes.c_int), ("cells", ctypes.c_int), ("cell_bits", ctypes.c_int),
-                ("hist_copies", ctypes.c_int), ("kernel_ms", ctypes.c_float), ("win_blocks", ctypes.c_uint64 * 6),
+                ("kernel_ms", ctypes.c_float), ("win_blocks", ctypes.c_uint64 * 6),
                 ("pruned_blocks", ctypes.c_uint64), ("lookup_share", ctypes.c_float)]
 
     def as_dict(self):
@@ -104,6 +105,7 @@ def lib() -> ctypes.CDLL:
             "tpcf_classify_fast": [vp, ctypes.c_float, ctypes.POINTER(i32)],
             "tpcf_plan": [vp, i32, u64, u64, ctypes.POINTER(u64)],
             "tpcf_plan_item_pairs": [vp, i32, u64, u64, u64, ctypes.POINTER(u64)],
+            "tpcf_count3": [vp, i32, vp],
             "tpcf_count_static": [i32, vp, i32, vp, sz, vp, sz, i32, vp, vp, ctypes.c_char_p, sz],
         }
         for name, args in sig.items():
@@ -258,6 +260,14 @@ def tpcf_estimate(ctx, nbins: int) -> np.ndarray:
     w = np.empty(nbins, dtype=np.float64)
     _check(ctx, lib().tpcf_estimate(ctx, _np_ptr(w)))
     return w
+
+
+def tpcf_count3(ctx, which: int, nbins: int) -> np.ndarray:
+    """Three-point counts of one loaded catalog: uint64 array [nbins+2]^3 over the ascending side slots (include/tpcf.h)."""
+    m = nbins + 2
+    h3 = np.zeros((m, m, m), dtype=np.uint64)
+    _check(ctx, lib().tpcf_count3(ctx, int(which), _np_ptr(h3)))
+    return h3
 
 
 def tpcf_estimate_cross(ctx, nbins: int) -> np.ndarray:
@@ -441,6 +451,9 @@ class Context:
 
     def estimate(self):
         return tpcf_estimate(self._ctx, self.nbins)
+
+    def count3(self, which="D"):
+        return tpcf_count3(self._ctx, _CATS.get(which, which), self.nbins)
 
     def estimate_cross(self):
         return tpcf_estimate_cross(self._ctx, self.nbins)

@@ -253,6 +253,11 @@ Sides sides_of(tpcf_kind k) {
     }
 }
 
+// SM count the plan's chunking balances for.  Under a partition (tpcf_set_partition) every rank must number the
+// same items, whatever GPU it runs on: the chunking then uses the constant kPlanSMs; the device's own SM count only
+// sizes the grid and the j-split of a launch.
+int plan_sms(const tpcf_ctx* ctx) { return ctx->nparts > 1 ? kPlanSMs : ctx->sm_count; }
+
 uint32_t items_of_part(uint64_t n_items, int part, int nparts) {
     if ((uint64_t)part >= n_items) return 0;
     return (uint32_t)((n_items - part + nparts - 1) / nparts);
@@ -309,7 +314,7 @@ tpcf_status enqueue_count(tpcf_ctx* ctx, tpcf_kind kind, const int64_t* rows_hos
         sc.release();
         if (e != cudaSuccess) return cuda_fail(ctx, e, "gather subset rows");
         if (bad) return fail(ctx, TPCF_EINVAL, "row index out of range");
-        make_plan(false, nrows, cj.n, ctx->sm_count, subset_plan);
+        make_plan(false, nrows, cj.n, plan_sms(ctx), subset_plan);
         plan = &subset_plan;
         p.xq = tmp->xq;
         p.cq = tmp->cq;
@@ -321,7 +326,7 @@ tpcf_status enqueue_count(tpcf_ctx* ctx, tpcf_kind kind, const int64_t* rows_hos
     } else {
         PlanCache& pc = ctx->plans[kind];
         if (!pc.valid) {
-            make_plan(sd.tri, ci.n, cj.n, ctx->sm_count, pc.plan);
+            make_plan(sd.tri, ci.n, cj.n, plan_sms(ctx), pc.plan);
             if (pc.d_row_start) cudaFree(pc.d_row_start);
             pc.d_row_start = nullptr;
             if (sd.tri) {
@@ -444,7 +449,6 @@ tpcf_status enqueue_count(tpcf_ctx* ctx, tpcf_kind kind, const int64_t* rows_hos
     ctx->stats.smem_bytes = li.smem_bytes;
     ctx->stats.cells = ctx->ft.ncells;
     ctx->stats.cell_bits = (ctx->ft.map == CellMap::LogBits) ? 23 - ctx->ft.shift : -1;
-    ctx->stats.hist_copies = 1;
     if (pairs_out) {
         uint64_t pairs = 0;
         if (ctx->nparts == 1) {
@@ -691,8 +695,11 @@ static tpcf_status enqueue_count_all(tpcf_ctx* ctx, unsigned long long* hist_dev
         }
         CU(cudaEventRecord(kev.first, st), "cudaEventRecord");
     }
-    ctx->time_kernels = false;
-    CU(cudaEventRecord(ctx->fork, st), "cudaEventRecord");
+    ctx->time_kernels = false;              // restored below on every path
+    {
+        const cudaError_t e = cudaEventRecord(ctx->fork, st);
+        if (e != cudaSuccess) s = cuda_fail(ctx, e, "cudaEventRecord");
+    }
     const tpcf_kind order[3] = {TPCF_DR, TPCF_DD, TPCF_RR};
     for (int k = 0; k < 3 && s == TPCF_OK; ++k) {
         cudaStream_t on = k == 0 ? st : ctx->side[k - 1];
@@ -702,10 +709,12 @@ static tpcf_status enqueue_count_all(tpcf_ctx* ctx, unsigned long long* hist_dev
         }
         s = enqueue_count(ctx, order[k], nullptr, 0, hist_dev + (size_t)order[k] * (nb + 2), nullptr, nullptr,
                           pairs_out ? pairs_out + order[k] : nullptr, &on);
-        if (s == TPCF_OK && k > 0) {
+        if (k > 0) {
+            // a side stream that was forked is joined back whether or not its count could be enqueued: the context's stream
+            // must never run ahead of work that reads the catalogs
             cudaError_t e = cudaEventRecord(ctx->join[k - 1], on);
             if (e == cudaSuccess) e = cudaStreamWaitEvent(st, ctx->join[k - 1], 0);
-            if (e != cudaSuccess) s = cuda_fail(ctx, e, "join side stream");
+            if (e != cudaSuccess && s == TPCF_OK) s = cuda_fail(ctx, e, "join side stream");
         }
     }
     ctx->time_kernels = timing;
@@ -769,13 +778,23 @@ tpcf_status tpcf_set_weights(tpcf_ctx* ctx, tpcf_cat which, const double* w, siz
     for (size_t k = 0; k < n; ++k)
         if (!(std::fabs(w[k]) <= 1.0e150)) return fail(ctx, TPCF_EINVAL, "non-finite weight");
     cudaStream_t st = ctx->stream;
-    if (!c.w64) CU(cudaMalloc(&c.w64, c.n_pad * sizeof(double)), "cudaMalloc weights");
+    // a failure below must not leave a weights array that tpcf_count_weighted would accept: the old one is dropped first
+    // and the new one is attached to the catalog only when it is complete
+    cudaFree(c.w64);
+    c.w64 = nullptr;
     s = arena_reserve(ctx, n * sizeof(double));
     if (s) return s;
+    double* w64 = nullptr;
+    CU(cudaMalloc(&w64, c.n_pad * sizeof(double)), "cudaMalloc weights");
     double* staged = static_cast<double*>(ctx->arena);
-    CU(cudaMemcpyAsync(staged, w, n * sizeof(double), cudaMemcpyHostToDevice, st), "copy weights");
-    CU(launch_scatter_weights(staged, c.inv, n, c.n_pad, c.w64, st), "scatter_weights_kernel launch");
-    CU(cudaStreamSynchronize(st), "set weights");
+    cudaError_t e = cudaMemcpyAsync(staged, w, n * sizeof(double), cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = launch_scatter_weights(staged, c.inv, n, c.n_pad, w64, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) {
+        cudaFree(w64);
+        return cuda_fail(ctx, e, "set weights");
+    }
+    c.w64 = w64;
     return TPCF_OK;
 }
 
@@ -793,7 +812,7 @@ tpcf_status tpcf_count_weighted(tpcf_ctx* ctx, tpcf_kind kind, double* wsum_out,
     cudaStream_t st = ctx->stream;
     const int nb = ctx->bin.nbins;
     Plan plan;
-    make_plan(sd.tri, ci.n, cj.n, ctx->sm_count, plan);
+    make_plan(sd.tri, ci.n, cj.n, plan_sms(ctx), plan);
     if (plan.n_items > 0xFFFFFFFFull) return fail(ctx, TPCF_EINVAL, "catalogs too large for the 32-bit work-item index");
     uint32_t* d_row_start = nullptr;
     if (sd.tri) {
@@ -835,6 +854,43 @@ tpcf_status tpcf_count_weighted(tpcf_ctx* ctx, tpcf_kind kind, double* wsum_out,
         under_over_out[0] = host[0];
         under_over_out[1] = host[nb + 1];
     }
+    return TPCF_OK;
+}
+
+tpcf_status tpcf_count3(tpcf_ctx* ctx, tpcf_cat which, uint64_t* hist3_out) {
+    if (!ctx) return TPCF_EINVAL;
+    if (!hist3_out) return fail(ctx, TPCF_EINVAL, "hist3_out is NULL");
+    if (which != TPCF_D && which != TPCF_R && which != TPCF_D2) return fail(ctx, TPCF_EINVAL, "which must be TPCF_D, TPCF_R or TPCF_D2");
+    const int nb = ctx->bin.nbins;
+    if (nb > TPCF_COUNT3_MAX_BINS) return fail(ctx, TPCF_EINVAL, "tpcf_count3: more than TPCF_COUNT3_MAX_BINS (30) bins");
+    tpcf_status s = ensure_cuda(ctx);
+    if (s) return s;
+    const Catalog& c = ctx->cat[which];
+    if (!c.n) return fail(ctx, TPCF_ESTATE, "tpcf_count3 before the catalog was loaded");
+    if (c.n > (uint64_t)TPCF_COUNT3_MAX_ROWS) return fail(ctx, TPCF_EINVAL, "tpcf_count3: more than TPCF_COUNT3_MAX_ROWS (16384) rows");
+    const size_t m = (size_t)nb + 2, cells = m * m * m;
+    cudaStream_t st = ctx->stream;
+    // scratch: the pair-slot matrix, the result cells and the row counter, carved from the context's arena (tpcf_load's scratch)
+    const size_t sbytes = count3_slot_bytes(c.n);
+    s = arena_reserve(ctx, sbytes + cells * sizeof(unsigned long long) + 3 * 256);
+    if (s) return s;
+    Carver cv{static_cast<char*>(ctx->arena)};
+    uint8_t* slots = cv.take<uint8_t>(sbytes);
+    unsigned long long* result3 = cv.take<unsigned long long>(cells);
+    unsigned long long* next_row = cv.take<unsigned long long>(1);
+    cudaError_t e = cudaMemsetAsync(result3, 0, cells * sizeof(unsigned long long), st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(next_row, 0, sizeof(unsigned long long), st);
+    if (e == cudaSuccess) e = cudaEventRecord(ctx->ev0, st);
+    if (e == cudaSuccess) e = launch_count3(c.x64, (uint32_t)c.n, ctx->d_thr, nb, slots, next_row, result3, ctx->sm_count, st);
+    if (e == cudaSuccess) e = cudaEventRecord(ctx->ev1, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(hist3_out, result3, cells * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "three-point counts");
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, ctx->ev0, ctx->ev1);
+    ctx->stats.kernel_ms = ms;
+    ctx->stats.pairs = c.n * (c.n - 1) * (c.n - 2) / 6;      // triples, here
+    ctx->stats.launches = 2;
     return TPCF_OK;
 }
 
@@ -955,6 +1011,8 @@ tpcf_status tpcf_set_guard_scale(tpcf_ctx* ctx, double scale) {
 tpcf_status tpcf_set_partition(tpcf_ctx* ctx, int part, int nparts) {
     if (!ctx) return TPCF_EINVAL;
     if (nparts < 1 || part < 0 || part >= nparts) return fail(ctx, TPCF_EINVAL, "need 0 <= part < nparts");
+    if ((ctx->nparts > 1) != (nparts > 1))
+        for (auto& pc : ctx->plans) pc.valid = false;       // the chunking differs between the two (plan_sms)
     ctx->part = part;
     ctx->nparts = nparts;
     return TPCF_OK;
@@ -1041,9 +1099,10 @@ tpcf_status tpcf_get_bands(const tpcf_ctx* ctx, int capacity, float* lo_out, flo
 
 tpcf_status tpcf_plan(const tpcf_ctx* ctx, tpcf_kind kind, uint64_t n_d, uint64_t n_r, uint64_t* n_items_out) {
     if (!ctx || !n_items_out || n_d == 0 || n_r == 0) return TPCF_EINVAL;
+    if ((int)kind < 0 || (int)kind > (int)TPCF_RR) return TPCF_EINVAL;      // the D2 kinds have a third size
     Plan p;
     const Sides sd = sides_of(kind);
-    make_plan(sd.tri, sd.ci == 0 ? n_d : n_r, sd.cj == 0 ? n_d : n_r, ctx->sm_count, p);
+    make_plan(sd.tri, sd.ci == 0 ? n_d : n_r, sd.cj == 0 ? n_d : n_r, plan_sms(ctx), p);
     *n_items_out = p.n_items;
     return TPCF_OK;
 }
@@ -1051,9 +1110,10 @@ tpcf_status tpcf_plan(const tpcf_ctx* ctx, tpcf_kind kind, uint64_t n_d, uint64_
 tpcf_status tpcf_plan_item_pairs(const tpcf_ctx* ctx, tpcf_kind kind, uint64_t n_d, uint64_t n_r, uint64_t w,
                                  uint64_t* pairs_out) {
     if (!ctx || !pairs_out || n_d == 0 || n_r == 0) return TPCF_EINVAL;
+    if ((int)kind < 0 || (int)kind > (int)TPCF_RR) return TPCF_EINVAL;
     Plan p;
     const Sides sd = sides_of(kind);
-    make_plan(sd.tri, sd.ci == 0 ? n_d : n_r, sd.cj == 0 ? n_d : n_r, ctx->sm_count, p);
+    make_plan(sd.tri, sd.ci == 0 ? n_d : n_r, sd.cj == 0 ? n_d : n_r, plan_sms(ctx), p);
     if (w >= p.n_items) return TPCF_EINVAL;
     *pairs_out = p.item_pairs(w);
     return TPCF_OK;

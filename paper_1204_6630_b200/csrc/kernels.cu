@@ -2,7 +2,7 @@
 //
 //   convert_kernel      RA/Dec (deg) -> fp64 unit vector + sort key                     (hot-path step a1)
 //   radix_* / permute / spheres   spatial sort of the catalog, fp32 copy, subtile bounding spheres (a1)
-//   pair_fast_kernel    the all-pairs count: fp32 squared chord; per (lane, 32-row j-subtile) window of
+//   pair_fast_kernel    the all-pairs count: fp32 squared chord; per (lane, 64-row j-subtile) window of
 //                       candidate bin edges from bounding spheres -> 1..3 threshold compares per pair with
 //                       register counters, else O(1) cell lookup + shared-memory partial histogram;
 //                       guard band -> fp64 recheck; uint64 merge                        (steps a3-a7)
@@ -471,7 +471,7 @@ __device__ __forceinline__ void subtile_pairs(const float4* __restrict__ js, con
             lookup_block<MAP, true>(js, sx, sy, sz, act, lk, g, slow, rq, qn, i0, j0);
         } else if (lk.multi || !__all_sync(0xffffffffu, act)) {
             lookup_block<MAP, false>(js, sx, sy, sz, act, lk, g, slow, rq, qn, i0, j0);
-        } else if (MAP == (int)CellMap::SqrtLin && __any_sync(0xffffffffu, __fmul_ru(hi, hi) > lk.clamp)) {
+        } else if (MAP == (int)CellMap::SqrtLin && __any_sync(0xffffffffu, __fadd_ru(__fmul_ru(hi, hi), g) > lk.clamp)) {      // hi bounds the TRUE chords; the fp32 q may exceed them by g
             lookup_block_fast<MAP, true>(js, sx2, sy2, sz2, lk, g, slow, rq, qn, i0, j0);
         } else {
             lookup_block_fast<MAP, false>(js, sx2, sy2, sz2, lk, g, slow, rq, qn, i0, j0);

@@ -50,11 +50,7 @@ def test_cross_catalog_counts_and_estimator(engine, oracle_threads):
         sub = full(*c.count("D2R", rows))                             # rows index D2
         osub = oracle.count_rows(d2, rows, r, False, e, validate=True, threads=oracle_threads)
         assert_parity(sub, osub, 300 * nr)
-    h = {k: o[k].hist.astype(np.float64) for k in o}
-    nrr = 0.5 * nr * (nr - 1.0)
-    frr = h["RR"] / nrr
-    with np.errstate(divide="ignore", invalid="ignore"):
-        ref = np.where(h["RR"] > 0, (h["D1D2"] / (nd * n2) - h["DR"] / (nd * nr) - h["D2R"] / (n2 * nr) + frr) / frr, np.nan)
+    ref = oracle.estimate_cross(o["D1D2"].hist, o["DR"].hist, o["D2R"].hist, o["RR"].hist, nd, n2, nr)      # pinned in test_oracle_pins.py
     assert_w(w12, ref)
 
 

@@ -306,3 +306,25 @@ def test_product_package_does_not_touch_the_oracle():
             if f.endswith((".py", ".cu", ".cuh", ".cpp", ".h")):
                 src = open(os.path.join(dirpath, f)).read()
                 assert "import oracle" not in src and "from oracle" not in src and "tpcf_oracle" not in src, f
+
+
+def test_plan_refuses_the_kinds_with_a_third_catalog_size():
+    """tpcf_plan takes (n_d, n_r) only: D1D2 and D2R pair a third catalog whose size it is not told."""
+    with T.Context(4, [0.1, 10.0], "log") as c:
+        for kind in (T.TPCF_D1D2, T.TPCF_D2R, 7, -1):
+            with pytest.raises(T.TpcfError):
+                c.plan(kind, 1000, 1000)
+            with pytest.raises(T.TpcfError):
+                c.plan_item_pairs(kind, 1000, 1000, 0)
+
+
+def test_plan_numbering_under_a_partition_is_the_fixed_one():
+    """With nparts > 1 the chunking is balanced for the constant 148 SMs on every rank (ranks on GPUs with
+    different SM counts must enumerate the same items).  Without a GPU the context has not seen a device, so both
+    numberings coincide here; what this pins is that setting and clearing a partition leaves the plan arithmetic intact."""
+    with T.Context(4, [0.1, 10.0], "log") as c:
+        base = [(k, c.plan(k, 430_000, 300_000)) for k in ("DD", "DR", "RR")]
+        c.set_partition(1, 3)
+        assert [(k, c.plan(k, 430_000, 300_000)) for k in ("DD", "DR", "RR")] == base
+        c.set_partition(0, 1)
+        assert [(k, c.plan(k, 430_000, 300_000)) for k in ("DD", "DR", "RR")] == base
