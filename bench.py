@@ -193,7 +193,13 @@ def run_ours(args):
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device: libtpcf has no CPU fallback")
-    local = local % torch.cuda.device_count()      # one rank per GPU; on a box with fewer GPUs than ranks (tests) ranks share
+    ndev = torch.cuda.device_count()
+    if world > ndev:
+        if args.backend == "nccl":      # one rank per GPU, no exceptions: NCCL cannot put two ranks on one device
+            print(f"[bench] {world} ranks but only {ndev} CUDA device(s) visible: --backend nccl needs one GPU per rank "
+                  f"(use --backend gloo to smoke-test the N > 1 path on fewer GPUs)", file=sys.stderr, flush=True)
+            return 2
+        local = local % ndev            # gloo smoke test on a box with fewer GPUs than ranks: ranks share devices
     torch.cuda.set_device(local)
     if world > 1:
         if args.backend == "nccl":
@@ -290,16 +296,21 @@ def run_ours(args):
     Dp, Rp = torch.from_numpy(D).pin_memory(), torch.from_numpy(R).pin_memory()
     e2e_steps = max(1, min(args.steps, 5))
 
+    e2e_out = torch.zeros_like(out)
+
     def e2e_step():
         ctx.load("D", Dp, stream=st.cuda_stream)            # H2D copy + on-device conversion
         ctx.load("R", Rp, stream=st.cuda_stream)
         tdist.apply_partition(ctx)
-        ca = ctx.count_all()                                # D2H of the three histograms inside
-        hs = [ca[k] for k in KINDS]
         if world > 1:
-            arr = np.stack([np.concatenate([[u], h.astype(np.int64), [o]]) for h, u, o in hs])
-            arr = tdist.allreduce_counts(arr)
-            return T.tpcf_estimate_from(arr[0][1:-1], arr[1][1:-1], arr[2][1:-1], nd, nr)
+            # the partial histograms stay on the device for the all-reduce; one D2H of the summed counts, then Eq. 1
+            with torch.cuda.stream(st):
+                ctx.count_all_async(e2e_out)
+                tdist.allreduce_counts(e2e_out)
+                arr = e2e_out.cpu().numpy()
+            return T.tpcf_estimate_from(arr[0][1:-1].astype(np.uint64), arr[1][1:-1].astype(np.uint64),
+                                        arr[2][1:-1].astype(np.uint64), nd, nr)
+        ctx.count_all()                                     # D2H of the three histograms inside
         return ctx.estimate()
 
     e2e_step()
@@ -338,6 +349,7 @@ def run_ours(args):
     # one CUDA-event pair per step around the three overlapping pair kernels (tpcf_count_all_async)
     pairs_per_s_kernel = (sum(share) * len(kernel_ms) / (sum(kernel_ms) * 1e-3)) if kernel_ms else pairs_step / world / (ms_step * 1e-3)
     achieved = pairs_per_s_kernel * OPS_PER_PAIR / 1e12
+    ppcs = pairs_per_s_kernel / (SM_COUNT * sm_max * 1e6)          # pairs per clock per SM at the maximum SM clock
     roofline = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "T lane-operations/s (FP32 FMA-pipe + ALU-pipe operations)",
                 "frac": achieved / peak, "traffic": prof.get("dram_bytes_per_launch"),
                 "kernel": "pair_tensor_kernel" if tensor_ran else "pair_fast_kernel", "ops_per_pair": OPS_PER_PAIR,
@@ -350,7 +362,12 @@ def run_ours(args):
                 "kernel_ms_note": "per step: from the start of the first to the end of the last of the three overlapping pair kernels",
                 "kernel_launches_timed": len(kernel_ms),
                 "kernel_share_of_step": (sum(kernel_ms) / ms_total) if kernel_ms else None,
-                "pairs_per_clk_per_sm_at_max_clock": pairs_per_s_kernel / (SM_COUNT * sm_max * 1e6),
+                "pairs_per_clk_per_sm_at_max_clock": ppcs,
+                # BASELINE.json north_star's own figure: N_SM x 128 x f / (executed instructions per pair), the count taken
+                # from the committed ncu capture of THIS (config, kernel variant) -- null when there is none
+                "frac_counted_instruction": (ppcs * prof["inst_per_pair"] / LANES_PER_CLK_PER_SM) if prof.get("inst_per_pair") else None,
+                # the pipe that binds the tensor kernel: 1.5 ALU-pipe instructions per pair at 64 lanes/clk/SM = 42.7 pairs/clk/SM
+                "frac_of_alu_pipe_bound": (ppcs / (64.0 / 1.5)) if tensor_ran else None,
                 "fma_pipe_bound_pairs_per_clk_per_sm": LANES_PER_CLK_PER_SM / 4.0,
                 "peak_source": f"{SM_COUNT} SMs x {LANES_PER_CLK_PER_SM} FP32 lanes/clk x {sm_max:.0f} MHz ({peak_src}); DESIGN.md section 7",
                 "frac_at_sampled_clock": (achieved / (SM_COUNT * LANES_PER_CLK_PER_SM * clocks["sm_mhz"] * 1e6 / 1e12)) if clocks.get("sm_mhz") else None}
@@ -386,7 +403,9 @@ def run_ours(args):
             "seconds_per_w_theta": ms_step * 1e-3,
             "e2e": {"value": pairs_step / e2e_s / 1e9, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "seconds_per_step": e2e_s, "steps": e2e_steps,
-                    "path": ("tpcf_load_xyz" if wl.spatial else "tpcf_load") + "(D), (R) from pinned host rows + tpcf_count_all + tpcf_estimate"},
+                    "path": ("tpcf_load_xyz" if wl.spatial else "tpcf_load") + "(D), (R) from pinned host rows + " +
+                            ("tpcf_count_all + tpcf_estimate" if world == 1 else
+                             "tpcf_count_all_async + all-reduce of the device histograms + one D2H + tpcf_estimate_from")},
             "gpu_launches": args.steps * 6,
             "gpu_launches_note": f"per step: 3 x ({'pair_tensor_kernel' if tensor_ran else 'pair_fast_kernel'} + finalize_kernel), the three pair kernels in flight together on three streams (tpcf_count_all_async); memsets are driver memset nodes; the e2e leg adds 2 x 29 load kernels per step",
             "other_engine": other,
@@ -395,6 +414,18 @@ def run_ours(args):
     if world > 1:
         dist.destroy_process_group()
     return 0
+
+
+def spawn_ranks(n: int) -> int:
+    """`python bench.py --gpus N` without a launcher: re-run this command line as N ranks (one per GPU) under
+    torch.distributed.run on this node, exactly as the driver launches the N > 1 line; rank 0 prints the JSON line."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n}", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
 
 
 def main():
@@ -417,6 +448,8 @@ def main():
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.steps < 1:
         ap.error("--steps must be >= 1")
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        return spawn_ranks(args.gpus)
     if args.impl == "reference":
         return run_reference(args)
     return run_ours(args)

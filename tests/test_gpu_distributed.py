@@ -90,3 +90,38 @@ def test_two_processes_count_their_partitions_and_allreduce(engine, oracle_threa
     for i, k in enumerate(KINDS):
         assert_parity(single[i], o[k], want[k])
     assert_w(w1, oracle.estimate(o["DD"].hist, o["DR"].hist, o["RR"].hist, ND, NR))
+
+
+def _run_bench(*flags):
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    return subprocess.run([sys.executable, os.path.join(root, "bench.py"), *flags], cwd=root, env=env, capture_output=True,
+                          text=True, timeout=900)
+
+
+def test_bench_gpus_2_starts_two_ranks_by_itself():
+    """`python bench.py --gpus 2` with no launcher around it must start the two ranks itself (it used to
+    count on one GPU and print n_gpus 1).  gloo, because this box has one GPU; the totals check inside bench.py runs on the
+    all-reduced histograms, so a rank that did not take its share of the plan fails the run."""
+    import json
+    r = _run_bench("--gpus", "2", "--backend", "gloo", "--config", "2", "--steps", "3", "--no-cpu-baseline")
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1, "exactly one JSON line, from rank 0"
+    line = json.loads(lines[0])
+    assert line["n_gpus"] == 2 and line["config"]["comm_nranks"] == 2
+    assert "communicator of 2 ranks" in r.stderr
+    assert line["e2e"]["value"] > 0 and "all-reduce of the device histograms" in line["e2e"]["path"]
+
+
+def test_bench_refuses_nccl_with_more_ranks_than_gpus():
+    """NCCL needs one device per rank: with fewer visible GPUs the run must stop with a clear message, not stack the ranks
+    on one device and still print n_gpus = world."""
+    import torch
+    n = torch.cuda.device_count() + 1
+    r = _run_bench("--gpus", str(n), "--backend", "nccl", "--config", "1", "--steps", "1", "--no-cpu-baseline")
+    assert r.returncode != 0
+    assert "needs one GPU per rank" in r.stderr
+    assert not [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
