@@ -9,7 +9,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtpcf.so")
-SOURCES = ["api.cu", "kernels.cu", "noalloc.cu", "tables.cpp"]
+SOURCES = ["api.cu", "count3.cu", "kernels.cu", "noalloc.cu", "tables.cpp"]
 HEADERS = ["kernels.cuh", "tables.h", os.path.join("..", "..", "include", "tpcf.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",

@@ -106,4 +106,11 @@ cudaError_t launch_scatter_weights(const double* w, const uint32_t* inv, uint64_
 cudaError_t launch_finalize(const unsigned long long* result, int nbins, int zero_slot, unsigned long long self_pairs,
                             unsigned long long* out, cudaStream_t st);
 
+// three-point counts (count3.cu): bytes of the n x n pair-slot matrix, and the two kernels: slots <- slot of every pair (fp64),
+// result3[(a * m + b) * m + c] += triples i<j<k whose side slots in ascending order are (a, b, c), m = nbins + 2;
+// next_row (one counter) and result3 (m^3) must be zero on entry
+size_t count3_slot_bytes(uint64_t n);
+cudaError_t launch_count3(const double4* x64, uint32_t n, const double* thr, int nbins, uint8_t* slots, unsigned long long* next_row,
+                          unsigned long long* result3, int sm_count, cudaStream_t st);
+
 }  // namespace tpcf
